@@ -1,0 +1,500 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+Nothing here touches the CUDA library.  Each test names the passage of
+/root/reference/PAPER.md (or the SURVEY.md section 8(c) pin) it follows.  The
+brute-force tests enumerate trajectories from the *definitions* (Eq. 8/11 for
+G, <dx_1 dx_n> for the VACF) and never call the recursion they check.
+"""
+import itertools
+import os
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+import lpc_inputs
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+GOLD = os.path.join(ROOT, "tests", "golden")
+
+
+def _mk(oracle_mod, lat, **kw):
+    return oracle_mod.Oracle.from_lattice(lat, **kw)
+
+
+def _uniform(shape, bc=(0, 0, 0), alpha=1.0, dt=1.0, a=1.0, omega=0.0):
+    lat = lpc_inputs.random_small(shape, bc=bc, p_block=0.0, alpha=alpha, seed=0)
+    lat.dF[...] = 0.0
+    lat.omega[...] = omega
+    lat.dt = dt
+    lat.a = a
+    return lat
+
+
+# --------------------------------------------------------------------------
+# helpers that restate the *model*, not the oracle's recursion
+# --------------------------------------------------------------------------
+def _metropolis(dFi, dFj):
+    """Eq. 1."""
+    return np.exp(-(dFj - dFi)) if dFj > dFi else 1.0
+
+
+def _moves(lat):
+    """For every site: list of (target, probability, displacement vector) incl. staying.
+
+    Lattice-gas rule of PAPER.md:51-55: one of z = 6 neighbours is tried with
+    probability alpha/6 (alpha: :101); the hop is accepted with Eq. 1; a move
+    into an obstacle or through a wall leaves the particle where it is.
+    """
+    shape = lat.shape
+    moves = {}
+    for idx in itertools.product(*[range(n) for n in shape]):
+        if lat.blocked[idx]:
+            continue
+        lst, stay = [], 1.0
+        for d in range(3):
+            for s in (-1, 1):
+                tgt = list(idx)
+                tgt[d] += s
+                if tgt[d] < 0 or tgt[d] >= shape[d]:
+                    if lat.bc[d]:
+                        continue
+                    tgt[d] %= shape[d]
+                tgt = tuple(tgt)
+                if lat.blocked[tgt]:
+                    continue
+                p = lat.alpha / 6.0 * _metropolis(lat.dF[idx], lat.dF[tgt])
+                disp = np.zeros(3)
+                disp[d] = s * lat.a
+                lst.append((tgt, p, disp))
+                stay -= p
+        lst.append((idx, stay, np.zeros(3)))
+        moves[idx] = lst
+    return moves
+
+
+def _boltzmann(lat):
+    """Eq. 2 with <rho> = 1/N so that the densities sum to one."""
+    e = np.where(lat.blocked != 0, 0.0, np.exp(-lat.dF))
+    return e / e.sum()
+
+
+def _enumerate(lat, n):
+    """All n-step trajectories: returns G[0..n] (Eq. 8/11) and C[d, m] = <dx_1 dx_m>, m = 1..n."""
+    moves = _moves(lat)
+    pi = _boltzmann(lat)
+    G = np.zeros(n + 1, dtype=complex)
+    Cm = np.zeros((3, n + 1))
+
+    def walk(site, prob, phase, depth, dx1):
+        # phase = dt * sum of omega over the sites visited at steps 1..depth (Eq. 11)
+        G[depth] += prob * np.exp(1j * phase)
+        if depth == n:
+            return
+        for tgt, p, disp in moves[site]:
+            if p == 0.0:
+                continue
+            first = disp if depth == 0 else dx1
+            Cm[:, depth + 1] += prob * p * first * disp
+            walk(tgt, prob * p, phase + lat.dt * lat.omega[tgt], depth + 1, first)
+
+    for site in moves:
+        walk(site, pi[site], 0.0, 0, None)
+    return G, Cm
+
+
+# --------------------------------------------------------------------------
+# P1 conservation / P2 detailed balance / P3 stationarity
+# --------------------------------------------------------------------------
+@pytest.mark.parametrize("bc", [(0, 0, 0), (1, 0, 0), (1, 1, 1)])
+def test_p1_total_density_is_conserved(oracle_mod, bc):
+    lat = lpc_inputs.random_small((6, 5, 7), bc=bc, p_block=0.3, alpha=0.8, seed=1)
+    o = _mk(oracle_mod, lat)
+    rng = np.random.default_rng(5)
+    rho = rng.random(lat.shape) * (lat.blocked == 0)
+    out = o.propagate_real(rho, 50)
+    assert abs(out.sum() - rho.sum()) <= 1e-13 * rho.sum()
+    assert np.all(out[lat.blocked != 0] == 0.0)
+    assert out.min() >= 0.0
+
+
+def test_p1_delta_source_keeps_unit_mass(oracle_mod):
+    lat = lpc_inputs.random_small((5, 5, 5), bc=(0, 1, 0), p_block=0.2, seed=2)
+    o = _mk(oracle_mod, lat)
+    open_sites = np.argwhere(lat.blocked == 0)
+    for k in (0, len(open_sites) // 2, len(open_sites) - 1):
+        rho = np.zeros(lat.shape)
+        rho[tuple(open_sites[k])] = 1.0
+        for n in (1, 2, 9):
+            assert abs(o.propagate_real(rho, n).sum() - 1.0) < 1e-14
+
+
+@pytest.mark.parametrize("bc", [(0, 0, 0), (1, 0, 1)])
+def test_p2_detailed_balance(oracle_mod, bc):
+    """pi_i p(i->j) = pi_j p(j->i) = (alpha/6) min(pi_i, pi_j)."""
+    lat = lpc_inputs.random_small((4, 5, 3), bc=bc, p_block=0.25, alpha=0.7, seed=3)
+    o = _mk(oracle_mod, lat)
+    pi = o.pi().reshape(-1)
+    blk = lat.blocked.reshape(-1)
+    for i in range(lat.n_sites):
+        for d in range(3):
+            for s in (-1, 1):
+                j = oracle_mod.neighbor(lat.shape, bc, i, d, s)
+                if j < 0:
+                    continue
+                pij = oracle_mod.hop(lat.shape, bc, lat.alpha, lat.dF, lat.blocked, i, j)
+                pji = oracle_mod.hop(lat.shape, bc, lat.alpha, lat.dF, lat.blocked, j, i)
+                if blk[i] or blk[j]:
+                    assert pij == 0.0 and pji == 0.0
+                    continue
+                want = lat.alpha / 6.0 * min(pi[i], pi[j])
+                assert abs(pi[i] * pij - want) <= 2e-15 * want
+                assert abs(pi[j] * pji - want) <= 2e-15 * want
+
+
+def test_o1_boltzmann_density(oracle_mod):
+    """Eq. 2: rho_i proportional to exp(-dF_i), zero on carbon, normalised."""
+    lat = lpc_inputs.config0(L=8, n_steps=0)
+    o = _mk(oracle_mod, lat)
+    pi = o.pi()
+    assert abs(pi.sum() - 1.0) < 1e-14
+    assert np.all(pi[lat.blocked != 0] == 0.0)
+    opn = np.argwhere(lat.blocked == 0)
+    i, j = tuple(opn[0]), tuple(opn[-1])
+    assert np.isclose(np.log(pi[i] / pi[j]), -(lat.dF[i] - lat.dF[j]), rtol=0, atol=1e-14)
+    assert np.isclose(o.partition_sum, np.exp(-lat.dF[lat.blocked == 0]).sum(), rtol=1e-14)
+
+
+@pytest.mark.parametrize("bc", [(0, 0, 0), (1, 0, 0)])
+def test_p3_boltzmann_is_stationary(oracle_mod, bc):
+    lat = lpc_inputs.random_small((6, 6, 6), bc=bc, p_block=0.3, seed=4)
+    o = _mk(oracle_mod, lat)
+    pi = o.pi()
+    out = o.propagate_real(pi, 200)
+    assert np.max(np.abs(out - pi)) <= 1e-13 * pi.max()
+
+
+def test_p3_magnetisation_without_shift_stays_at_pi(oracle_mod):
+    lat = lpc_inputs.random_small((5, 4, 6), p_block=0.3, seed=6)
+    lat.omega[...] = 0.0
+    o = _mk(oracle_mod, lat, max_steps=100)
+    o.step(100)
+    assert np.max(np.abs(o.g() - o.pi())) <= 1e-13 * o.pi().max()
+    assert np.allclose(o.fid(), 1.0, rtol=0, atol=1e-13)
+
+
+# --------------------------------------------------------------------------
+# P4 relaxation to exp(-dF) within each connected cluster
+# --------------------------------------------------------------------------
+def _clusters(lat):
+    shape = lat.shape
+    label = -np.ones(shape, dtype=int)
+    nlab = 0
+    for start in itertools.product(*[range(n) for n in shape]):
+        if lat.blocked[start] or label[start] >= 0:
+            continue
+        stack = [start]
+        label[start] = nlab
+        while stack:
+            cur = stack.pop()
+            for d in range(3):
+                for s in (-1, 1):
+                    t = list(cur)
+                    t[d] += s
+                    if t[d] < 0 or t[d] >= shape[d]:
+                        if lat.bc[d]:
+                            continue
+                        t[d] %= shape[d]
+                    t = tuple(t)
+                    if not lat.blocked[t] and label[t] < 0:
+                        label[t] = nlab
+                        stack.append(t)
+        nlab += 1
+    return label, nlab
+
+
+@pytest.mark.parametrize("bc", [(0, 0, 0), (1, 0, 0)])
+def test_p4_relaxes_to_boltzmann_per_cluster(oracle_mod, bc):
+    lat = lpc_inputs.random_small((8, 8, 8), bc=bc, p_block=0.3, alpha=0.9, seed=7, dF_span=2.0)
+    # carve two pockets cut off from the main pore network: a single site and a pair
+    for cell, keep in (((2, 2, 2), [(2, 2, 2)]), ((5, 5, 5), [(5, 5, 5), (5, 5, 6)])):
+        for k in keep:
+            for d in range(3):
+                for s in (-1, 1):
+                    t = list(k)
+                    t[d] += s
+                    lat.blocked[tuple(t)] = 1
+        for k in keep:
+            lat.blocked[k] = 0
+    o = _mk(oracle_mod, lat)
+    pi = o.pi()
+    rng = np.random.default_rng(11)
+    rho0 = rng.random(lat.shape) * (lat.blocked == 0)
+    out = o.propagate_real(rho0, 6000)
+    label, nlab = _clusters(lat)
+    assert nlab >= 3  # isolated pockets: the per-cluster statement matters
+    for c in range(nlab):
+        m = label == c
+        mass = rho0[m].sum()
+        assert abs(out[m].sum() - mass) <= 1e-12 * max(mass, 1e-300)
+        want = mass * pi[m] / pi[m].sum()
+        assert np.max(np.abs(out[m] - want)) <= 1e-9 * want.max()
+
+
+def test_p4_bipartite_lattice_never_relaxes_at_alpha_one(oracle_mod):
+    """SURVEY P4 caveat: alpha = 1 on a homogeneous even lattice has stay = 0 (period 2)."""
+    lat = _uniform((4, 4, 4), alpha=1.0)
+    o = _mk(oracle_mod, lat)
+    assert np.all(np.abs(o.stay()) <= 2.3e-16)  # 1 - 6 * (1/6) up to rounding
+    rho = np.zeros(lat.shape)
+    rho[0, 0, 0] = 1.0
+    out = o.propagate_real(rho, 1001)
+    parity = np.indices(lat.shape).sum(axis=0) % 2
+    assert out[parity == 0].sum() <= 1e-12  # an equilibrated lattice would hold one half here
+    assert abs(out[parity == 1].sum() - 1.0) <= 1e-12
+
+
+# --------------------------------------------------------------------------
+# P5 free diffusion closed form (Eq. 6, Eq. 7) -- golden values
+# --------------------------------------------------------------------------
+def _golden(name):
+    rows = []
+    with open(os.path.join(GOLD, name)) as fh:
+        for line in fh:
+            if line.strip() and not line.startswith("#"):
+                rows.append([float(v) for v in line.split()])
+    return rows
+
+
+@pytest.mark.parametrize("row", _golden("free_diffusion.txt"))
+def test_p5_free_diffusion(oracle_mod, row):
+    alpha, a, dt, D_want, Z1_want = row
+    L = 12
+    lat = _uniform((L, L, L), alpha=alpha, dt=dt, a=a)
+    o = _mk(oracle_mod, lat, n_moments=3, max_steps=8)
+    o.step(8)
+    vacf, D = o.moments()
+    assert np.allclose(vacf[:, 0], Z1_want, rtol=1e-14)
+    assert np.max(np.abs(vacf[:, 1:])) <= 1e-17  # uncorrelated successive jumps
+    assert np.allclose(D, D_want, rtol=1e-13)
+    # MSD(n) = n alpha a^2 from a delta start, while the cloud has not met its image (n < L/2)
+    rho = np.zeros(lat.shape)
+    rho[0, 0, 0] = 1.0
+    ax = np.minimum(np.arange(L), L - np.arange(L)) * a
+    r2 = ax[:, None, None] ** 2 + ax[None, :, None] ** 2 + ax[None, None, :] ** 2
+    for n in (1, 3, 5):
+        out = o.propagate_real(rho, n)
+        assert np.isclose((out * r2).sum(), n * alpha * a * a, rtol=1e-13)
+
+
+# --------------------------------------------------------------------------
+# P6 uniform shift -> one line at omega (Eq. 8) -- golden values
+# --------------------------------------------------------------------------
+@pytest.mark.parametrize("row", _golden("uniform_shift.txt"))
+def test_p6_uniform_shift_single_line(oracle_mod, row):
+    omega, dt, n, re, im = row
+    n = int(n)
+    lat = lpc_inputs.random_small((5, 6, 4), bc=(0, 1, 0), p_block=0.3, alpha=0.6, seed=8)
+    lat.omega[...] = omega
+    lat.dt = dt
+    o = _mk(oracle_mod, lat, max_steps=n)
+    o.step(n)
+    G = o.fid()
+    assert abs(G[n] - complex(re, im)) < 1e-12
+    k = np.arange(n + 1)
+    assert np.max(np.abs(G - np.exp(1j * omega * dt * k))) < 1e-12
+    assert np.max(np.abs(np.abs(G) - 1.0)) < 1e-12
+
+
+# --------------------------------------------------------------------------
+# P7 brute force: every trajectory, from the definitions
+# --------------------------------------------------------------------------
+@pytest.mark.parametrize("shape,bc,n,alpha", [
+    ((4, 4, 4), (0, 0, 0), 3, 1.0),
+    ((3, 2, 4), (1, 0, 1), 4, 0.7),
+    ((2, 1, 3), (0, 0, 0), 5, 0.9),   # degenerate axes: neighbours coincide / are the site itself (Q17)
+])
+def test_p7_trajectory_enumeration(oracle_mod, shape, bc, n, alpha):
+    lat = lpc_inputs.random_small(shape, bc=bc, p_block=0.25, alpha=alpha, seed=9, n_steps=n)
+    lat.dt = 2.0e-5  # larger phase steps than the default so that the test has teeth
+    o = _mk(oracle_mod, lat, n_moments=3, max_steps=n)
+    o.step(n)
+    G_def, C_def = _enumerate(lat, n)
+    G = o.fid()
+    assert np.max(np.abs(G - G_def)) < 1e-12   # the enumeration adds ~1e5 terms uncompensated
+    vacf, D = o.moments(n)
+    for d in range(3):
+        assert np.max(np.abs(vacf[d] - C_def[d, 1:])) < 1e-13
+    D_def = C_def[:, 1] / (2 * lat.dt) + C_def[:, 2:].sum(axis=1) / lat.dt   # Eq. 4
+    assert np.allclose(D, D_def, rtol=1e-10, atol=1e-10 * abs(D_def).max())
+
+
+def test_p7_dense_matrix_power_4cubed(oracle_mod):
+    """4^3: G[n] = 1^T (Phi W)^n pi with W built entry by entry from the move table."""
+    lat = lpc_inputs.config0(L=4, n_steps=50)
+    moves = _moves(lat)
+    N = lat.n_sites
+    flat = lambda idx: (idx[0] * lat.ny + idx[1]) * lat.nz + idx[2]
+    W = np.zeros((N, N))
+    for src, lst in moves.items():
+        for tgt, p, _ in lst:
+            W[flat(tgt), flat(src)] += p
+    Phi = np.diag(np.exp(1j * lat.omega.reshape(-1) * lat.dt))
+    v = _boltzmann(lat).reshape(-1).astype(complex)
+    o = _mk(oracle_mod, lat)
+    o.step(50)
+    G = o.fid()
+    for n in range(51):
+        assert abs(G[n] - v.sum()) < 1e-13
+        v = Phi @ (W @ v)
+    assert np.max(np.abs(o.g().reshape(-1) - np.linalg.matrix_power(Phi @ W, 50) @ _boltzmann(lat).reshape(-1))) < 1e-15
+
+
+# --------------------------------------------------------------------------
+# P8 bounds
+# --------------------------------------------------------------------------
+def test_p8_bounds(oracle_mod):
+    lat = lpc_inputs.config0(L=8, n_steps=300)
+    o = _mk(oracle_mod, lat)
+    pi = o.pi()
+    prev = 1.0
+    for _ in range(30):
+        o.step(10)
+        assert np.all(np.abs(o.g()) <= pi * (1 + 1e-12))
+        G, sabs = o.fid(with_scale=True)
+        assert sabs[-1] <= prev * (1 + 1e-14)
+        prev = sabs[-1]
+        assert abs(G[-1]) <= sabs[-1] + 1e-15
+    assert abs(G[0] - 1.0) < 1e-14 and abs(sabs[0] - 1.0) < 1e-14
+
+
+# --------------------------------------------------------------------------
+# P9 bounded system: D_x -> 0     P10 Lorentz gas first lag
+# --------------------------------------------------------------------------
+def test_p9_reflective_box_sum_rule(oracle_mod):
+    lat = lpc_inputs.random_small((6, 3, 3), bc=(1, 0, 0), p_block=0.0, alpha=0.8, seed=10, dF_span=1.5)
+    lat.dt = 1.0
+    n = 4000
+    o = _mk(oracle_mod, lat, n_moments=3, max_steps=n)
+    o.step(n)
+    vacf, D = o.moments()
+    assert abs(D[0]) < 1e-13          # confined along x: no long-time diffusion
+    assert D[1] > 1e-2 and D[2] > 1e-2  # free along the periodic axes
+
+
+def test_p10_lorentz_gas_first_lag(oracle_mod):
+    lat = lpc_inputs.random_small((10, 10, 10), p_block=0.3, alpha=0.8, seed=12)
+    lat.dF[...] = 0.0
+    o = _mk(oracle_mod, lat, n_moments=3, max_steps=1)
+    o.step(1)
+    vacf, _ = o.moments(2)
+    opn = (lat.blocked == 0).astype(float)
+    n_open = opn.sum()
+    for d in range(3):
+        diff = np.roll(opn, -1, axis=d) - np.roll(opn, 1, axis=d)
+        want2 = -(lat.alpha ** 2 * lat.a ** 2 / (36.0 * n_open)) * (opn * diff * diff).sum()
+        want1 = (lat.alpha * lat.a ** 2 / (6.0 * n_open)) * (opn * (np.roll(opn, -1, axis=d) + np.roll(opn, 1, axis=d))).sum()
+        assert np.isclose(vacf[d, 1], want2, rtol=1e-12)
+        assert np.isclose(vacf[d, 0], want1, rtol=1e-12)
+
+
+# --------------------------------------------------------------------------
+# P11 two-site exchange (Bloch-McConnell in discrete time), exact 2x2 form
+# --------------------------------------------------------------------------
+def test_p11_two_site_exchange(oracle_mod):
+    lat = lpc_inputs.random_small((2, 1, 1), p_block=0.0, alpha=0.6, seed=13)
+    lat.dF[:, 0, 0] = [0.0, 1.2]
+    lat.omega[:, 0, 0] = [0.0, -9000.0]
+    lat.dt = 2.0e-5
+    n = 200
+    o = _mk(oracle_mod, lat, max_steps=n)
+    o.step(n)
+    # site A <-> B through the two x links (both lead to the other site); y, z links lead back home
+    kAB = 2 * lat.alpha / 6 * np.exp(-1.2)
+    kBA = 2 * lat.alpha / 6
+    W = np.array([[1 - kAB, kBA], [kAB, 1 - kBA]])
+    Phi = np.diag(np.exp(1j * lat.omega[:, 0, 0] * lat.dt))
+    p = np.array([1.0, np.exp(-1.2)])
+    v = (p / p.sum()).astype(complex)
+    want = []
+    for _ in range(n + 1):
+        want.append(v.sum())
+        v = Phi @ (W @ v)
+    assert np.max(np.abs(o.fid() - np.array(want))) < 1e-14
+
+
+# --------------------------------------------------------------------------
+# P12 symmetries
+# --------------------------------------------------------------------------
+def test_p12_axis_permutation_and_translation(oracle_mod):
+    lat = lpc_inputs.random_small((5, 6, 7), bc=(1, 0, 0), p_block=0.25, alpha=0.9, seed=14)
+    n = 25
+    o = _mk(oracle_mod, lat, n_moments=3, max_steps=n)
+    o.step(n)
+    G, (vacf, D) = o.fid(), o.moments()
+    # permute axes (x,y,z) -> (z,x,y)
+    perm = (2, 0, 1)
+    lat2 = lpc_inputs.random_small((7, 5, 6), bc=tuple(lat.bc[p] for p in perm), alpha=0.9, seed=14)
+    lat2.dF = np.ascontiguousarray(lat.dF.transpose(perm))
+    lat2.blocked = np.ascontiguousarray(lat.blocked.transpose(perm))
+    lat2.omega = np.ascontiguousarray(lat.omega.transpose(perm))
+    o2 = _mk(oracle_mod, lat2, n_moments=3, max_steps=n)
+    o2.step(n)
+    assert np.max(np.abs(o2.fid() - G)) < 1e-14
+    vacf2, D2 = o2.moments()
+    for new_axis, old_axis in enumerate(perm):
+        assert np.allclose(vacf2[new_axis], vacf[old_axis], rtol=1e-11, atol=1e-16)
+        assert np.isclose(D2[new_axis], D[old_axis], rtol=1e-9)
+    assert np.max(np.abs(o2.g() - o.g().transpose(perm))) < 1e-16
+    # translate along the periodic axes
+    lat3 = lpc_inputs.random_small((5, 6, 7), bc=(1, 0, 0), alpha=0.9, seed=14)
+    for name in ("dF", "blocked", "omega"):
+        setattr(lat3, name, np.ascontiguousarray(np.roll(getattr(lat, name), (2, -3), axis=(1, 2))))
+    o3 = _mk(oracle_mod, lat3, max_steps=n)
+    o3.step(n)
+    assert np.max(np.abs(o3.fid() - G)) < 1e-14
+
+
+# --------------------------------------------------------------------------
+# Q16 isolated site, API guards, thread-count independence
+# --------------------------------------------------------------------------
+def test_q16_isolated_open_site_only_rotates(oracle_mod):
+    lat = lpc_inputs.random_small((4, 4, 4), p_block=0.0, seed=15)
+    lat.blocked[...] = 0
+    c = (2, 2, 2)
+    for d in range(3):
+        for s in (-1, 1):
+            t = list(c)
+            t[d] += s
+            lat.blocked[tuple(t)] = 1
+    o = _mk(oracle_mod, lat, max_steps=7)
+    o.step(7)
+    assert o.stay()[c] == 1.0
+    want = o.pi()[c] * np.exp(1j * lat.omega[c] * lat.dt * 7)
+    assert abs(o.g()[c] - want) < 1e-15 * abs(want) * 10
+
+
+def test_rejects_bad_inputs(oracle_mod):
+    lat = lpc_inputs.random_small((3, 3, 3), seed=16)
+    with pytest.raises(ValueError):
+        oracle_mod.Oracle(lat.shape, lat.bc, lat.dt, lat.a, 0.0, lat.dF, lat.blocked, lat.omega)
+    with pytest.raises(ValueError):
+        oracle_mod.Oracle(lat.shape, lat.bc, lat.dt, lat.a, 1.0, lat.dF, np.ones_like(lat.blocked), lat.omega)
+    o = _mk(oracle_mod, lat, max_steps=2)
+    with pytest.raises(ValueError):
+        o.step(3)
+
+
+def test_result_does_not_depend_on_thread_count():
+    code = (
+        "import sys; sys.path.insert(0, %r); import importlib.util, numpy as np, lpc_inputs;"
+        "s = importlib.util.spec_from_file_location('o', %r); m = importlib.util.module_from_spec(s); s.loader.exec_module(m);"
+        "lat = lpc_inputs.config0(L=12, n_steps=20, n_moments=3); o = m.Oracle.from_lattice(lat); o.step(20);"
+        "v, D = o.moments(); sys.stdout.write(o.fid().tobytes().hex() + v.tobytes().hex())"
+    ) % (ROOT, os.path.join(ROOT, "oracle", "lpc_oracle.py"))
+    outs = []
+    for nt in ("1", "3", "8"):
+        env = dict(os.environ, OMP_NUM_THREADS=nt)
+        outs.append(subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, check=True).stdout)
+    assert outs[0] == outs[1] == outs[2] and len(outs[0]) > 100
