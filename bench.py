@@ -1,0 +1,286 @@
+#!/usr/bin/env python
+"""bench.py -- GLUPS and HBM roofline of the LPC3D propagation step on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--size L]
+
+One "step" is one lattice time step: the whole hot path (propagate + phase-rotate +
+FID reduce) over every site of the lattice.  The workload is
+the configuration the north star quotes its target on: the 512^3 lattice of
+BASELINE.json configs[4] (monolith statistics, fp64, NMR kernel alone).  It is 8.6 GB
+of state and parameters, far larger than the 126 MB L2, so no L2 flush is needed
+between steps.
+
+N > 1 (torchrun): the path is benchmarked as independent replicas, one lattice per
+GPU, no data-path collective; value = all ranks' site updates
+divided by the slowest rank's time.
+
+--impl reference times the CPU oracle (oracle/) as it stands on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import lpc_inputs  # noqa: E402
+
+METRIC = "lattice site updates/sec (GLUPS), 1 step = propagate + phase-rotate + FID reduce over all sites"
+UNIT = "GLUPS"
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md
+
+
+def parse():
+    p = argparse.ArgumentParser()
+    p.add_argument("--gpus", type=int, default=1)
+    p.add_argument("--steps", type=int, default=1000)
+    p.add_argument("--warmup", type=int, default=100)
+    p.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    p.add_argument("--size", type=int, default=512, help="lattice edge L of the L^3 workload")
+    p.add_argument("--moments", type=int, default=0, choices=[0, 3], help="also propagate the 3 VACF fields")
+    p.add_argument("--precision", type=int, default=0, choices=[0, 1])
+    p.add_argument("--kernel", type=int, default=0, choices=[0, 1, 2])
+    p.add_argument("--no-cpu-baseline", action="store_true")
+    p.add_argument("--no-e2e", action="store_true")
+    return p.parse_args()
+
+
+def load_oracle():
+    import importlib.util
+
+    spec = importlib.util.spec_from_file_location("lpc_oracle", os.path.join(ROOT, "oracle", "lpc_oracle.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    return mod
+
+
+def workload_name(L, moments, precision):
+    return (f"configs[4] sweep: {L}^3 periodic, monolith statistics (Gaussian pore field ell=8, 20% blocked), "
+            f"{'fp32' if precision else 'fp64'}, {'NMR + 3 moment fields' if moments else 'NMR kernel alone'}")
+
+
+# --------------------------------------------------------------------------------------------
+# CPU oracle timing (cpu_baseline leg and --impl reference)
+# --------------------------------------------------------------------------------------------
+def oracle_sample(moments, steps=None, warmup=1, budget_s=12.0, L=160):
+    """Time the oracle on a bounded sample of the workload: an L^3 lattice with the same statistics."""
+    orc_mod = load_oracle()
+    lat = lpc_inputs.sweep(L, n_moments=moments)
+    cap = 100000
+    o = orc_mod.Oracle.from_lattice(lat, max_steps=cap)
+    o.step(warmup)
+    if steps is None:
+        t0 = time.perf_counter()
+        o.step(1)
+        one = time.perf_counter() - t0
+        steps = max(2, min(200, int(budget_s / max(one, 1e-6))))
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    return {
+        "value": lat.n_sites * steps / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+        "sample": f"{L}^3 sub-lattice with the workload's statistics, {steps} steps after {warmup} warm-up "
+                  f"(oracle/lpc_oracle.c, gcc -O2 -fopenmp, {dt:.1f} s)",
+    }, steps, dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cb, steps, dt = oracle_sample(args.moments, steps=args.steps if args.steps <= 200 else None, warmup=max(1, min(args.warmup, 3)))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": max(1, min(args.warmup, 3)), "ms_per_step": dt / steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(args.size, args.moments, 0), "sample": cb["sample"]},
+        "cpu_baseline": cb,
+        "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line))
+
+
+# --------------------------------------------------------------------------------------------
+# clocks
+# --------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), [v.strip() for v in line.split(",")]))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        rows = [r for t, r in self.rows if t0 <= t <= t1] or [r for _, r in self.rows]
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0]))
+                mx = float(r[1])
+            except Exception:
+                continue
+            for name, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# --------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2603_22553_b200 as lpc
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    torch.cuda.set_device(local)
+    dev = f"cuda:{local}"
+
+    L, K, W = args.size, args.steps, args.warmup
+    lat = lpc_inputs.sweep(L, n_moments=args.moments)
+    n_sites = lat.n_sites
+    # pinned host buffers: the inputs of the end-to-end job
+    host = [torch.from_numpy(a).pin_memory() for a in (lat.dF, lat.blocked, lat.omega)]
+    h2d_job = sum(t.numel() * t.element_size() for t in host)
+
+    sim = lpc.Lattice(lat.shape, bc=lat.bc, precision=args.precision, n_moments=args.moments, dt=lat.dt, a=lat.a,
+                      alpha=lat.alpha, max_steps=2 * K + W + 8, device=dev)
+    sim.set_kernel(args.kernel)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- end-to-end job through the C ABI with host buffers: upload + precompute + K steps, each step's G[n] read back
+    e2e = None
+    if not args.no_e2e:
+        sim.set_site_params(*host)          # warm the path once (page-in, module load)
+        lpc.lpc_step_n(sim.handle, 3)
+        barrier()
+        t0 = time.perf_counter()
+        sim.set_site_params(*host)
+        last = None
+        for k in range(K):
+            lpc.lpc_step_n(sim.handle, 1)
+            last = lpc.lpc_read_fid(sim.handle, k + 1, 1)
+        torch.cuda.synchronize()
+        t_e2e = time.perf_counter() - t0
+        te = torch.tensor([t_e2e], device=dev, dtype=torch.float64)
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * n_sites * K / float(te.item()) / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": h2d_job / K, "d2h_bytes_per_step": 16,
+               "what": "lpc_set_site_params from pinned host arrays (amortised over the K steps) + K x (lpc_step_n(1) + "
+                       "lpc_read_fid of that step's sample to the host)"}
+        assert np.isfinite(last).all()
+    else:
+        sim.set_site_params(*host)
+
+    # ---- device-timed region: W warm-up steps, then exactly K steps between CUDA events on the library's stream
+    lpc.lpc_step_n(sim.handle, W)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.25)
+    l0 = sim.launch_count
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    tw0 = time.perf_counter()
+    ev0.record()
+    lpc.lpc_step_n(sim.handle, K)
+    ev1.record()
+    barrier()
+    tw1 = time.perf_counter()
+    clocks = sampler.stop(tw0, tw1)
+    ms = ev0.elapsed_time(ev1)
+    launches = sim.launch_count - l0
+    tm = torch.tensor([ms], device=dev, dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(tm, op=dist.ReduceOp.MAX)
+    ms_max = float(tm.item())
+    fid = sim.fid()
+    assert np.isfinite(fid).all() and abs(fid[0] - 1.0) < 1e-12, "FID series is not sane"
+
+    if rank == 0:
+        value = world * n_sites * K / (ms_max * 1e-3) / 1e9
+        peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+        if os.path.exists(peaks_path):
+            peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (measured copy)"
+        else:
+            peak, peak_src = FALLBACK_HBM_GBS, "fallback of B200_PROFILING.md"
+        bps = sim.bytes_per_site_step
+        ms_kernel = ms / launches          # one launch per step; this rank's own time
+        achieved = bps * n_sites / (ms_kernel * 1e-3) / 1e9
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tpath):
+            t = json.load(open(tpath))
+            key = f"{L}^3/m{args.moments}/p{args.precision}"
+            traffic = t.get(key, {}).get("dram_bytes_per_launch")
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32" if args.precision else "f64", "data": "synthetic",
+            "config": {"workload": workload_name(L, args.moments, args.precision), "lattice": list(lat.shape),
+                       "sites": n_sites, "parallelism": f"{world} independent replica(s), no collective",
+                       "l2": "working set 8.6 GB per step >> 126 MB L2, no flush needed" if L >= 256 else
+                             "working set may fit L2: not an HBM measurement",
+                       "kernel": {0: "auto (tma)", 1: "direct", 2: "tma"}[args.kernel]},
+            "clocks": clocks,
+            "e2e": e2e,
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": traffic, "peak_source": peak_src, "bytes_per_site_step": bps,
+                         "kernel_ms": ms_kernel, "frac_of_8TBs_spec": achieved / 8000.0},
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = oracle_sample(args.moments)[0]
+        print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

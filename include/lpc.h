@@ -1,0 +1,150 @@
+/*
+ * lpc.h -- C ABI of liblpc.so: the LPC3D lattice-gas propagation step on one
+ * NVIDIA B200 (sm_100a).
+ *
+ * Method: arxiv 2603.22553.  Each time step propagates the complex
+ * NMR magnetisation g_i between neighbouring lattice sites with Metropolis hop
+ * probabilities (Eq. 1) that keep the Boltzmann density (Eq. 2,
+ * :66) stationary, multiplies by the site phase exp(i omega_i dt) (Eq. 13,
+ * :144) and sums all sites into one free-induction-decay sample G(n dt)
+ * (Eq. 12, :137).  Optionally the same sweep propagates the three
+ * moment-propagation fields of the velocity autocorrelation function
+ * (Eq. 4-5, :79-95; :84-86) and a real density field (:192).
+ *
+ * Conventions
+ *   - Site arrays are dense, C order, shape (nx, ny, nz), z fastest:
+ *     i = (x*ny + y)*nz + z.
+ *   - Energies are in kT.  omega_i = 2 pi nu_i in rad/s.
+ *   - Every pointer argument says "host", "device" or "host or device".  A
+ *     "host or device" pointer is classified with cudaPointerGetAttributes.
+ *   - All device work is enqueued on lpc_config.stream.  lpc_step_n does not
+ *     synchronise; every call that returns data to the host does.
+ *   - The library never allocates device memory: the caller passes one
+ *     workspace (lpc_workspace_bytes) that must outlive the lattice.
+ *   - Return value: 0 (LPC_OK) or a negative LPC_E* code; lpc_last_error()
+ *     gives a thread-local message.  No exception crosses this boundary and
+ *     there is no CPU fallback: without an sm_100 device calls return
+ *     LPC_ECUDA.
+ */
+#ifndef LPC_H_
+#define LPC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LPC_OK 0
+#define LPC_EINVAL (-1) /* bad dimension, null pointer, alpha outside (0,1], range, all sites blocked */
+#define LPC_ESTATE (-2) /* call out of order, e.g. lpc_step_n before lpc_set_site_params */
+#define LPC_ENOMEM (-3) /* workspace too small or misaligned */
+#define LPC_ECUDA (-4)  /* CUDA runtime / driver error, or no sm_100 device */
+
+/* lpc_read_field / lpc_set_state selectors */
+#define LPC_FIELD_G 0   /* complex magnetisation g_i: 2N doubles, interleaved re,im      */
+#define LPC_FIELD_PI 1  /* equilibrium density pi_i (Eq. 2, sums to 1): N doubles, read only */
+#define LPC_FIELD_PX 2  /* moment field P^x_i (needs n_moments = 3): N doubles            */
+#define LPC_FIELD_PY 3
+#define LPC_FIELD_PZ 4
+#define LPC_FIELD_RHO 5 /* real density rho_i (needs n_density = 1): N doubles            */
+
+/* lpc_set_kernel selectors */
+#define LPC_KERNEL_AUTO 0
+#define LPC_KERNEL_DIRECT 1 /* one thread per site pair, neighbours straight from global memory */
+#define LPC_KERNEL_TMA 2    /* TMA-staged x-marching tiles, mbarrier pipeline                  */
+
+typedef struct lpc_lattice lpc_lattice; /* opaque, host struct owned by the library */
+
+typedef struct lpc_config {
+  int32_t nx, ny, nz;  /* lattice size, each >= 1 ("system dimensions")            */
+  int32_t bc[3];       /* per axis: 0 periodic, 1 reflective zero-flux wall      */
+  int32_t precision;   /* 0: fp64 storage and arithmetic; 1: fp32 storage and arithmetic with   */
+                       /*    fp64 reductions                                                    */
+  int32_t n_moments;   /* 0, or 3 to propagate P^x, P^y, P^z for the VACF / D (Eq. 4)           */
+  int32_t n_density;   /* 0, or 1 to propagate a real density rho alongside      */
+  int32_t reserved;    /* must be 0                                                             */
+  double dt;           /* time step in s (5e-6)                                   */
+  double a;            /* lattice spacing; D comes out in a^2 / dt units of it    */
+  double alpha;        /* global jump factor in (0,1], Eq. 7                 */
+  int64_t max_steps;   /* capacity of the G and VACF series, >= 0                               */
+  void* stream;        /* cudaStream_t owned by the caller (e.g. a torch stream); NULL = legacy */
+                       /* default stream                                                        */
+} lpc_config;
+
+/* Bytes of device workspace lpc_create_lattice needs for this configuration.
+ * cfg: host.  bytes: host, out.  Errors: LPC_EINVAL.  Needs no GPU.                            */
+int lpc_workspace_bytes(const lpc_config* cfg, size_t* bytes);
+
+/* Create a lattice over a caller-owned device workspace (256-byte aligned, >= the size above).
+ * The workspace holds the packed per-site parameters, the ping-pong state, the per-block
+ * partial sums and the G / VACF series; the caller frees it after lpc_destroy.
+ * cfg: host.  workspace_dev: device.  out: host, receives the handle.
+ * Errors: LPC_EINVAL, LPC_ENOMEM, LPC_ECUDA.                                                    */
+int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes, lpc_lattice** out);
+
+/* Site-parameter precompute (north star (a); Eq. 1, Eq. 2, Eq. 13 phase, Eq. 5):
+ *   pi_i = exp(-dF_i) / sum_j exp(-dF_j) on open sites, 0 on blocked ones;
+ *   packed hop data: pi_i and kappa_i = (alpha/6) / pi_i, from which every hop probability
+ *   follows as p(i->j) = kappa_i * min(pi_i, pi_j)  (= (alpha/6) min(1, exp(-(dF_j - dF_i))));
+ *   phase factors cos(omega_i dt), sin(omega_i dt);
+ *   initial state g(0) = pi (or g0), P^d(1), Z_d[1], rho(0) = pi, G[0].
+ * dF_kT, omega_rad_s: host or device, N doubles.  blocked: host or device, N bytes (non-zero =
+ * carbon).  g0_or_null: host or device, 2N doubles (re,im) or NULL for g(0) = pi.  The arrays
+ * are read during the call and not referenced afterwards.  Values at blocked sites are ignored.
+ * Resets the step counter and both series.  Synchronises the stream.
+ * Errors: LPC_EINVAL (null pointer; every site blocked; exp(-dF) over- or underflows, i.e. the
+ * spread of dF exceeds about 700 kT), LPC_ECUDA.                                               */
+int lpc_set_site_params(lpc_lattice* lat, const double* dF_kT, const uint8_t* blocked,
+                        const double* omega_rad_s, const void* g0_or_null);
+
+/* Advance n time steps (north star (b), (c); Eq. 13 + Eq. 12, Eq. 4): per step one fused sweep
+ * that propagates, phase-rotates, reduces G[n] and (if enabled) Z_d[n+1], P^d, rho.
+ * Asynchronous on the stream.  Errors: LPC_ESTATE (no site parameters yet), LPC_EINVAL (n < 0 or
+ * steps_done + n > max_steps), LPC_ECUDA.                                                      */
+int lpc_step_n(lpc_lattice* lat, int64_t n);
+
+/* Copy G[first .. first+count) to the host as interleaved (re, im) doubles.  G[0] is the initial
+ * sum; the series has steps_done + 1 samples.  out_re_im_host: host, 2*count doubles.
+ * Synchronises.  Errors: LPC_EINVAL (range), LPC_ESTATE, LPC_ECUDA.                             */
+int lpc_read_fid(lpc_lattice* lat, int64_t first, int64_t count, double* out_re_im_host);
+
+/* VACF series and diffusion coefficients (Eq. 4):
+ *   vacf_xyz_host[d*count + (m-1)] = Z_d[m] = <dx_1 dx_m>,  m = 1..count  (count <= steps_done+1)
+ *   D_xyz[d] = Z_d[1] / (2 dt) + (1/dt) * sum_{m=2..count} Z_d[m]
+ * vacf_xyz_host: host, 3*count doubles, may be NULL.  D_xyz: host, 3 doubles.  Synchronises.
+ * Errors: LPC_ESTATE (n_moments == 0 or no parameters), LPC_EINVAL (range), LPC_ECUDA.         */
+int lpc_moments(lpc_lattice* lat, int64_t count, double* vacf_xyz_host, double D_xyz[3]);
+
+/* Read a site field into a dense (nx,ny,nz) array of doubles (see LPC_FIELD_*).
+ * out: host or device.  Synchronises.  Errors: LPC_EINVAL, LPC_ESTATE, LPC_ECUDA.              */
+int lpc_read_field(lpc_lattice* lat, int32_t which, void* out);
+
+/* Overwrite a state field (LPC_FIELD_G or LPC_FIELD_RHO) from a dense array; values at blocked
+ * sites are ignored (set to 0).  LPC_FIELD_G resets the step counter and series (G[0] = sum g).
+ * in: host or device.  Synchronises.  Errors: LPC_EINVAL, LPC_ESTATE, LPC_ECUDA.               */
+int lpc_set_state(lpc_lattice* lat, int32_t which, const void* in);
+
+/* Choose the step kernel (LPC_KERNEL_*).  AUTO picks TMA.  Errors: LPC_EINVAL.                 */
+int lpc_set_kernel(lpc_lattice* lat, int32_t which);
+
+/* Steps taken since the last lpc_set_site_params / lpc_set_state(G).                           */
+int64_t lpc_steps_done(const lpc_lattice* lat);
+
+/* Kernel launches this lattice has enqueued so far (all kernels, for accounting).              */
+int64_t lpc_launch_count(const lpc_lattice* lat);
+
+/* Algorithmic HBM bytes one step moves per lattice site with this configuration.   */
+double lpc_bytes_per_site_step(const lpc_lattice* lat);
+
+/* Free the host handle (the workspace stays with the caller).  NULL is allowed.                */
+void lpc_destroy(lpc_lattice* lat);
+
+/* Message of the last error on this thread ("" if none).                                       */
+const char* lpc_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LPC_H_ */

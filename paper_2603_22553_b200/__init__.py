@@ -1,0 +1,280 @@
+"""paper_2603_22553_b200 -- thin Python binding of liblpc.so (include/lpc.h).
+
+Argument marshalling only: every step of the LPC3D hot path (site-parameter
+precompute, fused propagate + phase-rotate + FID reduce, moment propagation)
+runs in the CUDA kernels of ``csrc/`` behind the C ABI.  PyTorch is used for
+device memory (the workspace) and streams, nothing else.
+
+There is no CPU fallback.  If ``liblpc.so`` has not been built
+(``python -m paper_2603_22553_b200.build``) the first call raises ImportError.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "liblpc.so")
+
+LPC_OK, LPC_EINVAL, LPC_ESTATE, LPC_ENOMEM, LPC_ECUDA = 0, -1, -2, -3, -4
+LPC_FIELD_G, LPC_FIELD_PI, LPC_FIELD_PX, LPC_FIELD_PY, LPC_FIELD_PZ, LPC_FIELD_RHO = range(6)
+LPC_KERNEL_AUTO, LPC_KERNEL_DIRECT, LPC_KERNEL_TMA = range(3)
+
+EXPORTS = (
+    "lpc_workspace_bytes", "lpc_create_lattice", "lpc_set_site_params", "lpc_step_n", "lpc_read_fid",
+    "lpc_moments", "lpc_read_field", "lpc_set_state", "lpc_set_kernel", "lpc_steps_done",
+    "lpc_launch_count", "lpc_bytes_per_site_step", "lpc_destroy", "lpc_last_error",
+)
+
+
+class LpcError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"liblpc error {code}: {msg}")
+        self.code = code
+
+
+class lpc_config(C.Structure):
+    _fields_ = [
+        ("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("bc", C.c_int32 * 3),
+        ("precision", C.c_int32), ("n_moments", C.c_int32), ("n_density", C.c_int32), ("reserved", C.c_int32),
+        ("dt", C.c_double), ("a", C.c_double), ("alpha", C.c_double),
+        ("max_steps", C.c_int64), ("stream", C.c_void_p),
+    ]
+
+
+_lib_handle = None
+
+
+def _load():
+    """Load liblpc.so on first use; there is no fallback if it is missing."""
+    global _lib_handle
+    if _lib_handle is not None:
+        return _lib_handle
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            f"{LIB_PATH} is missing: build the CUDA library with `python -m paper_2603_22553_b200.build` "
+            "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    lib.lpc_workspace_bytes.argtypes = [C.POINTER(lpc_config), C.POINTER(C.c_size_t)]
+    lib.lpc_create_lattice.argtypes = [C.POINTER(lpc_config), C.c_void_p, C.c_size_t, C.POINTER(C.c_void_p)]
+    lib.lpc_set_site_params.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.lpc_step_n.argtypes = [C.c_void_p, C.c_int64]
+    lib.lpc_read_fid.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_void_p]
+    lib.lpc_moments.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
+    lib.lpc_read_field.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
+    lib.lpc_set_state.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
+    lib.lpc_set_kernel.argtypes = [C.c_void_p, C.c_int32]
+    lib.lpc_steps_done.argtypes = [C.c_void_p]
+    lib.lpc_steps_done.restype = C.c_int64
+    lib.lpc_launch_count.argtypes = [C.c_void_p]
+    lib.lpc_launch_count.restype = C.c_int64
+    lib.lpc_bytes_per_site_step.argtypes = [C.c_void_p]
+    lib.lpc_bytes_per_site_step.restype = C.c_double
+    lib.lpc_destroy.argtypes = [C.c_void_p]
+    lib.lpc_destroy.restype = None
+    lib.lpc_last_error.restype = C.c_char_p
+    _lib_handle = lib
+    return lib
+
+
+class _LazyLib:
+    def __getattr__(self, name):
+        return getattr(_load(), name)
+
+
+_lib = _LazyLib()
+
+
+def lpc_last_error() -> str:
+    return _lib.lpc_last_error().decode()
+
+
+def _check(rc):
+    if rc != LPC_OK:
+        raise LpcError(rc, lpc_last_error())
+
+
+def _ptr(x, dtype=None, count=None):
+    """Address of a numpy array (host) or torch tensor (host or device); keeps nothing alive."""
+    if x is None:
+        return None
+    if isinstance(x, np.ndarray):
+        if dtype is not None and x.dtype != dtype:
+            raise TypeError(f"expected {dtype}, got {x.dtype}")
+        if not x.flags.c_contiguous:
+            raise ValueError("array must be C-contiguous")
+        if count is not None and x.size != count:
+            raise ValueError(f"expected {count} elements, got {x.size}")
+        return C.c_void_p(x.ctypes.data)
+    if hasattr(x, "data_ptr"):
+        if not x.is_contiguous():
+            raise ValueError("tensor must be contiguous")
+        if count is not None and x.numel() != count:
+            raise ValueError(f"expected {count} elements, got {x.numel()}")
+        return C.c_void_p(x.data_ptr())
+    raise TypeError(f"cannot take the address of {type(x)}")
+
+
+def make_config(nx, ny, nz, bc=(0, 0, 0), precision=0, n_moments=0, n_density=0, dt=5e-6, a=1.0, alpha=1.0,
+                max_steps=0, stream=None) -> lpc_config:
+    return lpc_config(int(nx), int(ny), int(nz), (C.c_int32 * 3)(*[int(b) for b in bc]), int(precision),
+                      int(n_moments), int(n_density), 0, float(dt), float(a), float(alpha), int(max_steps),
+                      C.c_void_p(stream) if stream else None)
+
+
+def lpc_workspace_bytes(cfg: lpc_config) -> int:
+    out = C.c_size_t(0)
+    _check(_lib.lpc_workspace_bytes(C.byref(cfg), C.byref(out)))
+    return int(out.value)
+
+
+def lpc_create_lattice(cfg: lpc_config, workspace, nbytes=None):
+    """workspace: torch uint8 CUDA tensor (or a raw device address with nbytes)."""
+    handle = C.c_void_p()
+    if hasattr(workspace, "data_ptr"):
+        addr, nbytes = workspace.data_ptr(), workspace.numel() * workspace.element_size()
+    else:
+        addr = int(workspace)
+    _check(_lib.lpc_create_lattice(C.byref(cfg), C.c_void_p(addr), C.c_size_t(int(nbytes)), C.byref(handle)))
+    return handle
+
+
+def lpc_set_site_params(handle, dF, blocked, omega, g0=None):
+    _check(_lib.lpc_set_site_params(handle, _ptr(dF), _ptr(blocked), _ptr(omega), _ptr(g0)))
+
+
+def lpc_step_n(handle, n):
+    _check(_lib.lpc_step_n(handle, int(n)))
+
+
+def lpc_read_fid(handle, first=0, count=None):
+    if count is None:
+        count = int(_lib.lpc_steps_done(handle)) + 1 - first
+    out = np.empty(count, dtype=np.complex128)
+    _check(_lib.lpc_read_fid(handle, int(first), int(count), C.c_void_p(out.ctypes.data)))
+    return out
+
+
+def lpc_moments(handle, count=None):
+    """(vacf[3, count] with vacf[d, m-1] = Z_d[m], D[3])."""
+    if count is None:
+        count = int(_lib.lpc_steps_done(handle)) + 1
+    vacf = np.empty((3, count), dtype=np.float64)
+    D = np.empty(3, dtype=np.float64)
+    _check(_lib.lpc_moments(handle, int(count), C.c_void_p(vacf.ctypes.data), C.c_void_p(D.ctypes.data)))
+    return vacf, D
+
+
+def lpc_read_field(handle, which, out):
+    _check(_lib.lpc_read_field(handle, int(which), _ptr(out)))
+    return out
+
+
+def lpc_set_state(handle, which, arr):
+    _check(_lib.lpc_set_state(handle, int(which), _ptr(arr)))
+
+
+def lpc_set_kernel(handle, which):
+    _check(_lib.lpc_set_kernel(handle, int(which)))
+
+
+def lpc_steps_done(handle) -> int:
+    return int(_lib.lpc_steps_done(handle))
+
+
+def lpc_launch_count(handle) -> int:
+    return int(_lib.lpc_launch_count(handle))
+
+
+def lpc_bytes_per_site_step(handle) -> float:
+    return float(_lib.lpc_bytes_per_site_step(handle))
+
+
+def lpc_destroy(handle):
+    _lib.lpc_destroy(handle)
+
+
+class Lattice:
+    """Owns the torch workspace and the handle; methods forward to the C calls one to one."""
+
+    def __init__(self, shape, bc=(0, 0, 0), precision=0, n_moments=0, n_density=0, dt=5e-6, a=1.0, alpha=1.0,
+                 max_steps=0, device="cuda:0", stream=None):
+        import torch
+
+        self.shape = tuple(int(v) for v in shape)
+        self.n = int(np.prod(self.shape))
+        self.device = torch.device(device)
+        if stream is None:
+            stream = torch.cuda.current_stream(self.device)
+        self.stream = stream
+        self.cfg = make_config(*self.shape, bc=bc, precision=precision, n_moments=n_moments, n_density=n_density,
+                               dt=dt, a=a, alpha=alpha, max_steps=max_steps, stream=stream.cuda_stream)
+        self.workspace_bytes = lpc_workspace_bytes(self.cfg)
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(self.workspace_bytes, dtype=torch.uint8, device=self.device)
+            self.handle = lpc_create_lattice(self.cfg, self.workspace)
+
+    @classmethod
+    def from_inputs(cls, lat, precision=0, n_moments=None, n_density=0, max_steps=None, device="cuda:0", g0=None):
+        """Build from an ``lpc_inputs.Lattice`` (host arrays) and run the precompute."""
+        self = cls(lat.shape, bc=lat.bc, precision=precision,
+                   n_moments=lat.n_moments if n_moments is None else n_moments, n_density=n_density,
+                   dt=lat.dt, a=lat.a, alpha=lat.alpha,
+                   max_steps=lat.n_steps if max_steps is None else max_steps, device=device)
+        self.set_site_params(lat.dF, lat.blocked, lat.omega, g0)
+        return self
+
+    def close(self):
+        if getattr(self, "handle", None):
+            lpc_destroy(self.handle)
+            self.handle = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_site_params(self, dF, blocked, omega, g0=None):
+        if isinstance(dF, np.ndarray):
+            dF = np.ascontiguousarray(dF, dtype=np.float64)
+            blocked = np.ascontiguousarray(blocked, dtype=np.uint8)
+            omega = np.ascontiguousarray(omega, dtype=np.float64)
+        if isinstance(g0, np.ndarray):
+            g0 = np.ascontiguousarray(g0, dtype=np.complex128)
+        lpc_set_site_params(self.handle, dF, blocked, omega, g0)
+
+    def step(self, n=1):
+        lpc_step_n(self.handle, n)
+
+    def fid(self, first=0, count=None):
+        return lpc_read_fid(self.handle, first, count)
+
+    def moments(self, count=None):
+        return lpc_moments(self.handle, count)
+
+    def field(self, which):
+        out = np.empty(self.shape, dtype=np.complex128 if which == LPC_FIELD_G else np.float64)
+        return lpc_read_field(self.handle, which, out)
+
+    def set_state(self, which, arr):
+        arr = np.ascontiguousarray(arr, dtype=np.complex128 if which == LPC_FIELD_G else np.float64)
+        lpc_set_state(self.handle, which, arr)
+
+    def set_kernel(self, which):
+        lpc_set_kernel(self.handle, which)
+
+    @property
+    def steps_done(self):
+        return lpc_steps_done(self.handle)
+
+    @property
+    def launch_count(self):
+        return lpc_launch_count(self.handle)
+
+    @property
+    def bytes_per_site_step(self):
+        return lpc_bytes_per_site_step(self.handle)

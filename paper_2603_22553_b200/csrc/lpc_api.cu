@@ -1,0 +1,605 @@
+// lpc_api.cu -- host side of liblpc.so: the C ABI of include/lpc.h.
+//
+// Workspace layout (device, all offsets 256-byte aligned):
+//   Ctl | fid[max_steps+1] | vacf[3][max_steps+2] | partials | pi | kcs[3] | F0[C] | F1[C] | staging
+// F0/F1 are the ping-pong state buffers in density-normalised, channel-planar (SoA) form.
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "../../include/lpc.h"
+#include "lpc_internal.cuh"
+#include "lpc_precompute.cuh"
+#include "lpc_step.cuh"
+
+using namespace lpc;
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+#define CUDA_TRY(expr)                                                                                  \
+  do {                                                                                                  \
+    cudaError_t e_ = (expr);                                                                            \
+    if (e_ != cudaSuccess) return fail(LPC_ECUDA, "%s: %s (%s:%d)", #expr, cudaGetErrorString(e_), __FILE__, __LINE__); \
+  } while (0)
+
+constexpr size_t ALIGN = 256;
+size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
+
+constexpr int DIRECT_MAX_BLOCKS = 148 * 8;
+constexpr int AUX_BLOCKS = 148 * 8;
+constexpr long long STAGE_SITES = 4ll << 20;  // sites per host<->device staging chunk
+
+struct Offsets {
+  size_t ctl, fid, vacf, partials, pi, kcs, f0, f1, staging, total;
+  size_t partial_slots;
+};
+
+}  // namespace
+
+struct lpc_lattice {
+  lpc_config cfg;
+  Layout L;
+  int C, nrho, nmom, sT;
+  long long N;
+  Offsets off;
+  unsigned char* ws;
+  cudaStream_t stream;
+  bool have_params;
+  int cur;  // index of the buffer holding the current state
+  long long steps;
+  long long launches;
+  int kernel;  // LPC_KERNEL_*
+  // TMA geometry
+  int ty, tz, nstage, xc, tiles_z, tiles_y, chunks_x;
+  bool tma_ok;
+  CUtensorMap tm_f[2], tm_pi, tm_kcs;
+};
+
+namespace {
+
+int check_cfg(const lpc_config* c) {
+  if (!c) return fail(LPC_EINVAL, "config is NULL");
+  if (c->nx < 1 || c->ny < 1 || c->nz < 1) return fail(LPC_EINVAL, "lattice dimensions must be >= 1 (got %d %d %d)", c->nx, c->ny, c->nz);
+  if ((long long)c->nx * c->ny * c->nz > (1ll << 40)) return fail(LPC_EINVAL, "lattice too large");
+  for (int d = 0; d < 3; ++d)
+    if (c->bc[d] != 0 && c->bc[d] != 1) return fail(LPC_EINVAL, "bc[%d] must be 0 (periodic) or 1 (reflective)", d);
+  if (c->precision != 0 && c->precision != 1) return fail(LPC_EINVAL, "precision must be 0 (fp64) or 1 (fp32)");
+  if (c->n_moments != 0 && c->n_moments != 3) return fail(LPC_EINVAL, "n_moments must be 0 or 3");
+  if (c->n_density != 0 && c->n_density != 1) return fail(LPC_EINVAL, "n_density must be 0 or 1");
+  if (c->reserved != 0) return fail(LPC_EINVAL, "reserved must be 0");
+  if (!(c->alpha > 0.0 && c->alpha <= 1.0)) return fail(LPC_EINVAL, "alpha must lie in (0,1]");
+  if (!(c->dt > 0.0) || !std::isfinite(c->dt)) return fail(LPC_EINVAL, "dt must be positive");
+  if (!(c->a > 0.0) || !std::isfinite(c->a)) return fail(LPC_EINVAL, "a must be positive");
+  if (c->max_steps < 0) return fail(LPC_EINVAL, "max_steps must be >= 0");
+  return LPC_OK;
+}
+
+Layout make_layout(const lpc_config* c) {
+  Layout L;
+  const int sT = c->precision ? 4 : 8;
+  L.nx = c->nx; L.ny = c->ny; L.nz = c->nz;
+  L.padz = 128 / sT;  // 128 bytes of ghost columns on each side keep every row 128-byte aligned
+  L.nxp = c->nx + 2;
+  L.nyp = c->ny + 2;
+  L.nzp = (c->nz + L.padz - 1) / L.padz * L.padz + 2 * L.padz;
+  L.sy = L.nzp;
+  L.sx = (long long)L.nyp * L.nzp;
+  L.np = (long long)L.nxp * L.sx;
+  return L;
+}
+
+// TMA tile geometry per channel count.
+void tma_geometry(int C, int nx, int ny, int nz, int* ty, int* tz, int* nstage, int* xc, int* tiles_z, int* tiles_y, int* chunks_x) {
+  *ty = 8; *tz = 64;
+  *nstage = (C <= 3) ? 4 : 3;
+  *tiles_z = (nz + *tz - 1) / *tz;
+  *tiles_y = (ny + *ty - 1) / *ty;
+  const long long tiles = (long long)*tiles_z * *tiles_y;
+  const long long resident = 148ll * ((C <= 3) ? 2 : 1);
+  long long chunks = (12 * resident + tiles - 1) / tiles;     // aim for ~12 waves of CTAs ...
+  chunks = std::min<long long>(chunks, std::max(1, nx / 32)); // ... but at least 32 planes per chunk
+  chunks = std::max<long long>(chunks, 1);
+  if (const char* e = getenv("LPC_XC")) {
+    const int v = atoi(e);
+    if (v > 0) chunks = (nx + v - 1) / v;
+  }
+  *xc = (int)((nx + chunks - 1) / chunks);
+  *chunks_x = (nx + *xc - 1) / *xc;
+}
+
+Offsets make_offsets(const lpc_config* c, const Layout& L) {
+  Offsets o;
+  const size_t sT = c->precision ? 4 : 8;
+  const int C = 2 + c->n_density + c->n_moments;
+  int ty, tz, ns, xc, tzs, tys, cxs;
+  tma_geometry(C, c->nx, c->ny, c->nz, &ty, &tz, &ns, &xc, &tzs, &tys, &cxs);
+  // the LPC_XC override may only shrink chunks at run time; size for the worst case (one plane per chunk)
+  const size_t tma_blocks = (size_t)tzs * tys * (size_t)c->nx;
+  o.partial_slots = std::max<size_t>(std::max<size_t>(DIRECT_MAX_BLOCKS, AUX_BLOCKS), std::min<size_t>(tma_blocks, 1u << 20));
+  const long long N = (long long)c->nx * c->ny * c->nz;
+  size_t p = 0;
+  o.ctl = p; p += align_up(sizeof(Ctl));
+  o.fid = p; p += align_up((size_t)(c->max_steps + 1) * sizeof(double2));
+  o.vacf = p; p += align_up((size_t)3 * (c->max_steps + 2) * sizeof(double));
+  o.partials = p; p += align_up(o.partial_slots * MAX_RED * sizeof(double));
+  o.pi = p; p += align_up((size_t)L.np * sT);
+  o.kcs = p; p += align_up((size_t)3 * L.np * sT);
+  o.f0 = p; p += align_up((size_t)C * L.np * sT);
+  o.f1 = p; p += align_up((size_t)C * L.np * sT);
+  o.staging = p; p += align_up((size_t)std::min<long long>(N, STAGE_SITES) * 16);
+  o.total = p;
+  return o;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+int get_encode_fn(EncodeTiledFn* out) {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q));
+    if (q != cudaDriverEntryPointSuccess || !p) return fail(LPC_ECUDA, "cuTensorMapEncodeTiled not available in this driver");
+    fn = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  *out = fn;
+  return LPC_OK;
+}
+
+int encode_map(CUtensorMap* m, bool f32, void* base, int rank, const cuuint64_t* dims, const cuuint32_t* box) {
+  EncodeTiledFn fn;
+  int rc = get_encode_fn(&fn);
+  if (rc) return rc;
+  const cuuint64_t sT = f32 ? 4 : 8;
+  cuuint64_t strides[4];
+  cuuint64_t s = sT;
+  for (int d = 0; d < rank - 1; ++d) {
+    s *= dims[d];
+    strides[d] = s;
+  }
+  cuuint32_t estr[4] = {1, 1, 1, 1};
+  CUresult r = fn(m, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, (cuuint32_t)rank, base, dims, strides, box,
+                  estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(LPC_ECUDA, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+  return LPC_OK;
+}
+
+template <typename T> T* wsp(lpc_lattice* h, size_t off) { return reinterpret_cast<T*>(h->ws + off); }
+
+bool is_device_ptr(const void* p) {
+  cudaPointerAttributes at;
+  if (cudaPointerGetAttributes(&at, p) != cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+int aux_grid(long long n) { return (int)std::max<long long>(1, std::min<long long>((n + 255) / 256, AUX_BLOCKS)); }
+
+// ---- launch of one sweep ---------------------------------------------------------------------
+template <typename T, int NRHO, int NMOM>
+int launch_step_t(lpc_lattice* h) {
+  StepArgs<T> a;
+  a.L = h->L;
+  a.fin = wsp<T>(h, h->cur ? h->off.f1 : h->off.f0);
+  a.fout = wsp<T>(h, h->cur ? h->off.f0 : h->off.f1);
+  a.pi = wsp<T>(h, h->off.pi);
+  a.kcs = wsp<T>(h, h->off.kcs);
+  a.partials = wsp<double>(h, h->off.partials);
+  a.ctl = wsp<Ctl>(h, h->off.ctl);
+  a.fid = wsp<double2>(h, h->off.fid);
+  a.vacf = wsp<double>(h, h->off.vacf);
+  a.vacf_stride = h->cfg.max_steps + 2;
+  a.zscale = h->cfg.a * h->cfg.alpha / 6.0;
+  for (int d = 0; d < 3; ++d) a.per[d] = h->cfg.bc[d] == 0;
+  a.xc = h->xc; a.tiles_z = h->tiles_z; a.tiles_y = h->tiles_y; a.chunks_x = h->chunks_x;
+
+  const bool use_tma = h->tma_ok && h->kernel != LPC_KERNEL_DIRECT;
+  if (use_tma) {
+    constexpr int C = 2 + NRHO + NMOM;
+    constexpr int NS = (C <= 3) ? 4 : 3;
+    using K = TmaCfg<T, NRHO, NMOM, 8, 64, NS>;
+    auto kern = step_tma_kernel<T, NRHO, NMOM, 8, 64, NS>;
+    static bool attr_set = false;
+    if (!attr_set) {
+      CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, K::SMEM_BYTES));
+      attr_set = true;
+    }
+    const unsigned grid = (unsigned)(h->tiles_z * h->tiles_y * h->chunks_x);
+    kern<<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(h->tm_f[h->cur], h->tm_pi, h->tm_kcs, a);
+  } else {
+    const long long npairs = (long long)((h->L.nz + 1) / 2) * h->L.ny * h->L.nx;
+    const int grid = (int)std::max<long long>(1, std::min<long long>((npairs + 255) / 256, DIRECT_MAX_BLOCKS));
+    step_direct_kernel<T, NRHO, NMOM><<<grid, 256, 0, h->stream>>>(a);
+  }
+  CUDA_TRY(cudaGetLastError());
+  h->launches++;
+  h->cur ^= 1;
+  return LPC_OK;
+}
+
+template <typename T>
+int launch_step(lpc_lattice* h) {
+  if (h->nrho == 0 && h->nmom == 0) return launch_step_t<T, 0, 0>(h);
+  if (h->nrho == 1 && h->nmom == 0) return launch_step_t<T, 1, 0>(h);
+  if (h->nrho == 0 && h->nmom == 3) return launch_step_t<T, 0, 3>(h);
+  return launch_step_t<T, 1, 3>(h);
+}
+
+// ---- staging helpers: run `body(dev_ptr, i0, n)` over chunks of a dense host/device array -----
+template <typename F>
+int for_chunks_in(lpc_lattice* h, const void* src, size_t bytes_per_site, F body) {
+  if (is_device_ptr(src)) return body(src, 0ll, h->N);
+  const long long chunk = std::min<long long>(h->N, STAGE_SITES);
+  unsigned char* stg = h->ws + h->off.staging;
+  for (long long i0 = 0; i0 < h->N; i0 += chunk) {
+    const long long n = std::min(chunk, h->N - i0);
+    CUDA_TRY(cudaMemcpyAsync(stg, static_cast<const unsigned char*>(src) + (size_t)i0 * bytes_per_site, (size_t)n * bytes_per_site,
+                             cudaMemcpyHostToDevice, h->stream));
+    int rc = body(stg, i0, n);
+    if (rc) return rc;
+    // the staging buffer is reused by the next chunk
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+  }
+  return LPC_OK;
+}
+
+template <typename T>
+int fill_state_ghosts(lpc_lattice* h) {
+  const Layout& L = h->L;
+  const long long cells = 2ll * ((long long)L.nx * L.ny + (long long)L.nx * L.nz + (long long)L.ny * L.nz) * h->C;
+  fill_ghosts_kernel<T><<<aux_grid(cells), 256, 0, h->stream>>>(wsp<T>(h, h->cur ? h->off.f1 : h->off.f0), h->C, L, h->cfg.bc[0] == 0,
+                                                                 h->cfg.bc[1] == 0, h->cfg.bc[2] == 0);
+  CUDA_TRY(cudaGetLastError());
+  h->launches++;
+  return LPC_OK;
+}
+
+template <typename T>
+int set_g_from(lpc_lattice* h, const void* g) {
+  T* f = wsp<T>(h, h->cur ? h->off.f1 : h->off.f0);
+  int rc = for_chunks_in(h, g, 16, [&](const void* d, long long i0, long long n) {
+    set_h_kernel<T><<<aux_grid(n), 256, 0, h->stream>>>(static_cast<const double*>(d), i0, n, h->L, wsp<T>(h, h->off.pi), f);
+    CUDA_TRY(cudaGetLastError());
+    h->launches++;
+    return LPC_OK;
+  });
+  if (rc) return rc;
+  reduce_g_kernel<T><<<aux_grid(h->N), 256, 0, h->stream>>>(h->L, wsp<T>(h, h->off.pi), f, wsp<double>(h, h->off.partials),
+                                                             wsp<Ctl>(h, h->off.ctl), wsp<double2>(h, h->off.fid));
+  CUDA_TRY(cudaGetLastError());
+  h->launches++;
+  return LPC_OK;
+}
+
+template <typename T>
+int set_site_params_t(lpc_lattice* h, const double* dF, const uint8_t* blocked, const double* omega, const void* g0) {
+  const Layout& L = h->L;
+  Ctl* ctl = wsp<Ctl>(h, h->off.ctl);
+  CUDA_TRY(cudaMemsetAsync(h->ws, 0, h->off.staging, h->stream));  // ghosts, series, control block, state: all zero
+  double* e = wsp<double>(h, h->off.f1);                            // dense scratch for exp(-dF), aliases the back buffer
+  int rc;
+  // pass 1: Boltzmann factors.  dF and blocked travel through the staging buffer together.
+  const bool dev_in = is_device_ptr(dF) && is_device_ptr(blocked);
+  if (dev_in) {
+    boltzmann_factor_kernel<<<aux_grid(h->N), 256, 0, h->stream>>>(dF, blocked, 0, h->N, e, ctl);
+    CUDA_TRY(cudaGetLastError());
+    h->launches++;
+  } else {
+    const long long chunk = std::min<long long>(h->N, STAGE_SITES);
+    unsigned char* stg = h->ws + h->off.staging;
+    for (long long i0 = 0; i0 < h->N; i0 += chunk) {
+      const long long n = std::min(chunk, h->N - i0);
+      CUDA_TRY(cudaMemcpyAsync(stg, dF + i0, (size_t)n * 8, cudaMemcpyDefault, h->stream));
+      CUDA_TRY(cudaMemcpyAsync(stg + (size_t)chunk * 8, blocked + i0, (size_t)n, cudaMemcpyDefault, h->stream));
+      boltzmann_factor_kernel<<<aux_grid(n), 256, 0, h->stream>>>(reinterpret_cast<const double*>(stg), stg + (size_t)chunk * 8, i0, n, e,
+                                                                   ctl);
+      CUDA_TRY(cudaGetLastError());
+      h->launches++;
+      CUDA_TRY(cudaStreamSynchronize(h->stream));
+    }
+  }
+  sum_kernel<<<aux_grid(h->N), 256, 0, h->stream>>>(e, h->N, wsp<double>(h, h->off.partials), ctl);
+  CUDA_TRY(cudaGetLastError());
+  h->launches++;
+  Ctl hc;
+  CUDA_TRY(cudaMemcpyAsync(&hc, ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  if (hc.bad != 0) return fail(LPC_EINVAL, "exp(-dF) under- or overflows on %llu open sites: the spread of dF is too wide", hc.bad);
+  if (!(hc.zsum > 0.0) || !std::isfinite(hc.zsum)) return fail(LPC_EINVAL, "every site is blocked (sum of Boltzmann factors = %g)", hc.zsum);
+
+  // pass 2: pi, kappa, phase factors
+  rc = for_chunks_in(h, omega, 8, [&](const void* d, long long i0, long long n) {
+    site_params_kernel<T><<<aux_grid(n), 256, 0, h->stream>>>(e, static_cast<const double*>(d), i0, n, L, h->cfg.alpha / 6.0, h->cfg.dt,
+                                                               ctl, wsp<T>(h, h->off.pi), wsp<T>(h, h->off.kcs));
+    CUDA_TRY(cudaGetLastError());
+    h->launches++;
+    return LPC_OK;
+  });
+  if (rc) return rc;
+  {
+    const long long cells = 2ll * ((long long)L.nx * L.ny + (long long)L.nx * L.nz + (long long)L.ny * L.nz);
+    fill_ghosts_kernel<T><<<aux_grid(cells), 256, 0, h->stream>>>(wsp<T>(h, h->off.pi), 1, L, h->cfg.bc[0] == 0, h->cfg.bc[1] == 0,
+                                                                   h->cfg.bc[2] == 0);
+    CUDA_TRY(cudaGetLastError());
+    h->launches++;
+  }
+  // the scratch aliased the back buffer: clear it again so that its ghosts and carbon sites are 0
+  CUDA_TRY(cudaMemsetAsync(h->ws + h->off.f1, 0, (size_t)h->C * L.np * h->sT, h->stream));
+
+  // initial state
+  h->cur = 0;
+  T* f = wsp<T>(h, h->off.f0);
+  auto init = [&](auto kern) {
+    kern<<<aux_grid(h->N), 256, 0, h->stream>>>(L, wsp<T>(h, h->off.pi), wsp<T>(h, h->off.kcs), f, h->cfg.a, wsp<double>(h, h->off.partials),
+                                                 ctl, wsp<double2>(h, h->off.fid), wsp<double>(h, h->off.vacf), h->cfg.max_steps + 2,
+                                                 h->cfg.a * h->cfg.a * h->cfg.alpha / 6.0);
+  };
+  if (h->nrho == 0 && h->nmom == 0) init(init_state_kernel<T, 0, 0>);
+  else if (h->nrho == 1 && h->nmom == 0) init(init_state_kernel<T, 1, 0>);
+  else if (h->nrho == 0 && h->nmom == 3) init(init_state_kernel<T, 0, 3>);
+  else init(init_state_kernel<T, 1, 3>);
+  CUDA_TRY(cudaGetLastError());
+  h->launches++;
+  if (g0) {
+    rc = set_g_from<T>(h, g0);
+    if (rc) return rc;
+  }
+  rc = fill_state_ghosts<T>(h);
+  if (rc) return rc;
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  h->steps = 0;
+  h->have_params = true;
+  return LPC_OK;
+}
+
+template <typename T>
+int read_field_t(lpc_lattice* h, int which, void* out) {
+  const Layout& L = h->L;
+  const T* f = wsp<T>(h, h->cur ? h->off.f1 : h->off.f0);
+  int mode;
+  const T* ch;
+  size_t bps = 8;
+  if (which == LPC_FIELD_G) { mode = 0; ch = f; bps = 16; }
+  else if (which == LPC_FIELD_PI) { mode = 1; ch = f; }
+  else if (which >= LPC_FIELD_PX && which <= LPC_FIELD_PZ) {
+    if (h->nmom != 3) return fail(LPC_ESTATE, "moment fields are not propagated (n_moments = 0)");
+    mode = 2; ch = f + (long long)(2 + h->nrho + (which - LPC_FIELD_PX)) * L.np;
+  } else if (which == LPC_FIELD_RHO) {
+    if (h->nrho != 1) return fail(LPC_ESTATE, "the density field is not propagated (n_density = 0)");
+    mode = 2; ch = f + 2 * L.np;
+  } else return fail(LPC_EINVAL, "unknown field %d", which);
+  const T* pi = wsp<T>(h, h->off.pi);
+  if (is_device_ptr(out)) {
+    gather_field_kernel<T><<<aux_grid(h->N), 256, 0, h->stream>>>(mode, 0, h->N, L, pi, ch, static_cast<double*>(out));
+    CUDA_TRY(cudaGetLastError());
+    h->launches++;
+  } else {
+    const long long chunk = std::min<long long>(h->N, STAGE_SITES);
+    double* stg = wsp<double>(h, h->off.staging);
+    for (long long i0 = 0; i0 < h->N; i0 += chunk) {
+      const long long n = std::min(chunk, h->N - i0);
+      gather_field_kernel<T><<<aux_grid(n), 256, 0, h->stream>>>(mode, i0, n, L, pi, ch, stg);
+      CUDA_TRY(cudaGetLastError());
+      h->launches++;
+      CUDA_TRY(cudaMemcpyAsync(static_cast<unsigned char*>(out) + (size_t)i0 * bps, stg, (size_t)n * bps, cudaMemcpyDeviceToHost, h->stream));
+      CUDA_TRY(cudaStreamSynchronize(h->stream));
+    }
+  }
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return LPC_OK;
+}
+
+template <typename T>
+int set_state_t(lpc_lattice* h, int which, const void* in) {
+  int rc;
+  if (which == LPC_FIELD_G) {
+    rc = set_g_from<T>(h, in);
+    if (rc) return rc;
+    h->steps = 0;
+  } else if (which == LPC_FIELD_RHO) {
+    if (h->nrho != 1) return fail(LPC_ESTATE, "the density field is not propagated (n_density = 0)");
+    T* ch = wsp<T>(h, h->cur ? h->off.f1 : h->off.f0) + 2 * h->L.np;
+    rc = for_chunks_in(h, in, 8, [&](const void* d, long long i0, long long n) {
+      set_real_kernel<T><<<aux_grid(n), 256, 0, h->stream>>>(static_cast<const double*>(d), i0, n, h->L, wsp<T>(h, h->off.pi), ch);
+      CUDA_TRY(cudaGetLastError());
+      h->launches++;
+      return LPC_OK;
+    });
+    if (rc) return rc;
+  } else {
+    return fail(LPC_EINVAL, "field %d cannot be set", which);
+  }
+  rc = fill_state_ghosts<T>(h);
+  if (rc) return rc;
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return LPC_OK;
+}
+
+}  // namespace
+
+// ================================================================================================
+extern "C" {
+
+const char* lpc_last_error(void) { return g_err; }
+
+int lpc_workspace_bytes(const lpc_config* cfg, size_t* bytes) {
+  int rc = check_cfg(cfg);
+  if (rc) return rc;
+  if (!bytes) return fail(LPC_EINVAL, "bytes is NULL");
+  *bytes = make_offsets(cfg, make_layout(cfg)).total;
+  return LPC_OK;
+}
+
+int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes, lpc_lattice** out) {
+  int rc = check_cfg(cfg);
+  if (rc) return rc;
+  if (!out) return fail(LPC_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (!workspace_dev) return fail(LPC_EINVAL, "workspace is NULL");
+  int dev = 0, major = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  CUDA_TRY(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+  if (major != 10) return fail(LPC_ECUDA, "liblpc is built for sm_100a only; device %d has compute capability major %d", dev, major);
+  lpc_lattice* h = new (std::nothrow) lpc_lattice();
+  if (!h) return fail(LPC_ENOMEM, "host allocation failed");
+  h->cfg = *cfg;
+  h->L = make_layout(cfg);
+  h->off = make_offsets(cfg, h->L);
+  if (bytes < h->off.total) {
+    delete h;
+    return fail(LPC_ENOMEM, "workspace of %zu bytes is smaller than the %zu needed", bytes, make_offsets(cfg, make_layout(cfg)).total);
+  }
+  if (reinterpret_cast<uintptr_t>(workspace_dev) % ALIGN != 0) {
+    delete h;
+    return fail(LPC_ENOMEM, "workspace must be %zu-byte aligned", ALIGN);
+  }
+  if (!is_device_ptr(workspace_dev)) {
+    delete h;
+    return fail(LPC_EINVAL, "workspace is not device memory");
+  }
+  h->nrho = cfg->n_density;
+  h->nmom = cfg->n_moments;
+  h->C = 2 + h->nrho + h->nmom;
+  h->sT = cfg->precision ? 4 : 8;
+  h->N = (long long)cfg->nx * cfg->ny * cfg->nz;
+  h->ws = static_cast<unsigned char*>(workspace_dev);
+  h->stream = static_cast<cudaStream_t>(cfg->stream);
+  h->have_params = false;
+  h->cur = 0;
+  h->steps = 0;
+  h->launches = 0;
+  h->kernel = LPC_KERNEL_AUTO;
+  if (const char* e = getenv("LPC_KERNEL")) {
+    if (!strcmp(e, "direct")) h->kernel = LPC_KERNEL_DIRECT;
+    if (!strcmp(e, "tma")) h->kernel = LPC_KERNEL_TMA;
+  }
+  tma_geometry(h->C, cfg->nx, cfg->ny, cfg->nz, &h->ty, &h->tz, &h->nstage, &h->xc, &h->tiles_z, &h->tiles_y, &h->chunks_x);
+  h->tma_ok = (size_t)h->tiles_z * h->tiles_y * h->chunks_x <= h->off.partial_slots;
+  if (h->tma_ok) {
+    const Layout& L = h->L;
+    const bool f32 = cfg->precision == 1;
+    const cuuint64_t d4[4] = {(cuuint64_t)L.nzp, (cuuint64_t)L.nyp, (cuuint64_t)L.nxp, (cuuint64_t)h->C};
+    const cuuint32_t b4[4] = {(cuuint32_t)(h->tz + 2 * (16 / h->sT)), (cuuint32_t)(h->ty + 2), 1, (cuuint32_t)h->C};
+    const cuuint64_t dk[4] = {(cuuint64_t)L.nzp, (cuuint64_t)L.nyp, (cuuint64_t)L.nxp, 3};
+    const cuuint32_t bk[4] = {(cuuint32_t)h->tz, (cuuint32_t)h->ty, 1, 3};
+    rc = encode_map(&h->tm_f[0], f32, h->ws + h->off.f0, 4, d4, b4);
+    if (!rc) rc = encode_map(&h->tm_f[1], f32, h->ws + h->off.f1, 4, d4, b4);
+    if (!rc) rc = encode_map(&h->tm_pi, f32, h->ws + h->off.pi, 3, d4, b4);
+    if (!rc) rc = encode_map(&h->tm_kcs, f32, h->ws + h->off.kcs, 4, dk, bk);
+    if (rc) {
+      delete h;
+      return rc;
+    }
+  }
+  *out = h;
+  return LPC_OK;
+}
+
+int lpc_set_site_params(lpc_lattice* h, const double* dF, const uint8_t* blocked, const double* omega, const void* g0) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (!dF || !blocked || !omega) return fail(LPC_EINVAL, "dF, blocked and omega must not be NULL");
+  h->have_params = false;
+  return h->cfg.precision ? set_site_params_t<float>(h, dF, blocked, omega, g0) : set_site_params_t<double>(h, dF, blocked, omega, g0);
+}
+
+int lpc_step_n(lpc_lattice* h, int64_t n) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
+  if (n < 0) return fail(LPC_EINVAL, "n must be >= 0");
+  if (h->steps + n > h->cfg.max_steps) return fail(LPC_EINVAL, "steps_done + n = %lld exceeds max_steps = %lld", (long long)(h->steps + n), (long long)h->cfg.max_steps);
+  for (int64_t k = 0; k < n; ++k) {
+    int rc = h->cfg.precision ? launch_step<float>(h) : launch_step<double>(h);
+    if (rc) return rc;
+    h->steps++;
+  }
+  return LPC_OK;
+}
+
+int lpc_read_fid(lpc_lattice* h, int64_t first, int64_t count, double* out) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
+  if (first < 0 || count < 0 || first + count > h->steps + 1) return fail(LPC_EINVAL, "range [%lld, %lld) is outside the %lld samples of the series", (long long)first, (long long)(first + count), (long long)(h->steps + 1));
+  if (count > 0 && !out) return fail(LPC_EINVAL, "out is NULL");
+  if (count > 0)
+    CUDA_TRY(cudaMemcpyAsync(out, wsp<double2>(h, h->off.fid) + first, (size_t)count * sizeof(double2), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return LPC_OK;
+}
+
+int lpc_moments(lpc_lattice* h, int64_t count, double* vacf_host, double D[3]) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
+  if (h->nmom != 3) return fail(LPC_ESTATE, "moment fields are not propagated (n_moments = 0)");
+  if (count < 1 || count > h->steps + 1) return fail(LPC_EINVAL, "count must lie in [1, steps_done + 1]");
+  if (!D) return fail(LPC_EINVAL, "D is NULL");
+  const long long stride = h->cfg.max_steps + 2;
+  double* vacf = wsp<double>(h, h->off.vacf);
+  Ctl* ctl = wsp<Ctl>(h, h->off.ctl);
+  diffusion_kernel<<<3, 256, 0, h->stream>>>(vacf, stride, count, h->cfg.dt, ctl);
+  CUDA_TRY(cudaGetLastError());
+  h->launches++;
+  CUDA_TRY(cudaMemcpyAsync(D, ctl->scratch, 3 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  if (vacf_host)
+    for (int d = 0; d < 3; ++d)
+      CUDA_TRY(cudaMemcpyAsync(vacf_host + (size_t)d * count, vacf + d * stride + 1, (size_t)count * sizeof(double), cudaMemcpyDeviceToHost,
+                               h->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return LPC_OK;
+}
+
+int lpc_read_field(lpc_lattice* h, int32_t which, void* out) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
+  if (!out) return fail(LPC_EINVAL, "out is NULL");
+  return h->cfg.precision ? read_field_t<float>(h, which, out) : read_field_t<double>(h, which, out);
+}
+
+int lpc_set_state(lpc_lattice* h, int32_t which, const void* in) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
+  if (!in) return fail(LPC_EINVAL, "in is NULL");
+  return h->cfg.precision ? set_state_t<float>(h, which, in) : set_state_t<double>(h, which, in);
+}
+
+int lpc_set_kernel(lpc_lattice* h, int32_t which) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (which < LPC_KERNEL_AUTO || which > LPC_KERNEL_TMA) return fail(LPC_EINVAL, "unknown kernel selector %d", which);
+  if (which == LPC_KERNEL_TMA && !h->tma_ok) return fail(LPC_EINVAL, "the TMA kernel is not available for this lattice");
+  h->kernel = which;
+  return LPC_OK;
+}
+
+int64_t lpc_steps_done(const lpc_lattice* h) { return h ? h->steps : 0; }
+int64_t lpc_launch_count(const lpc_lattice* h) { return h ? h->launches : 0; }
+
+double lpc_bytes_per_site_step(const lpc_lattice* h) {
+  if (!h) return 0.0;
+  // read C state channels + pi + kappa + cos + sin, write C state channels
+  return (double)h->sT * (2.0 * h->C + 4.0);
+}
+
+void lpc_destroy(lpc_lattice* h) { delete h; }
+
+}  // extern "C"

@@ -1,0 +1,328 @@
+"""Parity of the CUDA library (through the C ABI) against the CPU oracle, on a B200.
+
+Tolerances, fp64:
+  per site   |g_gpu - g_orc|_i  <= 1e-10 * pi_i            (|g_i(n)| <= pi_i for all n)
+  FID        |G_gpu - G_orc|[n] <= 1e-9 * sum_i |g_i(n)|   (the sum's own scale, <= G[0] = 1)
+  moments    |P_gpu - P_orc|_i  <= 1e-10 * a * pi_i,  |Z_gpu - Z_orc|[m] <= 1e-9 * Z[1],
+             |D_gpu - D_orc|    <= 1e-9 * Z[1] / (2 dt)
+fp32 mode: the same with 1e-5, checked at n <= 200.
+"""
+import importlib.util
+import os
+
+import numpy as np
+import pytest
+
+import lpc_inputs
+
+pytestmark = pytest.mark.gpu
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+FULL = os.environ.get("LPC_FULL", "0") == "1"
+
+
+@pytest.fixture(scope="module")
+def lpc():
+    import torch
+
+    assert torch.cuda.is_available(), "these tests need the B200"
+    spec = importlib.util.spec_from_file_location("_lpc_build", os.path.join(ROOT, "paper_2603_22553_b200", "build.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    mod.build()
+    import paper_2603_22553_b200 as m
+
+    return m
+
+
+def _check(lpc, lat, gpu, orc, n, tol_site=1e-10, tol_sum=1e-9, what=""):
+    pi = orc.pi()
+    G_o, sabs = orc.fid(with_scale=True)
+    G_g = gpu.fid()
+    assert G_g.shape == G_o.shape == (n + 1,)
+    err_G = np.abs(G_g - G_o) / sabs
+    assert err_G.max() <= tol_sum, f"{what} FID: max scaled error {err_G.max():.3e} at n={err_G.argmax()}"
+    g_o, g_g = orc.g(), gpu.field(lpc.LPC_FIELD_G)
+    opn = lat.blocked == 0
+    assert np.all(g_g[~opn] == 0)
+    err_g = np.abs(g_g - g_o)[opn] / pi[opn]
+    assert err_g.max() <= tol_site, f"{what} g: max scaled per-site error {err_g.max():.3e}"
+    out = {"err_G": float(err_G.max()), "err_g": float(err_g.max())}
+    if gpu.cfg.n_moments == 3:
+        v_o, D_o = orc.moments()
+        v_g, D_g = gpu.moments()
+        z1 = np.abs(v_o[:, :1])
+        err_Z = np.abs(v_g - v_o) / z1
+        assert err_Z.max() <= tol_sum, f"{what} VACF: max scaled error {err_Z.max():.3e}"
+        err_D = np.abs(D_g - D_o) / (z1[:, 0] / (2 * lat.dt))
+        assert err_D.max() <= tol_sum, f"{what} D: scaled error {err_D.max():.3e}"
+        for d in range(3):
+            P_o, P_g = orc.P(d), gpu.field(lpc.LPC_FIELD_PX + d)
+            err_P = np.abs(P_g - P_o)[opn] / (lat.a * pi[opn])
+            assert err_P.max() <= tol_site, f"{what} P^{d}: max scaled per-site error {err_P.max():.3e}"
+        out.update(err_Z=float(err_Z.max()), err_D=float(err_D.max()))
+    return out
+
+
+def _pair(lpc, oracle_mod, lat, n, kernel, n_moments=None, n_density=0, precision=0, g0=None):
+    nm = lat.n_moments if n_moments is None else n_moments
+    gpu = lpc.Lattice.from_inputs(lat, precision=precision, n_moments=nm, n_density=n_density, max_steps=n, g0=g0)
+    gpu.set_kernel(kernel)
+    orc = oracle_mod.Oracle.from_lattice(lat, n_moments=nm, max_steps=n)
+    if g0 is not None:
+        orc.set_g(g0)
+    return gpu, orc
+
+
+KERNELS = [1, 2]  # LPC_KERNEL_DIRECT, LPC_KERNEL_TMA
+
+
+# ---------------------------------------------------------------------------------------------
+# precompute (S0) against oracle O1-O4, O7
+# ---------------------------------------------------------------------------------------------
+def test_precompute_matches_oracle(lpc, oracle_mod):
+    lat = lpc_inputs.random_small((20, 13, 37), bc=(1, 0, 0), p_block=0.3, alpha=0.8, seed=21, n_moments=3)
+    gpu, orc = _pair(lpc, oracle_mod, lat, 0, 1)
+    pi_o, pi_g = orc.pi(), gpu.field(lpc.LPC_FIELD_PI)
+    opn = lat.blocked == 0
+    assert np.all(pi_g[~opn] == 0)
+    assert np.max(np.abs(pi_g - pi_o)[opn] / pi_o[opn]) < 5e-15
+    assert abs(gpu.fid()[0] - 1.0) < 1e-14
+    g = gpu.field(lpc.LPC_FIELD_G)
+    assert np.max(np.abs(g - pi_o)[opn] / pi_o[opn]) < 5e-15
+    v_o, _ = orc.moments(1)
+    v_g, _ = gpu.moments(1)
+    assert np.max(np.abs(v_g - v_o) / v_o) < 1e-13
+    for d in range(3):
+        P_o, P_g = orc.P(d), gpu.field(lpc.LPC_FIELD_PX + d)
+        assert np.max(np.abs(P_g - P_o)[opn] / (lat.a * pi_o[opn])) < 1e-14
+
+
+# ---------------------------------------------------------------------------------------------
+# BASELINE configs[0]: 32^3, 2000 steps, G(t) and density
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_config0_full(lpc, oracle_mod, kernel):
+    lat = lpc_inputs.config0()
+    n = lat.n_steps
+    gpu, orc = _pair(lpc, oracle_mod, lat, n, kernel, n_density=1)
+    gpu.step(n)
+    orc.step(n)
+    _check(lpc, lat, gpu, orc, n, what=f"config0 kernel={kernel}")
+    # "output G(t) and density": the density started at pi stays at pi (stationarity)
+    rho = gpu.field(lpc.LPC_FIELD_RHO)
+    pi = orc.pi()
+    opn = lat.blocked == 0
+    assert np.max(np.abs(rho - pi)[opn] / pi[opn]) <= 1e-10
+
+
+# ---------------------------------------------------------------------------------------------
+# several tiles + ragged tails, mixed boundary conditions, moments fused in
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("shape,bc,alpha", [
+    ((70, 19, 133), (1, 0, 0), 0.8),    # ragged in y and z, 3 z-tiles, 3 y-tiles, 2+ x-chunks, reflective x
+    ((33, 40, 64), (0, 1, 1), 1.0),     # exact z tile, reflective y and z
+    ((9, 8, 200), (0, 0, 0), 0.5),      # short x, 4 z-tiles
+    ((5, 3, 7), (0, 0, 0), 1.0),        # odd nz, smaller than one tile
+    ((2, 1, 3), (0, 0, 0), 0.9),        # degenerate axes (Q17)
+    ((1, 1, 1), (0, 0, 0), 1.0),        # a single site
+    ((4, 4, 4), (1, 1, 1), 1.0),        # closed box
+])
+def test_shapes_and_boundaries(lpc, oracle_mod, kernel, shape, bc, alpha):
+    lat = lpc_inputs.random_small(shape, bc=bc, p_block=0.3 if np.prod(shape) > 8 else 0.0, alpha=alpha, seed=22, n_moments=3)
+    lat.dt = 2.0e-5
+    n = 60
+    gpu, orc = _pair(lpc, oracle_mod, lat, n, kernel, n_density=1)
+    gpu.step(n)
+    orc.step(n)
+    _check(lpc, lat, gpu, orc, n, what=f"{shape} {bc} kernel={kernel}")
+    rho, pi = gpu.field(lpc.LPC_FIELD_RHO), orc.pi()
+    opn = lat.blocked == 0
+    assert np.max(np.abs(rho - pi)[opn] / pi[opn]) <= 1e-10
+
+
+@pytest.mark.parametrize("nm,nd", [(0, 0), (0, 1), (3, 0), (3, 1)])
+def test_channel_combinations_tma(lpc, oracle_mod, nm, nd):
+    lat = lpc_inputs.random_small((40, 24, 96), bc=(0, 0, 1), p_block=0.2, alpha=0.9, seed=23)
+    n = 40
+    gpu, orc = _pair(lpc, oracle_mod, lat, n, 2, n_moments=nm, n_density=nd)
+    gpu.step(17)
+    gpu.step(n - 17)     # series append across calls
+    orc.step(n)
+    _check(lpc, lat, gpu, orc, n, what=f"nm={nm} nd={nd}")
+
+
+def test_kernels_agree_bitwise_on_state_and_are_deterministic(lpc):
+    lat = lpc_inputs.random_small((48, 20, 130), bc=(1, 0, 0), p_block=0.25, seed=24, n_moments=3)
+    res = []
+    for kernel in (1, 2, 2):
+        gpu = lpc.Lattice.from_inputs(lat, max_steps=30)
+        gpu.set_kernel(kernel)
+        gpu.step(30)
+        res.append((gpu.field(lpc.LPC_FIELD_G), gpu.fid(), gpu.moments()[0]))
+    # same per-site arithmetic in both kernels: the fields agree bit for bit; the sums differ only by order
+    assert np.array_equal(res[0][0], res[1][0])
+    assert np.max(np.abs(res[0][1] - res[1][1])) < 1e-14
+    # repeated runs of one kernel are bitwise reproducible (fixed-order reduction, no atomics on data)
+    assert np.array_equal(res[1][0], res[2][0])
+    assert np.array_equal(res[1][1], res[2][1])
+    assert np.array_equal(res[1][2], res[2][2])
+
+
+# ---------------------------------------------------------------------------------------------
+# states set from outside, device-resident inputs
+# ---------------------------------------------------------------------------------------------
+def test_arbitrary_initial_magnetisation_and_relaxation(lpc, oracle_mod):
+    lat = lpc_inputs.random_small((16, 12, 34), bc=(0, 0, 0), p_block=0.2, alpha=0.7, seed=25)
+    rng = np.random.default_rng(3)
+    g0 = (rng.standard_normal(lat.shape) + 1j * rng.standard_normal(lat.shape))
+    n = 50
+    gpu, orc = _pair(lpc, oracle_mod, lat, n, 2, n_density=1, g0=g0)
+    pi = orc.pi()
+    G0 = gpu.fid()[0]
+    assert abs(G0 - g0[lat.blocked == 0].sum()) < 1e-12 * np.abs(g0).sum()
+    gpu.step(n)
+    orc.step(n)
+    G_o, G_g = orc.fid(), gpu.fid()
+    scale = np.abs(g0[lat.blocked == 0]).sum()
+    assert np.max(np.abs(G_g - G_o)) <= 1e-9 * scale
+    g_o, g_g = orc.g(), gpu.field(lpc.LPC_FIELD_G)
+    assert np.max(np.abs(g_g - g_o)) <= 1e-10 * np.abs(g0).max()
+    # relaxation of an arbitrary density towards exp(-dF) through lpc_set_state
+    rho0 = rng.random(lat.shape) * (lat.blocked == 0)
+    gpu2 = lpc.Lattice.from_inputs(lat, n_density=1, max_steps=400)
+    gpu2.set_state(lpc.LPC_FIELD_RHO, rho0)
+    gpu2.step(400)
+    want = orc.propagate_real(rho0, 400)
+    got = gpu2.field(lpc.LPC_FIELD_RHO)
+    assert np.max(np.abs(got - want)) <= 1e-10 * rho0.max()
+    assert abs(got.sum() - rho0.sum()) <= 1e-12 * rho0.sum()   # conservation of total density
+    assert np.abs(got / got.sum() - pi).max() < np.abs(rho0 / rho0.sum() - pi).max() * 0.5
+
+
+def test_device_resident_inputs_give_the_same_result(lpc):
+    import torch
+
+    lat = lpc_inputs.random_small((24, 16, 70), p_block=0.3, seed=26)
+    a = lpc.Lattice.from_inputs(lat, max_steps=10)
+    b = lpc.Lattice(lat.shape, bc=lat.bc, dt=lat.dt, a=lat.a, alpha=lat.alpha, max_steps=10)
+    dev = [torch.from_numpy(x).cuda() for x in (lat.dF, lat.blocked, lat.omega)]
+    b.set_site_params(*dev)
+    a.step(10)
+    b.step(10)
+    assert np.array_equal(a.fid(), b.fid())
+    out = torch.empty(lat.shape, dtype=torch.complex128, device="cuda")
+    lpc.lpc_read_field(b.handle, lpc.LPC_FIELD_G, out)
+    assert np.array_equal(out.cpu().numpy(), a.field(lpc.LPC_FIELD_G))
+
+
+# ---------------------------------------------------------------------------------------------
+# fp32 mode
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_fp32_mode(lpc, oracle_mod, kernel):
+    lat = lpc_inputs.random_small((40, 24, 100), bc=(1, 0, 0), p_block=0.2, alpha=0.9, seed=27, n_moments=3)
+    n = 200
+    gpu, orc = _pair(lpc, oracle_mod, lat, n, kernel, precision=1)
+    gpu.step(n)
+    orc.step(n)
+    _check(lpc, lat, gpu, orc, n, tol_site=1e-5, tol_sum=1e-5, what=f"fp32 kernel={kernel}")
+
+
+# ---------------------------------------------------------------------------------------------
+# BASELINE configs[1..3] at test sizes (and full length with LPC_FULL=1)
+# ---------------------------------------------------------------------------------------------
+def test_config1_particle(lpc, oracle_mod):
+    n = 20000 if FULL else 300
+    lat = lpc_inputs.particle(n_steps=n)
+    gpu, orc = _pair(lpc, oracle_mod, lat, n, 0)
+    gpu.step(n)
+    orc.step(n)
+    print(_check(lpc, lat, gpu, orc, n, what="config1"))
+
+
+def test_config2_monolith_scaled(lpc, oracle_mod):
+    L, n = (256, 200) if FULL else (96, 200)
+    lat = lpc_inputs.monolith(L=L, n_steps=n)
+    gpu, orc = _pair(lpc, oracle_mod, lat, n, 0)
+    gpu.step(n)
+    orc.step(n)
+    print(_check(lpc, lat, gpu, orc, n, what="config2"))
+
+
+def test_config3_supercap_scaled(lpc, oracle_mod):
+    shape, n = ((2048, 256, 256), 20) if FULL else ((256, 32, 64), 200)
+    lat = lpc_inputs.supercap(*shape, n_steps=n)
+    gpu, orc = _pair(lpc, oracle_mod, lat, n, 0)
+    gpu.step(n)
+    orc.step(n)
+    print(_check(lpc, lat, gpu, orc, n, what="config3"))
+    # reflective x: nothing leaks through the walls -- total magnetisation magnitude is bounded by 1
+    assert np.abs(gpu.fid()).max() <= 1 + 1e-12
+
+
+# ---------------------------------------------------------------------------------------------
+# properties that hold at any size, on the bench configuration (512^3 NMR kernel)
+# ---------------------------------------------------------------------------------------------
+def test_bench_size_properties(lpc):
+    import torch
+
+    L = 512
+    n_sites = L ** 3
+    # uniform shift on a heterogeneous lattice: G[n] = exp(i omega n dt) exactly (Eq. 8)
+    rng = np.random.default_rng(5)
+    dF = -3.0 * rng.random((L, L, L))
+    blocked = (rng.random((L, L, L)) < 0.2).astype(np.uint8)
+    omega = np.full((L, L, L), -12000.0)
+    gpu = lpc.Lattice((L, L, L), dt=5e-6, max_steps=20)
+    gpu.set_site_params(dF, blocked, omega)
+    gpu.step(20)
+    G = gpu.fid()
+    k = np.arange(21)
+    assert np.max(np.abs(G - np.exp(1j * -12000.0 * 5e-6 * k))) < 1e-12
+    # the reduction agrees with an independent fp64 sum of the field read back
+    g = gpu.field(lpc.LPC_FIELD_G)
+    assert abs(g.sum() - G[-1]) < 1e-12
+    del gpu, g
+    torch.cuda.empty_cache()
+
+
+# ---------------------------------------------------------------------------------------------
+# error behaviour through the ABI
+# ---------------------------------------------------------------------------------------------
+def test_error_codes(lpc):
+    import torch
+
+    lat = lpc_inputs.random_small((8, 8, 8), seed=28)
+    cfg = lpc.make_config(8, 8, 8, max_steps=3)
+    ws = torch.empty(lpc.lpc_workspace_bytes(cfg), dtype=torch.uint8, device="cuda")
+    with pytest.raises(lpc.LpcError) as e:
+        lpc.lpc_create_lattice(cfg, ws[: ws.numel() // 2])
+    assert e.value.code == lpc.LPC_ENOMEM
+    h = lpc.lpc_create_lattice(cfg, ws)
+    with pytest.raises(lpc.LpcError) as e:
+        lpc.lpc_step_n(h, 1)
+    assert e.value.code == lpc.LPC_ESTATE
+    with pytest.raises(lpc.LpcError) as e:
+        lpc.lpc_set_site_params(h, lat.dF, np.ones_like(lat.blocked), lat.omega)
+    assert e.value.code == lpc.LPC_EINVAL and "blocked" in str(e.value)
+    wide = lat.dF.copy()
+    wide[0, 0, 0] = 2000.0
+    with pytest.raises(lpc.LpcError) as e:
+        lpc.lpc_set_site_params(h, wide, np.zeros_like(lat.blocked), lat.omega)
+    assert e.value.code == lpc.LPC_EINVAL
+    lpc.lpc_set_site_params(h, lat.dF, lat.blocked, lat.omega)
+    lpc.lpc_step_n(h, 3)
+    with pytest.raises(lpc.LpcError) as e:
+        lpc.lpc_step_n(h, 1)
+    assert e.value.code == lpc.LPC_EINVAL
+    with pytest.raises(lpc.LpcError) as e:
+        lpc.lpc_read_fid(h, 2, 5)
+    assert e.value.code == lpc.LPC_EINVAL
+    with pytest.raises(lpc.LpcError) as e:
+        lpc.lpc_moments(h, 1)
+    assert e.value.code == lpc.LPC_ESTATE
+    assert lpc.lpc_read_fid(h).shape == (4,)
+    assert lpc.lpc_steps_done(h) == 3 and lpc.lpc_launch_count(h) > 3
+    lpc.lpc_destroy(h)
