@@ -71,7 +71,7 @@ def workload_name(L, moments, precision):
 # --------------------------------------------------------------------------------------------
 # CPU oracle timing (cpu_baseline leg and --impl reference)
 # --------------------------------------------------------------------------------------------
-def oracle_sample(moments, steps=None, warmup=1, budget_s=12.0, L=160):
+def oracle_sample(moments, steps=None, warmup=1, budget_s=12.0, L=256):
     """Time the oracle on a bounded sample of the workload: an L^3 lattice with the same statistics."""
     orc_mod = load_oracle()
     lat = lpc_inputs.sweep(L, n_moments=moments)
@@ -82,7 +82,7 @@ def oracle_sample(moments, steps=None, warmup=1, budget_s=12.0, L=160):
         t0 = time.perf_counter()
         o.step(1)
         one = time.perf_counter() - t0
-        steps = max(2, min(200, int(budget_s / max(one, 1e-6))))
+        steps = max(2, min(2000, int(budget_s / max(one, 1e-6))))
     t0 = time.perf_counter()
     o.step(steps)
     dt = time.perf_counter() - t0
