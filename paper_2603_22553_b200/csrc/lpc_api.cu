@@ -1,7 +1,7 @@
 // lpc_api.cu -- host side of liblpc.so: the C ABI of include/lpc.h.
 //
 // Workspace layout (device, all offsets 256-byte aligned):
-//   Ctl | fid[max_steps+1] | vacf[3][max_steps+2] | partials | pi | kcs[3] | F0[C] | F1[C] | staging
+//   Ctl | fid[max_steps+1] | vacf[3][max_steps+2] | partials | pi | cs[2] | F0[C] | F1[C] | staging
 // F0/F1 are the ping-pong state buffers in density-normalised, channel-planar (SoA) form.
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -47,7 +47,7 @@ constexpr int AUX_BLOCKS = 148 * 8;
 constexpr long long STAGE_SITES = 4ll << 20;  // sites per host<->device staging chunk
 
 struct Offsets {
-  size_t ctl, fid, vacf, partials, pi, kcs, f0, f1, staging, total;
+  size_t ctl, fid, vacf, partials, pi, cs, f0, f1, staging, total;
   size_t partial_slots;
 };
 
@@ -69,7 +69,7 @@ struct lpc_lattice {
   // TMA geometry
   int ty, tz, nstage, xc, tiles_z, tiles_y, chunks_x;
   bool tma_ok;
-  CUtensorMap tm_f[2], tm_pi, tm_kcs;
+  CUtensorMap tm_f[2], tm_pi, tm_cs;
 };
 
 namespace {
@@ -116,6 +116,9 @@ void tma_geometry(int C, int nx, int ny, int nz, int* ty, int* tz, int* nstage, 
   long long chunks = (12 * resident + tiles - 1) / tiles;     // aim for ~12 waves of CTAs ...
   chunks = std::min<long long>(chunks, std::max(1, nx / 32)); // ... but at least 32 planes per chunk
   chunks = std::max<long long>(chunks, 1);
+  // Small lattices (L2-resident, latency-bound): the march costs about 1 us per plane, so fill one
+  // wave of CTAs first and accept the two extra plane loads per chunk (measured: 64^3 35 -> 10 us/step).
+  if (tiles * chunks < resident) chunks = std::min<long long>((resident + tiles - 1) / tiles, std::max(1, nx / 2));
   if (const char* e = getenv("LPC_XC")) {
     const int v = atoi(e);
     if (v > 0) chunks = (nx + v - 1) / v;
@@ -140,7 +143,7 @@ Offsets make_offsets(const lpc_config* c, const Layout& L) {
   o.vacf = p; p += align_up((size_t)3 * (c->max_steps + 2) * sizeof(double));
   o.partials = p; p += align_up(o.partial_slots * MAX_RED * sizeof(double));
   o.pi = p; p += align_up((size_t)L.np * sT);
-  o.kcs = p; p += align_up((size_t)3 * L.np * sT);
+  o.cs = p; p += align_up((size_t)2 * L.np * sT);
   o.f0 = p; p += align_up((size_t)C * L.np * sT);
   o.f1 = p; p += align_up((size_t)C * L.np * sT);
   o.staging = p; p += align_up((size_t)std::min<long long>(N, STAGE_SITES) * 16);
@@ -205,7 +208,8 @@ int launch_step_t(lpc_lattice* h) {
   a.fin = wsp<T>(h, h->cur ? h->off.f1 : h->off.f0);
   a.fout = wsp<T>(h, h->cur ? h->off.f0 : h->off.f1);
   a.pi = wsp<T>(h, h->off.pi);
-  a.kcs = wsp<T>(h, h->off.kcs);
+  a.cs = wsp<T>(h, h->off.cs);
+  a.a6 = (T)(h->cfg.alpha / 6.0);
   a.partials = wsp<double>(h, h->off.partials);
   a.ctl = wsp<Ctl>(h, h->off.ctl);
   a.fid = wsp<double2>(h, h->off.fid);
@@ -227,7 +231,7 @@ int launch_step_t(lpc_lattice* h) {
       attr_set = true;
     }
     const unsigned grid = (unsigned)(h->tiles_z * h->tiles_y * h->chunks_x);
-    kern<<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(h->tm_f[h->cur], h->tm_pi, h->tm_kcs, a);
+    kern<<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(h->tm_f[h->cur], h->tm_pi, h->tm_cs, a);
   } else {
     const long long npairs = (long long)((h->L.nz + 1) / 2) * h->L.ny * h->L.nx;
     const int grid = (int)std::max<long long>(1, std::min<long long>((npairs + 255) / 256, DIRECT_MAX_BLOCKS));
@@ -331,8 +335,8 @@ int set_site_params_t(lpc_lattice* h, const double* dF, const uint8_t* blocked, 
 
   // pass 2: pi, kappa, phase factors
   rc = for_chunks_in(h, omega, 8, [&](const void* d, long long i0, long long n) {
-    site_params_kernel<T><<<aux_grid(n), 256, 0, h->stream>>>(e, static_cast<const double*>(d), i0, n, L, h->cfg.alpha / 6.0, h->cfg.dt,
-                                                               ctl, wsp<T>(h, h->off.pi), wsp<T>(h, h->off.kcs));
+    site_params_kernel<T><<<aux_grid(n), 256, 0, h->stream>>>(e, static_cast<const double*>(d), i0, n, L, h->cfg.dt, ctl,
+                                                               wsp<T>(h, h->off.pi), wsp<T>(h, h->off.cs));
     CUDA_TRY(cudaGetLastError());
     h->launches++;
     return LPC_OK;
@@ -352,7 +356,7 @@ int set_site_params_t(lpc_lattice* h, const double* dF, const uint8_t* blocked, 
   h->cur = 0;
   T* f = wsp<T>(h, h->off.f0);
   auto init = [&](auto kern) {
-    kern<<<aux_grid(h->N), 256, 0, h->stream>>>(L, wsp<T>(h, h->off.pi), wsp<T>(h, h->off.kcs), f, h->cfg.a, wsp<double>(h, h->off.partials),
+    kern<<<aux_grid(h->N), 256, 0, h->stream>>>(L, wsp<T>(h, h->off.pi), (T)(h->cfg.alpha / 6.0), f, h->cfg.a, wsp<double>(h, h->off.partials),
                                                  ctl, wsp<double2>(h, h->off.fid), wsp<double>(h, h->off.vacf), h->cfg.max_steps + 2,
                                                  h->cfg.a * h->cfg.a * h->cfg.alpha / 6.0);
   };
@@ -502,12 +506,12 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
     const bool f32 = cfg->precision == 1;
     const cuuint64_t d4[4] = {(cuuint64_t)L.nzp, (cuuint64_t)L.nyp, (cuuint64_t)L.nxp, (cuuint64_t)h->C};
     const cuuint32_t b4[4] = {(cuuint32_t)(h->tz + 2 * (16 / h->sT)), (cuuint32_t)(h->ty + 2), 1, (cuuint32_t)h->C};
-    const cuuint64_t dk[4] = {(cuuint64_t)L.nzp, (cuuint64_t)L.nyp, (cuuint64_t)L.nxp, 3};
-    const cuuint32_t bk[4] = {(cuuint32_t)h->tz, (cuuint32_t)h->ty, 1, 3};
+    const cuuint64_t dk[4] = {(cuuint64_t)L.nzp, (cuuint64_t)L.nyp, (cuuint64_t)L.nxp, 2};
+    const cuuint32_t bk[4] = {(cuuint32_t)h->tz, (cuuint32_t)h->ty, 1, 2};
     rc = encode_map(&h->tm_f[0], f32, h->ws + h->off.f0, 4, d4, b4);
     if (!rc) rc = encode_map(&h->tm_f[1], f32, h->ws + h->off.f1, 4, d4, b4);
     if (!rc) rc = encode_map(&h->tm_pi, f32, h->ws + h->off.pi, 3, d4, b4);
-    if (!rc) rc = encode_map(&h->tm_kcs, f32, h->ws + h->off.kcs, 4, dk, bk);
+    if (!rc) rc = encode_map(&h->tm_cs, f32, h->ws + h->off.cs, 4, dk, bk);
     if (rc) {
       delete h;
       return rc;
@@ -596,8 +600,8 @@ int64_t lpc_launch_count(const lpc_lattice* h) { return h ? h->launches : 0; }
 
 double lpc_bytes_per_site_step(const lpc_lattice* h) {
   if (!h) return 0.0;
-  // read C state channels + pi + kappa + cos + sin, write C state channels
-  return (double)h->sT * (2.0 * h->C + 4.0);
+  // read C state channels + pi + cos + sin, write C state channels
+  return (double)h->sT * (2.0 * h->C + 3.0);
 }
 
 void lpc_destroy(lpc_lattice* h) { delete h; }

@@ -64,25 +64,21 @@ __global__ void __launch_bounds__(256) sum_kernel(const double* __restrict__ e, 
   }
 }
 
-// pi_i = e_i / Z, kappa_i = (alpha/6) / pi_i (0 on carbon), phase factors of Eq. 13.
+// pi_i = e_i / Z and the phase factors cos, sin of omega_i dt of Eq. 13.
 // omega points at site i0.
 template <typename T>
 __global__ void site_params_kernel(const double* __restrict__ e, const double* __restrict__ omega, long long i0, long long n,
-                                   Layout L, double alpha6, double dt, const Ctl* ctl, T* __restrict__ pi, T* __restrict__ kcs) {
+                                   Layout L, double dt, const Ctl* ctl, T* __restrict__ pi, T* __restrict__ cs) {
   const double Z = ctl->zsum;
   for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (long long)gridDim.x * blockDim.x) {
     const long long i = i0 + k;
     const long long j = dense_to_padded(L, i);
     const double p = e[i] / Z;
-    double c = 1.0, s = 0.0, kap = 0.0;
-    if (p > 0.0) {
-      sincos(omega[k] * dt, &s, &c);
-      kap = alpha6 / p;
-    }
+    double c = 1.0, s = 0.0;
+    if (p > 0.0) sincos(omega[k] * dt, &s, &c);
     pi[j] = (T)p;
-    kcs[j] = (T)kap;
-    kcs[L.np + j] = (T)c;
-    kcs[2 * L.np + j] = (T)s;
+    cs[j] = (T)c;
+    cs[L.np + j] = (T)s;
   }
 }
 
@@ -118,7 +114,7 @@ __global__ void fill_ghosts_kernel(T* __restrict__ f, int nch, Layout L, int per
 // and the sums G[0] = sum pi h, Z_d[1] = a^2 (alpha/6) sum_i [m_{i,+d} + m_{i,-d}].
 template <typename T, int NRHO, int NMOM>
 __global__ void __launch_bounds__(256)
-    init_state_kernel(Layout L, const T* __restrict__ pi, const T* __restrict__ kcs, T* __restrict__ f, double a_len,
+    init_state_kernel(Layout L, const T* __restrict__ pi, T a6, T* __restrict__ f, double a_len,
                       double* partials, Ctl* ctl, double2* fid, double* vacf, long long vacf_stride, double zscale) {
   constexpr int NRED = 2 + NMOM;
   double acc[NRED];
@@ -138,7 +134,7 @@ __global__ void __launch_bounds__(256)
 #pragma unroll
       for (int d = 0; d < 3; ++d) {
         const T mm = tmin(p, pi[j - st[d]]), mp = tmin(p, pi[j + st[d]]);
-        f[(long long)(2 + NRHO + d) * L.np + j] = (T)a_len * kcs[j] * (mm - mp);
+        f[(long long)(2 + NRHO + d) * L.np + j] = (T)a_len * kappa_of(p, a6) * (mm - mp);
         acc[2 + d] += (double)mp + (double)mm;
       }
     }

@@ -61,9 +61,8 @@ __global__ void __launch_bounds__(256) step_direct_kernel(StepArgs<T> a) {
   for (int r = 0; r < NRED; ++r) acc[r] = 0.0;
 
   const T* __restrict__ pi = a.pi;
-  const T* __restrict__ kap = a.kcs;
-  const T* __restrict__ csv = a.kcs + L.np;
-  const T* __restrict__ snv = a.kcs + 2 * L.np;
+  const T* __restrict__ csv = a.cs;
+  const T* __restrict__ snv = a.cs + L.np;
 
   for (long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x; p < npairs; p += (long long)gridDim.x * blockDim.x) {
     const int z = 2 * (int)(p % zpairs);
@@ -78,7 +77,7 @@ __global__ void __launch_bounds__(256) step_direct_kernel(StepArgs<T> a) {
       if (s == 1 && !vb) break;
       const long long j = i + s;
       SiteUpdate<T, NRHO, NMOM> u;
-      u.weights(pi[j], pi[j - L.sx], pi[j + L.sx], pi[j - L.sy], pi[j + L.sy], pi[j - 1], pi[j + 1], kap[j], csv[j], snv[j]);
+      u.weights(pi[j], pi[j - L.sx], pi[j + L.sx], pi[j - L.sy], pi[j + L.sy], pi[j - 1], pi[j + 1], a.a6, csv[j], snv[j]);
 #pragma unroll
       for (int c = 0; c < C; ++c) {
         const T* __restrict__ f = a.fin + (long long)c * L.np;
@@ -120,7 +119,7 @@ struct TmaCfg {
   static constexpr int NTHREADS = NCONS + 32;
   static constexpr int F_RAW = C * TYH * TZW * (int)sizeof(T);
   static constexpr int PI_RAW = TYH * TZW * (int)sizeof(T);
-  static constexpr int KCS_RAW = 3 * TY * TZ * (int)sizeof(T);
+  static constexpr int KCS_RAW = 2 * TY * TZ * (int)sizeof(T);  // cos, sin (no halo)
   static constexpr int F_BYTES = (F_RAW + 127) / 128 * 128;
   static constexpr int PI_BYTES = (PI_RAW + 127) / 128 * 128;
   static constexpr int KCS_BYTES = (KCS_RAW + 127) / 128 * 128;
@@ -135,7 +134,7 @@ struct TmaCfg {
 template <typename T, int NRHO, int NMOM, int TY, int TZ, int NSTAGE>
 __global__ void __launch_bounds__(TY* TZ / 2 + 32)
     step_tma_kernel(const __grid_constant__ CUtensorMap tm_f, const __grid_constant__ CUtensorMap tm_pi,
-                    const __grid_constant__ CUtensorMap tm_kcs, StepArgs<T> a) {
+                    const __grid_constant__ CUtensorMap tm_cs, StepArgs<T> a) {
   using K = TmaCfg<T, NRHO, NMOM, TY, TZ, NSTAGE>;
   using V2 = typename Vec2<T>::type;
   constexpr int C = K::C, NRED = K::NRED, TZW = K::TZW, TYH = K::TYH, HZ = K::HZ;
@@ -173,7 +172,7 @@ __global__ void __launch_bounds__(TY* TZ / 2 + 32)
     if (lane == 0) {
       tma_prefetch_desc(&tm_f);
       tma_prefetch_desc(&tm_pi);
-      tma_prefetch_desc(&tm_kcs);
+      tma_prefetch_desc(&tm_cs);
       for (int j = 0; j < nloads; ++j) {
         const int s = j % NSTAGE;
         if (j >= NSTAGE) mbar_wait(&empty[s], ((j / NSTAGE) - 1) & 1);
@@ -183,7 +182,7 @@ __global__ void __launch_bounds__(TY* TZ / 2 + 32)
         // plane x0-1+j lives at padded x coordinate x0+j; box starts HZ columns / 1 row before the tile
         tma_load_4d(st, &tm_f, &full[s], L.padz + z0 - HZ, y0, x0 + j, 0);
         tma_load_3d(st + K::F_BYTES, &tm_pi, &full[s], L.padz + z0 - HZ, y0, x0 + j);
-        if (need_kcs) tma_load_4d(st + K::F_BYTES + K::PI_BYTES, &tm_kcs, &full[s], L.padz + z0, y0 + 1, x0 + j, 0);
+        if (need_kcs) tma_load_4d(st + K::F_BYTES + K::PI_BYTES, &tm_cs, &full[s], L.padz + z0, y0 + 1, x0 + j, 0);
       }
     }
   } else {
@@ -222,16 +221,15 @@ __global__ void __launch_bounds__(TY* TZ / 2 + 32)
       const T* sp = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES + K::F_BYTES);
       const T* sk = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES + K::F_BYTES + K::PI_BYTES);
       const int ek = ty * TZ + 2 * tp;
-      const V2 kap = *reinterpret_cast<const V2*>(sk + ek);
-      const V2 csv = *reinterpret_cast<const V2*>(sk + TY * TZ + ek);
-      const V2 snv = *reinterpret_cast<const V2*>(sk + 2 * TY * TZ + ek);
+      const V2 csv = *reinterpret_cast<const V2*>(sk + ek);
+      const V2 snv = *reinterpret_cast<const V2*>(sk + TY * TZ + ek);
       const V2 pym = *reinterpret_cast<const V2*>(sp + ec - TZW);
       const V2 pyp = *reinterpret_cast<const V2*>(sp + ec + TZW);
       const T pzm = sp[ec - 1], pzp = sp[ec + 2];
 
       SiteUpdate<T, NRHO, NMOM> ua, ub;
-      ua.weights(cpi.x, ppi.x, npi.x, pym.x, pyp.x, pzm, cpi.y, kap.x, csv.x, snv.x);
-      ub.weights(cpi.y, ppi.y, npi.y, pym.y, pyp.y, cpi.x, pzp, kap.y, csv.y, snv.y);
+      ua.weights(cpi.x, ppi.x, npi.x, pym.x, pyp.x, pzm, cpi.y, a.a6, csv.x, snv.x);
+      ub.weights(cpi.y, ppi.y, npi.y, pym.y, pyp.y, cpi.x, pzp, a.a6, csv.y, snv.y);
 
       T oa[C], ob[C];
 #pragma unroll
