@@ -342,6 +342,11 @@ int set_site_params_t(lpc_lattice* h, const double* dF, const uint8_t* blocked, 
     return LPC_OK;
   });
   if (rc) return rc;
+  CUDA_TRY(cudaMemcpyAsync(&hc, ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  if (hc.bad != 0)
+    return fail(LPC_EINVAL, "the equilibrium density underflows on %llu open sites: the spread of dF is too wide for %s", hc.bad,
+                h->cfg.precision ? "fp32" : "fp64");
   {
     const long long cells = 2ll * ((long long)L.nx * L.ny + (long long)L.nx * L.nz + (long long)L.ny * L.nz);
     fill_ghosts_kernel<T><<<aux_grid(cells), 256, 0, h->stream>>>(wsp<T>(h, h->off.pi), 1, L, h->cfg.bc[0] == 0, h->cfg.bc[1] == 0,

@@ -68,18 +68,22 @@ __global__ void __launch_bounds__(256) sum_kernel(const double* __restrict__ e, 
 // omega points at site i0.
 template <typename T>
 __global__ void site_params_kernel(const double* __restrict__ e, const double* __restrict__ omega, long long i0, long long n,
-                                   Layout L, double dt, const Ctl* ctl, T* __restrict__ pi, T* __restrict__ cs) {
+                                   Layout L, double dt, Ctl* ctl, T* __restrict__ pi, T* __restrict__ cs) {
   const double Z = ctl->zsum;
+  unsigned long long bad = 0;
   for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (long long)gridDim.x * blockDim.x) {
     const long long i = i0 + k;
     const long long j = dense_to_padded(L, i);
     const double p = e[i] / Z;
     double c = 1.0, s = 0.0;
     if (p > 0.0) sincos(omega[k] * dt, &s, &c);
+    // kappa_of() needs pi to be a normal number of T on every open site
+    if (e[i] > 0.0 && !((T)p >= (sizeof(T) == 8 ? (T)2.2250738585072014e-308 : (T)1.17549435e-38f))) bad++;
     pi[j] = (T)p;
     cs[j] = (T)c;
     cs[L.np + j] = (T)s;
   }
+  if (bad) atomicAdd(&ctl->bad, bad);
 }
 
 // Ghost layers of nch channel planes: periodic axis -> wrapped interior value, reflective -> 0.

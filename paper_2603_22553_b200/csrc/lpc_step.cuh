@@ -132,7 +132,7 @@ struct TmaCfg {
 };
 
 template <typename T, int NRHO, int NMOM, int TY, int TZ, int NSTAGE>
-__global__ void __launch_bounds__(TY* TZ / 2 + 32)
+__global__ void __launch_bounds__(TY* TZ / 2 + 64, (2 + NRHO + NMOM <= 3) ? 2 : 1)
     step_tma_kernel(const __grid_constant__ CUtensorMap tm_f, const __grid_constant__ CUtensorMap tm_pi,
                     const __grid_constant__ CUtensorMap tm_cs, StepArgs<T> a) {
   using K = TmaCfg<T, NRHO, NMOM, TY, TZ, NSTAGE>;
