@@ -126,6 +126,23 @@ int lpc_read_field(lpc_lattice* lat, int32_t which, void* out);
  * in: host or device.  Synchronises.  Errors: LPC_EINVAL, LPC_ESTATE, LPC_ECUDA.               */
 int lpc_set_state(lpc_lattice* lat, int32_t which, const void* in);
 
+/* Equilibration loop of the paper's workflow (Fig. 3 step 3): iterate
+ * the density update rho <- W rho on the density field (LPC_FIELD_RHO; needs n_density = 1) and
+ * compare rho(t) with rho(t+1); stop when delta = max_i |rho_i(t+1) - rho_i(t)| < threshold or
+ * after max_iters sweeps.  delta is reduced on the device inside every sweep; the host reads it
+ * back every check_every sweeps (>= 1; 1 reproduces the paper's loop exactly, larger values
+ * trade up to check_every - 1 extra sweeps for fewer synchronisations).  The magnetisation, the
+ * moment fields and both series are not touched.
+ * iters_done, last_delta: host, out (may be NULL).  Synchronises.
+ * Errors: LPC_ESTATE (n_density == 0 or no parameters), LPC_EINVAL, LPC_ECUDA.                 */
+int lpc_equilibrate(lpc_lattice* lat, double threshold, int64_t max_iters, int64_t check_every,
+                    int64_t* iters_done, double* last_delta);
+
+/* Start the propagation from the density field: g(0) <- rho (real), G[0] = sum_i rho_i; resets
+ * the step counter and the G series (Fig. 3: the equilibrated densities feed the propagation
+ * loop).  Synchronises.  Errors: LPC_ESTATE, LPC_ECUDA.                           */
+int lpc_seed_from_density(lpc_lattice* lat);
+
 /* Choose the step kernel (LPC_KERNEL_*).  AUTO picks TMA.  Errors: LPC_EINVAL.                 */
 int lpc_set_kernel(lpc_lattice* lat, int32_t which);
 

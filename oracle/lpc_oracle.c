@@ -29,6 +29,7 @@
  *   O6  G[n] = sum_i g_i(n)                         Eq. 12
  *   O7  first-step moments P^d(1), u^d, Z_d[1]      Eq. 4, 5 PAPER.md:79,92; :84-86
  *   O8  Z_d[k+1] = sum_i P^d_i u^d_i ; P^d <- W P^d ; D_d   Eq. 4
+ *   O9  equilibration loop rho <- W rho until max_i |rho(t+1)-rho(t)| < threshold
  *
  * Every global sum is Neumaier-compensated, taken plane by plane (x) and the
  * plane partials combined in x order, so results do not depend on the OpenMP
@@ -334,6 +335,34 @@ int lpco_propagate_real(const lpco_state *st, const double *rho_in, double *rho_
   memcpy(rho_out, a, (size_t)st->n * sizeof(double));
   free(a); free(b);
   return 0;
+}
+
+/* Equilibration loop of the paper's workflow (Fig. 3 step 3): iterate the
+ * density update rho <- W rho and compare rho(t) with rho(t+1); stop when the difference falls below
+ * `threshold` or after `max_iters` iterations.  The paper does not name the norm: DESIGN.md reading
+ * Q25 takes the largest per-site change, delta(t+1) = max_i |rho_i(t+1) - rho_i(t)|, and stops as soon
+ * as delta < threshold (the updated density is kept).  deltas_out (may be NULL) receives
+ * delta(1..iters).  Returns the number of iterations done, or -1 on bad arguments. */
+int64_t lpco_equilibrate(const lpco_state *st, double *rho_inout, double threshold, int64_t max_iters, double *deltas_out) {
+  if (!st || !rho_inout || max_iters < 0) return -1;
+  double *a = dalloc(st->n), *b = dalloc(st->n);
+  for (int64_t i = 0; i < st->n; ++i) a[i] = st->blocked[i] ? 0.0 : rho_inout[i];
+  int64_t it = 0;
+  while (it < max_iters) {
+    propagate_real(st, a, b);
+    double delta = 0.0;
+    for (int64_t i = 0; i < st->n; ++i) {
+      const double d = fabs(b[i] - a[i]);
+      if (d > delta) delta = d;
+    }
+    double *t = a; a = b; b = t;
+    if (deltas_out) deltas_out[it] = delta;
+    ++it;
+    if (delta < threshold) break;
+  }
+  memcpy(rho_inout, a, (size_t)st->n * sizeof(double));
+  free(a); free(b);
+  return it;
 }
 
 /* ---- read-outs ----------------------------------------------------------- */

@@ -37,6 +37,8 @@ _lib.lpco_destroy.argtypes = [C.c_void_p]
 _lib.lpco_step.argtypes = [C.c_void_p, C.c_int64]
 _lib.lpco_set_g.argtypes = [C.c_void_p, _dp]
 _lib.lpco_propagate_real.argtypes = [C.c_void_p, _dp, _dp, C.c_int64]
+_lib.lpco_equilibrate.restype = C.c_int64
+_lib.lpco_equilibrate.argtypes = [C.c_void_p, _dp, C.c_double, C.c_int64, _dp]
 _lib.lpco_steps.restype = C.c_int64
 _lib.lpco_steps.argtypes = [C.c_void_p]
 _lib.lpco_partition_sum.restype = C.c_double
@@ -131,6 +133,14 @@ class Oracle:
         out = np.empty_like(rho)
         _lib.lpco_propagate_real(self._h, _d(rho), _d(out), int(n_steps))
         return out.reshape(self.shape)
+
+    def equilibrate(self, rho, threshold, max_iters):
+        """The paper's equilibration loop: returns (rho, iterations, deltas[1..iterations])."""
+        rho = np.array(rho, dtype=np.float64).reshape(-1)
+        deltas = np.zeros(max(int(max_iters), 1), dtype=np.float64)
+        it = int(_lib.lpco_equilibrate(self._h, _d(rho), float(threshold), int(max_iters), _d(deltas)))
+        assert it >= 0
+        return rho.reshape(self.shape), it, deltas[:it]
 
     def _get(self, fn, *a):
         out = np.empty(self.n, dtype=np.float64)

@@ -24,7 +24,8 @@ LPC_KERNEL_AUTO, LPC_KERNEL_DIRECT, LPC_KERNEL_TMA = range(3)
 
 EXPORTS = (
     "lpc_workspace_bytes", "lpc_create_lattice", "lpc_set_site_params", "lpc_step_n", "lpc_read_fid",
-    "lpc_moments", "lpc_read_field", "lpc_set_state", "lpc_set_kernel", "lpc_steps_done",
+    "lpc_moments", "lpc_read_field", "lpc_set_state", "lpc_equilibrate", "lpc_seed_from_density", "lpc_set_kernel",
+    "lpc_steps_done",
     "lpc_launch_count", "lpc_bytes_per_site_step", "lpc_destroy", "lpc_last_error",
 )
 
@@ -66,6 +67,8 @@ def _load():
     lib.lpc_read_field.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
     lib.lpc_set_state.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
     lib.lpc_set_kernel.argtypes = [C.c_void_p, C.c_int32]
+    lib.lpc_equilibrate.argtypes = [C.c_void_p, C.c_double, C.c_int64, C.c_int64, C.POINTER(C.c_int64), C.POINTER(C.c_double)]
+    lib.lpc_seed_from_density.argtypes = [C.c_void_p]
     lib.lpc_steps_done.argtypes = [C.c_void_p]
     lib.lpc_steps_done.restype = C.c_int64
     lib.lpc_launch_count.argtypes = [C.c_void_p]
@@ -176,6 +179,17 @@ def lpc_set_state(handle, which, arr):
     _check(_lib.lpc_set_state(handle, int(which), _ptr(arr)))
 
 
+def lpc_equilibrate(handle, threshold, max_iters, check_every=1):
+    """(iterations done, delta of the last sweep)."""
+    iters, delta = C.c_int64(0), C.c_double(0.0)
+    _check(_lib.lpc_equilibrate(handle, float(threshold), int(max_iters), int(check_every), C.byref(iters), C.byref(delta)))
+    return int(iters.value), float(delta.value)
+
+
+def lpc_seed_from_density(handle):
+    _check(_lib.lpc_seed_from_density(handle))
+
+
 def lpc_set_kernel(handle, which):
     _check(_lib.lpc_set_kernel(handle, int(which)))
 
@@ -263,6 +277,12 @@ class Lattice:
     def set_state(self, which, arr):
         arr = np.ascontiguousarray(arr, dtype=np.complex128 if which == LPC_FIELD_G else np.float64)
         lpc_set_state(self.handle, which, arr)
+
+    def equilibrate(self, threshold, max_iters, check_every=1):
+        return lpc_equilibrate(self.handle, threshold, max_iters, check_every)
+
+    def seed_from_density(self):
+        lpc_seed_from_density(self.handle)
 
     def set_kernel(self, which):
         lpc_set_kernel(self.handle, which)

@@ -18,6 +18,7 @@
 #include "lpc_internal.cuh"
 #include "lpc_precompute.cuh"
 #include "lpc_step.cuh"
+#include "lpc_equil.cuh"
 
 using namespace lpc;
 
@@ -105,19 +106,28 @@ Layout make_layout(const lpc_config* c) {
   return L;
 }
 
-// TMA tile geometry per channel count.
+// TMA tile geometry: 8 x 64 tiles of the y-z plane, 8 warps per CTA; two CTAs per
+// SM up to 3 channels, one with 5.  (16 x 64 tiles with one 16-warp CTA per SM measured the same at 512^3
+// and slightly worse at 256^3, so there is one tile shape.)
+constexpr int SM_COUNT = 148;
+
 void tma_geometry(int C, int nx, int ny, int nz, int* ty, int* tz, int* nstage, int* xc, int* tiles_z, int* tiles_y, int* chunks_x) {
   *ty = 8; *tz = 64;
   *nstage = (C <= 3) ? 4 : 3;
   *tiles_z = (nz + *tz - 1) / *tz;
   *tiles_y = (ny + *ty - 1) / *ty;
   const long long tiles = (long long)*tiles_z * *tiles_y;
-  const long long resident = 148ll * ((C <= 3) ? 2 : 1);
-  long long chunks = (12 * resident + tiles - 1) / tiles;     // aim for ~12 waves of CTAs ...
-  chunks = std::min<long long>(chunks, std::max(1, nx / 32)); // ... but at least 32 planes per chunk
-  chunks = std::max<long long>(chunks, 1);
-  // Small lattices (L2-resident, latency-bound): the march costs about 1 us per plane, so fill one
-  // wave of CTAs first and accept the two extra plane loads per chunk (measured: 64^3 35 -> 10 us/step).
+  const long long resident = (long long)SM_COUNT * ((C <= 3) ? 2 : 1);
+  // Split x into chunks of about 32 planes.  Measured on 512^3 fp64 (ms per step, xc = 8 / 16 / 24 / 32 /
+  // 48 / 74 / 128 / 256): 1.44 / 1.32 / 1.29 / 1.29 / 1.32 / 1.38 / 1.49 / 1.55 -- long chunks keep all SMs
+  // marching through the same planes in lockstep, which makes the DRAM traffic come in read bursts and
+  // write bursts; many short CTAs desynchronise and keep the mix even.  Below 24 planes the two extra
+  // plane loads per chunk cost more than that gains, unless the grid is short of waves (256^3: 16 planes
+  // per chunk measured 2% faster than 32), so chunks shrink to 16 planes to reach 8 waves.  Small,
+  // L2-resident lattices are latency-bound: they get as many chunks as it takes to fill the SMs once
+  // (measured 64^3: 35 -> 10 us/step).
+  long long chunks = std::max(1, (nx + 16) / 32);
+  chunks = std::max(chunks, std::min<long long>(std::max(1, nx / 16), (8 * resident + tiles - 1) / tiles));
   if (tiles * chunks < resident) chunks = std::min<long long>((resident + tiles - 1) / tiles, std::max(1, nx / 2));
   if (const char* e = getenv("LPC_XC")) {
     const int v = atoi(e);
@@ -222,16 +232,20 @@ int launch_step_t(lpc_lattice* h) {
   const bool use_tma = h->tma_ok && h->kernel != LPC_KERNEL_DIRECT;
   if (use_tma) {
     constexpr int C = 2 + NRHO + NMOM;
-    constexpr int NS = (C <= 3) ? 4 : 3;
-    using K = TmaCfg<T, NRHO, NMOM, 8, 64, NS>;
-    auto kern = step_tma_kernel<T, NRHO, NMOM, 8, 64, NS>;
-    static bool attr_set = false;
-    if (!attr_set) {
-      CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, K::SMEM_BYTES));
-      attr_set = true;
-    }
     const unsigned grid = (unsigned)(h->tiles_z * h->tiles_y * h->chunks_x);
-    kern<<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(h->tm_f[h->cur], h->tm_pi, h->tm_cs, a);
+    auto launch = [&](auto kern, auto cfg) -> int {
+      using K = decltype(cfg);
+      static bool attr_set = false;
+      if (!attr_set) {
+        CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, K::SMEM_BYTES));
+        attr_set = true;
+      }
+      kern<<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(h->tm_f[h->cur], h->tm_pi, h->tm_cs, a);
+      return LPC_OK;
+    };
+    constexpr int NS = (C <= 3) ? 4 : 3;
+    int rc = launch(step_tma_kernel<T, NRHO, NMOM, 8, 64, NS>, TmaCfg<T, NRHO, NMOM, 8, 64, NS>());
+    if (rc) return rc;
   } else {
     const long long npairs = (long long)((h->L.nz + 1) / 2) * h->L.ny * h->L.nx;
     const int grid = (int)std::max<long long>(1, std::min<long long>((npairs + 255) / 256, DIRECT_MAX_BLOCKS));
@@ -446,6 +460,63 @@ int set_state_t(lpc_lattice* h, int which, const void* in) {
   return LPC_OK;
 }
 
+template <typename T>
+int equilibrate_t(lpc_lattice* h, double threshold, int64_t max_iters, int64_t check_every, int64_t* iters_done, double* last_delta) {
+  const Layout& L = h->L;
+  Ctl* ctl = wsp<Ctl>(h, h->off.ctl);
+  T* ch[2] = {wsp<T>(h, h->off.f0) + 2 * L.np, wsp<T>(h, h->off.f1) + 2 * L.np};  // density channel of F0 / F1
+  int src = h->cur;  // the current state buffer holds rho(t)
+  CUDA_TRY(cudaMemsetAsync(&ctl->scratch[4], 0, 2 * sizeof(double), h->stream));
+  EquilArgs<T> a;
+  a.L = L;
+  a.pi = wsp<T>(h, h->off.pi);
+  a.a6 = (T)(h->cfg.alpha / 6.0);
+  a.partials = wsp<double>(h, h->off.partials);
+  a.ctl = ctl;
+  for (int d = 0; d < 3; ++d) a.per[d] = h->cfg.bc[d] == 0;
+  const long long npairs = (long long)((L.nz + 1) / 2) * L.ny * L.nx;
+  const int grid = (int)std::max<long long>(1, std::min<long long>((npairs + 255) / 256, DIRECT_MAX_BLOCKS));
+  int64_t done = 0;
+  double delta = 0.0;
+  while (done < max_iters) {
+    const int64_t batch = std::min<int64_t>(check_every, max_iters - done);
+    for (int64_t k = 0; k < batch; ++k) {
+      a.rin = ch[src];
+      a.rout = ch[src ^ 1];
+      equil_kernel<T><<<grid, 256, 0, h->stream>>>(a);
+      CUDA_TRY(cudaGetLastError());
+      h->launches++;
+      src ^= 1;
+    }
+    done += batch;
+    CUDA_TRY(cudaMemcpyAsync(&delta, &ctl->scratch[4], sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    if (delta < threshold) break;
+  }
+  // the other channels live in buffer `cur`: bring the density back there if it ended in the other one
+  if (src != h->cur) CUDA_TRY(cudaMemcpyAsync(ch[h->cur], ch[src], (size_t)L.np * sizeof(T), cudaMemcpyDeviceToDevice, h->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  if (iters_done) *iters_done = done;
+  if (last_delta) *last_delta = delta;
+  return LPC_OK;
+}
+
+template <typename T>
+int seed_from_density_t(lpc_lattice* h) {
+  const Layout& L = h->L;
+  T* f = wsp<T>(h, h->cur ? h->off.f1 : h->off.f0);
+  seed_h_from_r_kernel<T><<<aux_grid(L.np), 256, 0, h->stream>>>(L.np, f + 2 * L.np, f, f + L.np);
+  CUDA_TRY(cudaGetLastError());
+  h->launches++;
+  reduce_g_kernel<T><<<aux_grid(h->N), 256, 0, h->stream>>>(L, wsp<T>(h, h->off.pi), f, wsp<double>(h, h->off.partials),
+                                                             wsp<Ctl>(h, h->off.ctl), wsp<double2>(h, h->off.fid));
+  CUDA_TRY(cudaGetLastError());
+  h->launches++;
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  h->steps = 0;
+  return LPC_OK;
+}
+
 }  // namespace
 
 // ================================================================================================
@@ -590,6 +661,24 @@ int lpc_set_state(lpc_lattice* h, int32_t which, const void* in) {
   if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
   if (!in) return fail(LPC_EINVAL, "in is NULL");
   return h->cfg.precision ? set_state_t<float>(h, which, in) : set_state_t<double>(h, which, in);
+}
+
+int lpc_equilibrate(lpc_lattice* h, double threshold, int64_t max_iters, int64_t check_every, int64_t* iters_done, double* last_delta) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
+  if (h->nrho != 1) return fail(LPC_ESTATE, "the density field is not propagated (n_density = 0)");
+  if (max_iters < 0) return fail(LPC_EINVAL, "max_iters must be >= 0");
+  if (check_every < 1) return fail(LPC_EINVAL, "check_every must be >= 1");
+  if (!(threshold == threshold)) return fail(LPC_EINVAL, "threshold is NaN");
+  return h->cfg.precision ? equilibrate_t<float>(h, threshold, max_iters, check_every, iters_done, last_delta)
+                          : equilibrate_t<double>(h, threshold, max_iters, check_every, iters_done, last_delta);
+}
+
+int lpc_seed_from_density(lpc_lattice* h) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
+  if (h->nrho != 1) return fail(LPC_ESTATE, "the density field is not propagated (n_density = 0)");
+  return h->cfg.precision ? seed_from_density_t<float>(h) : seed_from_density_t<double>(h);
 }
 
 int lpc_set_kernel(lpc_lattice* h, int32_t which) {

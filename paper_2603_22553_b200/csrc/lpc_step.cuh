@@ -3,10 +3,11 @@
 // Two kernels compute the same thing with the same per-site arithmetic (SiteUpdate):
 //   step_direct_kernel : one thread per z-pair of sites, neighbours read straight from global
 //                        memory (L1/L2 serve the reuse).  Works for every size; the fallback.
-//   step_tma_kernel    : a CTA owns a (TY x TZ) tile of the y-z plane and marches along x.  A
-//                        producer warp streams one x-plane per stage into shared memory with
-//                        cp.async.bulk.tensor (TMA, halo included) behind a full/empty mbarrier
-//                        ring; consumer warps keep the x-1 / x / x+1 centre values in registers
+//   step_tma_kernel    : a CTA owns a (TY x TZ) tile of the y-z plane and marches along x.  One
+//                        x-plane per stage is streamed into shared memory with cp.async.bulk.tensor
+//                        (TMA, halo included) behind a full/empty mbarrier ring; thread 0 issues the
+//                        loads between planes (no producer warp: 16 warps per SM leave 128 registers
+//                        per thread).  The threads keep the x-1 / x / x+1 centre values in registers
 //                        and read the in-plane neighbours from shared memory.
 // Both end with one block partial per CTA and a fixed-order final sum by the last CTA.
 #pragma once
@@ -43,6 +44,28 @@ __device__ __forceinline__ void store_with_ghosts(T* __restrict__ base, const La
   if (per[0]) {
     if (x == 0) store_pair(base, i + (long long)L.nx * L.sx, oa, ob, vb);
     if (x == L.nx - 1) store_pair(base, i - (long long)L.nx * L.sx, oa, ob, vb);
+  }
+}
+
+// One channel of a pair that lies on a periodic face (rare; kept out of line, with scalar arguments
+// only, so that the march of the TMA kernel stays small and the kernel parameters stay in the
+// constant bank).  i is the padded index of (x, y, z); permask bit d = axis d is periodic.
+template <typename T>
+__device__ __noinline__ void store_face_pair(T* __restrict__ base, long long i, int nx, int ny, int nz, long long sy, long long sx,
+                                             int permask, int x, int y, int z, T oa, T ob, bool vb) {
+  store_pair(base, i, oa, ob, vb);
+  if (permask & 4) {
+    if (z == 0) base[i + nz] = oa;
+    if (z == nz - 1) base[i - nz] = oa;
+    if (vb && z + 1 == nz - 1) base[i + 1 - nz] = ob;
+  }
+  if (permask & 2) {
+    if (y == 0) store_pair(base, i + (long long)ny * sy, oa, ob, vb);
+    if (y == ny - 1) store_pair(base, i - (long long)ny * sy, oa, ob, vb);
+  }
+  if (permask & 1) {
+    if (x == 0) store_pair(base, i + (long long)nx * sx, oa, ob, vb);
+    if (x == nx - 1) store_pair(base, i - (long long)nx * sx, oa, ob, vb);
   }
 }
 
@@ -116,7 +139,7 @@ struct TmaCfg {
   static constexpr int TYH = TY + 2;
   static constexpr int NCONS = TY * TZ / 2;  // consumer threads, one per z-pair
   static constexpr int NCW = NCONS / 32;
-  static constexpr int NTHREADS = NCONS + 32;
+  static constexpr int NTHREADS = NCONS;      // no producer warp: thread 0 issues the TMA loads between planes
   static constexpr int F_RAW = C * TYH * TZW * (int)sizeof(T);
   static constexpr int PI_RAW = TYH * TZW * (int)sizeof(T);
   static constexpr int KCS_RAW = 2 * TY * TZ * (int)sizeof(T);  // cos, sin (no halo)
@@ -127,12 +150,16 @@ struct TmaCfg {
   static constexpr int BAR_OFF = NSTAGE * STAGE_BYTES;
   static constexpr int RED_OFF = BAR_OFF + 2 * NSTAGE * 8;
   static constexpr int SMEM_BYTES = RED_OFF + ((NTHREADS / 32) * NRED + 1) * 8 + 128;  // +128: manual alignment slack
+  // Resident CTAs per SM the registers are budgeted for: two 8-warp CTAs (TY = 8, up to 3 channels) or
+  // one.  16 warps per SM are 4 per scheduler, i.e. up to 128 registers per thread.
+  static constexpr int LB_CTAS = (TY == 8 && C <= 3) ? 2 : 1;
+  static constexpr int LB_THREADS = NTHREADS;
   static_assert(NCONS % 32 == 0, "consumer threads must fill whole warps");
   static_assert(TZ % 2 == 0, "TZ must be even");
 };
 
 template <typename T, int NRHO, int NMOM, int TY, int TZ, int NSTAGE>
-__global__ void __launch_bounds__(TY* TZ / 2 + 64, (2 + NRHO + NMOM <= 3) ? 2 : 1)
+__global__ void __launch_bounds__(TmaCfg<T, NRHO, NMOM, TY, TZ, NSTAGE>::LB_THREADS, TmaCfg<T, NRHO, NMOM, TY, TZ, NSTAGE>::LB_CTAS)
     step_tma_kernel(const __grid_constant__ CUtensorMap tm_f, const __grid_constant__ CUtensorMap tm_pi,
                     const __grid_constant__ CUtensorMap tm_cs, StepArgs<T> a) {
   using K = TmaCfg<T, NRHO, NMOM, TY, TZ, NSTAGE>;
@@ -152,7 +179,7 @@ __global__ void __launch_bounds__(TY* TZ / 2 + 64, (2 + NRHO + NMOM <= 3) ? 2 : 
   const int z0 = bz * TZ, y0 = by * TY, x0 = bx * a.xc;
   const int nplanes = min(a.xc, L.nx - x0);
   const int nloads = nplanes + 2;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int lane = threadIdx.x & 31;
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < NSTAGE; ++s) {
@@ -167,25 +194,27 @@ __global__ void __launch_bounds__(TY* TZ / 2 + 64, (2 + NRHO + NMOM <= 3) ? 2 : 
 #pragma unroll
   for (int r = 0; r < NRED; ++r) acc[r] = 0.0;
 
-  if (warp == K::NCW) {
-    // ===== producer warp: one elected lane issues the TMA loads =====
-    if (lane == 0) {
-      tma_prefetch_desc(&tm_f);
-      tma_prefetch_desc(&tm_pi);
-      tma_prefetch_desc(&tm_cs);
-      for (int j = 0; j < nloads; ++j) {
-        const int s = j % NSTAGE;
-        if (j >= NSTAGE) mbar_wait(&empty[s], ((j / NSTAGE) - 1) & 1);
-        unsigned char* st = smem + s * K::STAGE_BYTES;
-        const bool need_kcs = (j >= 1 && j <= nplanes);
-        mbar_expect_tx(&full[s], K::F_RAW + K::PI_RAW + (need_kcs ? K::KCS_RAW : 0));
-        // plane x0-1+j lives at padded x coordinate x0+j; box starts HZ columns / 1 row before the tile
-        tma_load_4d(st, &tm_f, &full[s], L.padz + z0 - HZ, y0, x0 + j, 0);
-        tma_load_3d(st + K::F_BYTES, &tm_pi, &full[s], L.padz + z0 - HZ, y0, x0 + j);
-        if (need_kcs) tma_load_4d(st + K::F_BYTES + K::PI_BYTES, &tm_cs, &full[s], L.padz + z0, y0 + 1, x0 + j, 0);
-      }
-    }
-  } else {
+  // ----- TMA issue (thread 0): load j brings plane x0-1+j into stage j % NSTAGE -----
+  int jl = 0;  // next load to issue (thread 0 only)
+  auto issue_load = [&]() {
+    const int s = jl % NSTAGE;
+    if (jl >= NSTAGE) mbar_wait(&empty[s], ((jl / NSTAGE) - 1) & 1);   // every warp is done with the plane it held
+    unsigned char* st = smem + s * K::STAGE_BYTES;
+    const bool need_kcs = (jl >= 1 && jl <= nplanes);
+    mbar_expect_tx(&full[s], K::F_RAW + K::PI_RAW + (need_kcs ? K::KCS_RAW : 0));
+    // plane x0-1+j lives at padded x coordinate x0+j; box starts HZ columns / 1 row before the tile
+    tma_load_4d(st, &tm_f, &full[s], L.padz + z0 - HZ, y0, x0 + jl, 0);
+    tma_load_3d(st + K::F_BYTES, &tm_pi, &full[s], L.padz + z0 - HZ, y0, x0 + jl);
+    if (need_kcs) tma_load_4d(st + K::F_BYTES + K::PI_BYTES, &tm_cs, &full[s], L.padz + z0, y0 + 1, x0 + jl, 0);
+    ++jl;
+  };
+  if (threadIdx.x == 0) {
+    tma_prefetch_desc(&tm_f);
+    tma_prefetch_desc(&tm_pi);
+    tma_prefetch_desc(&tm_cs);
+    for (int j = 0; j < NSTAGE && j < nloads; ++j) issue_load();
+  }
+  {
     // ===== consumer warps =====
     const int ty = threadIdx.x / (TZ / 2);   // row inside the tile
     const int tp = threadIdx.x % (TZ / 2);   // pair inside the row
@@ -193,34 +222,49 @@ __global__ void __launch_bounds__(TY* TZ / 2 + 64, (2 + NRHO + NMOM <= 3) ? 2 : 
     const bool va = (y < L.ny) && (z < L.nz);
     const bool vb = (y < L.ny) && (z + 1 < L.nz);
     const int ec = (ty + 1) * TZW + 2 * tp + HZ;  // element offset of the centre pair in a halo'd tile
+    const int ek = ty * TZ + 2 * tp;              // element offset of the pair in a tile without halo
+    // sites on a periodic face also write their ghost copies: rare, so it is a separate path
+    const bool edge_yz = (a.per[1] && (y == 0 || y == L.ny - 1)) || (a.per[2] && (z == 0 || z + 2 >= L.nz - 1));
+    const int permask = (a.per[0] ? 1 : 0) | (a.per[1] ? 2 : 0) | (a.per[2] ? 4 : 0);
+    T* outp = a.fout + L.idx(x0, y, z);
 
-    V2 prev[C], ctr[C], nxt[C], ppi, cpi, npi;
-    auto load_centres = [&](int s, V2(&f)[C], V2& p) {
-      const T* sf = reinterpret_cast<const T*>(smem + s * K::STAGE_BYTES);
-      const T* sp = reinterpret_cast<const T*>(smem + s * K::STAGE_BYTES + K::F_BYTES);
+    // One x-plane as a consumer thread holds it: the centre pair of every channel and of pi, kappa of
+    // the pair, and mlo = min(pi, pi of the plane below) -- the symmetric link weight m_ij of the -x
+    // link (which is the +x link of the plane below).
+    struct Plane {
+      V2 f[C];
+      V2 pi, kap, mlo;
+    };
+    Plane P0, P1, P2;
+    int sj = 0;            // stage of the next plane to take from the ring
+    uint32_t phj = 0;      // and its phase bit
+    auto take = [&](Plane& n, const Plane* below) {
+      mbar_wait(&full[sj], phj);
+      const T* sf = reinterpret_cast<const T*>(smem + sj * K::STAGE_BYTES);
+      const T* sp = reinterpret_cast<const T*>(smem + sj * K::STAGE_BYTES + K::F_BYTES);
 #pragma unroll
-      for (int c = 0; c < C; ++c) f[c] = *reinterpret_cast<const V2*>(sf + c * TYH * TZW + ec);
-      p = *reinterpret_cast<const V2*>(sp + ec);
+      for (int c = 0; c < C; ++c) n.f[c] = *reinterpret_cast<const V2*>(sf + c * TYH * TZW + ec);
+      n.pi = *reinterpret_cast<const V2*>(sp + ec);
+      n.kap.x = kappa_of(n.pi.x, a.a6);
+      n.kap.y = kappa_of(n.pi.y, a.a6);
+      if (below) {
+        n.mlo.x = tmin(n.pi.x, below->pi.x);
+        n.mlo.y = tmin(n.pi.y, below->pi.y);
+      }
+      if (++sj == NSTAGE) {
+        sj = 0;
+        phj ^= 1u;
+      }
     };
 
-    mbar_wait(&full[0], 0);
-    load_centres(0, prev, ppi);
-    __syncwarp();
-    if (lane == 0) mbar_arrive(&empty[0]);
-    mbar_wait(&full[1 % NSTAGE], (1 / NSTAGE) & 1);
-    load_centres(1 % NSTAGE, ctr, cpi);
-
-    for (int p = 0; p < nplanes; ++p) {
-      const int x = x0 + p;
-      const int jn = p + 2, sn_ = jn % NSTAGE;
-      mbar_wait(&full[sn_], (jn / NSTAGE) & 1);
-      load_centres(sn_, nxt, npi);
-
-      const int sc = (p + 1) % NSTAGE;
+    // one plane of the march: prv / ctr / nxt are the planes x-1 / x / x+1, sc the stage that holds x
+    auto plane = [&](int x, int sc, const Plane& prv, const Plane& ctr, Plane& nxt) {
+      // refill the stage that held plane x-1 (released when the previous plane was finished)
+      if (threadIdx.x == 0 && jl < nloads) issue_load();
+      take(nxt, &ctr);
       const T* sf = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES);
       const T* sp = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES + K::F_BYTES);
       const T* sk = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES + K::F_BYTES + K::PI_BYTES);
-      const int ek = ty * TZ + 2 * tp;
       const V2 csv = *reinterpret_cast<const V2*>(sk + ek);
       const V2 snv = *reinterpret_cast<const V2*>(sk + TY * TZ + ek);
       const V2 pym = *reinterpret_cast<const V2*>(sp + ec - TZW);
@@ -228,8 +272,16 @@ __global__ void __launch_bounds__(TY* TZ / 2 + 64, (2 + NRHO + NMOM <= 3) ? 2 : 
       const T pzm = sp[ec - 1], pzp = sp[ec + 2];
 
       SiteUpdate<T, NRHO, NMOM> ua, ub;
-      ua.weights(cpi.x, ppi.x, npi.x, pym.x, pyp.x, pzm, cpi.y, a.a6, csv.x, snv.x);
-      ub.weights(cpi.y, ppi.y, npi.y, pym.y, pyp.y, cpi.x, pzp, a.a6, csv.y, snv.y);
+      ua.pc = ctr.pi.x; ub.pc = ctr.pi.y;
+      ua.kap = ctr.kap.x; ub.kap = ctr.kap.y;
+      ua.mxm = ctr.mlo.x; ub.mxm = ctr.mlo.y;
+      ua.mxp = nxt.mlo.x; ub.mxp = nxt.mlo.y;
+      ua.mym = tmin(ctr.pi.x, pym.x); ub.mym = tmin(ctr.pi.y, pym.y);
+      ua.myp = tmin(ctr.pi.x, pyp.x); ub.myp = tmin(ctr.pi.y, pyp.y);
+      ua.mzm = tmin(ctr.pi.x, pzm);
+      ua.mzp = tmin(ctr.pi.x, ctr.pi.y);
+      ub.mzm = ua.mzp;
+      ub.mzp = tmin(ctr.pi.y, pzp);
 
       T oa[C], ob[C];
 #pragma unroll
@@ -243,12 +295,12 @@ __global__ void __launch_bounds__(TY* TZ / 2 + 64, (2 + NRHO + NMOM <= 3) ? 2 : 
           const T dma = (d == 0) ? (ua.mxp - ua.mxm) : (d == 1) ? (ua.myp - ua.mym) : (ua.mzp - ua.mzm);
           const T dmb = (d == 0) ? (ub.mxp - ub.mxm) : (d == 1) ? (ub.myp - ub.mym) : (ub.mzp - ub.mzm);
           double t = 0.0;
-          if (va) t += (double)ctr[c].x * (double)dma;
-          if (vb) t += (double)ctr[c].y * (double)dmb;
+          if (va) t += (double)ctr.f[c].x * (double)dma;
+          if (vb) t += (double)ctr.f[c].y * (double)dmb;
           acc[2 + d] += t;
         }
-        oa[c] = ua.gather(ctr[c].x, prev[c].x, nxt[c].x, fym.x, fyp.x, fzm, ctr[c].y);
-        ob[c] = ub.gather(ctr[c].y, prev[c].y, nxt[c].y, fym.y, fyp.y, ctr[c].x, fzp);
+        oa[c] = ua.gather(ctr.f[c].x, prv.f[c].x, nxt.f[c].x, fym.x, fyp.x, fzm, ctr.f[c].y);
+        ob[c] = ub.gather(ctr.f[c].y, prv.f[c].y, nxt.f[c].y, fym.y, fyp.y, ctr.f[c].x, fzp);
       }
       // every shared-memory read of stage sc is done: hand it back to the producer
       __syncwarp();
@@ -256,30 +308,47 @@ __global__ void __launch_bounds__(TY* TZ / 2 + 64, (2 + NRHO + NMOM <= 3) ? 2 : 
 
       {
         const T ar = oa[0], ai = oa[1], br = ob[0], bi = ob[1];
-        oa[0] = ua.cs * ar - ua.sn * ai;
-        oa[1] = ua.cs * ai + ua.sn * ar;
-        ob[0] = ub.cs * br - ub.sn * bi;
-        ob[1] = ub.cs * bi + ub.sn * br;
+        oa[0] = csv.x * ar - snv.x * ai;
+        oa[1] = csv.x * ai + snv.x * ar;
+        ob[0] = csv.y * br - snv.y * bi;
+        ob[1] = csv.y * bi + snv.y * br;
       }
       if (va) {
-        acc[0] += (double)cpi.x * (double)oa[0];
-        acc[1] += (double)cpi.x * (double)oa[1];
+        acc[0] += (double)ctr.pi.x * (double)oa[0];
+        acc[1] += (double)ctr.pi.x * (double)oa[1];
         if (vb) {
-          acc[0] += (double)cpi.y * (double)ob[0];
-          acc[1] += (double)cpi.y * (double)ob[1];
+          acc[0] += (double)ctr.pi.y * (double)ob[0];
+          acc[1] += (double)ctr.pi.y * (double)ob[1];
         }
-        const long long i = L.idx(x, y, z);
+        if (edge_yz || (a.per[0] && (x == 0 || x == L.nx - 1))) {
+          const long long i = L.idx(x, y, z);
 #pragma unroll
-        for (int c = 0; c < C; ++c) store_with_ghosts(a.fout + (long long)c * L.np, L, a.per, i, x, y, z, oa[c], ob[c], vb);
-      }
+          for (int c = 0; c < C; ++c)
+            store_face_pair<T>(a.fout + (long long)c * L.np, i, L.nx, L.ny, L.nz, L.sy, L.sx, permask, x, y, z, oa[c], ob[c], vb);
+        } else {
 #pragma unroll
-      for (int c = 0; c < C; ++c) {
-        prev[c] = ctr[c];
-        ctr[c] = nxt[c];
+          for (int c = 0; c < C; ++c) store_pair(outp + (long long)c * L.np, 0, oa[c], ob[c], vb);
+        }
       }
-      ppi = cpi;
-      cpi = npi;
+      outp += L.sx;
+    };
+
+    take(P0, nullptr);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty[0]);   // the plane below the chunk is only needed for its centres
+    take(P1, &P0);
+
+    // the march, unrolled by three so that the planes keep their registers while their roles rotate
+    int sc = 1 % NSTAGE;
+    auto next_stage = [&]() { if (++sc == NSTAGE) sc = 0; };
+    int p = 0;
+    for (; p + 3 <= nplanes; p += 3) {
+      plane(x0 + p, sc, P0, P1, P2); next_stage();
+      plane(x0 + p + 1, sc, P1, P2, P0); next_stage();
+      plane(x0 + p + 2, sc, P2, P0, P1); next_stage();
     }
+    if (p < nplanes) { plane(x0 + p, sc, P0, P1, P2); next_stage(); ++p; }
+    if (p < nplanes) { plane(x0 + p, sc, P1, P2, P0); next_stage(); ++p; }
   }
   block_reduce_finalize<NRED, FIN_STEP, NMOM>(acc, red, a.partials, a.ctl, a.fid, a.vacf, a.vacf_stride, a.zscale, gridDim.x,
                                               blockIdx.x);

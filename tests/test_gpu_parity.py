@@ -201,6 +201,91 @@ def test_arbitrary_initial_magnetisation_and_relaxation(lpc, oracle_mod):
     assert np.abs(got / got.sum() - pi).max() < np.abs(rho0 / rho0.sum() - pi).max() * 0.5
 
 
+# ---------------------------------------------------------------------------------------------
+# equilibration loop against oracle O9
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("shape,bc,precision", [((24, 20, 70), (1, 0, 0), 0), ((17, 9, 33), (0, 0, 0), 0),
+                                                ((24, 20, 70), (0, 1, 0), 1)])
+def test_equilibration_loop_matches_oracle(lpc, oracle_mod, shape, bc, precision):
+    lat = lpc_inputs.random_small(shape, bc=bc, p_block=0.25, alpha=0.9, seed=31)
+    tol = 1e-5 if precision else 1e-10
+    rng = np.random.default_rng(4)
+    opn = lat.blocked == 0
+    rho0 = rng.random(lat.shape) * opn
+    rho0 /= rho0.sum()
+    orc = oracle_mod.Oracle.from_lattice(lat, n_moments=0, max_steps=8)
+    pi = orc.pi()
+    # a threshold the loop crosses after a few dozen sweeps, placed mid-way between two oracle deltas so
+    # that rounding cannot move the stopping iteration (both sides decide in fp64 on an fp64 delta)
+    _, _, dl = orc.equilibrate(rho0, 0.0, 60)
+    k_stop = 41
+    thr = float(np.sqrt(dl[k_stop - 1] * dl[k_stop - 2]))
+    assert dl[k_stop - 1] < thr < dl[k_stop - 2] and np.all(dl[: k_stop - 1] > thr)
+    rho_o, it_o, deltas = orc.equilibrate(rho0, thr, 5000)
+    assert it_o == k_stop
+
+    gpu = lpc.Lattice.from_inputs(lat, precision=precision, n_density=1, max_steps=8)
+    gpu.set_state(lpc.LPC_FIELD_RHO, rho0)
+    it_g, d_g = gpu.equilibrate(thr, 5000, 1)
+    if precision == 0:
+        assert it_g == it_o
+        assert abs(d_g - deltas[-1]) <= tol * rho0.max()
+        assert np.max(np.abs(gpu.field(lpc.LPC_FIELD_RHO) - rho_o)) <= tol * rho0.max()
+    else:
+        # fp32 storage: the per-sweep delta is resolved to about 1e-7 rho, compare the state at equal sweeps
+        want = orc.propagate_real(rho0, it_g)
+        assert np.max(np.abs(gpu.field(lpc.LPC_FIELD_RHO) - want)) <= tol * rho0.max()
+    assert abs(gpu.field(lpc.LPC_FIELD_RHO).sum() - 1.0) <= (1e-5 if precision else 1e-12)
+    # the magnetisation and its series are untouched
+    assert gpu.steps_done == 0 and abs(gpu.fid()[0] - 1.0) < (1e-5 if precision else 1e-13)
+    assert np.max(np.abs(gpu.field(lpc.LPC_FIELD_G) - pi)[opn] / pi[opn]) < (1e-5 if precision else 1e-13)
+
+    # host checks every 7 sweeps: stops at the first multiple of 7 at or after the paper's stopping sweep
+    gpu.set_state(lpc.LPC_FIELD_RHO, rho0)
+    it7, d7 = gpu.equilibrate(thr, 5000, 7)
+    if precision == 0:
+        assert it7 == 7 * ((it_o + 6) // 7)
+    want = orc.propagate_real(rho0, it7)
+    assert np.max(np.abs(gpu.field(lpc.LPC_FIELD_RHO) - want)) <= tol * rho0.max()
+    # iteration cap, even and odd (the density ends in either ping-pong buffer)
+    for cap in (3, 4):
+        gpu.set_state(lpc.LPC_FIELD_RHO, rho0)
+        itc, dc = gpu.equilibrate(0.0, cap, 1)
+        assert itc == cap
+        assert abs(dc - dl[cap - 1]) <= tol * rho0.max()
+        assert np.max(np.abs(gpu.field(lpc.LPC_FIELD_RHO) - orc.propagate_real(rho0, cap))) <= tol * rho0.max()
+    assert gpu.equilibrate(1.0, 0, 1)[0] == 0
+
+    # Fig. 3: the equilibrated density starts the propagation loop
+    gpu.set_state(lpc.LPC_FIELD_RHO, rho0)
+    it_g, _ = gpu.equilibrate(thr, 5000, 1)
+    rho_g = gpu.field(lpc.LPC_FIELD_RHO)
+    gpu.seed_from_density()
+    assert abs(gpu.fid()[0] - rho_g.sum()) <= 1e-12
+    gpu.step(8)
+    orc.set_g(rho_g.astype(np.complex128))
+    orc.step(8)
+    G_o, sabs = orc.fid(with_scale=True)
+    assert np.max(np.abs(gpu.fid() - G_o) / sabs) <= (1e-5 if precision else 1e-9)
+    assert np.max(np.abs(gpu.field(lpc.LPC_FIELD_G) - orc.g())) <= tol * rho0.max()
+
+
+def test_equilibration_errors(lpc):
+    lat = lpc_inputs.random_small((8, 8, 8), seed=32)
+    gpu = lpc.Lattice.from_inputs(lat, n_density=0, max_steps=2)
+    with pytest.raises(lpc.LpcError) as e:
+        gpu.equilibrate(1e-9, 10)
+    assert e.value.code == lpc.LPC_ESTATE
+    with pytest.raises(lpc.LpcError) as e:
+        gpu.seed_from_density()
+    assert e.value.code == lpc.LPC_ESTATE
+    gpu = lpc.Lattice.from_inputs(lat, n_density=1, max_steps=2)
+    for bad in ((1e-9, -1, 1), (1e-9, 10, 0), (float("nan"), 10, 1)):
+        with pytest.raises(lpc.LpcError) as e:
+            gpu.equilibrate(*bad)
+        assert e.value.code == lpc.LPC_EINVAL
+
+
 def test_device_resident_inputs_give_the_same_result(lpc):
     import torch
 
@@ -286,6 +371,49 @@ def test_bench_size_properties(lpc):
     assert abs(g.sum() - G[-1]) < 1e-12
     del gpu, g
     torch.cuda.empty_cache()
+
+
+def test_bench_workload_sampled_sites_against_oracle(lpc, oracle_mod):
+    """The bench workload itself (512^3 sweep lattice, launch configuration of bench.py), sampled outputs.
+
+    g_i(n) depends only on the sites within n hops of i (Eq. 13, is a nearest-neighbour
+    recurrence) and on dF one site further (Eq. 1).  The oracle therefore reproduces g_i(n) exactly on a
+    (2n+5)^3 box cut around i (walls n+2 sites away cannot reach the centre in n steps); only the
+    normalisation of Eq. 2 differs, by the known factor Z_box / Z_lattice.
+    """
+    import torch
+
+    L, n = 512, 6
+    lat = lpc_inputs.sweep(L)
+    gpu = lpc.Lattice.from_inputs(lat, max_steps=n)
+    gpu.step(n)
+    g_gpu = gpu.field(lpc.LPC_FIELD_G)
+    del gpu
+    torch.cuda.empty_cache()
+    opn = lat.blocked == 0
+    z_full = np.exp(-lat.dF[opn]).sum()
+    r = n + 2
+    rng = np.random.default_rng(77)
+    sites = [(0, 0, 0), (L - 1, L - 1, L - 1), (0, 255, L - 1), (L - 1, 0, 256), (63, 64, 65), (7, 8, 63), (300, 7, 64)]
+    sites += [tuple(int(v) for v in rng.integers(0, L, 3)) for _ in range(9)]
+    checked = 0
+    for c in sites:
+        # nearest open site along z so that the sample carries a value
+        while lat.blocked[c]:
+            c = (c[0], c[1], (c[2] + 1) % L)
+        ix = [(c[d] + np.arange(-r, r + 1)) % L for d in range(3)]
+        sub = np.ix_(*ix)
+        dF, blk, om = (np.ascontiguousarray(a[sub]) for a in (lat.dF, lat.blocked, lat.omega))
+        orc = oracle_mod.Oracle(dF.shape, (1, 1, 1), lat.dt, lat.a, lat.alpha, dF, blk, om, n_moments=0, max_steps=n)
+        orc.step(n)
+        z_box = np.exp(-dF[blk == 0]).sum()
+        want = orc.g()[r, r, r] * (z_box / z_full)
+        pi_c = np.exp(-lat.dF[c]) / z_full
+        err = abs(g_gpu[c] - want) / pi_c
+        assert err <= 1e-10, f"site {c}: scaled error {err:.3e}"
+        assert abs(want) > 0
+        checked += 1
+    assert checked == len(sites)
 
 
 # ---------------------------------------------------------------------------------------------

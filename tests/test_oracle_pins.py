@@ -256,6 +256,50 @@ def test_p4_bipartite_lattice_never_relaxes_at_alpha_one(oracle_mod):
 
 
 # --------------------------------------------------------------------------
+# P13 equilibration loop (O9): closed-form iteration count and deltas on a single Fourier mode
+# --------------------------------------------------------------------------
+@pytest.mark.parametrize("alpha,L,thr", [(0.6, 12, 1e-9), (0.9, 8, 3e-7), (0.3, 16, 1e-6)])
+def test_p13_equilibration_loop_single_mode_closed_form(oracle_mod, alpha, L, thr):
+    """Homogeneous periodic lattice, rho(0) = 1/N + eps cos(2 pi x / L): the cosine is an eigenvector of W
+    with eigenvalue lam = 1 - (alpha/3)(1 - cos(2 pi / L)) (one hop in +-x with probability alpha/6 each),
+    so delta(k) = max_i |rho_i(k) - rho_i(k-1)| = eps (1 - lam) lam^(k-1) exactly, and the loop of
+    PAPER.md:190-194 stops at the first k with delta(k) < threshold."""
+    lat = _uniform((L, 4, 4), alpha=alpha)
+    o = _mk(oracle_mod, lat)
+    N, eps = L * 16, 1e-3
+    x = np.arange(L)[:, None, None]
+    rho0 = 1.0 / N + eps / N * np.cos(2 * np.pi * x / L) * np.ones(lat.shape)
+    lam = 1.0 - (alpha / 3.0) * (1.0 - np.cos(2 * np.pi / L))
+    k = np.arange(1, 5000)
+    want_delta = eps / N * (1.0 - lam) * lam ** (k - 1)
+    want_iters = int(k[np.argmax(want_delta < thr / N)])
+    rho, iters, deltas = o.equilibrate(rho0, thr / N, 5000)
+    assert iters == want_iters and 3 < iters < 4000
+    # delta is a difference of nearly equal densities: it is exact to a few spacings of rho, not of delta
+    assert np.max(np.abs(deltas - want_delta[:iters])) < 8 * np.spacing(rho0.max())
+    assert abs(rho.sum() - rho0.sum()) < 1e-12
+    want_rho = 1.0 / N + eps / N * lam ** iters * np.cos(2 * np.pi * x / L) * np.ones(lat.shape)
+    assert np.max(np.abs(rho - want_rho)) < 1e-13 / N
+    # the iteration cap is honoured and reported
+    _, it2, d2 = o.equilibrate(rho0, 0.0, 7)
+    assert it2 == 7 and d2.shape == (7,)
+    _, it0, _ = o.equilibrate(rho0, 1.0, 0)
+    assert it0 == 0
+
+
+def test_p13_equilibration_reaches_boltzmann(oracle_mod):
+    """From a flat density the loop ends at the Boltzmann density of Eq. 2 on a connected lattice."""
+    lat = lpc_inputs.random_small((6, 6, 6), p_block=0.0, alpha=0.9, seed=5, dF_span=2.0)
+    o = _mk(oracle_mod, lat)
+    rho0 = np.full(lat.shape, 1.0 / lat.n_sites)
+    rho, iters, deltas = o.equilibrate(rho0, 1e-15, 100000)
+    assert 10 < iters < 100000 and deltas[-1] < 1e-15 and np.all(deltas[:-1] >= 1e-15)
+    want = np.exp(-lat.dF)
+    want /= want.sum()
+    assert np.max(np.abs(rho - want) / want) < 1e-9
+
+
+# --------------------------------------------------------------------------
 # P5 free diffusion closed form (Eq. 6, Eq. 7) -- golden values
 # --------------------------------------------------------------------------
 def _golden(name):
