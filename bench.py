@@ -6,9 +6,9 @@
 One "step" is one lattice time step: the whole hot path (propagate + phase-rotate +
 FID reduce) over every site of the lattice.  The workload is
 the configuration the north star quotes its target on: the 512^3 lattice of
-BASELINE.json configs[4] (monolith statistics, fp64, NMR kernel alone).  It is 8.6 GB
-of state and parameters, far larger than the 126 MB L2, so no L2 flush is needed
-between steps.
+BASELINE.json configs[4] (monolith statistics, fp64, NMR kernel alone).  One step
+moves 7.5 GB of state and parameters, far more than the 126 MB L2, so no L2 flush is
+needed between steps.
 
 N > 1 (torchrun): the path is benchmarked as independent replicas, one lattice per
 GPU, no data-path collective; value = all ranks' site updates
@@ -256,8 +256,8 @@ def run_ours(args):
             "dtype": "f32" if args.precision else "f64", "data": "synthetic",
             "config": {"workload": workload_name(L, args.moments, args.precision), "lattice": list(lat.shape),
                        "sites": n_sites, "parallelism": f"{world} independent replica(s), no collective",
-                       "l2": "working set 8.6 GB per step >> 126 MB L2, no flush needed" if L >= 256 else
-                             "working set may fit L2: not an HBM measurement",
+                       "l2": (f"working set {bps * n_sites / 1e9:.2f} GB per step >> 126 MB L2, no flush needed"
+                              if bps * n_sites > 4 * 126e6 else "working set is L2-sized: not an HBM measurement"),
                        "kernel": {0: "auto (tma)", 1: "direct", 2: "tma"}[args.kernel]},
             "clocks": clocks,
             "e2e": e2e,
