@@ -64,7 +64,7 @@ typedef struct lpc_config {
                        /*    fp64 reductions                                                    */
   int32_t n_moments;   /* 0, or 3 to propagate P^x, P^y, P^z for the VACF / D (Eq. 4)           */
   int32_t n_density;   /* 0, or 1 to propagate a real density rho alongside      */
-  int32_t reserved;    /* must be 0                                                             */
+  int32_t n_regions;   /* 0, or 1..8 regions ("blocks") for a region-resolved FID        */
   double dt;           /* time step in s (5e-6)                                   */
   double a;            /* lattice spacing; D comes out in a^2 / dt units of it    */
   double alpha;        /* global jump factor in (0,1], Eq. 7                 */
@@ -86,8 +86,8 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
 
 /* Site-parameter precompute (north star (a); Eq. 1, Eq. 2, Eq. 13 phase, Eq. 5):
  *   pi_i = exp(-dF_i) / sum_j exp(-dF_j) on open sites, 0 on blocked ones;
- *   packed hop data: pi_i and kappa_i = (alpha/6) / pi_i, from which every hop probability
- *   follows as p(i->j) = kappa_i * min(pi_i, pi_j)  (= (alpha/6) min(1, exp(-(dF_j - dF_i))));
+ *   packed hop data: pi_i alone, from which every hop probability follows in the sweep as
+ *   p(i->j) = kappa_i * min(pi_i, pi_j), kappa_i = (alpha/6) / pi_i  (= (alpha/6) min(1, exp(-(dF_j - dF_i))));
  *   phase factors cos(omega_i dt), sin(omega_i dt);
  *   initial state g(0) = pi (or g0), P^d(1), Z_d[1], rho(0) = pi, G[0].
  * dF_kT, omega_rad_s: host or device, N doubles.  blocked: host or device, N bytes (non-zero =
@@ -142,6 +142,31 @@ int lpc_equilibrate(lpc_lattice* lat, double threshold, int64_t max_iters, int64
  * the step counter and the G series (Fig. 3: the equilibrated densities feed the propagation
  * loop).  Synchronises.  Errors: LPC_ESTATE, LPC_ECUDA.                           */
 int lpc_seed_from_density(lpc_lattice* lat);
+
+/* Region labels for the region-resolved FID (the paper's electrode / bulk "blocks", PAPER.md:180,
+ * and the signal of "different parts" of the system, Fig. 9, :275-281; needs n_regions >= 1).
+ * region[i] in 0..n_regions-1 puts site i into that region, any other value into none.  From this
+ * call on every step also reduces G_r[n] = sum_{i in r} g_i(n) (Eq. 12, :137, restricted to r) with
+ * one extra pass over the state; G_r[steps_done] is computed at once.  lpc_set_site_params drops the
+ * labels; lpc_set_state(G) and lpc_seed_from_density restart the regional series with the G series.
+ * region: host or device, N bytes.  Synchronises.
+ * Errors: LPC_ESTATE (n_regions == 0 or no parameters), LPC_EINVAL, LPC_ECUDA.                  */
+int lpc_set_regions(lpc_lattice* lat, const uint8_t* region);
+
+/* Copy G_r[first .. first+count) of one region to the host as interleaved (re, im) doubles; the
+ * series starts at the step at which lpc_set_regions was called.  Synchronises.
+ * Errors: LPC_ESTATE (no labels), LPC_EINVAL (region or range), LPC_ECUDA.                       */
+int lpc_read_fid_region(lpc_lattice* lat, int32_t region, int64_t first, int64_t count, double* out_re_im_host);
+
+/* Spectrum of a FID series (Eq. 9, "Fourier transformed", :202) on a frequency grid:
+ *   F(f_k) = dt * sum_{n=0}^{count-1} G[n] exp(-pi lb n dt) exp(-2 pi i f_k n dt),  f_k = f0 + k df,
+ * k = 0..n_freq-1 (Hz; delta in ppm = f / (nu_0 * 1e-6)); lb_hz >= 0 is an optional Lorentzian line
+ * broadening, 0 = the plain sum.  region = -1 takes the FID of the whole lattice, 0..n_regions-1 a
+ * regional one (which must have been recorded from step 0).  count <= steps_done + 1.
+ * out_re_im_host: host, 2*n_freq doubles.  Synchronises.
+ * Errors: LPC_ESTATE, LPC_EINVAL, LPC_ECUDA.                                                    */
+int lpc_spectrum(lpc_lattice* lat, int32_t region, int64_t count, double f0_hz, double df_hz, int64_t n_freq,
+                 double lb_hz, double* out_re_im_host);
 
 /* Choose the step kernel (LPC_KERNEL_*).  AUTO picks TMA.  Errors: LPC_EINVAL.                 */
 int lpc_set_kernel(lpc_lattice* lat, int32_t which);

@@ -142,6 +142,20 @@ class Oracle:
         assert it >= 0
         return rho.reshape(self.shape), it, deltas[:it]
 
+    def step_with_regions(self, region, n_regions, n_steps):
+        """Region-resolved FID (PAPER.md:180 blocks, Fig. 9 :275-281): Eq. 12 (:137) restricted to each
+        region, G_r[k] = sum_{i in r} g_i(k), for k = current step .. current step + n_steps, taken from the
+        site values after every single step.  Returns an array [n_regions, n_steps + 1]."""
+        region = np.asarray(region).reshape(self.shape)
+        out = np.zeros((n_regions, n_steps + 1), dtype=np.complex128)
+        for k in range(n_steps + 1):
+            if k:
+                self.step(1)
+            g = self.g()
+            for r in range(n_regions):
+                out[r, k] = g[region == r].sum()
+        return out
+
     def _get(self, fn, *a):
         out = np.empty(self.n, dtype=np.float64)
         fn(self._h, *a, _d(out))
@@ -185,3 +199,16 @@ class Oracle:
         if _lib.lpco_get_moments(self._h, int(count), _d(vacf), _d(D)) != 0:
             raise ValueError("lpco_get_moments: range or no moments")
         return vacf, D
+
+
+def spectrum(G, dt, freqs_hz, lb_hz=0.0):
+    """Eq. 9, F(f) = int G(t) exp(-2 i pi f t) dt, as the plain sum over the samples
+    (reading Q23): F(f) = dt * sum_n G[n] exp(-pi lb n dt) exp(-2 pi i f n dt).  lb_hz is an
+    optional Lorentzian line broadening (0 = none).  One frequency at a time, written out."""
+    G = np.asarray(G, dtype=np.complex128)
+    t = np.arange(G.size) * float(dt)
+    w = np.exp(-np.pi * float(lb_hz) * t)
+    out = np.empty(len(freqs_hz), dtype=np.complex128)
+    for k, f in enumerate(np.asarray(freqs_hz, dtype=np.float64)):
+        out[k] = float(dt) * np.sum(G * w * np.exp(-2j * np.pi * f * t))
+    return out

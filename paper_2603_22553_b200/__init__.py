@@ -24,7 +24,7 @@ LPC_KERNEL_AUTO, LPC_KERNEL_DIRECT, LPC_KERNEL_TMA = range(3)
 
 EXPORTS = (
     "lpc_workspace_bytes", "lpc_create_lattice", "lpc_set_site_params", "lpc_step_n", "lpc_read_fid",
-    "lpc_moments", "lpc_read_field", "lpc_set_state", "lpc_equilibrate", "lpc_seed_from_density", "lpc_set_kernel",
+    "lpc_moments", "lpc_read_field", "lpc_set_state", "lpc_equilibrate", "lpc_seed_from_density", "lpc_set_regions", "lpc_read_fid_region", "lpc_spectrum", "lpc_set_kernel",
     "lpc_steps_done",
     "lpc_launch_count", "lpc_bytes_per_site_step", "lpc_destroy", "lpc_last_error",
 )
@@ -39,7 +39,7 @@ class LpcError(RuntimeError):
 class lpc_config(C.Structure):
     _fields_ = [
         ("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("bc", C.c_int32 * 3),
-        ("precision", C.c_int32), ("n_moments", C.c_int32), ("n_density", C.c_int32), ("reserved", C.c_int32),
+        ("precision", C.c_int32), ("n_moments", C.c_int32), ("n_density", C.c_int32), ("n_regions", C.c_int32),
         ("dt", C.c_double), ("a", C.c_double), ("alpha", C.c_double),
         ("max_steps", C.c_int64), ("stream", C.c_void_p),
     ]
@@ -69,6 +69,9 @@ def _load():
     lib.lpc_set_kernel.argtypes = [C.c_void_p, C.c_int32]
     lib.lpc_equilibrate.argtypes = [C.c_void_p, C.c_double, C.c_int64, C.c_int64, C.POINTER(C.c_int64), C.POINTER(C.c_double)]
     lib.lpc_seed_from_density.argtypes = [C.c_void_p]
+    lib.lpc_set_regions.argtypes = [C.c_void_p, C.c_void_p]
+    lib.lpc_read_fid_region.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_int64, C.c_void_p]
+    lib.lpc_spectrum.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_double, C.c_double, C.c_int64, C.c_double, C.c_void_p]
     lib.lpc_steps_done.argtypes = [C.c_void_p]
     lib.lpc_steps_done.restype = C.c_int64
     lib.lpc_launch_count.argtypes = [C.c_void_p]
@@ -121,9 +124,9 @@ def _ptr(x, dtype=None, count=None):
 
 
 def make_config(nx, ny, nz, bc=(0, 0, 0), precision=0, n_moments=0, n_density=0, dt=5e-6, a=1.0, alpha=1.0,
-                max_steps=0, stream=None) -> lpc_config:
+                max_steps=0, stream=None, n_regions=0) -> lpc_config:
     return lpc_config(int(nx), int(ny), int(nz), (C.c_int32 * 3)(*[int(b) for b in bc]), int(precision),
-                      int(n_moments), int(n_density), 0, float(dt), float(a), float(alpha), int(max_steps),
+                      int(n_moments), int(n_density), int(n_regions), float(dt), float(a), float(alpha), int(max_steps),
                       C.c_void_p(stream) if stream else None)
 
 
@@ -190,6 +193,28 @@ def lpc_seed_from_density(handle):
     _check(_lib.lpc_seed_from_density(handle))
 
 
+def lpc_set_regions(handle, region):
+    _check(_lib.lpc_set_regions(handle, _ptr(region)))
+
+
+def lpc_read_fid_region(handle, region, first=0, count=None):
+    if count is None:
+        count = int(_lib.lpc_steps_done(handle)) + 1 - first
+    out = np.empty(count, dtype=np.complex128)
+    _check(_lib.lpc_read_fid_region(handle, int(region), int(first), int(count), C.c_void_p(out.ctypes.data)))
+    return out
+
+
+def lpc_spectrum(handle, f0_hz, df_hz, n_freq, lb_hz=0.0, region=-1, count=None):
+    """F(f0 + k df), k = 0..n_freq-1, of G[0..count) (Eq. 9); region = -1 takes the whole lattice."""
+    if count is None:
+        count = int(_lib.lpc_steps_done(handle)) + 1
+    out = np.empty(max(int(n_freq), 0), dtype=np.complex128)
+    _check(_lib.lpc_spectrum(handle, int(region), int(count), float(f0_hz), float(df_hz), int(n_freq), float(lb_hz),
+                             C.c_void_p(out.ctypes.data)))
+    return out
+
+
 def lpc_set_kernel(handle, which):
     _check(_lib.lpc_set_kernel(handle, int(which)))
 
@@ -214,7 +239,7 @@ class Lattice:
     """Owns the torch workspace and the handle; methods forward to the C calls one to one."""
 
     def __init__(self, shape, bc=(0, 0, 0), precision=0, n_moments=0, n_density=0, dt=5e-6, a=1.0, alpha=1.0,
-                 max_steps=0, device="cuda:0", stream=None):
+                 max_steps=0, device="cuda:0", stream=None, n_regions=0):
         import torch
 
         self.shape = tuple(int(v) for v in shape)
@@ -224,19 +249,20 @@ class Lattice:
             stream = torch.cuda.current_stream(self.device)
         self.stream = stream
         self.cfg = make_config(*self.shape, bc=bc, precision=precision, n_moments=n_moments, n_density=n_density,
-                               dt=dt, a=a, alpha=alpha, max_steps=max_steps, stream=stream.cuda_stream)
+                               dt=dt, a=a, alpha=alpha, max_steps=max_steps, stream=stream.cuda_stream, n_regions=n_regions)
         self.workspace_bytes = lpc_workspace_bytes(self.cfg)
         with torch.cuda.device(self.device):
             self.workspace = torch.empty(self.workspace_bytes, dtype=torch.uint8, device=self.device)
             self.handle = lpc_create_lattice(self.cfg, self.workspace)
 
     @classmethod
-    def from_inputs(cls, lat, precision=0, n_moments=None, n_density=0, max_steps=None, device="cuda:0", g0=None):
+    def from_inputs(cls, lat, precision=0, n_moments=None, n_density=0, max_steps=None, device="cuda:0", g0=None,
+                    n_regions=0):
         """Build from an ``lpc_inputs.Lattice`` (host arrays) and run the precompute."""
         self = cls(lat.shape, bc=lat.bc, precision=precision,
                    n_moments=lat.n_moments if n_moments is None else n_moments, n_density=n_density,
                    dt=lat.dt, a=lat.a, alpha=lat.alpha,
-                   max_steps=lat.n_steps if max_steps is None else max_steps, device=device)
+                   max_steps=lat.n_steps if max_steps is None else max_steps, device=device, n_regions=n_regions)
         self.set_site_params(lat.dF, lat.blocked, lat.omega, g0)
         return self
 
@@ -283,6 +309,17 @@ class Lattice:
 
     def seed_from_density(self):
         lpc_seed_from_density(self.handle)
+
+    def set_regions(self, region):
+        if isinstance(region, np.ndarray):
+            region = np.ascontiguousarray(region, dtype=np.uint8)
+        lpc_set_regions(self.handle, region)
+
+    def fid_region(self, region, first=0, count=None):
+        return lpc_read_fid_region(self.handle, region, first, count)
+
+    def spectrum(self, f0_hz, df_hz, n_freq, lb_hz=0.0, region=-1, count=None):
+        return lpc_spectrum(self.handle, f0_hz, df_hz, n_freq, lb_hz, region, count)
 
     def set_kernel(self, which):
         lpc_set_kernel(self.handle, which)

@@ -19,6 +19,7 @@
 #include "lpc_precompute.cuh"
 #include "lpc_step.cuh"
 #include "lpc_equil.cuh"
+#include "lpc_regions.cuh"
 
 using namespace lpc;
 
@@ -46,9 +47,10 @@ size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 constexpr int DIRECT_MAX_BLOCKS = 148 * 8;
 constexpr int AUX_BLOCKS = 148 * 8;
 constexpr long long STAGE_SITES = 4ll << 20;  // sites per host<->device staging chunk
+constexpr long long SPEC_BATCH = 4096;        // frequencies per spectrum launch
 
 struct Offsets {
-  size_t ctl, fid, vacf, partials, pi, cs, f0, f1, staging, total;
+  size_t ctl, fid, vacf, partials, pi, cs, f0, f1, regions, fidr, rpartials, spec, staging, total;
   size_t partial_slots;
 };
 
@@ -63,6 +65,8 @@ struct lpc_lattice {
   unsigned char* ws;
   cudaStream_t stream;
   bool have_params;
+  bool have_regions;
+  long long region_first;  // first sample of the regional series
   int cur;  // index of the buffer holding the current state
   long long steps;
   long long launches;
@@ -84,7 +88,7 @@ int check_cfg(const lpc_config* c) {
   if (c->precision != 0 && c->precision != 1) return fail(LPC_EINVAL, "precision must be 0 (fp64) or 1 (fp32)");
   if (c->n_moments != 0 && c->n_moments != 3) return fail(LPC_EINVAL, "n_moments must be 0 or 3");
   if (c->n_density != 0 && c->n_density != 1) return fail(LPC_EINVAL, "n_density must be 0 or 1");
-  if (c->reserved != 0) return fail(LPC_EINVAL, "reserved must be 0");
+  if (c->n_regions < 0 || c->n_regions > MAX_REGIONS) return fail(LPC_EINVAL, "n_regions must lie in [0, %d]", MAX_REGIONS);
   if (!(c->alpha > 0.0 && c->alpha <= 1.0)) return fail(LPC_EINVAL, "alpha must lie in (0,1]");
   if (!(c->dt > 0.0) || !std::isfinite(c->dt)) return fail(LPC_EINVAL, "dt must be positive");
   if (!(c->a > 0.0) || !std::isfinite(c->a)) return fail(LPC_EINVAL, "a must be positive");
@@ -156,6 +160,10 @@ Offsets make_offsets(const lpc_config* c, const Layout& L) {
   o.cs = p; p += align_up((size_t)2 * L.np * sT);
   o.f0 = p; p += align_up((size_t)C * L.np * sT);
   o.f1 = p; p += align_up((size_t)C * L.np * sT);
+  o.regions = p; p += align_up(c->n_regions ? (size_t)N : 0);
+  o.fidr = p; p += align_up((size_t)c->n_regions * (c->max_steps + 1) * sizeof(double2));
+  o.rpartials = p; p += align_up(c->n_regions ? (size_t)AUX_BLOCKS * 2 * MAX_REGIONS * sizeof(double) : 0);
+  o.spec = p; p += align_up((size_t)SPEC_BATCH * sizeof(double2));
   o.staging = p; p += align_up((size_t)std::min<long long>(N, STAGE_SITES) * 16);
   o.total = p;
   return o;
@@ -281,6 +289,21 @@ int for_chunks_in(lpc_lattice* h, const void* src, size_t bytes_per_site, F body
     CUDA_TRY(cudaStreamSynchronize(h->stream));
   }
   return LPC_OK;
+}
+
+// G_r[sample] of every region from the current state
+template <typename T>
+int region_reduce_t(lpc_lattice* h, long long sample) {
+  region_reduce_kernel<T><<<aux_grid(h->N), 256, 0, h->stream>>>(
+      h->L, wsp<T>(h, h->off.pi), wsp<T>(h, h->cur ? h->off.f1 : h->off.f0), h->ws + h->off.regions, h->cfg.n_regions,
+      wsp<double>(h, h->off.rpartials), wsp<Ctl>(h, h->off.ctl), wsp<double2>(h, h->off.fidr), h->cfg.max_steps + 1, sample);
+  CUDA_TRY(cudaGetLastError());
+  h->launches++;
+  return LPC_OK;
+}
+
+int region_reduce(lpc_lattice* h, long long sample) {
+  return h->cfg.precision ? region_reduce_t<float>(h, sample) : region_reduce_t<double>(h, sample);
 }
 
 template <typename T>
@@ -441,6 +464,11 @@ int set_state_t(lpc_lattice* h, int which, const void* in) {
     rc = set_g_from<T>(h, in);
     if (rc) return rc;
     h->steps = 0;
+    if (h->have_regions) {
+      h->region_first = 0;
+      rc = region_reduce_t<T>(h, 0);
+      if (rc) return rc;
+    }
   } else if (which == LPC_FIELD_RHO) {
     if (h->nrho != 1) return fail(LPC_ESTATE, "the density field is not propagated (n_density = 0)");
     T* ch = wsp<T>(h, h->cur ? h->off.f1 : h->off.f0) + 2 * h->L.np;
@@ -512,8 +540,13 @@ int seed_from_density_t(lpc_lattice* h) {
                                                              wsp<Ctl>(h, h->off.ctl), wsp<double2>(h, h->off.fid));
   CUDA_TRY(cudaGetLastError());
   h->launches++;
-  CUDA_TRY(cudaStreamSynchronize(h->stream));
   h->steps = 0;
+  if (h->have_regions) {
+    h->region_first = 0;
+    int rc = region_reduce_t<T>(h, 0);
+    if (rc) return rc;
+  }
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
   return LPC_OK;
 }
 
@@ -567,6 +600,8 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
   h->ws = static_cast<unsigned char*>(workspace_dev);
   h->stream = static_cast<cudaStream_t>(cfg->stream);
   h->have_params = false;
+  h->have_regions = false;
+  h->region_first = 0;
   h->cur = 0;
   h->steps = 0;
   h->launches = 0;
@@ -601,6 +636,7 @@ int lpc_set_site_params(lpc_lattice* h, const double* dF, const uint8_t* blocked
   if (!h) return fail(LPC_EINVAL, "lattice is NULL");
   if (!dF || !blocked || !omega) return fail(LPC_EINVAL, "dF, blocked and omega must not be NULL");
   h->have_params = false;
+  h->have_regions = false;
   return h->cfg.precision ? set_site_params_t<float>(h, dF, blocked, omega, g0) : set_site_params_t<double>(h, dF, blocked, omega, g0);
 }
 
@@ -613,6 +649,10 @@ int lpc_step_n(lpc_lattice* h, int64_t n) {
     int rc = h->cfg.precision ? launch_step<float>(h) : launch_step<double>(h);
     if (rc) return rc;
     h->steps++;
+    if (h->have_regions) {
+      rc = region_reduce(h, h->steps);
+      if (rc) return rc;
+    }
   }
   return LPC_OK;
 }
@@ -681,6 +721,65 @@ int lpc_seed_from_density(lpc_lattice* h) {
   return h->cfg.precision ? seed_from_density_t<float>(h) : seed_from_density_t<double>(h);
 }
 
+int lpc_set_regions(lpc_lattice* h, const uint8_t* region) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
+  if (h->cfg.n_regions < 1) return fail(LPC_ESTATE, "the lattice was created with n_regions = 0");
+  if (!region) return fail(LPC_EINVAL, "region is NULL");
+  CUDA_TRY(cudaMemcpyAsync(h->ws + h->off.regions, region, (size_t)h->N, cudaMemcpyDefault, h->stream));
+  h->have_regions = true;
+  h->region_first = h->steps;
+  int rc = region_reduce(h, h->steps);
+  if (rc) return rc;
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return LPC_OK;
+}
+
+int lpc_read_fid_region(lpc_lattice* h, int32_t region, int64_t first, int64_t count, double* out) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
+  if (!h->have_regions) return fail(LPC_ESTATE, "lpc_set_regions has not been called");
+  if (region < 0 || region >= h->cfg.n_regions) return fail(LPC_EINVAL, "region %d is outside [0, %d)", region, h->cfg.n_regions);
+  if (first < h->region_first || count < 0 || first + count > h->steps + 1)
+    return fail(LPC_EINVAL, "range [%lld, %lld) is outside the recorded samples [%lld, %lld]", (long long)first, (long long)(first + count),
+                h->region_first, (long long)h->steps);
+  if (count > 0 && !out) return fail(LPC_EINVAL, "out is NULL");
+  if (count > 0)
+    CUDA_TRY(cudaMemcpyAsync(out, wsp<double2>(h, h->off.fidr) + (size_t)region * (h->cfg.max_steps + 1) + first,
+                             (size_t)count * sizeof(double2), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return LPC_OK;
+}
+
+int lpc_spectrum(lpc_lattice* h, int32_t region, int64_t count, double f0, double df, int64_t n_freq, double lb, double* out) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
+  if (count < 1 || count > h->steps + 1) return fail(LPC_EINVAL, "count must lie in [1, steps_done + 1]");
+  if (n_freq < 0) return fail(LPC_EINVAL, "n_freq must be >= 0");
+  if (!(lb >= 0.0) || !std::isfinite(f0) || !std::isfinite(df)) return fail(LPC_EINVAL, "lb must be >= 0 and the frequency grid finite");
+  if (n_freq > 0 && !out) return fail(LPC_EINVAL, "out is NULL");
+  const double2* series;
+  if (region == -1) {
+    series = wsp<double2>(h, h->off.fid);
+  } else {
+    if (!h->have_regions) return fail(LPC_ESTATE, "lpc_set_regions has not been called");
+    if (region < 0 || region >= h->cfg.n_regions) return fail(LPC_EINVAL, "region %d is outside [-1, %d)", region, h->cfg.n_regions);
+    if (h->region_first != 0) return fail(LPC_ESTATE, "the regional series starts at step %lld, not 0", h->region_first);
+    series = wsp<double2>(h, h->off.fidr) + (size_t)region * (h->cfg.max_steps + 1);
+  }
+  double2* spec = wsp<double2>(h, h->off.spec);
+  for (int64_t k0 = 0; k0 < n_freq; k0 += SPEC_BATCH) {
+    const int64_t nb = std::min<int64_t>(SPEC_BATCH, n_freq - k0);
+    spectrum_kernel<<<(unsigned)nb, 256, 0, h->stream>>>(series, count, h->cfg.dt, f0, df, k0, lb, spec);
+    CUDA_TRY(cudaGetLastError());
+    h->launches++;
+    CUDA_TRY(cudaMemcpyAsync(out + 2 * k0, spec, (size_t)nb * sizeof(double2), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+  }
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return LPC_OK;
+}
+
 int lpc_set_kernel(lpc_lattice* h, int32_t which) {
   if (!h) return fail(LPC_EINVAL, "lattice is NULL");
   if (which < LPC_KERNEL_AUTO || which > LPC_KERNEL_TMA) return fail(LPC_EINVAL, "unknown kernel selector %d", which);
@@ -694,8 +793,9 @@ int64_t lpc_launch_count(const lpc_lattice* h) { return h ? h->launches : 0; }
 
 double lpc_bytes_per_site_step(const lpc_lattice* h) {
   if (!h) return 0.0;
-  // read C state channels + pi + cos + sin, write C state channels
-  return (double)h->sT * (2.0 * h->C + 3.0);
+  // read C state channels + pi + cos + sin, write C state channels; with region labels one more pass
+  // reads h (2 channels), pi and the label
+  return (double)h->sT * (2.0 * h->C + 3.0) + (h->have_regions ? 3.0 * h->sT + 1.0 : 0.0);
 }
 
 void lpc_destroy(lpc_lattice* h) { delete h; }

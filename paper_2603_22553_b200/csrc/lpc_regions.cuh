@@ -1,0 +1,112 @@
+// lpc_regions.cuh -- region-resolved FID and the spectrum.
+//
+// The paper splits the system into "blocks" (electrodes, bulk) and plots the NMR signal of
+// "different parts" of it (Fig. 9, :275-281).  A region is a per-site label 0..n_regions-1 (any other
+// value = in no region); the regional FID is Eq. 12 (:137) restricted to the region,
+//     G_r[n] = sum_{i in r} g_i(n),
+// and the spectrum is Eq. 9 (:115) of a FID series on a caller-chosen frequency grid.
+#pragma once
+
+#include "lpc_internal.cuh"
+#include "lpc_precompute.cuh"
+
+namespace lpc {
+
+constexpr int MAX_REGIONS = 8;
+
+// G_r[sample] for all regions: one pass over the current state (16 B) + pi (8 B) + label (1 B) per site.
+// Per-thread accumulators are selected by predicate (no indexed registers), reduced per warp and block,
+// and the last block sums the block partials in a fixed order.
+template <typename T>
+__global__ void __launch_bounds__(256)
+    region_reduce_kernel(Layout L, const T* __restrict__ pi, const T* __restrict__ f, const uint8_t* __restrict__ label, int n_regions,
+                         double* partials, Ctl* ctl, double2* fidr, long long stride, long long sample) {
+  double ar[MAX_REGIONS], ai[MAX_REGIONS];
+#pragma unroll
+  for (int r = 0; r < MAX_REGIONS; ++r) ar[r] = ai[r] = 0.0;
+  const long long n = (long long)L.nx * L.ny * L.nz;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+    const long long j = dense_to_padded(L, i);
+    const double p = (double)pi[j];
+    const double gr = p * (double)f[j], gi = p * (double)f[L.np + j];
+    const int lab = label[i];
+#pragma unroll
+    for (int r = 0; r < MAX_REGIONS; ++r) {
+      ar[r] += (lab == r) ? gr : 0.0;
+      ai[r] += (lab == r) ? gi : 0.0;
+    }
+  }
+  __shared__ double red[8][2 * MAX_REGIONS];
+  __shared__ unsigned int s_last;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int r = 0; r < MAX_REGIONS; ++r) {
+    const double vr = warp_sum(ar[r]), vi = warp_sum(ai[r]);
+    if (lane == 0) {
+      red[warp][2 * r] = vr;
+      red[warp][2 * r + 1] = vi;
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x < 2 * MAX_REGIONS) {
+    double v = 0.0;
+    for (int w = 0; w < 8; ++w) v += red[w][threadIdx.x];
+    partials[(size_t)blockIdx.x * 2 * MAX_REGIONS + threadIdx.x] = v;
+    __threadfence();
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) s_last = (atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1);
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  // 16 threads, one per (region, re/im), each sums its column of the partials in block order
+  if (threadIdx.x < 2 * MAX_REGIONS) {
+    double v = 0.0;
+    for (unsigned int b = 0; b < gridDim.x; ++b) v += __ldcg(&partials[(size_t)b * 2 * MAX_REGIONS + threadIdx.x]);
+    const int r = threadIdx.x >> 1;
+    if (r < n_regions) reinterpret_cast<double*>(fidr + r * stride + sample)[threadIdx.x & 1] = v;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    ctl->ticket = 0;
+    __threadfence();
+  }
+}
+
+// F(f_k) = dt * sum_{n=0}^{M-1} G[n] exp(-pi lb n dt) exp(-2 pi i f_k n dt),  f_k = f0 + k df
+// (Eq. 9, as a plain discrete sum over the samples; lb = Lorentzian line broadening in Hz,
+// 0 = none).  One block per frequency, fixed summation order.
+__global__ void __launch_bounds__(256)
+    spectrum_kernel(const double2* __restrict__ series, long long M, double dt, double f0, double df, long long k0, double lb,
+                    double2* __restrict__ out) {
+  const double f = f0 + (double)(k0 + blockIdx.x) * df;
+  double sr = 0.0, si = 0.0;
+  for (long long n = threadIdx.x; n < M; n += blockDim.x) {
+    const double t = (double)n * dt;
+    double s, c;
+    sincospi(2.0 * f * t, &s, &c);        // e^{-2 pi i f t} = c - i s
+    const double w = exp(-M_PI * lb * t);
+    const double2 g = series[n];
+    sr += w * (g.x * c + g.y * s);
+    si += w * (g.y * c - g.x * s);
+  }
+  __shared__ double red[8][2];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  sr = warp_sum(sr);
+  si = warp_sum(si);
+  if (lane == 0) {
+    red[warp][0] = sr;
+    red[warp][1] = si;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double a = 0.0, b = 0.0;
+    for (int w = 0; w < 8; ++w) {
+      a += red[w][0];
+      b += red[w][1];
+    }
+    out[blockIdx.x] = make_double2(dt * a, dt * b);
+  }
+}
+
+}  // namespace lpc

@@ -286,6 +286,89 @@ def test_equilibration_errors(lpc):
         assert e.value.code == lpc.LPC_EINVAL
 
 
+# ---------------------------------------------------------------------------------------------
+# region-resolved FID and spectrum (Eq. 9 :115)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel,precision", [(1, 0), (2, 0), (2, 1)])
+def test_regional_fid_and_spectrum_match_oracle(lpc, oracle_mod, kernel, precision):
+    import torch
+
+    lat = lpc_inputs.supercap(96, 24, 70, n_steps=120)        # electrodes | bulk | electrodes along x
+    n, nreg = 120, 3
+    tol = 1e-5 if precision else 1e-9
+    x = np.arange(lat.nx)[:, None, None] * np.ones(lat.shape, dtype=int)
+    region = np.where(x < lat.nx * 3 // 8, 0, np.where(x < lat.nx * 5 // 8, 1, 2)).astype(np.uint8)
+    region[:, 0, 0] = 200                                     # a few sites in no region
+    gpu = lpc.Lattice.from_inputs(lat, precision=precision, max_steps=n, n_regions=nreg)
+    gpu.set_kernel(kernel)
+    gpu.set_regions(region)
+    assert gpu.bytes_per_site_step == (4 if precision else 8) * 10 + 1
+    gpu.step(n)
+    orc = oracle_mod.Oracle.from_lattice(lat, n_moments=0, max_steps=n)
+    Gr_o = orc.step_with_regions(region, nreg, n)
+    _, sabs = orc.fid(with_scale=True)
+    for r in range(nreg):
+        Gr_g = gpu.fid_region(r)
+        assert Gr_g.shape == (n + 1,)
+        assert np.max(np.abs(Gr_g - Gr_o[r]) / sabs) <= tol, f"region {r}"
+    # the whole-lattice FID is what it is without regions, and the regions never exceed it
+    assert np.max(np.abs(gpu.fid() - orc.fid()) / sabs) <= tol
+    # spectra: whole lattice and one region, with and without line broadening, against Eq. 9 written out
+    f0, df, nf = -4500.0, 37.5, 161
+    freqs = f0 + df * np.arange(nf)
+    for reg, series in ((-1, orc.fid()), (0, Gr_o[0]), (2, Gr_o[2])):
+        for lb in (0.0, 200.0):
+            want = oracle_mod.spectrum(series, lat.dt, freqs, lb)
+            got = gpu.spectrum(f0, df, nf, lb, region=reg)
+            scale = lat.dt * np.abs(series).sum()
+            assert np.max(np.abs(got - want)) <= tol * scale, f"spectrum region {reg} lb {lb}"
+    # a shorter record, device-resident labels, and a restart of both series from a new initial state
+    want = oracle_mod.spectrum(orc.fid()[:50], lat.dt, freqs[:7], 0.0)
+    assert np.max(np.abs(gpu.spectrum(f0, df, 7, 0.0, count=50) - want)) <= tol * lat.dt * 50
+    gpu.set_regions(torch.from_numpy(region).cuda())
+    assert np.max(np.abs(gpu.fid_region(1, first=n, count=1) - Gr_o[1][n:]) / sabs[n:]) <= tol
+    with pytest.raises(lpc.LpcError) as e:
+        gpu.fid_region(1, first=0, count=5)                   # recorded from step n only now
+    assert e.value.code == lpc.LPC_EINVAL
+    with pytest.raises(lpc.LpcError) as e:
+        gpu.spectrum(f0, df, 3, region=1)
+    assert e.value.code == lpc.LPC_ESTATE
+    g0 = orc.g()
+    gpu.set_state(lpc.LPC_FIELD_G, g0)
+    assert gpu.steps_done == 0
+    for r in range(nreg):
+        assert abs(gpu.fid_region(r, 0, 1)[0] - Gr_o[r][n]) <= tol * sabs[n]
+
+
+def test_regional_fid_large_spectrum_batches_and_errors(lpc):
+    lat = lpc_inputs.random_small((12, 10, 20), seed=43, p_block=0.1)
+    lat.omega[...] = -2 * np.pi * 2500.0
+    n = 64
+    gpu = lpc.Lattice.from_inputs(lat, max_steps=n, n_regions=0)
+    with pytest.raises(lpc.LpcError) as e:
+        gpu.set_regions(np.zeros(lat.shape, dtype=np.uint8))
+    assert e.value.code == lpc.LPC_ESTATE
+    gpu.step(n)
+    # uniform shift: G[n] = exp(i w n dt) (Eq. 8), whose spectrum is the geometric sum in closed form;
+    # 9000 frequencies span three launches of the spectrum kernel
+    nf, f0, df = 9000, -5000.0, 1.0
+    f = f0 + df * np.arange(nf)
+    q = np.exp(1j * (-2 * np.pi * 2500.0 - 2 * np.pi * f) * lat.dt)
+    with np.errstate(invalid="ignore", divide="ignore"):
+        want = lat.dt * np.where(np.abs(1 - q) < 1e-14, n + 1, (1 - q ** (n + 1)) / (1 - q))
+    got = gpu.spectrum(f0, df, nf)
+    assert np.max(np.abs(got - want)) <= 1e-9 * lat.dt * (n + 1)
+    assert abs(f[np.argmax(got.real)] + 2500.0) <= df
+    for bad in (dict(n_freq=-1), dict(lb_hz=-1.0), dict(count=n + 2), dict(count=0), dict(region=0)):
+        kw = dict(f0_hz=0.0, df_hz=1.0, n_freq=4)
+        kw.update(bad)
+        with pytest.raises(lpc.LpcError):
+            gpu.spectrum(**kw)
+    with pytest.raises(lpc.LpcError) as e:
+        lpc.make_config(8, 8, 8, n_regions=9) and lpc.lpc_workspace_bytes(lpc.make_config(8, 8, 8, n_regions=9))
+    assert e.value.code == lpc.LPC_EINVAL
+
+
 def test_device_resident_inputs_give_the_same_result(lpc):
     import torch
 

@@ -300,6 +300,57 @@ def test_p13_equilibration_reaches_boltzmann(oracle_mod):
 
 
 # --------------------------------------------------------------------------
+# P14 spectrum (Eq. 9) and P15 region-resolved FID
+# --------------------------------------------------------------------------
+def test_p14_spectrum_single_line_closed_form_and_fft(oracle_mod):
+    """G[n] = exp((i w0 - 1/T2) n dt) sums to a geometric series: F(f) = dt (1 - q^M)/(1 - q),
+    q = exp((i (w0 - 2 pi f) - 1/T2 - pi lb) dt); on the grid f_k = k/(M dt) the sum is numpy's FFT."""
+    dt, M, w0, T2 = 5e-6, 400, -2 * np.pi * 3200.0, 4e-4
+    n = np.arange(M)
+    G = np.exp((1j * w0 - 1.0 / T2) * n * dt)
+    f = np.array([-3200.0, -3000.0, 0.0, 1234.5, 99000.0])
+    for lb in (0.0, 150.0):
+        q = np.exp((1j * (w0 - 2 * np.pi * f) - 1.0 / T2 - np.pi * lb) * dt)
+        want = dt * (1 - q ** M) / (1 - q)
+        got = oracle_mod.spectrum(G, dt, f, lb)
+        assert np.max(np.abs(got - want)) < 1e-12 * np.abs(want).max()
+    # the line sits at f = w0 / 2 pi, and the broadening lowers and widens it (Lorentzian: height ~ 1/(1/T2 + pi lb))
+    grid = np.linspace(-6400.0, 0.0, 257)
+    s0, s1 = oracle_mod.spectrum(G, dt, grid, 0.0), oracle_mod.spectrum(G, dt, grid, 800.0)
+    assert grid[np.argmax(s0.real)] == -3200.0 and grid[np.argmax(s1.real)] == -3200.0
+    assert s1.real.max() < 0.6 * s0.real.max()
+    fk = np.arange(M) / (M * dt)
+    assert np.max(np.abs(oracle_mod.spectrum(G, dt, fk) - dt * np.fft.fft(G))) < 1e-12 * M * dt
+
+
+def test_p15_regional_fid_closed_form_on_sealed_pockets(oracle_mod):
+    """Two pore pockets sealed from each other by carbon, each with its own uniform shift: nothing crosses
+    the wall, so G_r[n] = (sum_{i in r} pi_i) exp(i w_r n dt) whatever dF is inside (Eq. 8 on each pocket),
+    and the regions add up to G."""
+    lat = lpc_inputs.random_small((10, 6, 6), bc=(1, 0, 0), p_block=0.2, alpha=0.8, seed=41, dF_span=2.0)
+    lat.blocked[4:6] = 1                      # the wall
+    region = np.zeros(lat.shape, dtype=np.uint8)
+    region[5:] = 1
+    w = (-9000.0, 4000.0)
+    lat.omega[:5], lat.omega[5:] = w
+    n = 60
+    o = _mk(oracle_mod, lat, max_steps=n)
+    pi = o.pi()
+    Gr = o.step_with_regions(region, 2, n)
+    k = np.arange(n + 1)
+    for r in range(2):
+        mass = pi[region == r].sum()
+        assert 0.2 < mass < 0.8
+        assert np.max(np.abs(Gr[r] - mass * np.exp(1j * w[r] * lat.dt * k))) < 1e-13
+    assert np.max(np.abs(Gr.sum(axis=0) - o.fid())) < 1e-14
+    # a label outside 0..n_regions-1 belongs to no region
+    region[0] = 7
+    o2 = _mk(oracle_mod, lat, max_steps=3)
+    Gr2 = o2.step_with_regions(region, 2, 3)
+    assert np.max(np.abs(Gr2[1] - Gr[1][:4])) < 1e-15 and np.all(np.abs(Gr2[0]) < np.abs(Gr[0][:4]))
+
+
+# --------------------------------------------------------------------------
 # P5 free diffusion closed form (Eq. 6, Eq. 7) -- golden values
 # --------------------------------------------------------------------------
 def _golden(name):
