@@ -74,7 +74,7 @@ struct lpc_lattice {
   // TMA geometry
   int ty, tz, nstage, xc, tiles_z, tiles_y, chunks_x;
   bool tma_ok;
-  CUtensorMap tm_f[2], tm_pi, tm_cs;
+  CUtensorMap tm_f[2], tm_m[2], tm_pi, tm_cs;  // tm_f: magnetisation (+ density) channels, tm_m: the 3 moment channels
 };
 
 namespace {
@@ -110,18 +110,19 @@ Layout make_layout(const lpc_config* c) {
   return L;
 }
 
-// TMA tile geometry: 8 x 64 tiles of the y-z plane, 8 warps per CTA; two CTAs per
-// SM up to 3 channels, one with 5.  (16 x 64 tiles with one 16-warp CTA per SM measured the same at 512^3
+// TMA tile geometry: 8 x 64 tiles of the y-z plane, 8 warps per CTA, two CTAs per
+// SM (a sweep carries at most 3 channels: the moment fields have a sweep of their own).  (16 x 64 tiles with one 16-warp CTA per SM measured the same at 512^3
 // and slightly worse at 256^3, so there is one tile shape.)
 constexpr int SM_COUNT = 148;
 
 void tma_geometry(int C, int nx, int ny, int nz, int* ty, int* tz, int* nstage, int* xc, int* tiles_z, int* tiles_y, int* chunks_x) {
   *ty = 8; *tz = 64;
-  *nstage = (C <= 3) ? 4 : 3;
+  *nstage = 4;   // 3 when the density rides along (3 channels); informational, the kernels fix it
   *tiles_z = (nz + *tz - 1) / *tz;
   *tiles_y = (ny + *ty - 1) / *ty;
   const long long tiles = (long long)*tiles_z * *tiles_y;
-  const long long resident = (long long)SM_COUNT * ((C <= 3) ? 2 : 1);
+  const long long resident = (long long)SM_COUNT * 2;   // every TMA sweep carries at most 3 channels
+  (void)C;
   // Split x into chunks of about 32 planes.  Measured on 512^3 fp64 (ms per step, xc = 8 / 16 / 24 / 32 /
   // 48 / 74 / 128 / 256): 1.44 / 1.32 / 1.29 / 1.29 / 1.32 / 1.38 / 1.49 / 1.55 -- long chunks keep all SMs
   // marching through the same planes in lockstep, which makes the DRAM traffic come in read bursts and
@@ -239,24 +240,40 @@ int launch_step_t(lpc_lattice* h) {
 
   const bool use_tma = h->tma_ok && h->kernel != LPC_KERNEL_DIRECT;
   if (use_tma) {
-    constexpr int C = 2 + NRHO + NMOM;
     const unsigned grid = (unsigned)(h->tiles_z * h->tiles_y * h->chunks_x);
-    auto launch = [&](auto kern, auto cfg) -> int {
+    auto launch = [&](auto kern, auto cfg, const CUtensorMap& tm, const StepArgs<T>& args) -> int {
       using K = decltype(cfg);
       static bool attr_set = false;
       if (!attr_set) {
         CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, K::SMEM_BYTES));
         attr_set = true;
       }
-      kern<<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(h->tm_f[h->cur], h->tm_pi, h->tm_cs, a);
+      kern<<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(tm, h->tm_pi, h->tm_cs, args);
+      CUDA_TRY(cudaGetLastError());
+      h->launches++;
       return LPC_OK;
     };
-    constexpr int NS = (C <= 3) ? 4 : 3;
-    int rc = launch(step_tma_kernel<T, NRHO, NMOM, 8, 64, NS>, TmaCfg<T, NRHO, NMOM, 8, 64, NS>());
+    // With moment fields the step is two sweeps over the same pair of buffers: the three moment
+    // channels first (Z_d[k+1], P^d <- W P^d; no phase, no cos/sin traffic), then the magnetisation
+    // (and density) channels, which also advance the step counter.  One 5-channel sweep needs more
+    // than 200 registers per thread and leaves one 8-warp CTA per SM (measured 42 GLUPS at 512^3).
+    if constexpr (NMOM == 3) {
+      StepArgs<T> am = a;
+      am.c0 = 2 + NRHO;
+      am.fout = a.fout + (long long)am.c0 * h->L.np;
+      int rc = launch(step_tma_kernel<T, 0, 0, 3, 8, 64, 4>, TmaCfg<T, 0, 0, 3, 8, 64, 4>(), h->tm_m[h->cur], am);
+      if (rc) return rc;
+    }
+    a.c0 = 0;
+    constexpr int NS = (NRHO == 0) ? 4 : 3;   // two CTAs per SM must fit in shared memory
+    int rc = launch(step_tma_kernel<T, 2, NRHO, 0, 8, 64, NS>, TmaCfg<T, 2, NRHO, 0, 8, 64, NS>(), h->tm_f[h->cur], a);
     if (rc) return rc;
+    h->cur ^= 1;
+    return LPC_OK;
   } else {
     const long long npairs = (long long)((h->L.nz + 1) / 2) * h->L.ny * h->L.nx;
     const int grid = (int)std::max<long long>(1, std::min<long long>((npairs + 255) / 256, DIRECT_MAX_BLOCKS));
+    a.c0 = 0;
     step_direct_kernel<T, NRHO, NMOM><<<grid, 256, 0, h->stream>>>(a);
   }
   CUDA_TRY(cudaGetLastError());
@@ -619,8 +636,13 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
     const cuuint32_t b4[4] = {(cuuint32_t)(h->tz + 2 * (16 / h->sT)), (cuuint32_t)(h->ty + 2), 1, (cuuint32_t)h->C};
     const cuuint64_t dk[4] = {(cuuint64_t)L.nzp, (cuuint64_t)L.nyp, (cuuint64_t)L.nxp, 2};
     const cuuint32_t bk[4] = {(cuuint32_t)h->tz, (cuuint32_t)h->ty, 1, 2};
-    rc = encode_map(&h->tm_f[0], f32, h->ws + h->off.f0, 4, d4, b4);
-    if (!rc) rc = encode_map(&h->tm_f[1], f32, h->ws + h->off.f1, 4, d4, b4);
+    // the channel dimension of the box: the magnetisation (+ density) channels, and the 3 moment channels
+    const cuuint32_t bf[4] = {b4[0], b4[1], 1, (cuuint32_t)(2 + h->nrho)};
+    const cuuint32_t bm[4] = {b4[0], b4[1], 1, 3};
+    rc = encode_map(&h->tm_f[0], f32, h->ws + h->off.f0, 4, d4, bf);
+    if (!rc) rc = encode_map(&h->tm_f[1], f32, h->ws + h->off.f1, 4, d4, bf);
+    if (!rc && h->nmom == 3) rc = encode_map(&h->tm_m[0], f32, h->ws + h->off.f0, 4, d4, bm);
+    if (!rc && h->nmom == 3) rc = encode_map(&h->tm_m[1], f32, h->ws + h->off.f1, 4, d4, bm);
     if (!rc) rc = encode_map(&h->tm_pi, f32, h->ws + h->off.pi, 3, d4, b4);
     if (!rc) rc = encode_map(&h->tm_cs, f32, h->ws + h->off.cs, 4, dk, bk);
     if (rc) {

@@ -130,9 +130,10 @@ __global__ void __launch_bounds__(256) step_direct_kernel(StepArgs<T> a) {
 // ---------------------------------------------------------------------------------------------
 // TMA kernel.
 // ---------------------------------------------------------------------------------------------
-template <typename T, int NRHO, int NMOM, int TY, int TZ, int NSTAGE>
+// NH = 2: the sweep carries the magnetisation (h_re, h_im, phase multiply, G); NH = 0: real channels only.
+template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE>
 struct TmaCfg {
-  static constexpr int C = 2 + NRHO + NMOM;
+  static constexpr int C = NH + NRHO + NMOM;
   static constexpr int NRED = 2 + NMOM;
   static constexpr int HZ = 16 / (int)sizeof(T);  // z halo of 16 bytes on each side keeps the centre pairs 16-byte aligned
   static constexpr int TZW = TZ + 2 * HZ;
@@ -142,7 +143,7 @@ struct TmaCfg {
   static constexpr int NTHREADS = NCONS;      // no producer warp: thread 0 issues the TMA loads between planes
   static constexpr int F_RAW = C * TYH * TZW * (int)sizeof(T);
   static constexpr int PI_RAW = TYH * TZW * (int)sizeof(T);
-  static constexpr int KCS_RAW = 2 * TY * TZ * (int)sizeof(T);  // cos, sin (no halo)
+  static constexpr int KCS_RAW = NH * TY * TZ * (int)sizeof(T);  // cos, sin (no halo); none without the magnetisation
   static constexpr int F_BYTES = (F_RAW + 127) / 128 * 128;
   static constexpr int PI_BYTES = (PI_RAW + 127) / 128 * 128;
   static constexpr int KCS_BYTES = (KCS_RAW + 127) / 128 * 128;
@@ -158,11 +159,11 @@ struct TmaCfg {
   static_assert(TZ % 2 == 0, "TZ must be even");
 };
 
-template <typename T, int NRHO, int NMOM, int TY, int TZ, int NSTAGE>
-__global__ void __launch_bounds__(TmaCfg<T, NRHO, NMOM, TY, TZ, NSTAGE>::LB_THREADS, TmaCfg<T, NRHO, NMOM, TY, TZ, NSTAGE>::LB_CTAS)
+template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE>
+__global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE>::LB_THREADS, TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE>::LB_CTAS)
     step_tma_kernel(const __grid_constant__ CUtensorMap tm_f, const __grid_constant__ CUtensorMap tm_pi,
                     const __grid_constant__ CUtensorMap tm_cs, StepArgs<T> a) {
-  using K = TmaCfg<T, NRHO, NMOM, TY, TZ, NSTAGE>;
+  using K = TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE>;
   using V2 = typename Vec2<T>::type;
   constexpr int C = K::C, NRED = K::NRED, TZW = K::TZW, TYH = K::TYH, HZ = K::HZ;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -200,10 +201,10 @@ __global__ void __launch_bounds__(TmaCfg<T, NRHO, NMOM, TY, TZ, NSTAGE>::LB_THRE
     const int s = jl % NSTAGE;
     if (jl >= NSTAGE) mbar_wait(&empty[s], ((jl / NSTAGE) - 1) & 1);   // every warp is done with the plane it held
     unsigned char* st = smem + s * K::STAGE_BYTES;
-    const bool need_kcs = (jl >= 1 && jl <= nplanes);
+    const bool need_kcs = (NH == 2) && (jl >= 1 && jl <= nplanes);
     mbar_expect_tx(&full[s], K::F_RAW + K::PI_RAW + (need_kcs ? K::KCS_RAW : 0));
     // plane x0-1+j lives at padded x coordinate x0+j; box starts HZ columns / 1 row before the tile
-    tma_load_4d(st, &tm_f, &full[s], L.padz + z0 - HZ, y0, x0 + jl, 0);
+    tma_load_4d(st, &tm_f, &full[s], L.padz + z0 - HZ, y0, x0 + jl, a.c0);
     tma_load_3d(st + K::F_BYTES, &tm_pi, &full[s], L.padz + z0 - HZ, y0, x0 + jl);
     if (need_kcs) tma_load_4d(st + K::F_BYTES + K::PI_BYTES, &tm_cs, &full[s], L.padz + z0, y0 + 1, x0 + jl, 0);
     ++jl;
@@ -265,8 +266,11 @@ __global__ void __launch_bounds__(TmaCfg<T, NRHO, NMOM, TY, TZ, NSTAGE>::LB_THRE
       const T* sf = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES);
       const T* sp = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES + K::F_BYTES);
       const T* sk = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES + K::F_BYTES + K::PI_BYTES);
-      const V2 csv = *reinterpret_cast<const V2*>(sk + ek);
-      const V2 snv = *reinterpret_cast<const V2*>(sk + TY * TZ + ek);
+      V2 csv, snv;
+      if (NH == 2) {
+        csv = *reinterpret_cast<const V2*>(sk + ek);
+        snv = *reinterpret_cast<const V2*>(sk + TY * TZ + ek);
+      }
       const V2 pym = *reinterpret_cast<const V2*>(sp + ec - TZW);
       const V2 pyp = *reinterpret_cast<const V2*>(sp + ec + TZW);
       const T pzm = sp[ec - 1], pzp = sp[ec + 2];
@@ -290,8 +294,8 @@ __global__ void __launch_bounds__(TmaCfg<T, NRHO, NMOM, TY, TZ, NSTAGE>::LB_THRE
         const V2 fym = *reinterpret_cast<const V2*>(fcn + ec - TZW);
         const V2 fyp = *reinterpret_cast<const V2*>(fcn + ec + TZW);
         const T fzm = fcn[ec - 1], fzp = fcn[ec + 2];
-        if (NMOM == 3 && c >= 2 + NRHO) {
-          const int d = c - 2 - NRHO;
+        if (NMOM == 3 && c >= NH + NRHO) {
+          const int d = c - NH - NRHO;
           const T dma = (d == 0) ? (ua.mxp - ua.mxm) : (d == 1) ? (ua.myp - ua.mym) : (ua.mzp - ua.mzm);
           const T dmb = (d == 0) ? (ub.mxp - ub.mxm) : (d == 1) ? (ub.myp - ub.mym) : (ub.mzp - ub.mzm);
           double t = 0.0;
@@ -306,7 +310,7 @@ __global__ void __launch_bounds__(TmaCfg<T, NRHO, NMOM, TY, TZ, NSTAGE>::LB_THRE
       __syncwarp();
       if (lane == 0) mbar_arrive(&empty[sc]);
 
-      {
+      if (NH == 2) {
         const T ar = oa[0], ai = oa[1], br = ob[0], bi = ob[1];
         oa[0] = csv.x * ar - snv.x * ai;
         oa[1] = csv.x * ai + snv.x * ar;
@@ -314,11 +318,13 @@ __global__ void __launch_bounds__(TmaCfg<T, NRHO, NMOM, TY, TZ, NSTAGE>::LB_THRE
         ob[1] = csv.y * bi + snv.y * br;
       }
       if (va) {
-        acc[0] += (double)ctr.pi.x * (double)oa[0];
-        acc[1] += (double)ctr.pi.x * (double)oa[1];
-        if (vb) {
-          acc[0] += (double)ctr.pi.y * (double)ob[0];
-          acc[1] += (double)ctr.pi.y * (double)ob[1];
+        if (NH == 2) {
+          acc[0] += (double)ctr.pi.x * (double)oa[0];
+          acc[1] += (double)ctr.pi.x * (double)oa[1];
+          if (vb) {
+            acc[0] += (double)ctr.pi.y * (double)ob[0];
+            acc[1] += (double)ctr.pi.y * (double)ob[1];
+          }
         }
         if (edge_yz || (a.per[0] && (x == 0 || x == L.nx - 1))) {
           const long long i = L.idx(x, y, z);
@@ -350,7 +356,7 @@ __global__ void __launch_bounds__(TmaCfg<T, NRHO, NMOM, TY, TZ, NSTAGE>::LB_THRE
     if (p < nplanes) { plane(x0 + p, sc, P0, P1, P2); next_stage(); ++p; }
     if (p < nplanes) { plane(x0 + p, sc, P1, P2, P0); next_stage(); ++p; }
   }
-  block_reduce_finalize<NRED, FIN_STEP, NMOM>(acc, red, a.partials, a.ctl, a.fid, a.vacf, a.vacf_stride, a.zscale, gridDim.x,
+  block_reduce_finalize<NRED, (NH == 2) ? FIN_STEP : FIN_MOM, NMOM>(acc, red, a.partials, a.ctl, a.fid, a.vacf, a.vacf_stride, a.zscale, gridDim.x,
                                               blockIdx.x);
 }
 
