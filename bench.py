@@ -46,9 +46,12 @@ def parse():
     p.add_argument("--warmup", type=int, default=100)
     p.add_argument("--impl", default="ours", choices=["ours", "reference"])
     p.add_argument("--size", type=int, default=512, help="lattice edge L of the L^3 workload")
+    p.add_argument("--workload", default="sweep", choices=["sweep", "config0", "particle", "monolith", "supercap"],
+                   help="sweep: configs[4] L^3 (default, the headline workload); the others are BASELINE.json configs[0..3] "
+                        "at their full sizes (particle 128^3, monolith 256^3 + moment fields, supercap 2048x256x256)")
     p.add_argument("--moments", type=int, default=0, choices=[0, 3], help="also propagate the 3 VACF fields")
     p.add_argument("--precision", type=int, default=0, choices=[0, 1])
-    p.add_argument("--kernel", type=int, default=0, choices=[0, 1, 2])
+    p.add_argument("--kernel", type=int, default=0, choices=[0, 1, 2, 3])
     p.add_argument("--no-cpu-baseline", action="store_true")
     p.add_argument("--no-e2e", action="store_true")
     p.add_argument("--ref-sample-size", type=int, default=int(os.environ.get("LPC_REF_SAMPLE_L", "256")),
@@ -65,9 +68,27 @@ def load_oracle():
     return mod
 
 
-def workload_name(L, moments, precision):
-    return (f"configs[4] sweep: {L}^3 periodic, monolith statistics (Gaussian pore field ell=8, 20% blocked), "
-            f"{'fp32' if precision else 'fp64'}, {'NMR + 3 moment fields' if moments else 'NMR kernel alone'}")
+def workload_name(L, moments, precision, workload="sweep"):
+    tail = f"{'fp32' if precision else 'fp64'}, {'NMR + 3 moment fields' if moments else 'NMR kernel alone'}"
+    if workload == "sweep":
+        return f"configs[4] sweep: {L}^3 periodic, monolith statistics (Gaussian pore field ell=8, 20% blocked), {tail}"
+    return {"config0": "configs[0]: 32^3 periodic, 30% blocked iid, dF ~ U[-3,0] kT, delta ~ U[-10,0] ppm",
+            "particle": "configs[1] single porous carbon particle: 128^3 periodic, sphere R=48 porous (ell=4, 10% blocked), bulk outside",
+            "monolith": "configs[2] carbon monolith: 256^3 periodic, pore field ell=8, 20% blocked",
+            "supercap": "configs[3] supercapacitor cell: 2048x256x256, reflective x, two film electrodes + bulk"}[workload] + ", " + tail
+
+
+def make_workload(args):
+    """The seeded synthetic lattice of the chosen workload (lpc_inputs) and its moment-field count."""
+    if args.workload == "sweep":
+        return lpc_inputs.sweep(args.size, n_moments=args.moments)
+    if args.workload == "config0":
+        return lpc_inputs.config0(n_moments=args.moments)
+    if args.workload == "particle":
+        return lpc_inputs.particle(n_moments=args.moments)
+    if args.workload == "monolith":
+        return lpc_inputs.monolith(n_moments=args.moments)
+    return lpc_inputs.supercap(n_moments=args.moments)
 
 
 # --------------------------------------------------------------------------------------------
@@ -171,7 +192,7 @@ def run_ours(args):
     dev = f"cuda:{local}"
 
     L, K, W = args.size, args.steps, args.warmup
-    lat = lpc_inputs.sweep(L, n_moments=args.moments)
+    lat = make_workload(args)
     n_sites = lat.n_sites
     # pinned host buffers: the inputs of the end-to-end job
     host = [torch.from_numpy(a).pin_memory() for a in (lat.dF, lat.blocked, lat.omega)]
@@ -248,7 +269,7 @@ def run_ours(args):
         # (profiles/traffic.csv: key,dram_bytes_per_launch,source)
         tpath = os.path.join(ROOT, "profiles", "traffic.csv")
         if os.path.exists(tpath):
-            key = f"{L}^3/m{args.moments}/p{args.precision}"
+            key = f"{L}^3/m{args.moments}/p{args.precision}" if args.workload == "sweep" else f"{args.workload}/m{args.moments}/p{args.precision}"
             for row in open(tpath):
                 cols = row.strip().split(",")
                 if cols and cols[0] == key:
@@ -257,11 +278,11 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32" if args.precision else "f64", "data": "synthetic",
-            "config": {"workload": workload_name(L, args.moments, args.precision), "lattice": list(lat.shape),
+            "config": {"workload": workload_name(L, args.moments, args.precision, args.workload), "lattice": list(lat.shape),
                        "sites": n_sites, "parallelism": f"{world} independent replica(s), no collective",
                        "l2": (f"working set {bps * n_sites / 1e9:.2f} GB per step >> 126 MB L2, no flush needed"
                               if bps * n_sites > 4 * 126e6 else "working set is L2-sized: not an HBM measurement"),
-                       "kernel": {0: "auto (tma)", 1: "direct", 2: "tma"}[args.kernel]},
+                       "kernel": {0: "auto", 1: "direct", 2: "tma", 3: "persistent"}[args.kernel]},
             "clocks": clocks,
             "e2e": e2e,
             "gpu_launches": int(launches),

@@ -54,6 +54,8 @@ extern "C" {
 #define LPC_KERNEL_AUTO 0
 #define LPC_KERNEL_DIRECT 1 /* one thread per site pair, neighbours straight from global memory */
 #define LPC_KERNEL_TMA 2    /* TMA-staged x-marching tiles, mbarrier pipeline                  */
+#define LPC_KERNEL_PERSIST 3 /* all n steps of lpc_step_n in one cooperative launch, grid barrier
+                                between steps; for lattices that stay in L2 (launch-bound otherwise) */
 
 typedef struct lpc_lattice lpc_lattice; /* opaque, host struct owned by the library */
 
@@ -168,7 +170,8 @@ int lpc_read_fid_region(lpc_lattice* lat, int32_t region, int64_t first, int64_t
 int lpc_spectrum(lpc_lattice* lat, int32_t region, int64_t count, double f0_hz, double df_hz, int64_t n_freq,
                  double lb_hz, double* out_re_im_host);
 
-/* Choose the step kernel (LPC_KERNEL_*).  AUTO picks TMA.  Errors: LPC_EINVAL.                 */
+/* Choose the step kernel (LPC_KERNEL_*).  AUTO picks PERSIST when one step's state and parameters
+ * stay in L2 (<= 48 MB) and no region labels are set, else TMA.  Errors: LPC_EINVAL.             */
 int lpc_set_kernel(lpc_lattice* lat, int32_t which);
 
 /* Steps taken since the last lpc_set_site_params / lpc_set_state(G).                           */

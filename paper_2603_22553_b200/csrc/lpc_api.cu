@@ -282,6 +282,67 @@ int launch_step_t(lpc_lattice* h) {
   return LPC_OK;
 }
 
+// ---- all n steps in one cooperative launch (L2-resident lattices) ------------------------------
+constexpr int PERSIST_MAX_BLOCKS = SM_COUNT * 4;   // 2 * blocks * MAX_RED partials fit the partial slots
+
+template <typename T, int NRHO, int NMOM>
+int launch_persist_t(lpc_lattice* h, int64_t n) {
+  StepArgs<T> a;
+  a.L = h->L;
+  a.fin = nullptr;
+  a.fout = nullptr;
+  a.pi = wsp<T>(h, h->off.pi);
+  a.cs = wsp<T>(h, h->off.cs);
+  a.a6 = (T)(h->cfg.alpha / 6.0);
+  a.partials = wsp<double>(h, h->off.partials);
+  a.ctl = wsp<Ctl>(h, h->off.ctl);
+  a.fid = wsp<double2>(h, h->off.fid);
+  a.vacf = wsp<double>(h, h->off.vacf);
+  a.vacf_stride = h->cfg.max_steps + 2;
+  a.zscale = h->cfg.a * h->cfg.alpha / 6.0;
+  for (int d = 0; d < 3; ++d) a.per[d] = h->cfg.bc[d] == 0;
+  a.c0 = 0; a.xc = 0; a.tiles_z = a.tiles_y = a.chunks_x = 0;
+  auto kern = step_persist_kernel<T, NRHO, NMOM>;
+  static int per_sm = 0;
+  if (!per_sm) CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 256, 0));
+  if (per_sm < 1) return fail(LPC_ECUDA, "the persistent kernel does not fit on an SM");
+  const long long npairs = (long long)((h->L.nz + 1) / 2) * h->L.ny * h->L.nx;
+  const int grid = (int)std::max<long long>(1, std::min<long long>({(npairs + 255) / 256, (long long)per_sm * SM_COUNT, (long long)PERSIST_MAX_BLOCKS}));
+  unsigned long long* bar = reinterpret_cast<unsigned long long*>(&wsp<Ctl>(h, h->off.ctl)->scratch[6]);
+  T* buf_a = wsp<T>(h, h->cur ? h->off.f1 : h->off.f0);
+  T* buf_b = wsp<T>(h, h->cur ? h->off.f0 : h->off.f1);
+  while (n > 0) {
+    const int chunk = (int)std::min<int64_t>(n, 1 << 20);
+    CUDA_TRY(cudaMemsetAsync(bar, 0, sizeof(unsigned long long), h->stream));
+    int nsteps = chunk;
+    void* args[] = {&a, &buf_a, &buf_b, &nsteps, &bar};
+    CUDA_TRY(cudaLaunchCooperativeKernel(reinterpret_cast<void*>(kern), dim3(grid), dim3(256), args, 0, h->stream));
+    h->launches++;
+    if (chunk & 1) {
+      std::swap(buf_a, buf_b);
+      h->cur ^= 1;
+    }
+    h->steps += chunk;
+    n -= chunk;
+  }
+  return LPC_OK;
+}
+
+template <typename T>
+int launch_persist(lpc_lattice* h, int64_t n) {
+  if (h->nrho == 0 && h->nmom == 0) return launch_persist_t<T, 0, 0>(h, n);
+  if (h->nrho == 1 && h->nmom == 0) return launch_persist_t<T, 1, 0>(h, n);
+  if (h->nrho == 0 && h->nmom == 3) return launch_persist_t<T, 0, 3>(h, n);
+  return launch_persist_t<T, 1, 3>(h, n);
+}
+
+// AUTO takes the persistent kernel when one step's state and parameters stay in L2
+bool persist_by_default(const lpc_lattice* h) {
+  long long limit = 48ll << 20;
+  if (const char* e = getenv("LPC_PERSIST_MAX_MB")) limit = (long long)atoll(e) << 20;
+  return (long long)h->N * h->sT * (2 * h->C + 3) <= limit;
+}
+
 template <typename T>
 int launch_step(lpc_lattice* h) {
   if (h->nrho == 0 && h->nmom == 0) return launch_step_t<T, 0, 0>(h);
@@ -626,6 +687,7 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
   if (const char* e = getenv("LPC_KERNEL")) {
     if (!strcmp(e, "direct")) h->kernel = LPC_KERNEL_DIRECT;
     if (!strcmp(e, "tma")) h->kernel = LPC_KERNEL_TMA;
+    if (!strcmp(e, "persist")) h->kernel = LPC_KERNEL_PERSIST;
   }
   tma_geometry(h->C, cfg->nx, cfg->ny, cfg->nz, &h->ty, &h->tz, &h->nstage, &h->xc, &h->tiles_z, &h->tiles_y, &h->chunks_x);
   h->tma_ok = (size_t)h->tiles_z * h->tiles_y * h->chunks_x <= h->off.partial_slots;
@@ -667,6 +729,9 @@ int lpc_step_n(lpc_lattice* h, int64_t n) {
   if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
   if (n < 0) return fail(LPC_EINVAL, "n must be >= 0");
   if (h->steps + n > h->cfg.max_steps) return fail(LPC_EINVAL, "steps_done + n = %lld exceeds max_steps = %lld", (long long)(h->steps + n), (long long)h->cfg.max_steps);
+  const bool persist = !h->have_regions && n >= 2 &&
+                       (h->kernel == LPC_KERNEL_PERSIST || (h->kernel == LPC_KERNEL_AUTO && persist_by_default(h)));
+  if (persist) return h->cfg.precision ? launch_persist<float>(h, n) : launch_persist<double>(h, n);
   for (int64_t k = 0; k < n; ++k) {
     int rc = h->cfg.precision ? launch_step<float>(h) : launch_step<double>(h);
     if (rc) return rc;
@@ -804,7 +869,7 @@ int lpc_spectrum(lpc_lattice* h, int32_t region, int64_t count, double f0, doubl
 
 int lpc_set_kernel(lpc_lattice* h, int32_t which) {
   if (!h) return fail(LPC_EINVAL, "lattice is NULL");
-  if (which < LPC_KERNEL_AUTO || which > LPC_KERNEL_TMA) return fail(LPC_EINVAL, "unknown kernel selector %d", which);
+  if (which < LPC_KERNEL_AUTO || which > LPC_KERNEL_PERSIST) return fail(LPC_EINVAL, "unknown kernel selector %d", which);
   if (which == LPC_KERNEL_TMA && !h->tma_ok) return fail(LPC_EINVAL, "the TMA kernel is not available for this lattice");
   h->kernel = which;
   return LPC_OK;

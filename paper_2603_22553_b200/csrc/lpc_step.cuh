@@ -72,17 +72,21 @@ __device__ __noinline__ void store_face_pair(T* __restrict__ base, long long i, 
 // ---------------------------------------------------------------------------------------------
 // Direct kernel.
 // ---------------------------------------------------------------------------------------------
-template <typename T, int NRHO, int NMOM>
-__global__ void __launch_bounds__(256) step_direct_kernel(StepArgs<T> a) {
+// One sweep over all site pairs, grid-stride.  COHERENT reads the state with ld.global.cg (L2 only): the
+// persistent kernel needs that, because another CTA wrote those values one grid barrier ago and L1 is not
+// coherent.  The parameters (pi, cos, sin) are read-only and always go through L1.
+template <typename T, bool COHERENT>
+__device__ __forceinline__ T ld_state(const T* p) {
+  return COHERENT ? __ldcg(p) : *p;
+}
+
+template <typename T, int NRHO, int NMOM, bool COHERENT>
+__device__ __forceinline__ void direct_sweep(const StepArgs<T>& a, const T* __restrict__ fin, T* __restrict__ fout,
+                                             double (&acc)[2 + NMOM]) {
   constexpr int C = 2 + NRHO + NMOM;
-  constexpr int NRED = 2 + NMOM;
   const Layout& L = a.L;
   const long long zpairs = (L.nz + 1) / 2;
   const long long npairs = zpairs * L.ny * L.nx;
-  double acc[NRED];
-#pragma unroll
-  for (int r = 0; r < NRED; ++r) acc[r] = 0.0;
-
   const T* __restrict__ pi = a.pi;
   const T* __restrict__ csv = a.cs;
   const T* __restrict__ snv = a.cs + L.np;
@@ -103,14 +107,16 @@ __global__ void __launch_bounds__(256) step_direct_kernel(StepArgs<T> a) {
       u.weights(pi[j], pi[j - L.sx], pi[j + L.sx], pi[j - L.sy], pi[j + L.sy], pi[j - 1], pi[j + 1], a.a6, csv[j], snv[j]);
 #pragma unroll
       for (int c = 0; c < C; ++c) {
-        const T* __restrict__ f = a.fin + (long long)c * L.np;
-        const T fc = f[j];
+        const T* __restrict__ f = fin + (long long)c * L.np;
+        const T fc = ld_state<T, COHERENT>(f + j);
         if (NMOM == 3 && c >= 2 + NRHO) {
           const int d = c - 2 - NRHO;
           const T dm = (d == 0) ? (u.mxp - u.mxm) : (d == 1) ? (u.myp - u.mym) : (u.mzp - u.mzm);
           acc[2 + d] += (double)fc * (double)dm;  // P^d_i u^d_i / (a alpha/6), before propagation
         }
-        out[s][c] = u.gather(fc, f[j - L.sx], f[j + L.sx], f[j - L.sy], f[j + L.sy], f[j - 1], f[j + 1]);
+        out[s][c] = u.gather(fc, ld_state<T, COHERENT>(f + j - L.sx), ld_state<T, COHERENT>(f + j + L.sx),
+                             ld_state<T, COHERENT>(f + j - L.sy), ld_state<T, COHERENT>(f + j + L.sy),
+                             ld_state<T, COHERENT>(f + j - 1), ld_state<T, COHERENT>(f + j + 1));
       }
       const T hr = out[s][0], hi = out[s][1];
       out[s][0] = u.cs * hr - u.sn * hi;
@@ -120,11 +126,103 @@ __global__ void __launch_bounds__(256) step_direct_kernel(StepArgs<T> a) {
     }
 #pragma unroll
     for (int c = 0; c < C; ++c)
-      store_with_ghosts(a.fout + (long long)c * L.np, L, a.per, i, x, y, z, out[0][c], vb ? out[1][c] : (T)0, vb);
+      store_with_ghosts(fout + (long long)c * L.np, L, a.per, i, x, y, z, out[0][c], vb ? out[1][c] : (T)0, vb);
   }
+}
+
+template <typename T, int NRHO, int NMOM>
+__global__ void __launch_bounds__(256) step_direct_kernel(StepArgs<T> a) {
+  constexpr int NRED = 2 + NMOM;
+  double acc[NRED];
+#pragma unroll
+  for (int r = 0; r < NRED; ++r) acc[r] = 0.0;
+  direct_sweep<T, NRHO, NMOM, false>(a, a.fin, a.fout, acc);
   __shared__ double red[8 * NRED + 1];
   block_reduce_finalize<NRED, FIN_STEP, NMOM>(acc, red, a.partials, a.ctl, a.fid, a.vacf, a.vacf_stride, a.zscale, gridDim.x,
                                               blockIdx.x);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Persistent kernel for lattices whose state and parameters stay in L2: all n steps of lpc_step_n in
+// ONE cooperative launch, a grid barrier between steps instead of a kernel boundary (a launch costs
+// more than a 32^3 .. 64^3 sweep).  Same per-site arithmetic as the other kernels.  Per step: sweep ->
+// block partial into partials[step parity] -> grid barrier -> block 0 sums the partials in block order
+// and writes G[step+1] (Z_d[step+2]) while the others start the next sweep; block 0 joins the next
+// barrier only after that, so a partial slot is never overwritten while it is still being read.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void grid_barrier(unsigned long long* bar, unsigned long long target) {
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    atomicAdd(bar, 1ull);
+    unsigned long long v;
+    do {
+      asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(bar) : "memory");
+    } while (v < target);
+  }
+  __syncthreads();
+}
+
+template <typename T, int NRHO, int NMOM>
+__global__ void __launch_bounds__(256) step_persist_kernel(StepArgs<T> a, T* buf_a, T* buf_b, int nsteps, unsigned long long* bar) {
+  constexpr int NRED = 2 + NMOM;
+  __shared__ double red[8 * NRED];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const size_t slot = (size_t)gridDim.x * NRED;   // partials of one step parity
+  T* fin = buf_a;
+  T* fout = buf_b;
+  for (int s = 0; s < nsteps; ++s) {
+    double acc[NRED];
+#pragma unroll
+    for (int r = 0; r < NRED; ++r) acc[r] = 0.0;
+    direct_sweep<T, NRHO, NMOM, true>(a, fin, fout, acc);
+    double* part = a.partials + (size_t)(s & 1) * slot;
+#pragma unroll
+    for (int r = 0; r < NRED; ++r) {
+      const double v = warp_sum(acc[r]);
+      if (lane == 0) red[warp * NRED + r] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < NRED) {
+      double v = 0.0;
+      for (int w = 0; w < 8; ++w) v += red[w * NRED + threadIdx.x];
+      part[(size_t)blockIdx.x * NRED + threadIdx.x] = v;
+    }
+    grid_barrier(bar, (unsigned long long)(s + 1) * gridDim.x);
+    if (blockIdx.x == 0) {
+      // fixed-order sum of the block partials: thread r < NRED takes column r
+      double tot[NRED];
+#pragma unroll
+      for (int r = 0; r < NRED; ++r) tot[r] = 0.0;
+      for (unsigned int b = threadIdx.x; b < gridDim.x; b += blockDim.x) {
+#pragma unroll
+        for (int r = 0; r < NRED; ++r) tot[r] += __ldcg(&part[(size_t)b * NRED + r]);
+      }
+#pragma unroll
+      for (int r = 0; r < NRED; ++r) {
+        const double v = warp_sum(tot[r]);
+        if (lane == 0) red[warp * NRED + r] = v;
+      }
+      __syncthreads();
+      if (threadIdx.x == 0) {
+        double out[NRED];
+        for (int r = 0; r < NRED; ++r) {
+          double v = 0.0;
+          for (int w = 0; w < 8; ++w) v += red[w * NRED + r];
+          out[r] = v;
+        }
+        const long long st = a.ctl->step;
+        a.fid[st + 1] = make_double2(out[0], out[1]);
+        if (NMOM == 3)
+          for (int d = 0; d < 3; ++d) a.vacf[d * a.vacf_stride + st + 2] = a.zscale * out[2 + d];
+        a.ctl->step = st + 1;
+      }
+      __syncthreads();
+    }
+    T* t = fin;
+    fin = fout;
+    fout = t;
+  }
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -74,7 +74,7 @@ def _pair(lpc, oracle_mod, lat, n, kernel, n_moments=None, n_density=0, precisio
     return gpu, orc
 
 
-KERNELS = [1, 2]  # LPC_KERNEL_DIRECT, LPC_KERNEL_TMA
+KERNELS = [1, 2, 3]  # LPC_KERNEL_DIRECT, LPC_KERNEL_TMA, LPC_KERNEL_PERSIST
 
 
 # ---------------------------------------------------------------------------------------------
@@ -156,8 +156,8 @@ def test_channel_combinations_tma(lpc, oracle_mod, nm, nd):
 def test_kernels_agree_bitwise_on_state_and_are_deterministic(lpc):
     lat = lpc_inputs.random_small((48, 20, 130), bc=(1, 0, 0), p_block=0.25, seed=24, n_moments=3)
     res = []
-    for kernel in (1, 2, 2):
-        gpu = lpc.Lattice.from_inputs(lat, max_steps=30)
+    for kernel in (1, 2, 2, 3, 3):
+        gpu = lpc.Lattice.from_inputs(lat, max_steps=31)
         gpu.set_kernel(kernel)
         gpu.step(30)
         res.append((gpu.field(lpc.LPC_FIELD_G), gpu.fid(), gpu.moments()[0]))
@@ -168,6 +168,21 @@ def test_kernels_agree_bitwise_on_state_and_are_deterministic(lpc):
     assert np.array_equal(res[1][0], res[2][0])
     assert np.array_equal(res[1][1], res[2][1])
     assert np.array_equal(res[1][2], res[2][2])
+    # the persistent kernel (30 steps in one launch): same state bits, reproducible series
+    assert np.array_equal(res[0][0], res[3][0])
+    assert np.max(np.abs(res[0][1] - res[3][1])) < 1e-14
+    assert np.max(np.abs(res[0][2] - res[3][2])) < 1e-14 * np.abs(res[0][2][:, :1]).max()
+    assert np.array_equal(res[3][1], res[4][1]) and np.array_equal(res[3][2], res[4][2])
+    # odd step counts, repeated calls and a single step (which takes the per-step path) keep the buffers straight
+    a, b = lpc.Lattice.from_inputs(lat, max_steps=31), lpc.Lattice.from_inputs(lat, max_steps=31)
+    a.set_kernel(3)
+    b.set_kernel(1)
+    for n in (7, 1, 2, 21):
+        a.step(n)
+        b.step(n)
+    assert a.steps_done == b.steps_done == 31 and a.launch_count < b.launch_count
+    assert np.array_equal(a.field(lpc.LPC_FIELD_G), b.field(lpc.LPC_FIELD_G))
+    assert np.max(np.abs(a.fid() - b.fid())) < 1e-14
 
 
 # ---------------------------------------------------------------------------------------------
