@@ -128,12 +128,24 @@ void tma_geometry(int C, int nx, int ny, int nz, int* ty, int* tz, int* nstage, 
   // marching through the same planes in lockstep, which makes the DRAM traffic come in read bursts and
   // write bursts; many short CTAs desynchronise and keep the mix even.  Below 24 planes the two extra
   // plane loads per chunk cost more than that gains, unless the grid is short of waves (256^3: 16 planes
-  // per chunk measured 2% faster than 32), so chunks shrink to 16 planes to reach 8 waves.  Small,
-  // L2-resident lattices are latency-bound: they get as many chunks as it takes to fill the SMs once
-  // (measured 64^3: 35 -> 10 us/step).
+  // per chunk measured 2% faster than 32), so chunks shrink to 16 planes to reach 8 waves.
   long long chunks = std::max(1, (nx + 16) / 32);
   chunks = std::max(chunks, std::min<long long>(std::max(1, nx / 16), (8 * resident + tiles - 1) / tiles));
-  if (tiles * chunks < resident) chunks = std::min<long long>((resident + tiles - 1) / tiles, std::max(1, nx / 2));
+  if (tiles * std::max(1, nx / 16) < 3 * resident) {
+    // Few waves: wave quantisation decides.  A CTA costs its planes plus two halo planes plus about six
+    // plane times of pipeline fill and final reduce; take the chunk count with the cheapest last wave
+    // (128^3: 9 chunks = 288 CTAs in one wave instead of 10 = 320 CTAs in two, 44 -> 30 us/step).
+    long long best = 1, best_cost = -1;
+    for (long long c = 1; c <= std::max(1, nx / 2); ++c) {
+      const long long len = (nx + c - 1) / c;
+      const long long cost = ((tiles * ((nx + len - 1) / len) + resident - 1) / resident) * (len + 8);
+      if (best_cost < 0 || cost < best_cost) {
+        best = c;
+        best_cost = cost;
+      }
+    }
+    chunks = best;
+  }
   if (const char* e = getenv("LPC_XC")) {
     const int v = atoi(e);
     if (v > 0) chunks = (nx + v - 1) / v;
