@@ -160,6 +160,15 @@ int lpc_set_regions(lpc_lattice* lat, const uint8_t* region);
  * Errors: LPC_ESTATE (no labels), LPC_EINVAL (region or range), LPC_ECUDA.                       */
 int lpc_read_fid_region(lpc_lattice* lat, int32_t region, int64_t first, int64_t count, double* out_re_im_host);
 
+/* Regional VACF and diffusion coefficients (the regional D of Table 1): Eq. 4
+ * (:79) restricted to the particles that sit in the region when the later displacement starts,
+ * normalised by the region's equilibrium population w_r = sum_{i in r} pi_i:
+ *   Z^r_d[1] = sum_{i in r} pi_i sum_s p(i -> i + s e_d) a^2 / w_r,
+ *   Z^r_d[m] = sum_{i in r} P^d_i(m-1) u^d_i / w_r  (m >= 2),   D^r_d as in lpc_moments.
+ * Needs n_moments = 3, n_regions >= 1 and labels set before the first step; costs one more pass
+ * over pi, the moment fields and the labels per step.  Layout and errors as lpc_moments.         */
+int lpc_moments_region(lpc_lattice* lat, int32_t region, int64_t count, double* vacf_xyz_host, double D_xyz[3]);
+
 /* Spectrum of a FID series (Eq. 9, "Fourier transformed", :202) on a frequency grid:
  *   F(f_k) = dt * sum_{n=0}^{count-1} G[n] exp(-pi lb n dt) exp(-2 pi i f_k n dt),  f_k = f0 + k df,
  * k = 0..n_freq-1 (Hz; delta in ppm = f / (nu_0 * 1e-6)); lb_hz >= 0 is an optional Lorentzian line

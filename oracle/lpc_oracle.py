@@ -88,6 +88,8 @@ class Oracle:
         self.shape = tuple(int(v) for v in shape)
         self.n = int(np.prod(self.shape))
         self.n_moments = int(n_moments)
+        self.bc = tuple(int(b) for b in bc)
+        self.a = float(a)
         self.cfg = _cfg(shape, bc, dt, a, alpha)
         dF = np.ascontiguousarray(dF, dtype=np.float64).reshape(-1)
         blocked = np.ascontiguousarray(blocked, dtype=np.uint8).reshape(-1)
@@ -155,6 +157,40 @@ class Oracle:
             for r in range(n_regions):
                 out[r, k] = g[region == r].sum()
         return out
+
+    def step_with_regional_moments(self, region, n_regions, n_steps):
+        """Regional VACF (the regional D of Table 1; reading Q27): the sum of
+        Eq. 4 (:79) over the sites of region r only -- the site a particle occupies when the later
+        displacement starts -- divided by the region's equilibrium population w_r = sum_{i in r} pi_i:
+            Z^r_d[1] = sum_{i in r} pi_i sum_s p(i -> i + s e_d) a^2 / w_r            (Eq. 5, :92)
+            Z^r_d[m] = sum_{i in r} P^d_i(m-1) u^d_i / w_r,  m = 2 .. n_steps + 1     (O8)
+        Must be called at step 0.  Returns (Z[n_regions, 3, n_steps + 1] with Z[r, d, m-1], w[n_regions])."""
+        assert self.n_moments == 3 and self.steps == 0
+        region = np.asarray(region).reshape(self.shape)
+        pi = self.pi()
+        w = np.array([pi[region == r].sum() for r in range(n_regions)])
+        Z = np.zeros((n_regions, 3, n_steps + 1))
+        for d in range(3):
+            # p(i -> i + e_d) is the probability with which i + e_d receives from its -d neighbour, and likewise for -e_d
+            out_plus = np.roll(self.p_in(2 * d), -1, axis=d)
+            out_minus = np.roll(self.p_in(2 * d + 1), +1, axis=d)
+            if self.bc[d]:  # reflective: no neighbour beyond the wall
+                idx = [slice(None)] * 3
+                idx[d] = -1
+                out_plus[tuple(idx)] = 0.0
+                idx[d] = 0
+                out_minus[tuple(idx)] = 0.0
+            z1 = pi * (out_plus + out_minus) * self.a ** 2
+            for r in range(n_regions):
+                Z[r, d, 0] = z1[region == r].sum() / w[r]
+        u = [self.u(d) for d in range(3)]
+        for m in range(1, n_steps + 1):
+            for d in range(3):
+                prod = self.P(d) * u[d]
+                for r in range(n_regions):
+                    Z[r, d, m] = prod[region == r].sum() / w[r]
+            self.step(1)
+        return Z, w
 
     def _get(self, fn, *a):
         out = np.empty(self.n, dtype=np.float64)

@@ -24,7 +24,7 @@ LPC_KERNEL_AUTO, LPC_KERNEL_DIRECT, LPC_KERNEL_TMA, LPC_KERNEL_PERSIST = range(4
 
 EXPORTS = (
     "lpc_workspace_bytes", "lpc_create_lattice", "lpc_set_site_params", "lpc_step_n", "lpc_read_fid",
-    "lpc_moments", "lpc_read_field", "lpc_set_state", "lpc_equilibrate", "lpc_seed_from_density", "lpc_set_regions", "lpc_read_fid_region", "lpc_spectrum", "lpc_set_kernel",
+    "lpc_moments", "lpc_read_field", "lpc_set_state", "lpc_equilibrate", "lpc_seed_from_density", "lpc_set_regions", "lpc_read_fid_region", "lpc_moments_region", "lpc_spectrum", "lpc_set_kernel",
     "lpc_steps_done",
     "lpc_launch_count", "lpc_bytes_per_site_step", "lpc_destroy", "lpc_last_error",
 )
@@ -71,6 +71,7 @@ def _load():
     lib.lpc_seed_from_density.argtypes = [C.c_void_p]
     lib.lpc_set_regions.argtypes = [C.c_void_p, C.c_void_p]
     lib.lpc_read_fid_region.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_int64, C.c_void_p]
+    lib.lpc_moments_region.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_void_p, C.c_void_p]
     lib.lpc_spectrum.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_double, C.c_double, C.c_int64, C.c_double, C.c_void_p]
     lib.lpc_steps_done.argtypes = [C.c_void_p]
     lib.lpc_steps_done.restype = C.c_int64
@@ -205,6 +206,16 @@ def lpc_read_fid_region(handle, region, first=0, count=None):
     return out
 
 
+def lpc_moments_region(handle, region, count=None):
+    """(vacf[3, count], D[3]) of one region."""
+    if count is None:
+        count = int(_lib.lpc_steps_done(handle)) + 1
+    vacf = np.empty((3, max(count, 0)), dtype=np.float64)
+    D = np.empty(3, dtype=np.float64)
+    _check(_lib.lpc_moments_region(handle, int(region), int(count), C.c_void_p(vacf.ctypes.data), C.c_void_p(D.ctypes.data)))
+    return vacf, D
+
+
 def lpc_spectrum(handle, f0_hz, df_hz, n_freq, lb_hz=0.0, region=-1, count=None):
     """F(f0 + k df), k = 0..n_freq-1, of G[0..count) (Eq. 9); region = -1 takes the whole lattice."""
     if count is None:
@@ -317,6 +328,9 @@ class Lattice:
 
     def fid_region(self, region, first=0, count=None):
         return lpc_read_fid_region(self.handle, region, first, count)
+
+    def moments_region(self, region, count=None):
+        return lpc_moments_region(self.handle, region, count)
 
     def spectrum(self, f0_hz, df_hz, n_freq, lb_hz=0.0, region=-1, count=None):
         return lpc_spectrum(self.handle, f0_hz, df_hz, n_freq, lb_hz, region, count)

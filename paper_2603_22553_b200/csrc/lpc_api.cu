@@ -50,7 +50,7 @@ constexpr long long STAGE_SITES = 4ll << 20;  // sites per host<->device staging
 constexpr long long SPEC_BATCH = 4096;        // frequencies per spectrum launch
 
 struct Offsets {
-  size_t ctl, fid, vacf, partials, pi, cs, f0, f1, regions, fidr, rpartials, spec, staging, total;
+  size_t ctl, fid, vacf, partials, pi, cs, f0, f1, regions, fidr, vacfr, wr, rpartials, spec, staging, total;
   size_t partial_slots;
 };
 
@@ -67,6 +67,7 @@ struct lpc_lattice {
   bool have_params;
   bool have_regions;
   long long region_first;  // first sample of the regional series
+  bool region_moments;     // the regional VACF is being recorded (labels were set at step 0)
   int cur;  // index of the buffer holding the current state
   long long steps;
   long long launches;
@@ -175,7 +176,9 @@ Offsets make_offsets(const lpc_config* c, const Layout& L) {
   o.f1 = p; p += align_up((size_t)C * L.np * sT);
   o.regions = p; p += align_up(c->n_regions ? (size_t)N : 0);
   o.fidr = p; p += align_up((size_t)c->n_regions * (c->max_steps + 1) * sizeof(double2));
-  o.rpartials = p; p += align_up(c->n_regions ? (size_t)AUX_BLOCKS * 2 * MAX_REGIONS * sizeof(double) : 0);
+  o.vacfr = p; p += align_up((c->n_regions && c->n_moments) ? (size_t)c->n_regions * 3 * (c->max_steps + 2) * sizeof(double) : 0);
+  o.wr = p; p += align_up(c->n_regions ? MAX_REGIONS * sizeof(double) : 0);
+  o.rpartials = p; p += align_up(c->n_regions ? (size_t)AUX_BLOCKS * 4 * MAX_REGIONS * sizeof(double) : 0);
   o.spec = p; p += align_up((size_t)SPEC_BATCH * sizeof(double2));
   o.staging = p; p += align_up((size_t)std::min<long long>(N, STAGE_SITES) * 16);
   o.total = p;
@@ -394,6 +397,24 @@ int region_reduce_t(lpc_lattice* h, long long sample) {
 
 int region_reduce(lpc_lattice* h, long long sample) {
   return h->cfg.precision ? region_reduce_t<float>(h, sample) : region_reduce_t<double>(h, sample);
+}
+
+// regional VACF sample: INIT writes w_r and Z^r_d[1], otherwise Z^r_d[steps + 2] from the moment fields before the sweep
+template <typename T, bool INIT>
+int region_moment_t(lpc_lattice* h) {
+  const T* q = wsp<T>(h, h->cur ? h->off.f1 : h->off.f0) + (long long)(2 + h->nrho) * h->L.np;
+  const double scale = INIT ? h->cfg.a * h->cfg.a * h->cfg.alpha / 6.0 : h->cfg.a * h->cfg.alpha / 6.0;
+  region_moment_kernel<T, INIT><<<aux_grid(h->N), 256, 0, h->stream>>>(
+      h->L, wsp<T>(h, h->off.pi), q, h->ws + h->off.regions, h->cfg.n_regions, wsp<double>(h, h->off.rpartials), wsp<Ctl>(h, h->off.ctl),
+      wsp<double>(h, h->off.wr), wsp<double>(h, h->off.vacfr), h->cfg.max_steps + 2, INIT ? 1 : h->steps + 2, scale);
+  CUDA_TRY(cudaGetLastError());
+  h->launches++;
+  return LPC_OK;
+}
+
+template <bool INIT>
+int region_moment(lpc_lattice* h) {
+  return h->cfg.precision ? region_moment_t<float, INIT>(h) : region_moment_t<double, INIT>(h);
 }
 
 template <typename T>
@@ -691,6 +712,7 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
   h->stream = static_cast<cudaStream_t>(cfg->stream);
   h->have_params = false;
   h->have_regions = false;
+  h->region_moments = false;
   h->region_first = 0;
   h->cur = 0;
   h->steps = 0;
@@ -733,6 +755,7 @@ int lpc_set_site_params(lpc_lattice* h, const double* dF, const uint8_t* blocked
   if (!dF || !blocked || !omega) return fail(LPC_EINVAL, "dF, blocked and omega must not be NULL");
   h->have_params = false;
   h->have_regions = false;
+  h->region_moments = false;
   return h->cfg.precision ? set_site_params_t<float>(h, dF, blocked, omega, g0) : set_site_params_t<double>(h, dF, blocked, omega, g0);
 }
 
@@ -745,6 +768,10 @@ int lpc_step_n(lpc_lattice* h, int64_t n) {
                        (h->kernel == LPC_KERNEL_PERSIST || (h->kernel == LPC_KERNEL_AUTO && persist_by_default(h)));
   if (persist) return h->cfg.precision ? launch_persist<float>(h, n) : launch_persist<double>(h, n);
   for (int64_t k = 0; k < n; ++k) {
+    if (h->region_moments) {
+      int rc = region_moment<false>(h);
+      if (rc) return rc;
+    }
     int rc = h->cfg.precision ? launch_step<float>(h) : launch_step<double>(h);
     if (rc) return rc;
     h->steps++;
@@ -830,6 +857,12 @@ int lpc_set_regions(lpc_lattice* h, const uint8_t* region) {
   h->region_first = h->steps;
   int rc = region_reduce(h, h->steps);
   if (rc) return rc;
+  // the regional VACF needs the whole series: it is recorded when the labels arrive before the first step
+  h->region_moments = (h->nmom == 3 && h->steps == 0);
+  if (h->region_moments) {
+    rc = region_moment<true>(h);
+    if (rc) return rc;
+  }
   CUDA_TRY(cudaStreamSynchronize(h->stream));
   return LPC_OK;
 }
@@ -875,6 +908,29 @@ int lpc_spectrum(lpc_lattice* h, int32_t region, int64_t count, double f0, doubl
     CUDA_TRY(cudaMemcpyAsync(out + 2 * k0, spec, (size_t)nb * sizeof(double2), cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(cudaStreamSynchronize(h->stream));
   }
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return LPC_OK;
+}
+
+int lpc_moments_region(lpc_lattice* h, int32_t region, int64_t count, double* vacf_host, double D[3]) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
+  if (h->nmom != 3) return fail(LPC_ESTATE, "moment fields are not propagated (n_moments = 0)");
+  if (!h->have_regions || !h->region_moments) return fail(LPC_ESTATE, "region labels must be set before the first step to record the regional VACF");
+  if (region < 0 || region >= h->cfg.n_regions) return fail(LPC_EINVAL, "region %d is outside [0, %d)", region, h->cfg.n_regions);
+  if (count < 1 || count > h->steps + 1) return fail(LPC_EINVAL, "count must lie in [1, steps_done + 1]");
+  if (!D) return fail(LPC_EINVAL, "D is NULL");
+  const long long stride = h->cfg.max_steps + 2;
+  double* vacf = wsp<double>(h, h->off.vacfr) + (size_t)region * 3 * stride;
+  Ctl* ctl = wsp<Ctl>(h, h->off.ctl);
+  diffusion_kernel<<<3, 256, 0, h->stream>>>(vacf, stride, count, h->cfg.dt, ctl);
+  CUDA_TRY(cudaGetLastError());
+  h->launches++;
+  CUDA_TRY(cudaMemcpyAsync(D, ctl->scratch, 3 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  if (vacf_host)
+    for (int d = 0; d < 3; ++d)
+      CUDA_TRY(cudaMemcpyAsync(vacf_host + (size_t)d * count, vacf + d * stride + 1, (size_t)count * sizeof(double), cudaMemcpyDeviceToHost,
+                               h->stream));
   CUDA_TRY(cudaStreamSynchronize(h->stream));
   return LPC_OK;
 }

@@ -73,6 +73,84 @@ __global__ void __launch_bounds__(256)
   }
 }
 
+// Regional VACF (the regional diffusion coefficients of Table 1):
+// the sum of Eq. 4 (:79) restricted to the particles that sit in region r when the later displacement
+// starts, normalised by the region's equilibrium population w_r = sum_{i in r} pi_i (Q27):
+//   INIT: w_r, and Z^r_d[1]   = (a^2 alpha/6) sum_{i in r} (m_{i,+d} + m_{i,-d}) / w_r
+//   STEP: Z^r_d[k+1] = (a alpha/6) sum_{i in r} q^d_i(k) (m_{i,+d} - m_{i,-d}) / w_r     (q = P/pi before the sweep)
+// One pass over pi (with neighbours), the three moment channels and the labels; predicate-selected
+// accumulators, block partials, fixed-order sum by the last block.
+template <typename T, bool INIT>
+__global__ void __launch_bounds__(256)
+    region_moment_kernel(Layout L, const T* __restrict__ pi, const T* __restrict__ q, const uint8_t* __restrict__ label, int n_regions,
+                         double* partials, Ctl* ctl, double* wr, double* vacfr, long long stride, long long index, double scale) {
+  constexpr int NV = INIT ? 4 : 3;   // INIT also sums pi
+  double acc[MAX_REGIONS][NV];
+#pragma unroll
+  for (int r = 0; r < MAX_REGIONS; ++r)
+#pragma unroll
+    for (int v = 0; v < NV; ++v) acc[r][v] = 0.0;
+  const long long n = (long long)L.nx * L.ny * L.nz;
+  const long long st[3] = {L.sx, L.sy, 1};
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+    const long long j = dense_to_padded(L, i);
+    const int lab = label[i];
+    const T p = pi[j];
+    double v[NV];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      const T mm = tmin(p, pi[j - st[d]]), mp = tmin(p, pi[j + st[d]]);
+      v[d] = INIT ? (double)mp + (double)mm : (double)q[(long long)d * L.np + j] * (double)(mp - mm);
+    }
+    if (INIT) v[NV - 1] = (double)p;
+#pragma unroll
+    for (int r = 0; r < MAX_REGIONS; ++r)
+#pragma unroll
+      for (int k = 0; k < NV; ++k) acc[r][k] += (lab == r) ? v[k] : 0.0;
+  }
+  constexpr int NC = MAX_REGIONS * NV;
+  __shared__ double red[8][NC];
+  __shared__ unsigned int s_last;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int r = 0; r < MAX_REGIONS; ++r)
+#pragma unroll
+    for (int k = 0; k < NV; ++k) {
+      const double t = warp_sum(acc[r][k]);
+      if (lane == 0) red[warp][r * NV + k] = t;
+    }
+  __syncthreads();
+  if (threadIdx.x < NC) {
+    double t = 0.0;
+    for (int w = 0; w < 8; ++w) t += red[w][threadIdx.x];
+    partials[(size_t)blockIdx.x * NC + threadIdx.x] = t;
+    __threadfence();
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) s_last = (atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1);
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  double* tot = &red[0][0];
+  if (threadIdx.x < NC) {
+    double t = 0.0;
+    for (unsigned int b = 0; b < gridDim.x; ++b) t += __ldcg(&partials[(size_t)b * NC + threadIdx.x]);
+    tot[threadIdx.x] = t;
+  }
+  __syncthreads();
+  if (threadIdx.x < n_regions) {
+    const int r = threadIdx.x;
+    if (INIT) wr[r] = tot[r * NV + 3];
+    const double w = INIT ? tot[r * NV + 3] : wr[r];
+    for (int d = 0; d < 3; ++d) vacfr[((long long)r * 3 + d) * stride + index] = (w > 0.0) ? scale * tot[r * NV + d] / w : 0.0;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    ctl->ticket = 0;
+    __threadfence();
+  }
+}
+
 // F(f_k) = dt * sum_{n=0}^{M-1} G[n] exp(-pi lb n dt) exp(-2 pi i f_k n dt),  f_k = f0 + k df
 // (Eq. 9, as a plain discrete sum over the samples; lb = Lorentzian line broadening in Hz,
 // 0 = none).  One block per frequency, fixed summation order.

@@ -355,6 +355,48 @@ def test_regional_fid_and_spectrum_match_oracle(lpc, oracle_mod, kernel, precisi
         assert abs(gpu.fid_region(r, 0, 1)[0] - Gr_o[r][n]) <= tol * sabs[n]
 
 
+@pytest.mark.parametrize("kernel,precision", [(1, 0), (2, 0), (2, 1)])
+def test_regional_vacf_and_diffusion_match_oracle(lpc, oracle_mod, kernel, precision):
+    """Regional D (Table 1) on a small supercapacitor-shaped lattice."""
+    n, nreg = 80, 3
+    lat = lpc_inputs.supercap(64, 16, 70, n_steps=n, n_moments=3)
+    tol = 1e-5 if precision else 1e-9
+    x = np.arange(lat.nx)[:, None, None] * np.ones(lat.shape, dtype=int)
+    region = np.where(x < lat.nx * 3 // 8, 0, np.where(x < lat.nx * 5 // 8, 1, 2)).astype(np.uint8)
+    gpu = lpc.Lattice.from_inputs(lat, precision=precision, max_steps=n, n_regions=nreg)
+    gpu.set_kernel(kernel)
+    gpu.set_regions(region)
+    gpu.step(n)
+    orc = oracle_mod.Oracle.from_lattice(lat, n_moments=3, max_steps=n)
+    Zr_o, w = orc.step_with_regional_moments(region, nreg, n)
+    Zall_g, D_all = gpu.moments()
+    acc = np.zeros_like(Zall_g)
+    for r in range(nreg):
+        Z_g, D_g = gpu.moments_region(r)
+        assert Z_g.shape == (3, n + 1)
+        z1 = np.abs(Zr_o[r][:, :1])
+        assert np.max(np.abs(Z_g - Zr_o[r]) / z1) <= tol, f"region {r}"
+        D_o = Zr_o[r][:, 0] / (2 * lat.dt) + Zr_o[r][:, 1:].sum(axis=1) / lat.dt
+        assert np.max(np.abs(D_g - D_o) / (z1[:, 0] / (2 * lat.dt))) <= tol
+        acc += w[r] * Z_g
+        # a shorter record
+        Z_s, D_s = gpu.moments_region(r, count=10)
+        assert np.array_equal(Z_s, Z_g[:, :10])
+    # the regions tile the lattice: population-weighted, they add up to the whole-lattice VACF
+    assert np.max(np.abs(acc - Zall_g) / np.abs(Zall_g[:, :1])) <= tol
+    # the bulk region (dF = 0, no carbon) is faster than the electrodes in the transverse directions
+    assert gpu.moments_region(1)[1][1] > gpu.moments_region(0)[1][1]
+    # labels that arrive after the first step cannot give the series
+    late = lpc.Lattice.from_inputs(lat, max_steps=4, n_regions=nreg)
+    late.step(1)
+    late.set_regions(region)
+    late.step(2)
+    with pytest.raises(lpc.LpcError) as e:
+        late.moments_region(0)
+    assert e.value.code == lpc.LPC_ESTATE
+    assert late.fid_region(0, first=1).shape == (3,)
+
+
 def test_regional_fid_large_spectrum_batches_and_errors(lpc):
     lat = lpc_inputs.random_small((12, 10, 20), seed=43, p_block=0.1)
     lat.omega[...] = -2 * np.pi * 2500.0

@@ -351,6 +351,47 @@ def test_p15_regional_fid_closed_form_on_sealed_pockets(oracle_mod):
 
 
 # --------------------------------------------------------------------------
+# P16 regional VACF / D
+# --------------------------------------------------------------------------
+def test_p16_regional_vacf_adds_up_and_matches_closed_forms(oracle_mod):
+    """(i) sum_r w_r Z^r_d[m] = Z_d[m] of the whole lattice; (ii) on a homogeneous lattice every region has the
+    free-diffusion values of Eq. 7, Z_d[1] = alpha a^2 / 3 and Z_d[m >= 2] = 0, hence D_r = alpha a^2 / (6 dt);
+    (iii) a sealed pocket has the regional series of the pocket run on its own."""
+    n = 25
+    lat = lpc_inputs.random_small((9, 7, 8), bc=(1, 0, 0), p_block=0.25, alpha=0.8, seed=51, dF_span=2.0, n_moments=3)
+    region = (np.indices(lat.shape)[1] % 3).astype(np.uint8)
+    o = _mk(oracle_mod, lat, n_moments=3, max_steps=n)
+    Zr, w = o.step_with_regional_moments(region, 3, n)
+    Zall, _ = o.moments()
+    assert abs(w.sum() - 1.0) < 1e-14
+    assert np.max(np.abs(np.einsum("r,rdm->dm", w, Zr) - Zall)) < 1e-15
+    assert np.all(np.abs(Zr[:, :, 2:]) > 0)   # a heterogeneous lattice has memory
+
+    a, alpha = 1.7, 0.6
+    lat = _uniform((8, 6, 6), alpha=alpha, a=a)
+    region = (np.indices(lat.shape)[0] >= 4).astype(np.uint8)
+    o = _mk(oracle_mod, lat, n_moments=3, max_steps=6)
+    Zr, w = o.step_with_regional_moments(region, 2, 6)
+    assert np.allclose(w, 0.5, atol=1e-15)
+    assert np.max(np.abs(Zr[:, :, 0] - alpha * a * a / 3.0)) < 1e-15 and np.max(np.abs(Zr[:, :, 1:])) < 1e-16
+
+    # sealed pocket: x < 4 is cut off from the rest by a carbon wall at x = 4 (reflective x closes the other side)
+    lat = lpc_inputs.random_small((9, 5, 5), bc=(1, 0, 0), p_block=0.15, alpha=0.9, seed=52, dF_span=1.5, n_moments=3)
+    lat.blocked[4] = 1
+    region = (np.indices(lat.shape)[0] > 4).astype(np.uint8)
+    o = _mk(oracle_mod, lat, n_moments=3, max_steps=n)
+    Zr, w = o.step_with_regional_moments(region, 2, n)
+    import copy
+    sub = copy.copy(lat)
+    sub.nx = 4
+    sub.dF, sub.blocked, sub.omega = (np.ascontiguousarray(v[:4]) for v in (lat.dF, lat.blocked, lat.omega))
+    o_sub = _mk(oracle_mod, sub, n_moments=3, max_steps=n)
+    o_sub.step(n)
+    Zsub, _ = o_sub.moments()
+    assert np.max(np.abs(Zr[0] - Zsub)) < 1e-14
+
+
+# --------------------------------------------------------------------------
 # P5 free diffusion closed form (Eq. 6, Eq. 7) -- golden values
 # --------------------------------------------------------------------------
 def _golden(name):
