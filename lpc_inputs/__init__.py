@@ -105,10 +105,10 @@ def pore_site_fields(w: np.ndarray):
     return dF, delta
 
 
-def _finish(name, shape, bc, n_steps, n_moments, dF, blocked, delta, alpha=1.0, notes=None):
+def _finish(name, shape, bc, n_steps, n_moments, dF, blocked, delta, alpha=1.0, notes=None, larmor_mhz=LARMOR_MHZ):
     blocked = np.ascontiguousarray(blocked, dtype=np.uint8)
     dF = np.ascontiguousarray(dF, dtype=np.float64)
-    omega = np.ascontiguousarray(ppm_to_omega(np.asarray(delta, dtype=np.float64)))
+    omega = np.ascontiguousarray(ppm_to_omega(np.asarray(delta, dtype=np.float64)) * (larmor_mhz / LARMOR_MHZ))
     return Lattice(
         name=name, nx=shape[0], ny=shape[1], nz=shape[2], bc=tuple(bc), dt=DT_DEFAULT,
         a=1.0, alpha=alpha, n_steps=n_steps, n_moments=n_moments,
@@ -193,3 +193,66 @@ def random_small(shape, bc=(0, 0, 0), p_block=0.3, alpha=1.0, seed=0, n_steps=10
     delta = -ppm_span * rng.random(shape)
     lat = _finish("random_small", tuple(shape), bc, n_steps, n_moments, dF, blocked, delta, alpha)
     return lat
+
+
+def film(nx: int = 100, ny: int = 100, nz: int = 300, radius: float = 9.0, spacing: int = 20, ell: float = 4.0,
+         p_block: float = 0.1, alpha: float = 0.025, n_steps: int = 50000, n_moments: int = 0) -> Lattice:
+    """Film-electrode supercapacitor of PAPER.md:236-248: a 100 x 100 x 300 lattice, no periodic
+    boundary in z, two electrodes made of monodisperse porous carbon particles of radius 9 sites that fill 38% of
+    the electrode volume, bulk electrolyte between the particles and between the electrodes.
+
+    Stand-in recipe (the paper's particle positions are not given): the electrodes are z < nz/3 and z >= 2nz/3;
+    particle centres sit on a simple-cubic grid of `spacing` sites (20: (4/3) pi 9^3 / 20^3 = 0.382) with a seeded
+    jitter of -1..1 sites per axis; inside the particles the pore field of configs[1] (ell = 4, 10% blocked), the
+    positive / negative electrode shifted by +-0.5 kT as in configs[3]; everything else is bulk (dF = delta = 0,
+    open).  alpha = dt / tau = 5 us / 0.2 ms, 19F at 282 MHz (:248).  notes["particle"] is the particle
+    mask (1 positive-electrode particle, 2 negative, 0 bulk).
+    """
+    shape = (nx, ny, nz)
+    rng = _rng(5, 0)
+    label = np.zeros(shape, dtype=np.uint8)
+    zel = nz // 3
+    R = int(np.ceil(radius)) + 1
+    off = np.arange(-R, R + 1)
+    ball = (off[:, None, None] ** 2 + off[None, :, None] ** 2 + off[None, None, :] ** 2) <= radius * radius
+    half = spacing // 2
+    for zlo, lab in ((0, 1), (nz - zel, 2)):
+        for cx in range(half, nx - half + 1, spacing):
+            for cy in range(half, ny - half + 1, spacing):
+                for cz in range(zlo + half, zlo + zel - half + 1, spacing):
+                    j = rng.integers(-1, 2, size=3)
+                    c = np.array([cx, cy, cz]) + j
+                    c[2] = min(max(c[2], zlo + R), zlo + zel - R - 1) if zel > 2 * R + 1 else c[2]
+                    ix = (c[0] + off) % nx
+                    iy = (c[1] + off) % ny
+                    iz = np.clip(c[2] + off, 0, nz - 1)
+                    sub = label[np.ix_(ix, iy, iz)]
+                    sub[ball] = lab
+                    label[np.ix_(ix, iy, iz)] = sub
+    inside = label > 0
+    xi = gaussian_field(shape, ell, _rng(5, 1))
+    dF, delta = pore_site_fields(pore_width_nm(xi))
+    del xi
+    blocked = (rng.random(shape) < p_block) & inside
+    dF = np.where(label == 1, dF + 0.5, np.where(label == 2, dF - 0.5, 0.0))
+    delta = np.where(inside, delta, 0.0)
+    return _finish("film_supercap", shape, (0, 0, 1), n_steps, n_moments, dF, blocked, delta, alpha=alpha,
+                   notes={"radius": radius, "spacing": spacing, "particle": label, "fraction": float(inside[:, :, :zel].mean())},
+                   larmor_mhz=282.0)
+
+
+def random_links(shape, seed=0, lo=0.1) -> np.ndarray:
+    """Seeded iid per-link mobility factors alpha_ij ~ U[lo, 1]: [3, nx, ny, nz], entry [d, i] belongs to
+    the link between site i and its +d neighbour."""
+    rng = np.random.Generator(np.random.PCG64(SEED_BASE + 2000 + seed))
+    return lo + (1.0 - lo) * rng.random((3,) + tuple(shape))
+
+
+def confined_links(confined: np.ndarray, mu: float) -> np.ndarray:
+    """Link factors for "mobility decreased due to confinement": a link has factor mu when either of
+    its two ends lies in the confined region (a particle or an electrode) and 1 between two bulk sites."""
+    c = np.asarray(confined) != 0
+    out = np.ones((3,) + c.shape)
+    for d in range(3):
+        out[d][c | np.roll(c, -1, axis=d)] = mu
+    return out

@@ -30,6 +30,8 @@
  *   O7  first-step moments P^d(1), u^d, Z_d[1]      Eq. 4, 5 PAPER.md:79,92; :84-86
  *   O8  Z_d[k+1] = sum_i P^d_i u^d_i ; P^d <- W P^d ; D_d   Eq. 4
  *   O9  equilibration loop rho <- W rho until max_i |rho(t+1)-rho(t)| < threshold
+ *   O10 per-link mobility factor alpha_ij: p(i->j) and p(j->i) are both multiplied by the factor of
+ *       the link (detailed balance kept)
  *
  * Every global sum is Neumaier-compensated, taken plane by plane (x) and the
  * plane partials combined in x order, so results do not depend on the OpenMP
@@ -62,6 +64,7 @@ typedef struct lpco_state {
   int n_moments;   /* 0 or 3 */
   uint8_t *blocked;
   double *dF;
+  double *link;    /* O10: 3n link factors or NULL; link[d*n + i] belongs to the link between i and i + e_d */
   double *pi;      /* O1 */
   double Zpart;    /* sum_j exp(-dF_j) */
   double *p_in[6]; /* p(nb_k(i) -> i), k = 2*d + (s>0) */
@@ -115,6 +118,16 @@ double lpco_hop(const lpco_config *c, const double *dF, const uint8_t *blocked,
   return (c->alpha / 6.0) * acc;
 }
 
+/* ---- O10: per-link mobility factor alpha_ij ---------------
+ * "a factor alpha_ij can be defined for each link between neighboring lattice sites i and j ... if the
+ * probability of jumping from site i to site j is reduced, the probability of jumping from j to i must be
+ * reduced by the same factor".  One number per link, stored at its lower end: link[d*n + i] is the factor of
+ * the link between i and nb(i, d, +1), whichever way it is crossed.  j = nb(i, d, s).  No array: 1.      */
+static double link_alpha(const double *link, int64_t n, int64_t i, int64_t j, int d, int s) {
+  if (!link || j < 0) return 1.0;
+  return (s > 0) ? link[(int64_t)d * n + i] : link[(int64_t)d * n + j];
+}
+
 static const int K_D[6] = {0, 0, 1, 1, 2, 2};
 static const int K_S[6] = {-1, +1, -1, +1, -1, +1};
 
@@ -122,7 +135,7 @@ static double *dalloc(int64_t n) { return (double *)calloc((size_t)(n > 0 ? n : 
 
 void lpco_destroy(lpco_state *st) {
   if (!st) return;
-  free(st->blocked); free(st->dF); free(st->pi); free(st->stay); free(st->cs); free(st->sn);
+  free(st->blocked); free(st->dF); free(st->link); free(st->pi); free(st->stay); free(st->cs); free(st->sn);
   for (int k = 0; k < 6; ++k) free(st->p_in[k]);
   free(st->g_re); free(st->g_im); free(st->t_re); free(st->t_im);
   for (int d = 0; d < 3; ++d) { free(st->P[d]); free(st->Pt[d]); free(st->u[d]); }
@@ -174,8 +187,8 @@ static double plane_sum_prod(const lpco_state *st, const double *a, const double
   return ns_val(&t);
 }
 
-lpco_state *lpco_create(const lpco_config *c, const double *dF, const uint8_t *blocked,
-                        const double *omega, int n_moments, int64_t max_steps) {
+lpco_state *lpco_create_links(const lpco_config *c, const double *dF, const uint8_t *blocked,
+                              const double *omega, const double *link, int n_moments, int64_t max_steps) {
   if (!c || !dF || !blocked || !omega) return NULL;
   if (c->nx < 1 || c->ny < 1 || c->nz < 1) return NULL;
   if (!(c->alpha > 0.0 && c->alpha <= 1.0)) return NULL;
@@ -191,6 +204,12 @@ lpco_state *lpco_create(const lpco_config *c, const double *dF, const uint8_t *b
   memcpy(st->blocked, blocked, (size_t)n);
   st->dF = dalloc(n);
   memcpy(st->dF, dF, (size_t)n * sizeof(double));
+  if (link) {
+    for (int64_t k = 0; k < 3 * n; ++k)
+      if (!(link[k] >= 0.0 && link[k] <= 1.0)) { lpco_destroy(st); return NULL; }
+    st->link = dalloc(3 * n);
+    memcpy(st->link, link, (size_t)(3 * n) * sizeof(double));
+  }
   st->pi = dalloc(n); st->stay = dalloc(n); st->cs = dalloc(n); st->sn = dalloc(n);
   for (int k = 0; k < 6; ++k) st->p_in[k] = dalloc(n);
   st->g_re = dalloc(n); st->g_im = dalloc(n); st->t_re = dalloc(n); st->t_im = dalloc(n);
@@ -212,8 +231,9 @@ lpco_state *lpco_create(const lpco_config *c, const double *dF, const uint8_t *b
     double out = 0.0;
     for (int k = 0; k < 6; ++k) {
       int64_t j = lpco_neighbor(c, i, K_D[k], K_S[k]);
-      st->p_in[k][i] = (j < 0) ? 0.0 : lpco_hop(c, dF, blocked, j, i);
-      out += lpco_hop(c, dF, blocked, i, j);
+      const double aij = link_alpha(st->link, n, i, j, K_D[k], K_S[k]);   /* O10: same factor both ways */
+      st->p_in[k][i] = (j < 0) ? 0.0 : aij * lpco_hop(c, dF, blocked, j, i);
+      out += aij * lpco_hop(c, dF, blocked, i, j);
     }
     st->stay[i] = 1.0 - out;
     st->cs[i] = cos(omega[i] * c->dt);
@@ -236,8 +256,9 @@ lpco_state *lpco_create(const lpco_config *c, const double *dF, const uint8_t *b
           int64_t j = lpco_neighbor(c, i, d, s);
           if (j < 0) continue;
           /* arrival at i from j = i + s e_d: displacement -s a */
-          P1 += st->pi[j] * lpco_hop(c, dF, blocked, j, i) * (-(double)s * c->a);
-          double po = lpco_hop(c, dF, blocked, i, j);
+          const double aij = link_alpha(st->link, n, i, j, d, s);
+          P1 += st->pi[j] * (aij * lpco_hop(c, dF, blocked, j, i)) * (-(double)s * c->a);
+          double po = aij * lpco_hop(c, dF, blocked, i, j);
           ui += po * ((double)s * c->a);
           m2 += po * c->a * c->a;
         }
@@ -251,6 +272,11 @@ lpco_state *lpco_create(const lpco_config *c, const double *dF, const uint8_t *b
   }
   st->steps = 0;
   return st;
+}
+
+lpco_state *lpco_create(const lpco_config *c, const double *dF, const uint8_t *blocked,
+                        const double *omega, int n_moments, int64_t max_steps) {
+  return lpco_create_links(c, dF, blocked, omega, NULL, n_moments, max_steps);
 }
 
 /* O5 for a real field (no phase): out_i = stay_i f_i + sum_k p_in[k][i] f_{nb_k(i)} */

@@ -33,6 +33,8 @@ _dp = C.POINTER(C.c_double)
 _u8p = C.POINTER(C.c_uint8)
 _lib.lpco_create.restype = C.c_void_p
 _lib.lpco_create.argtypes = [C.POINTER(_Cfg), _dp, _u8p, _dp, C.c_int, C.c_int64]
+_lib.lpco_create_links.restype = C.c_void_p
+_lib.lpco_create_links.argtypes = [C.POINTER(_Cfg), _dp, _u8p, _dp, _dp, C.c_int, C.c_int64]
 _lib.lpco_destroy.argtypes = [C.c_void_p]
 _lib.lpco_step.argtypes = [C.c_void_p, C.c_int64]
 _lib.lpco_set_g.argtypes = [C.c_void_p, _dp]
@@ -84,7 +86,9 @@ def hop(shape, bc, alpha, dF, blocked, i, j):
 class Oracle:
     """One oracle run: create from the site arrays, step, read series and fields."""
 
-    def __init__(self, shape, bc, dt, a, alpha, dF, blocked, omega, n_moments=0, max_steps=0):
+    def __init__(self, shape, bc, dt, a, alpha, dF, blocked, omega, n_moments=0, max_steps=0, link=None):
+        """link: None, or 3 x shape factors alpha_ij in [0, 1] (O10): link[d][i] belongs to the
+        link between site i and its +d neighbour and scales the hop both ways."""
         self.shape = tuple(int(v) for v in shape)
         self.n = int(np.prod(self.shape))
         self.n_moments = int(n_moments)
@@ -95,16 +99,22 @@ class Oracle:
         blocked = np.ascontiguousarray(blocked, dtype=np.uint8).reshape(-1)
         omega = np.ascontiguousarray(omega, dtype=np.float64).reshape(-1)
         assert dF.size == self.n and blocked.size == self.n and omega.size == self.n
-        self._h = _lib.lpco_create(C.byref(self.cfg), _d(dF), blocked.ctypes.data_as(_u8p), _d(omega),
-                                   self.n_moments, int(max_steps))
+        if link is None:
+            self._h = _lib.lpco_create(C.byref(self.cfg), _d(dF), blocked.ctypes.data_as(_u8p), _d(omega),
+                                       self.n_moments, int(max_steps))
+        else:
+            link = np.ascontiguousarray(link, dtype=np.float64).reshape(-1)
+            assert link.size == 3 * self.n
+            self._h = _lib.lpco_create_links(C.byref(self.cfg), _d(dF), blocked.ctypes.data_as(_u8p), _d(omega), _d(link),
+                                             self.n_moments, int(max_steps))
         if not self._h:
             raise ValueError("lpco_create rejected the inputs")
 
     @classmethod
-    def from_lattice(cls, lat, n_moments=None, max_steps=None):
+    def from_lattice(cls, lat, n_moments=None, max_steps=None, link=None):
         return cls(lat.shape, lat.bc, lat.dt, lat.a, lat.alpha, lat.dF, lat.blocked, lat.omega,
                    lat.n_moments if n_moments is None else n_moments,
-                   lat.n_steps if max_steps is None else max_steps)
+                   lat.n_steps if max_steps is None else max_steps, link=link)
 
     def close(self):
         if getattr(self, "_h", None):

@@ -40,8 +40,11 @@ def _metropolis(dFi, dFj):
     return np.exp(-(dFj - dFi)) if dFj > dFi else 1.0
 
 
-def _moves(lat):
+def _moves(lat, link=None):
     """For every site: list of (target, probability, displacement vector) incl. staying.
+
+    link: optional [3, nx, ny, nz] factors alpha_ij of PAPER.md:105; link[d][i] belongs to the link between i and
+    its +d neighbour and multiplies the hop probability in both directions.
 
     Lattice-gas rule of PAPER.md:51-55: one of z = 6 neighbours is tried with
     probability alpha/6 (alpha: :101); the hop is accepted with Eq. 1; a move
@@ -65,6 +68,8 @@ def _moves(lat):
                 if lat.blocked[tgt]:
                     continue
                 p = lat.alpha / 6.0 * _metropolis(lat.dF[idx], lat.dF[tgt])
+                if link is not None:
+                    p *= link[d][idx] if s > 0 else link[d][tgt]
                 disp = np.zeros(3)
                 disp[d] = s * lat.a
                 lst.append((tgt, p, disp))
@@ -80,9 +85,9 @@ def _boltzmann(lat):
     return e / e.sum()
 
 
-def _enumerate(lat, n):
+def _enumerate(lat, n, link=None):
     """All n-step trajectories: returns G[0..n] (Eq. 8/11) and C[d, m] = <dx_1 dx_m>, m = 1..n."""
-    moves = _moves(lat)
+    moves = _moves(lat, link)
     pi = _boltzmann(lat)
     G = np.zeros(n + 1, dtype=complex)
     Cm = np.zeros((3, n + 1))
@@ -389,6 +394,97 @@ def test_p16_regional_vacf_adds_up_and_matches_closed_forms(oracle_mod):
     o_sub.step(n)
     Zsub, _ = o_sub.moments()
     assert np.max(np.abs(Zr[0] - Zsub)) < 1e-14
+
+
+# --------------------------------------------------------------------------
+# P17 per-link mobility factors alpha_ij (O10)
+# --------------------------------------------------------------------------
+@pytest.mark.parametrize("shape,bc,n", [((3, 3, 4), (0, 0, 0), 3), ((3, 2, 4), (1, 0, 1), 4)])
+def test_p17_links_trajectory_enumeration(oracle_mod, shape, bc, n):
+    """Eq. 8/11 and <dx_1 dx_m> over every trajectory of the lattice gas whose hops carry alpha_ij."""
+    lat = lpc_inputs.random_small(shape, bc=bc, p_block=0.2, alpha=0.9, seed=61, n_steps=n)
+    lat.dt = 2.0e-5
+    link = lpc_inputs.random_links(shape, seed=1, lo=0.0)
+    o = _mk(oracle_mod, lat, n_moments=3, max_steps=n, link=link)
+    o.step(n)
+    G_def, C_def = _enumerate(lat, n, link)
+    assert np.max(np.abs(o.fid() - G_def)) < 1e-12
+    vacf, D = o.moments(n)
+    assert np.max(np.abs(vacf - C_def[:, 1:])) < 1e-13
+    # the factors matter: without them the answer is different
+    G0, _ = _enumerate(lat, n)
+    assert np.max(np.abs(G0 - G_def)) > 1e-6
+
+
+def test_p17_links_keep_detailed_balance_and_boltzmann(oracle_mod):
+    """":105: the same factor both ways, so that the equilibrium stays Eq. 2": pi_i p(i->j) = pi_j p(j->i) =
+    alpha_ij (alpha/6) min(pi_i, pi_j), W pi = pi, mass conserved."""
+    shape, bc = (6, 5, 7), (0, 1, 0)
+    lat = lpc_inputs.random_small(shape, bc=bc, p_block=0.25, alpha=0.8, seed=62)
+    link = lpc_inputs.random_links(shape, seed=2)
+    o = _mk(oracle_mod, lat, n_moments=0, max_steps=30, link=link)
+    pi = _boltzmann(lat)
+    assert np.max(np.abs(o.pi() - pi)) < 1e-16
+    for d in range(3):
+        # p_in(2d+1)[i] = p(i + e_d -> i), p_in(2d)[i] = p(i - e_d -> i)
+        flow_back = pi * 0 + np.roll(pi, -1, axis=d) * o.p_in(2 * d + 1)          # pi_j p(j -> i), j = i + e_d
+        flow_fwd = np.roll(np.roll(pi, 1, axis=d) * o.p_in(2 * d), -1, axis=d)    # pi_i p(i -> j) read at j, moved back to i
+        want = link[d] * (lat.alpha / 6.0) * np.minimum(pi, np.roll(pi, -1, axis=d))
+        if bc[d]:
+            idx = [slice(None)] * 3
+            idx[d] = -1
+            want[tuple(idx)] = 0.0
+        assert np.max(np.abs(flow_back - want)) < 1e-17 and np.max(np.abs(flow_fwd - want)) < 1e-17
+    rho = o.propagate_real(pi, 30)
+    assert np.max(np.abs(rho - pi) / np.where(pi > 0, pi, 1)) < 1e-13
+    rng = np.random.default_rng(5)
+    r0 = rng.random(shape) * (lat.blocked == 0)
+    assert abs(o.propagate_real(r0, 30).sum() - r0.sum()) < 1e-12 * r0.sum()
+    # the stay probability is what the moves leave over
+    assert np.all(o.stay() >= 1.0 - lat.alpha - 1e-15) and np.all(o.stay() <= 1.0)
+
+
+def test_p17_links_special_cases(oracle_mod):
+    """(i) all factors 1 = no factors, bit for bit; (ii) anisotropic uniform factors on a homogeneous lattice: Eq. 7
+    per axis, D_d = alpha alpha_d a^2 / (6 dt), Z_d[1] = alpha alpha_d a^2 / 3, Z_d[m >= 2] = 0; (iii) factor 0 on
+    the links that close a periodic axis = a reflective wall there."""
+    n = 20
+    lat = lpc_inputs.random_small((5, 6, 4), p_block=0.2, alpha=0.9, seed=63, n_steps=n)
+    a = _mk(oracle_mod, lat, n_moments=3, max_steps=n)
+    b = _mk(oracle_mod, lat, n_moments=3, max_steps=n, link=np.ones((3,) + lat.shape))
+    a.step(n); b.step(n)
+    assert np.array_equal(a.fid(), b.fid()) and np.array_equal(a.moments()[0], b.moments()[0]) and np.array_equal(a.g(), b.g())
+
+    alpha, aa, dt = 0.7, 1.3, 2.0
+    ad = np.array([1.0, 0.5, 0.125])
+    lat = _uniform((6, 6, 8), alpha=alpha, a=aa, dt=dt)
+    link = np.ones((3,) + lat.shape) * ad[:, None, None, None]
+    o = _mk(oracle_mod, lat, n_moments=3, max_steps=8, link=link)
+    o.step(8)
+    Z, D = o.moments()
+    assert np.max(np.abs(Z[:, 0] - alpha * ad * aa * aa / 3.0)) < 1e-15 and np.max(np.abs(Z[:, 1:])) < 1e-16
+    assert np.max(np.abs(D - alpha * ad * aa * aa / (6.0 * dt))) < 1e-15
+    # mean-square displacement of a delta source along each axis: n alpha alpha_d a^2 / 3 (n < L/2)
+    src = np.zeros(lat.shape); src[3, 3, 4] = 1.0
+    rho = o.propagate_real(src, 2)
+    for d, L in enumerate(lat.shape):
+        x = (np.arange(L) - (3, 3, 4)[d]) * aa
+        msd = (rho.sum(axis=tuple(k for k in range(3) if k != d)) * x * x).sum()
+        assert abs(msd - 2 * alpha * ad[d] * aa * aa / 3.0) < 1e-14
+
+    lat = lpc_inputs.random_small((6, 4, 5), bc=(0, 0, 0), p_block=0.2, alpha=1.0, seed=64, n_steps=n)
+    link = np.ones((3,) + lat.shape)
+    link[0][-1] = 0.0   # the links between x = nx-1 and x = 0
+    cut = _mk(oracle_mod, lat, n_moments=3, max_steps=n, link=link)
+    import copy
+    wall = copy.copy(lat); wall.bc = (1, 0, 0)
+    ref = _mk(oracle_mod, wall, n_moments=3, max_steps=n)
+    cut.step(n); ref.step(n)
+    assert np.max(np.abs(cut.fid() - ref.fid())) < 1e-15 and np.max(np.abs(cut.moments()[0] - ref.moments()[0])) < 1e-16
+    # factors outside [0, 1] are rejected
+    bad = np.ones((3,) + lat.shape); bad[1, 0, 0, 0] = 1.5
+    with pytest.raises(ValueError):
+        _mk(oracle_mod, lat, link=bad)
 
 
 # --------------------------------------------------------------------------
