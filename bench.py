@@ -46,9 +46,12 @@ def parse():
     p.add_argument("--warmup", type=int, default=100)
     p.add_argument("--impl", default="ours", choices=["ours", "reference"])
     p.add_argument("--size", type=int, default=512, help="lattice edge L of the L^3 workload")
-    p.add_argument("--workload", default="sweep", choices=["sweep", "config0", "particle", "monolith", "supercap"],
+    p.add_argument("--workload", default="sweep", choices=["sweep", "config0", "particle", "monolith", "supercap", "film"],
                    help="sweep: configs[4] L^3 (default, the headline workload); the others are BASELINE.json configs[0..3] "
-                        "at their full sizes (particle 128^3, monolith 256^3 + moment fields, supercap 2048x256x256)")
+                        "at their full sizes (particle 128^3, monolith 256^3 + moment fields, supercap 2048x256x256); "
+                        "film: the 100x100x300 film-electrode cell of PAPER.md:236-248")
+    p.add_argument("--links", action="store_true",
+                   help="per-link mobility factors alpha_ij (PAPER.md:105): 0.25 on links that touch a porous site, 1 in the bulk")
     p.add_argument("--moments", type=int, default=0, choices=[0, 3], help="also propagate the 3 VACF fields")
     p.add_argument("--precision", type=int, default=0, choices=[0, 1])
     p.add_argument("--kernel", type=int, default=0, choices=[0, 1, 2, 3])
@@ -75,7 +78,9 @@ def workload_name(L, moments, precision, workload="sweep"):
     return {"config0": "configs[0]: 32^3 periodic, 30% blocked iid, dF ~ U[-3,0] kT, delta ~ U[-10,0] ppm",
             "particle": "configs[1] single porous carbon particle: 128^3 periodic, sphere R=48 porous (ell=4, 10% blocked), bulk outside",
             "monolith": "configs[2] carbon monolith: 256^3 periodic, pore field ell=8, 20% blocked",
-            "supercap": "configs[3] supercapacitor cell: 2048x256x256, reflective x, two film electrodes + bulk"}[workload] + ", " + tail
+            "supercap": "configs[3] supercapacitor cell: 2048x256x256, reflective x, two film electrodes + bulk",
+            "film": "film-electrode cell (PAPER.md:236-248): 100x100x300, reflective z, particles R=9 at 38% of the electrode volume, "
+                    "alpha=0.025"}[workload] + ", " + tail
 
 
 def make_workload(args):
@@ -88,6 +93,8 @@ def make_workload(args):
         return lpc_inputs.particle(n_moments=args.moments)
     if args.workload == "monolith":
         return lpc_inputs.monolith(n_moments=args.moments)
+    if args.workload == "film":
+        return lpc_inputs.film(n_moments=args.moments)
     return lpc_inputs.supercap(n_moments=args.moments)
 
 
@@ -199,8 +206,18 @@ def run_ours(args):
     h2d_job = sum(t.numel() * t.element_size() for t in host)
 
     sim = lpc.Lattice(lat.shape, bc=lat.bc, precision=args.precision, n_moments=args.moments, dt=lat.dt, a=lat.a,
-                      alpha=lat.alpha, max_steps=2 * K + W + 8, device=dev)
+                      alpha=lat.alpha, max_steps=2 * K + W + 8, device=dev, link_mobility=1 if args.links else 0)
     sim.set_kernel(args.kernel)
+    link = None
+    if args.links:
+        # reduced mobility under confinement: every link that touches a porous (dF != 0) site
+        link = torch.from_numpy(lpc_inputs.confined_links(lat.dF != 0.0, 0.25)).pin_memory()
+        h2d_job += link.numel() * link.element_size()
+
+    def set_params():
+        sim.set_site_params(*host)
+        if link is not None:
+            sim.set_link_mobility(link)
 
     def barrier():
         if world > 1:
@@ -210,11 +227,11 @@ def run_ours(args):
     # ---- end-to-end job through the C ABI with host buffers: upload + precompute + K steps, each step's G[n] read back
     e2e = None
     if not args.no_e2e:
-        sim.set_site_params(*host)          # warm the path once (page-in, module load)
+        set_params()          # warm the path once (page-in, module load)
         lpc.lpc_step_n(sim.handle, 3)
         barrier()
         t0 = time.perf_counter()
-        sim.set_site_params(*host)
+        set_params()
         last = None
         for k in range(K):
             lpc.lpc_step_n(sim.handle, 1)
@@ -228,7 +245,7 @@ def run_ours(args):
                        "lpc_read_fid of that step's sample to the host)"}
         assert np.isfinite(last).all()
     else:
-        sim.set_site_params(*host)
+        set_params()
 
     # ---- device-timed region: W warm-up steps, then exactly K steps between CUDA events on the library's stream
     lpc.lpc_step_n(sim.handle, W)
@@ -270,6 +287,8 @@ def run_ours(args):
         tpath = os.path.join(ROOT, "profiles", "traffic.csv")
         if os.path.exists(tpath):
             key = f"{L}^3/m{args.moments}/p{args.precision}" if args.workload == "sweep" else f"{args.workload}/m{args.moments}/p{args.precision}"
+            if args.links:
+                key += "/links"
             for row in open(tpath):
                 cols = row.strip().split(",")
                 if cols and cols[0] == key:
@@ -282,7 +301,8 @@ def run_ours(args):
                        "sites": n_sites, "parallelism": f"{world} independent replica(s), no collective",
                        "l2": (f"working set {bps * n_sites / 1e9:.2f} GB per step >> 126 MB L2, no flush needed"
                               if bps * n_sites > 4 * 126e6 else "working set is L2-sized: not an HBM measurement"),
-                       "kernel": {0: "auto", 1: "direct", 2: "tma", 3: "persistent"}[args.kernel]},
+                       "kernel": {0: "auto", 1: "direct", 2: "tma", 3: "persistent"}[args.kernel],
+                       "links": "alpha_ij = 0.25 on links that touch a porous site" if args.links else "none"},
             "clocks": clocks,
             "e2e": e2e,
             "gpu_launches": int(launches),

@@ -67,6 +67,7 @@ typedef struct lpc_config {
   int32_t n_moments;   /* 0, or 3 to propagate P^x, P^y, P^z for the VACF / D (Eq. 4)           */
   int32_t n_density;   /* 0, or 1 to propagate a real density rho alongside      */
   int32_t n_regions;   /* 0, or 1..8 regions ("blocks") for a region-resolved FID        */
+  int32_t link_mobility; /* 0, or 1 to reserve room for per-link mobility factors alpha_ij */
   double dt;           /* time step in s (5e-6)                                   */
   double a;            /* lattice spacing; D comes out in a^2 / dt units of it    */
   double alpha;        /* global jump factor in (0,1], Eq. 7                 */
@@ -100,6 +101,20 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
  * spread of dF exceeds about 700 kT), LPC_ECUDA.                                               */
 int lpc_set_site_params(lpc_lattice* lat, const double* dF_kT, const uint8_t* blocked,
                         const double* omega_rad_s, const void* g0_or_null);
+
+/* Per-link mobility factors alpha_ij ("a factor alpha_ij can be defined for each link between
+ * neighboring lattice sites i and j"; :305 reduced mobility under confinement):
+ *   p(i->j) = alpha_ij (alpha/6) min(1, exp(-(dF_j - dF_i))),  alpha_ij = alpha_ji in [0, 1],
+ * the same factor in both directions, so detailed balance and the Boltzmann density of Eq. 2 are kept.
+ * alpha_link: host or device, 3N doubles; alpha_link[d*N + i] is the factor of the link between site i and its
+ * +d neighbour (d = 0 x, 1 y, 2 z; on a periodic axis the last site links to the first, on a reflective axis
+ * the entry of the last site is ignored).  NULL removes the factors.  Needs link_mobility = 1 at creation
+ * (24 B per site more workspace in fp64) and must come after lpc_set_site_params and before the first step;
+ * it resets the state to g(0) = pi, P^d(1), Z_d[1] of the new hop probabilities and drops region labels (set
+ * state and labels afterwards).  The sweeps then read three stored link weights per site (80 B per site
+ * update in fp64 instead of 56); every kernel (TMA, direct, persistent) has that path.  Synchronises the stream.
+ * Errors: LPC_ESTATE (order, or created without link_mobility), LPC_EINVAL (a factor outside [0,1]), LPC_ECUDA. */
+int lpc_set_link_mobility(lpc_lattice* lat, const double* alpha_link);
 
 /* Advance n time steps (north star (b), (c); Eq. 13 + Eq. 12, Eq. 4): per step one fused sweep
  * that propagates, phase-rotates, reduces G[n] and (if enabled) Z_d[n+1], P^d, rho.

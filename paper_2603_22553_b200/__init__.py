@@ -23,7 +23,7 @@ LPC_FIELD_G, LPC_FIELD_PI, LPC_FIELD_PX, LPC_FIELD_PY, LPC_FIELD_PZ, LPC_FIELD_R
 LPC_KERNEL_AUTO, LPC_KERNEL_DIRECT, LPC_KERNEL_TMA, LPC_KERNEL_PERSIST = range(4)
 
 EXPORTS = (
-    "lpc_workspace_bytes", "lpc_create_lattice", "lpc_set_site_params", "lpc_step_n", "lpc_read_fid",
+    "lpc_workspace_bytes", "lpc_create_lattice", "lpc_set_site_params", "lpc_set_link_mobility", "lpc_step_n", "lpc_read_fid",
     "lpc_moments", "lpc_read_field", "lpc_set_state", "lpc_equilibrate", "lpc_seed_from_density", "lpc_set_regions", "lpc_read_fid_region", "lpc_moments_region", "lpc_spectrum", "lpc_set_kernel",
     "lpc_steps_done",
     "lpc_launch_count", "lpc_bytes_per_site_step", "lpc_destroy", "lpc_last_error",
@@ -40,6 +40,7 @@ class lpc_config(C.Structure):
     _fields_ = [
         ("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("bc", C.c_int32 * 3),
         ("precision", C.c_int32), ("n_moments", C.c_int32), ("n_density", C.c_int32), ("n_regions", C.c_int32),
+        ("link_mobility", C.c_int32),
         ("dt", C.c_double), ("a", C.c_double), ("alpha", C.c_double),
         ("max_steps", C.c_int64), ("stream", C.c_void_p),
     ]
@@ -61,6 +62,7 @@ def _load():
     lib.lpc_workspace_bytes.argtypes = [C.POINTER(lpc_config), C.POINTER(C.c_size_t)]
     lib.lpc_create_lattice.argtypes = [C.POINTER(lpc_config), C.c_void_p, C.c_size_t, C.POINTER(C.c_void_p)]
     lib.lpc_set_site_params.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.lpc_set_link_mobility.argtypes = [C.c_void_p, C.c_void_p]
     lib.lpc_step_n.argtypes = [C.c_void_p, C.c_int64]
     lib.lpc_read_fid.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_void_p]
     lib.lpc_moments.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
@@ -125,9 +127,9 @@ def _ptr(x, dtype=None, count=None):
 
 
 def make_config(nx, ny, nz, bc=(0, 0, 0), precision=0, n_moments=0, n_density=0, dt=5e-6, a=1.0, alpha=1.0,
-                max_steps=0, stream=None, n_regions=0) -> lpc_config:
+                max_steps=0, stream=None, n_regions=0, link_mobility=0) -> lpc_config:
     return lpc_config(int(nx), int(ny), int(nz), (C.c_int32 * 3)(*[int(b) for b in bc]), int(precision),
-                      int(n_moments), int(n_density), int(n_regions), float(dt), float(a), float(alpha), int(max_steps),
+                      int(n_moments), int(n_density), int(n_regions), int(link_mobility), float(dt), float(a), float(alpha), int(max_steps),
                       C.c_void_p(stream) if stream else None)
 
 
@@ -150,6 +152,11 @@ def lpc_create_lattice(cfg: lpc_config, workspace, nbytes=None):
 
 def lpc_set_site_params(handle, dF, blocked, omega, g0=None):
     _check(_lib.lpc_set_site_params(handle, _ptr(dF), _ptr(blocked), _ptr(omega), _ptr(g0)))
+
+
+def lpc_set_link_mobility(handle, alpha_link):
+    """alpha_link: [3, nx, ny, nz] float64 (host numpy or CUDA tensor), or None to remove the factors."""
+    _check(_lib.lpc_set_link_mobility(handle, _ptr(alpha_link)))
 
 
 def lpc_step_n(handle, n):
@@ -250,7 +257,7 @@ class Lattice:
     """Owns the torch workspace and the handle; methods forward to the C calls one to one."""
 
     def __init__(self, shape, bc=(0, 0, 0), precision=0, n_moments=0, n_density=0, dt=5e-6, a=1.0, alpha=1.0,
-                 max_steps=0, device="cuda:0", stream=None, n_regions=0):
+                 max_steps=0, device="cuda:0", stream=None, n_regions=0, link_mobility=0):
         import torch
 
         self.shape = tuple(int(v) for v in shape)
@@ -260,7 +267,8 @@ class Lattice:
             stream = torch.cuda.current_stream(self.device)
         self.stream = stream
         self.cfg = make_config(*self.shape, bc=bc, precision=precision, n_moments=n_moments, n_density=n_density,
-                               dt=dt, a=a, alpha=alpha, max_steps=max_steps, stream=stream.cuda_stream, n_regions=n_regions)
+                               dt=dt, a=a, alpha=alpha, max_steps=max_steps, stream=stream.cuda_stream, n_regions=n_regions,
+                               link_mobility=link_mobility)
         self.workspace_bytes = lpc_workspace_bytes(self.cfg)
         with torch.cuda.device(self.device):
             self.workspace = torch.empty(self.workspace_bytes, dtype=torch.uint8, device=self.device)
@@ -268,13 +276,18 @@ class Lattice:
 
     @classmethod
     def from_inputs(cls, lat, precision=0, n_moments=None, n_density=0, max_steps=None, device="cuda:0", g0=None,
-                    n_regions=0):
+                    n_regions=0, link=None):
         """Build from an ``lpc_inputs.Lattice`` (host arrays) and run the precompute."""
         self = cls(lat.shape, bc=lat.bc, precision=precision,
                    n_moments=lat.n_moments if n_moments is None else n_moments, n_density=n_density,
                    dt=lat.dt, a=lat.a, alpha=lat.alpha,
-                   max_steps=lat.n_steps if max_steps is None else max_steps, device=device, n_regions=n_regions)
-        self.set_site_params(lat.dF, lat.blocked, lat.omega, g0)
+                   max_steps=lat.n_steps if max_steps is None else max_steps, device=device, n_regions=n_regions,
+                   link_mobility=0 if link is None else 1)
+        self.set_site_params(lat.dF, lat.blocked, lat.omega, None if link is not None else g0)
+        if link is not None:
+            self.set_link_mobility(link)
+            if g0 is not None:
+                self.set_state(LPC_FIELD_G, g0)
         return self
 
     def close(self):
@@ -297,6 +310,11 @@ class Lattice:
         if isinstance(g0, np.ndarray):
             g0 = np.ascontiguousarray(g0, dtype=np.complex128)
         lpc_set_site_params(self.handle, dF, blocked, omega, g0)
+
+    def set_link_mobility(self, alpha_link):
+        if isinstance(alpha_link, np.ndarray):
+            alpha_link = np.ascontiguousarray(alpha_link, dtype=np.float64)
+        lpc_set_link_mobility(self.handle, alpha_link)
 
     def step(self, n=1):
         lpc_step_n(self.handle, n)

@@ -50,7 +50,7 @@ constexpr long long STAGE_SITES = 4ll << 20;  // sites per host<->device staging
 constexpr long long SPEC_BATCH = 4096;        // frequencies per spectrum launch
 
 struct Offsets {
-  size_t ctl, fid, vacf, partials, pi, cs, f0, f1, regions, fidr, vacfr, wr, rpartials, spec, staging, total;
+  size_t ctl, fid, vacf, partials, pi, cs, mlink, f0, f1, regions, fidr, vacfr, wr, rpartials, spec, staging, total;
   size_t partial_slots;
 };
 
@@ -68,6 +68,7 @@ struct lpc_lattice {
   bool have_regions;
   long long region_first;  // first sample of the regional series
   bool region_moments;     // the regional VACF is being recorded (labels were set at step 0)
+  bool have_links;         // per-link mobility factors are set: the sweeps read the stored link weights
   int cur;  // index of the buffer holding the current state
   long long steps;
   long long launches;
@@ -75,6 +76,7 @@ struct lpc_lattice {
   // TMA geometry
   int ty, tz, nstage, xc, tiles_z, tiles_y, chunks_x;
   bool tma_ok;
+  TmaLinkMaps tm_l;  // pi centres and the three link-weight channels (link_mobility = 1)
   CUtensorMap tm_f[2], tm_m[2], tm_pi, tm_cs;  // tm_f: magnetisation (+ density) channels, tm_m: the 3 moment channels
 };
 
@@ -89,6 +91,7 @@ int check_cfg(const lpc_config* c) {
   if (c->precision != 0 && c->precision != 1) return fail(LPC_EINVAL, "precision must be 0 (fp64) or 1 (fp32)");
   if (c->n_moments != 0 && c->n_moments != 3) return fail(LPC_EINVAL, "n_moments must be 0 or 3");
   if (c->n_density != 0 && c->n_density != 1) return fail(LPC_EINVAL, "n_density must be 0 or 1");
+  if (c->link_mobility != 0 && c->link_mobility != 1) return fail(LPC_EINVAL, "link_mobility must be 0 or 1");
   if (c->n_regions < 0 || c->n_regions > MAX_REGIONS) return fail(LPC_EINVAL, "n_regions must lie in [0, %d]", MAX_REGIONS);
   if (!(c->alpha > 0.0 && c->alpha <= 1.0)) return fail(LPC_EINVAL, "alpha must lie in (0,1]");
   if (!(c->dt > 0.0) || !std::isfinite(c->dt)) return fail(LPC_EINVAL, "dt must be positive");
@@ -172,6 +175,7 @@ Offsets make_offsets(const lpc_config* c, const Layout& L) {
   o.partials = p; p += align_up(o.partial_slots * MAX_RED * sizeof(double));
   o.pi = p; p += align_up((size_t)L.np * sT);
   o.cs = p; p += align_up((size_t)2 * L.np * sT);
+  o.mlink = p; p += align_up(c->link_mobility ? (size_t)3 * L.np * sT : 0);
   o.f0 = p; p += align_up((size_t)C * L.np * sT);
   o.f1 = p; p += align_up((size_t)C * L.np * sT);
   o.regions = p; p += align_up(c->n_regions ? (size_t)N : 0);
@@ -222,6 +226,7 @@ int encode_map(CUtensorMap* m, bool f32, void* base, int rank, const cuuint64_t*
 }
 
 template <typename T> T* wsp(lpc_lattice* h, size_t off) { return reinterpret_cast<T*>(h->ws + off); }
+template <typename T> const T* mlink_of(lpc_lattice* h) { return h->have_links ? wsp<T>(h, h->off.mlink) : nullptr; }
 
 bool is_device_ptr(const void* p) {
   cudaPointerAttributes at;
@@ -243,6 +248,7 @@ int launch_step_t(lpc_lattice* h) {
   a.fout = wsp<T>(h, h->cur ? h->off.f0 : h->off.f1);
   a.pi = wsp<T>(h, h->off.pi);
   a.cs = wsp<T>(h, h->off.cs);
+  a.mlink = mlink_of<T>(h);
   a.a6 = (T)(h->cfg.alpha / 6.0);
   a.partials = wsp<double>(h, h->off.partials);
   a.ctl = wsp<Ctl>(h, h->off.ctl);
@@ -272,16 +278,33 @@ int launch_step_t(lpc_lattice* h) {
     // channels first (Z_d[k+1], P^d <- W P^d; no phase, no cos/sin traffic), then the magnetisation
     // (and density) channels, which also advance the step counter.  One 5-channel sweep needs more
     // than 200 registers per thread and leaves one 8-warp CTA per SM (measured 42 GLUPS at 512^3).
+    // With stored link weights (per-link mobility) the same two sweeps run as step_tma_links_kernel, with one
+    // stage less where the link boxes would not leave room for two CTAs per SM.
+    auto launch_links = [&](auto kern, auto cfg, const CUtensorMap& tm, const StepArgs<T>& args) -> int {
+      using K = decltype(cfg);
+      static bool attr_set = false;
+      if (!attr_set) {
+        CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, K::SMEM_BYTES));
+        attr_set = true;
+      }
+      kern<<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(tm, h->tm_cs, h->tm_l, args);
+      CUDA_TRY(cudaGetLastError());
+      h->launches++;
+      return LPC_OK;
+    };
     if constexpr (NMOM == 3) {
       StepArgs<T> am = a;
       am.c0 = 2 + NRHO;
       am.fout = a.fout + (long long)am.c0 * h->L.np;
-      int rc = launch(step_tma_kernel<T, 0, 0, 3, 8, 64, 4>, TmaCfg<T, 0, 0, 3, 8, 64, 4>(), h->tm_m[h->cur], am);
+      int rc = h->have_links ? launch_links(step_tma_links_kernel<T, 0, 0, 3, 8, 64, 3>, TmaCfg<T, 0, 0, 3, 8, 64, 3, 1>(), h->tm_m[h->cur], am)
+                             : launch(step_tma_kernel<T, 0, 0, 3, 8, 64, 4>, TmaCfg<T, 0, 0, 3, 8, 64, 4>(), h->tm_m[h->cur], am);
       if (rc) return rc;
     }
     a.c0 = 0;
     constexpr int NS = (NRHO == 0) ? 4 : 3;   // two CTAs per SM must fit in shared memory
-    int rc = launch(step_tma_kernel<T, 2, NRHO, 0, 8, 64, NS>, TmaCfg<T, 2, NRHO, 0, 8, 64, NS>(), h->tm_f[h->cur], a);
+    constexpr int NSL = (NRHO == 0) ? 3 : 2;
+    int rc = h->have_links ? launch_links(step_tma_links_kernel<T, 2, NRHO, 0, 8, 64, NSL>, TmaCfg<T, 2, NRHO, 0, 8, 64, NSL, 1>(), h->tm_f[h->cur], a)
+                           : launch(step_tma_kernel<T, 2, NRHO, 0, 8, 64, NS>, TmaCfg<T, 2, NRHO, 0, 8, 64, NS>(), h->tm_f[h->cur], a);
     if (rc) return rc;
     h->cur ^= 1;
     return LPC_OK;
@@ -308,6 +331,7 @@ int launch_persist_t(lpc_lattice* h, int64_t n) {
   a.fout = nullptr;
   a.pi = wsp<T>(h, h->off.pi);
   a.cs = wsp<T>(h, h->off.cs);
+  a.mlink = mlink_of<T>(h);
   a.a6 = (T)(h->cfg.alpha / 6.0);
   a.partials = wsp<double>(h, h->off.partials);
   a.ctl = wsp<Ctl>(h, h->off.ctl);
@@ -405,7 +429,7 @@ int region_moment_t(lpc_lattice* h) {
   const T* q = wsp<T>(h, h->cur ? h->off.f1 : h->off.f0) + (long long)(2 + h->nrho) * h->L.np;
   const double scale = INIT ? h->cfg.a * h->cfg.a * h->cfg.alpha / 6.0 : h->cfg.a * h->cfg.alpha / 6.0;
   region_moment_kernel<T, INIT><<<aux_grid(h->N), 256, 0, h->stream>>>(
-      h->L, wsp<T>(h, h->off.pi), q, h->ws + h->off.regions, h->cfg.n_regions, wsp<double>(h, h->off.rpartials), wsp<Ctl>(h, h->off.ctl),
+      h->L, wsp<T>(h, h->off.pi), mlink_of<T>(h), q, h->ws + h->off.regions, h->cfg.n_regions, wsp<double>(h, h->off.rpartials), wsp<Ctl>(h, h->off.ctl),
       wsp<double>(h, h->off.wr), wsp<double>(h, h->off.vacfr), h->cfg.max_steps + 2, INIT ? 1 : h->steps + 2, scale);
   CUDA_TRY(cudaGetLastError());
   h->launches++;
@@ -440,6 +464,28 @@ int set_g_from(lpc_lattice* h, const void* g) {
   if (rc) return rc;
   reduce_g_kernel<T><<<aux_grid(h->N), 256, 0, h->stream>>>(h->L, wsp<T>(h, h->off.pi), f, wsp<double>(h, h->off.partials),
                                                              wsp<Ctl>(h, h->off.ctl), wsp<double2>(h, h->off.fid));
+  CUDA_TRY(cudaGetLastError());
+  h->launches++;
+  return LPC_OK;
+}
+
+// Initial state: h = 1 (g(0) = pi), r = 1, q^d(1), and the sums G[0], Z_d[1]; uses the link weights if they are set.
+template <typename T>
+int init_state_t(lpc_lattice* h) {
+  const Layout& L = h->L;
+  Ctl* ctl = wsp<Ctl>(h, h->off.ctl);
+  h->cur = 0;
+  T* f = wsp<T>(h, h->off.f0);
+  auto init = [&](auto kern) {
+    kern<<<aux_grid(h->N), 256, 0, h->stream>>>(L, wsp<T>(h, h->off.pi), mlink_of<T>(h), (T)(h->cfg.alpha / 6.0), f, h->cfg.a,
+                                                 wsp<double>(h, h->off.partials), ctl, wsp<double2>(h, h->off.fid),
+                                                 wsp<double>(h, h->off.vacf), h->cfg.max_steps + 2,
+                                                 h->cfg.a * h->cfg.a * h->cfg.alpha / 6.0);
+  };
+  if (h->nrho == 0 && h->nmom == 0) init(init_state_kernel<T, 0, 0>);
+  else if (h->nrho == 1 && h->nmom == 0) init(init_state_kernel<T, 1, 0>);
+  else if (h->nrho == 0 && h->nmom == 3) init(init_state_kernel<T, 0, 3>);
+  else init(init_state_kernel<T, 1, 3>);
   CUDA_TRY(cudaGetLastError());
   h->launches++;
   return LPC_OK;
@@ -506,19 +552,8 @@ int set_site_params_t(lpc_lattice* h, const double* dF, const uint8_t* blocked, 
   CUDA_TRY(cudaMemsetAsync(h->ws + h->off.f1, 0, (size_t)h->C * L.np * h->sT, h->stream));
 
   // initial state
-  h->cur = 0;
-  T* f = wsp<T>(h, h->off.f0);
-  auto init = [&](auto kern) {
-    kern<<<aux_grid(h->N), 256, 0, h->stream>>>(L, wsp<T>(h, h->off.pi), (T)(h->cfg.alpha / 6.0), f, h->cfg.a, wsp<double>(h, h->off.partials),
-                                                 ctl, wsp<double2>(h, h->off.fid), wsp<double>(h, h->off.vacf), h->cfg.max_steps + 2,
-                                                 h->cfg.a * h->cfg.a * h->cfg.alpha / 6.0);
-  };
-  if (h->nrho == 0 && h->nmom == 0) init(init_state_kernel<T, 0, 0>);
-  else if (h->nrho == 1 && h->nmom == 0) init(init_state_kernel<T, 1, 0>);
-  else if (h->nrho == 0 && h->nmom == 3) init(init_state_kernel<T, 0, 3>);
-  else init(init_state_kernel<T, 1, 3>);
-  CUDA_TRY(cudaGetLastError());
-  h->launches++;
+  rc = init_state_t<T>(h);
+  if (rc) return rc;
   if (g0) {
     rc = set_g_from<T>(h, g0);
     if (rc) return rc;
@@ -528,6 +563,49 @@ int set_site_params_t(lpc_lattice* h, const double* dF, const uint8_t* blocked, 
   CUDA_TRY(cudaStreamSynchronize(h->stream));
   h->steps = 0;
   h->have_params = true;
+  return LPC_OK;
+}
+
+// Per-link mobility factors: stored link weights m_{i,+d} = alpha_{i,i+e_d} min(pi_i, pi_{i+e_d}), then the initial state again
+// (q^d(1) and Z_d[1] depend on the hop probabilities).
+template <typename T>
+int set_link_mobility_t(lpc_lattice* h, const double* alpha_link) {
+  const Layout& L = h->L;
+  Ctl* ctl = wsp<Ctl>(h, h->off.ctl);
+  h->have_links = false;
+  int rc;
+  if (alpha_link) {
+    T* m = wsp<T>(h, h->off.mlink);
+    CUDA_TRY(cudaMemsetAsync(m, 0, (size_t)3 * L.np * sizeof(T), h->stream));
+    CUDA_TRY(cudaMemsetAsync(&ctl->bad, 0, sizeof(ctl->bad), h->stream));
+    const long long stride[3] = {L.sx, L.sy, 1};
+    for (int d = 0; d < 3; ++d) {
+      rc = for_chunks_in(h, alpha_link + (size_t)d * h->N, 8, [&](const void* src, long long i0, long long n) {
+        link_weights_kernel<T><<<aux_grid(n), 256, 0, h->stream>>>(static_cast<const double*>(src), i0, n, L, stride[d],
+                                                                    wsp<T>(h, h->off.pi), m + (long long)d * L.np, ctl);
+        CUDA_TRY(cudaGetLastError());
+        h->launches++;
+        return LPC_OK;
+      });
+      if (rc) return rc;
+    }
+    const long long cells = 2ll * ((long long)L.nx * L.ny + (long long)L.nx * L.nz + (long long)L.ny * L.nz) * 3;
+    fill_ghosts_kernel<T><<<aux_grid(cells), 256, 0, h->stream>>>(m, 3, L, h->cfg.bc[0] == 0, h->cfg.bc[1] == 0, h->cfg.bc[2] == 0);
+    CUDA_TRY(cudaGetLastError());
+    h->launches++;
+    unsigned long long bad = 0;
+    CUDA_TRY(cudaMemcpyAsync(&bad, &ctl->bad, sizeof(bad), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    if (bad) return fail(LPC_EINVAL, "%llu link factors lie outside [0, 1]", bad);
+    h->have_links = true;
+  }
+  CUDA_TRY(cudaMemsetAsync(h->ws + h->off.f0, 0, (size_t)h->C * L.np * h->sT, h->stream));
+  CUDA_TRY(cudaMemsetAsync(h->ws + h->off.f1, 0, (size_t)h->C * L.np * h->sT, h->stream));
+  rc = init_state_t<T>(h);
+  if (rc) return rc;
+  rc = fill_state_ghosts<T>(h);
+  if (rc) return rc;
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
   return LPC_OK;
 }
 
@@ -609,6 +687,7 @@ int equilibrate_t(lpc_lattice* h, double threshold, int64_t max_iters, int64_t c
   EquilArgs<T> a;
   a.L = L;
   a.pi = wsp<T>(h, h->off.pi);
+  a.mlink = mlink_of<T>(h);
   a.a6 = (T)(h->cfg.alpha / 6.0);
   a.partials = wsp<double>(h, h->off.partials);
   a.ctl = ctl;
@@ -713,6 +792,7 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
   h->have_params = false;
   h->have_regions = false;
   h->region_moments = false;
+  h->have_links = false;
   h->region_first = 0;
   h->cur = 0;
   h->steps = 0;
@@ -741,6 +821,17 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
     if (!rc && h->nmom == 3) rc = encode_map(&h->tm_m[1], f32, h->ws + h->off.f1, 4, d4, bm);
     if (!rc) rc = encode_map(&h->tm_pi, f32, h->ws + h->off.pi, 3, d4, b4);
     if (!rc) rc = encode_map(&h->tm_cs, f32, h->ws + h->off.cs, 4, dk, bk);
+    if (!rc && cfg->link_mobility) {
+      // pi centres and m_x: the tile itself; m_y: one more row below; m_z: 16 bytes of columns below
+      const size_t chan = (size_t)L.np * h->sT;
+      const cuuint32_t bc[3] = {(cuuint32_t)h->tz, (cuuint32_t)h->ty, 1};
+      const cuuint32_t by[3] = {(cuuint32_t)h->tz, (cuuint32_t)(h->ty + 1), 1};
+      const cuuint32_t bz[3] = {(cuuint32_t)(h->tz + 16 / h->sT), (cuuint32_t)h->ty, 1};
+      rc = encode_map(&h->tm_l.pic, f32, h->ws + h->off.pi, 3, d4, bc);
+      if (!rc) rc = encode_map(&h->tm_l.mx, f32, h->ws + h->off.mlink, 3, d4, bc);
+      if (!rc) rc = encode_map(&h->tm_l.my, f32, h->ws + h->off.mlink + chan, 3, d4, by);
+      if (!rc) rc = encode_map(&h->tm_l.mz, f32, h->ws + h->off.mlink + 2 * chan, 3, d4, bz);
+    }
     if (rc) {
       delete h;
       return rc;
@@ -756,7 +847,18 @@ int lpc_set_site_params(lpc_lattice* h, const double* dF, const uint8_t* blocked
   h->have_params = false;
   h->have_regions = false;
   h->region_moments = false;
+  h->have_links = false;
   return h->cfg.precision ? set_site_params_t<float>(h, dF, blocked, omega, g0) : set_site_params_t<double>(h, dF, blocked, omega, g0);
+}
+
+int lpc_set_link_mobility(lpc_lattice* h, const double* alpha_link) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
+  if (!h->cfg.link_mobility) return fail(LPC_ESTATE, "the lattice was created without link_mobility = 1");
+  if (h->steps != 0) return fail(LPC_ESTATE, "link factors must be set before the first step");
+  h->have_regions = false;
+  h->region_moments = false;
+  return h->cfg.precision ? set_link_mobility_t<float>(h, alpha_link) : set_link_mobility_t<double>(h, alpha_link);
 }
 
 int lpc_step_n(lpc_lattice* h, int64_t n) {
@@ -950,7 +1052,8 @@ double lpc_bytes_per_site_step(const lpc_lattice* h) {
   if (!h) return 0.0;
   // read C state channels + pi + cos + sin, write C state channels; with region labels one more pass
   // reads h (2 channels), pi and the label
-  return (double)h->sT * (2.0 * h->C + 3.0) + (h->have_regions ? 3.0 * h->sT + 1.0 : 0.0);
+  // with per-link mobility factors the sweep also reads three stored link weights per site
+  return (double)h->sT * (2.0 * h->C + 3.0 + (h->have_links ? 3.0 : 0.0)) + (h->have_regions ? 3.0 * h->sT + 1.0 : 0.0);
 }
 
 void lpc_destroy(lpc_lattice* h) { delete h; }

@@ -20,6 +20,7 @@ struct EquilArgs {
   const T* rin;   // density channel of the buffer that holds rho(t)
   T* rout;        // density channel of the other buffer
   const T* pi;
+  const T* mlink;  // nullptr or the stored link weights (per-link mobility)
   T a6;
   double* partials;
   Ctl* ctl;
@@ -48,7 +49,10 @@ __global__ void __launch_bounds__(256) equil_kernel(EquilArgs<T> a) {
       if (s == 1 && !vb) break;
       const long long j = i + s;
       SiteUpdate<T, 0, 0> u;
-      u.weights(pi[j], pi[j - L.sx], pi[j + L.sx], pi[j - L.sy], pi[j + L.sy], pi[j - 1], pi[j + 1], a.a6, (T)1, (T)0);
+      if (a.mlink)
+        u.weights_links(pi[j], a.mlink + j, L.np, L.sx, L.sy, a.a6, (T)1, (T)0);
+      else
+        u.weights(pi[j], pi[j - L.sx], pi[j + L.sx], pi[j - L.sy], pi[j + L.sy], pi[j - 1], pi[j + 1], a.a6, (T)1, (T)0);
       const T fc = f[j];
       out[s] = u.gather(fc, f[j - L.sx], f[j + L.sx], f[j - L.sy], f[j + L.sy], f[j - 1], f[j + 1]);
       // rho' - rho = pi (r' - r); the product and the difference are taken in fp64

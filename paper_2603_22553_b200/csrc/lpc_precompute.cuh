@@ -112,13 +112,29 @@ __global__ void fill_ghosts_kernel(T* __restrict__ f, int nch, Layout L, int per
   }
 }
 
+// Stored link weights for per-link mobility factors: m_{i,+d} = alpha_{i,i+e_d} min(pi_i, pi_{i+e_d})
+// for the interior sites of channel d; `link` points at site i0 of the dense factor array of that axis.  The
+// ghosts of pi are in place (wrapped value or 0), so a link through a reflective wall gets weight 0.
+template <typename T>
+__global__ void link_weights_kernel(const double* __restrict__ link, long long i0, long long n, Layout L, long long stride,
+                                    const T* __restrict__ pi, T* __restrict__ m, Ctl* ctl) {
+  unsigned long long bad = 0;
+  for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (long long)gridDim.x * blockDim.x) {
+    const long long j = dense_to_padded(L, i0 + k);
+    const double a = link[k];
+    if (!(a >= 0.0 && a <= 1.0)) bad++;
+    m[j] = (T)a * tmin(pi[j], pi[j + stride]);
+  }
+  if (bad) atomicAdd(&ctl->bad, bad);
+}
+
 // Initial state in density-normalised form:
 //   h = 1 on open sites (g(0) = pi, real), r = 1 (rho(0) = pi),
 //   q^d(1) = P^d(1)/pi = a kappa_i [m_{i,-d} - m_{i,+d}]                       (O7; Eq. 4, 5)
 // and the sums G[0] = sum pi h, Z_d[1] = a^2 (alpha/6) sum_i [m_{i,+d} + m_{i,-d}].
 template <typename T, int NRHO, int NMOM>
 __global__ void __launch_bounds__(256)
-    init_state_kernel(Layout L, const T* __restrict__ pi, T a6, T* __restrict__ f, double a_len,
+    init_state_kernel(Layout L, const T* __restrict__ pi, const T* __restrict__ mlink, T a6, T* __restrict__ f, double a_len,
                       double* partials, Ctl* ctl, double2* fid, double* vacf, long long vacf_stride, double zscale) {
   constexpr int NRED = 2 + NMOM;
   double acc[NRED];
@@ -137,7 +153,8 @@ __global__ void __launch_bounds__(256)
       const long long st[3] = {L.sx, L.sy, 1};
 #pragma unroll
       for (int d = 0; d < 3; ++d) {
-        const T mm = tmin(p, pi[j - st[d]]), mp = tmin(p, pi[j + st[d]]);
+        const T* ml = mlink + (long long)d * L.np + j;
+        const T mm = mlink ? ml[-st[d]] : tmin(p, pi[j - st[d]]), mp = mlink ? ml[0] : tmin(p, pi[j + st[d]]);
         f[(long long)(2 + NRHO + d) * L.np + j] = (T)a_len * kappa_of(p, a6) * (mm - mp);
         acc[2 + d] += (double)mp + (double)mm;
       }

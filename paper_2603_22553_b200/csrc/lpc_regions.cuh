@@ -82,7 +82,8 @@ __global__ void __launch_bounds__(256)
 // accumulators, block partials, fixed-order sum by the last block.
 template <typename T, bool INIT>
 __global__ void __launch_bounds__(256)
-    region_moment_kernel(Layout L, const T* __restrict__ pi, const T* __restrict__ q, const uint8_t* __restrict__ label, int n_regions,
+    region_moment_kernel(Layout L, const T* __restrict__ pi, const T* __restrict__ mlink, const T* __restrict__ q,
+                         const uint8_t* __restrict__ label, int n_regions,
                          double* partials, Ctl* ctl, double* wr, double* vacfr, long long stride, long long index, double scale) {
   constexpr int NV = INIT ? 4 : 3;   // INIT also sums pi
   double acc[MAX_REGIONS][NV];
@@ -99,7 +100,8 @@ __global__ void __launch_bounds__(256)
     double v[NV];
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
-      const T mm = tmin(p, pi[j - st[d]]), mp = tmin(p, pi[j + st[d]]);
+      const T* ml = mlink + (long long)d * L.np + j;
+      const T mm = mlink ? ml[-st[d]] : tmin(p, pi[j - st[d]]), mp = mlink ? ml[0] : tmin(p, pi[j + st[d]]);
       v[d] = INIT ? (double)mp + (double)mm : (double)q[(long long)d * L.np + j] * (double)(mp - mm);
     }
     if (INIT) v[NV - 1] = (double)p;

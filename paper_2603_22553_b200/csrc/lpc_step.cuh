@@ -104,7 +104,10 @@ __device__ __forceinline__ void direct_sweep(const StepArgs<T>& a, const T* __re
       if (s == 1 && !vb) break;
       const long long j = i + s;
       SiteUpdate<T, NRHO, NMOM> u;
-      u.weights(pi[j], pi[j - L.sx], pi[j + L.sx], pi[j - L.sy], pi[j + L.sy], pi[j - 1], pi[j + 1], a.a6, csv[j], snv[j]);
+      if (a.mlink)
+        u.weights_links(pi[j], a.mlink + j, L.np, L.sx, L.sy, a.a6, csv[j], snv[j]);
+      else
+        u.weights(pi[j], pi[j - L.sx], pi[j + L.sx], pi[j - L.sy], pi[j + L.sy], pi[j - 1], pi[j + 1], a.a6, csv[j], snv[j]);
 #pragma unroll
       for (int c = 0; c < C; ++c) {
         const T* __restrict__ f = fin + (long long)c * L.np;
@@ -229,7 +232,15 @@ __global__ void __launch_bounds__(256) step_persist_kernel(StepArgs<T> a, T* buf
 // TMA kernel.
 // ---------------------------------------------------------------------------------------------
 // NH = 2: the sweep carries the magnetisation (h_re, h_im, phase multiply, G); NH = 0: real channels only.
-template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE>
+// LK = 1: per-link mobility factors.  The symmetric link weights m_{i,+d} are stored (3 channels) and
+// staged per plane instead of being rebuilt from pi: m_x without halo (the -x link is the +x link of the plane
+// below, carried in registers), m_y with one halo row below, m_z with one halo column (HZ wide) below; pi is then
+// needed at the centres only.
+struct TmaLinkMaps {
+  CUtensorMap pic, mx, my, mz;   // pi centres, the three link channels
+};
+
+template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int LK = 0>
 struct TmaCfg {
   static constexpr int C = NH + NRHO + NMOM;
   static constexpr int NRED = 2 + NMOM;
@@ -240,12 +251,23 @@ struct TmaCfg {
   static constexpr int NCW = NCONS / 32;
   static constexpr int NTHREADS = NCONS;      // no producer warp: thread 0 issues the TMA loads between planes
   static constexpr int F_RAW = C * TYH * TZW * (int)sizeof(T);
-  static constexpr int PI_RAW = TYH * TZW * (int)sizeof(T);
+  static constexpr int TZM = TZ + HZ;         // row length of the staged m_z box
+  static constexpr int PI_RAW = (LK ? TY * TZ : TYH * TZW) * (int)sizeof(T);
+  static constexpr int MX_RAW = LK ? TY * TZ * (int)sizeof(T) : 0;
+  static constexpr int MY_RAW = LK ? (TY + 1) * TZ * (int)sizeof(T) : 0;
+  static constexpr int MZ_RAW = LK ? TY * TZM * (int)sizeof(T) : 0;
+  static constexpr int MX_BYTES = (MX_RAW + 127) / 128 * 128;
+  static constexpr int MY_BYTES = (MY_RAW + 127) / 128 * 128;
+  static constexpr int MZ_BYTES = (MZ_RAW + 127) / 128 * 128;
   static constexpr int KCS_RAW = NH * TY * TZ * (int)sizeof(T);  // cos, sin (no halo); none without the magnetisation
   static constexpr int F_BYTES = (F_RAW + 127) / 128 * 128;
   static constexpr int PI_BYTES = (PI_RAW + 127) / 128 * 128;
   static constexpr int KCS_BYTES = (KCS_RAW + 127) / 128 * 128;
-  static constexpr int STAGE_BYTES = F_BYTES + PI_BYTES + KCS_BYTES;
+  static constexpr int MX_OFF = F_BYTES + PI_BYTES + KCS_BYTES;
+  static constexpr int MY_OFF = MX_OFF + MX_BYTES;
+  static constexpr int MZ_OFF = MY_OFF + MY_BYTES;
+  static constexpr int STAGE_BYTES = MZ_OFF + MZ_BYTES;
+  static constexpr int TX_BYTES = F_RAW + PI_RAW + MX_RAW + MY_RAW + MZ_RAW;   // per stage, without cos/sin
   static constexpr int BAR_OFF = NSTAGE * STAGE_BYTES;
   static constexpr int RED_OFF = BAR_OFF + 2 * NSTAGE * 8;
   static constexpr int SMEM_BYTES = RED_OFF + ((NTHREADS / 32) * NRED + 1) * 8 + 128;  // +128: manual alignment slack
@@ -257,11 +279,10 @@ struct TmaCfg {
   static_assert(TZ % 2 == 0, "TZ must be even");
 };
 
-template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE>
-__global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE>::LB_THREADS, TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE>::LB_CTAS)
-    step_tma_kernel(const __grid_constant__ CUtensorMap tm_f, const __grid_constant__ CUtensorMap tm_pi,
-                    const __grid_constant__ CUtensorMap tm_cs, StepArgs<T> a) {
-  using K = TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE>;
+template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int LK, typename LM>
+__device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUtensorMap& tm_pi, const CUtensorMap& tm_cs, const LM& lm,
+                                              const StepArgs<T>& a) {
+  using K = TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, LK>;
   using V2 = typename Vec2<T>::type;
   constexpr int C = K::C, NRED = K::NRED, TZW = K::TZW, TYH = K::TYH, HZ = K::HZ;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -300,16 +321,30 @@ __global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE>::LB_
     if (jl >= NSTAGE) mbar_wait(&empty[s], ((jl / NSTAGE) - 1) & 1);   // every warp is done with the plane it held
     unsigned char* st = smem + s * K::STAGE_BYTES;
     const bool need_kcs = (NH == 2) && (jl >= 1 && jl <= nplanes);
-    mbar_expect_tx(&full[s], K::F_RAW + K::PI_RAW + (need_kcs ? K::KCS_RAW : 0));
+    mbar_expect_tx(&full[s], K::TX_BYTES + (need_kcs ? K::KCS_RAW : 0));
     // plane x0-1+j lives at padded x coordinate x0+j; box starts HZ columns / 1 row before the tile
     tma_load_4d(st, &tm_f, &full[s], L.padz + z0 - HZ, y0, x0 + jl, a.c0);
-    tma_load_3d(st + K::F_BYTES, &tm_pi, &full[s], L.padz + z0 - HZ, y0, x0 + jl);
+    if constexpr (LK) {
+      tma_load_3d(st + K::F_BYTES, &lm.pic, &full[s], L.padz + z0, y0 + 1, x0 + jl);
+      tma_load_3d(st + K::MX_OFF, &lm.mx, &full[s], L.padz + z0, y0 + 1, x0 + jl);
+      tma_load_3d(st + K::MY_OFF, &lm.my, &full[s], L.padz + z0, y0, x0 + jl);           // rows y0-1 .. y0+TY-1
+      tma_load_3d(st + K::MZ_OFF, &lm.mz, &full[s], L.padz + z0 - HZ, y0 + 1, x0 + jl);  // columns z0-HZ .. z0+TZ-1
+    } else {
+      tma_load_3d(st + K::F_BYTES, &tm_pi, &full[s], L.padz + z0 - HZ, y0, x0 + jl);
+    }
     if (need_kcs) tma_load_4d(st + K::F_BYTES + K::PI_BYTES, &tm_cs, &full[s], L.padz + z0, y0 + 1, x0 + jl, 0);
     ++jl;
   };
   if (threadIdx.x == 0) {
     tma_prefetch_desc(&tm_f);
-    tma_prefetch_desc(&tm_pi);
+    if constexpr (LK) {
+      tma_prefetch_desc(&lm.pic);
+      tma_prefetch_desc(&lm.mx);
+      tma_prefetch_desc(&lm.my);
+      tma_prefetch_desc(&lm.mz);
+    } else {
+      tma_prefetch_desc(&tm_pi);
+    }
     tma_prefetch_desc(&tm_cs);
     for (int j = 0; j < NSTAGE && j < nloads; ++j) issue_load();
   }
@@ -329,7 +364,8 @@ __global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE>::LB_
 
     // One x-plane as a consumer thread holds it: the centre pair of every channel and of pi, kappa of
     // the pair, and mlo = min(pi, pi of the plane below) -- the symmetric link weight m_ij of the -x
-    // link (which is the +x link of the plane below).
+    // link (which is the +x link of the plane below).  With stored link weights (LK) mlo holds the plane's
+    // own +x link weight instead, which is the -x link of the plane above.
     struct Plane {
       V2 f[C];
       V2 pi, kap, mlo;
@@ -343,10 +379,12 @@ __global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE>::LB_
       const T* sp = reinterpret_cast<const T*>(smem + sj * K::STAGE_BYTES + K::F_BYTES);
 #pragma unroll
       for (int c = 0; c < C; ++c) n.f[c] = *reinterpret_cast<const V2*>(sf + c * TYH * TZW + ec);
-      n.pi = *reinterpret_cast<const V2*>(sp + ec);
+      n.pi = *reinterpret_cast<const V2*>(sp + (LK ? ek : ec));
       n.kap.x = kappa_of(n.pi.x, a.a6);
       n.kap.y = kappa_of(n.pi.y, a.a6);
-      if (below) {
+      if constexpr (LK) {
+        n.mlo = *reinterpret_cast<const V2*>(reinterpret_cast<const T*>(smem + sj * K::STAGE_BYTES + K::MX_OFF) + ek);
+      } else if (below) {
         n.mlo.x = tmin(n.pi.x, below->pi.x);
         n.mlo.y = tmin(n.pi.y, below->pi.y);
       }
@@ -369,21 +407,36 @@ __global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE>::LB_
         csv = *reinterpret_cast<const V2*>(sk + ek);
         snv = *reinterpret_cast<const V2*>(sk + TY * TZ + ek);
       }
-      const V2 pym = *reinterpret_cast<const V2*>(sp + ec - TZW);
-      const V2 pyp = *reinterpret_cast<const V2*>(sp + ec + TZW);
-      const T pzm = sp[ec - 1], pzp = sp[ec + 2];
-
       SiteUpdate<T, NRHO, NMOM> ua, ub;
       ua.pc = ctr.pi.x; ub.pc = ctr.pi.y;
       ua.kap = ctr.kap.x; ub.kap = ctr.kap.y;
-      ua.mxm = ctr.mlo.x; ub.mxm = ctr.mlo.y;
-      ua.mxp = nxt.mlo.x; ub.mxp = nxt.mlo.y;
-      ua.mym = tmin(ctr.pi.x, pym.x); ub.mym = tmin(ctr.pi.y, pym.y);
-      ua.myp = tmin(ctr.pi.x, pyp.x); ub.myp = tmin(ctr.pi.y, pyp.y);
-      ua.mzm = tmin(ctr.pi.x, pzm);
-      ua.mzp = tmin(ctr.pi.x, ctr.pi.y);
-      ub.mzm = ua.mzp;
-      ub.mzp = tmin(ctr.pi.y, pzp);
+      if constexpr (LK) {
+        const T* smy = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES + K::MY_OFF) + ek;          // row y-1 of the box
+        const T* smz = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES + K::MZ_OFF) + ty * K::TZM + HZ + 2 * tp;
+        const V2 mym = *reinterpret_cast<const V2*>(smy);
+        const V2 myp = *reinterpret_cast<const V2*>(smy + TZ);
+        const V2 mzp = *reinterpret_cast<const V2*>(smz);
+        ua.mxm = prv.mlo.x; ub.mxm = prv.mlo.y;
+        ua.mxp = ctr.mlo.x; ub.mxp = ctr.mlo.y;
+        ua.mym = mym.x; ub.mym = mym.y;
+        ua.myp = myp.x; ub.myp = myp.y;
+        ua.mzm = smz[-1];
+        ua.mzp = mzp.x;
+        ub.mzm = mzp.x;
+        ub.mzp = mzp.y;
+      } else {
+        const V2 pym = *reinterpret_cast<const V2*>(sp + ec - TZW);
+        const V2 pyp = *reinterpret_cast<const V2*>(sp + ec + TZW);
+        const T pzm = sp[ec - 1], pzp = sp[ec + 2];
+        ua.mxm = ctr.mlo.x; ub.mxm = ctr.mlo.y;
+        ua.mxp = nxt.mlo.x; ub.mxp = nxt.mlo.y;
+        ua.mym = tmin(ctr.pi.x, pym.x); ub.mym = tmin(ctr.pi.y, pym.y);
+        ua.myp = tmin(ctr.pi.x, pyp.x); ub.myp = tmin(ctr.pi.y, pyp.y);
+        ua.mzm = tmin(ctr.pi.x, pzm);
+        ua.mzp = tmin(ctr.pi.x, ctr.pi.y);
+        ub.mzm = ua.mzp;
+        ub.mzp = tmin(ctr.pi.y, pzp);
+      }
 
       T oa[C], ob[C];
 #pragma unroll
@@ -456,6 +509,23 @@ __global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE>::LB_
   }
   block_reduce_finalize<NRED, (NH == 2) ? FIN_STEP : FIN_MOM, NMOM>(acc, red, a.partials, a.ctl, a.fid, a.vacf, a.vacf_stride, a.zscale, gridDim.x,
                                               blockIdx.x);
+}
+
+struct NoLinkMaps {};
+
+template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE>
+__global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE>::LB_THREADS, TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE>::LB_CTAS)
+    step_tma_kernel(const __grid_constant__ CUtensorMap tm_f, const __grid_constant__ CUtensorMap tm_pi,
+                    const __grid_constant__ CUtensorMap tm_cs, StepArgs<T> a) {
+  step_tma_body<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 0>(tm_f, tm_pi, tm_cs, NoLinkMaps(), a);
+}
+
+// the same sweep with stored link weights (per-link mobility factors)
+template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE>
+__global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1>::LB_THREADS, TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1>::LB_CTAS)
+    step_tma_links_kernel(const __grid_constant__ CUtensorMap tm_f, const __grid_constant__ CUtensorMap tm_cs,
+                          const __grid_constant__ TmaLinkMaps lm, StepArgs<T> a) {
+  step_tma_body<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1>(tm_f, tm_f, tm_cs, lm, a);
 }
 
 }  // namespace lpc

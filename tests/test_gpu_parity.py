@@ -397,6 +397,132 @@ def test_regional_vacf_and_diffusion_match_oracle(lpc, oracle_mod, kernel, preci
     assert late.fid_region(0, first=1).shape == (3,)
 
 
+# ---------------------------------------------------------------------------------------------
+# f3: per-link mobility factors alpha_ij (oracle O10)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel,precision,bc", [(0, 0, (1, 0, 0)), (1, 0, (0, 0, 0)), (3, 0, (0, 1, 0)), (1, 1, (1, 0, 0)), (2, 0, (0, 0, 1)),
+                                                 (2, 0, (0, 0, 0)), (2, 1, (0, 1, 0))])
+def test_link_mobility_matches_oracle(lpc, oracle_mod, kernel, precision, bc):
+    n = 80
+    lat = lpc_inputs.random_small((22, 18, 70), bc=bc, p_block=0.25, alpha=0.9, seed=71, n_steps=n, n_moments=3)
+    link = lpc_inputs.random_links(lat.shape, seed=3, lo=0.0)
+    link[:, 5:9, 3:6, 10:20] = 0.0   # a pocket of dead links
+    tol_site, tol_sum = (1e-5, 1e-5) if precision else (1e-10, 1e-9)
+    gpu = lpc.Lattice.from_inputs(lat, precision=precision, n_moments=3, n_density=1, max_steps=n, link=link)
+    gpu.set_kernel(kernel)
+    assert gpu.bytes_per_site_step == (4 if precision else 8) * (2 * 6 + 3 + 3)
+    orc = oracle_mod.Oracle.from_lattice(lat, n_moments=3, max_steps=n, link=link)
+    # the precompute: Z_d[1] and P^d(1) of the scaled hop probabilities
+    v_o, _ = orc.moments(1)
+    v_g, _ = gpu.moments(1)
+    assert np.max(np.abs(v_g - v_o) / v_o) < (1e-5 if precision else 1e-13)
+    gpu.step(n)
+    orc.step(n)
+    print(_check(lpc, lat, gpu, orc, n, tol_site=tol_site, tol_sum=tol_sum, what="links"))
+    # the density channel started at pi and stays there (the factors keep Eq. 2 stationary)
+    pi = orc.pi()
+    opn = lat.blocked == 0
+    assert np.max(np.abs(gpu.field(lpc.LPC_FIELD_RHO) - pi)[opn] / pi[opn]) < (1e-4 if precision else 1e-12)
+    # and the result differs from the run without factors by far more than the tolerance
+    plain = lpc.Lattice.from_inputs(lat, precision=precision, n_moments=3, n_density=1, max_steps=n)
+    plain.step(n)
+    assert np.max(np.abs(plain.fid() - gpu.fid())) > 1e-3
+
+
+def test_link_mobility_kernels_agree_bitwise(lpc):
+    lat = lpc_inputs.random_small((40, 21, 131), bc=(0, 1, 0), p_block=0.25, seed=73, n_moments=3)
+    link = lpc_inputs.random_links(lat.shape, seed=4, lo=0.0)
+    res = []
+    for kernel, prec in ((1, 0), (2, 0), (3, 0), (1, 1), (2, 1)):
+        gpu = lpc.Lattice.from_inputs(lat, precision=prec, n_density=1, max_steps=25, link=link)
+        gpu.set_kernel(kernel)
+        gpu.step(25)
+        res.append([gpu.field(w) for w in (lpc.LPC_FIELD_G, lpc.LPC_FIELD_PX, lpc.LPC_FIELD_PY, lpc.LPC_FIELD_PZ, lpc.LPC_FIELD_RHO)])
+    for k in (1, 2):
+        assert all(np.array_equal(x, y) for x, y in zip(res[0], res[k])), f"fp64 kernel {k}"
+    assert all(np.array_equal(x, y) for x, y in zip(res[3], res[4])), "fp32"
+
+
+def test_link_mobility_regions_equilibration_and_errors(lpc, oracle_mod):
+    n, nreg = 40, 2
+    lat = lpc_inputs.random_small((20, 16, 40), bc=(1, 0, 0), p_block=0.2, alpha=0.8, seed=72, n_steps=n, n_moments=3)
+    confined = np.zeros(lat.shape, dtype=np.uint8)
+    confined[:10] = 1
+    link = lpc_inputs.confined_links(confined, 0.25)
+    region = (1 - confined).astype(np.uint8)
+    gpu = lpc.Lattice.from_inputs(lat, n_moments=3, n_density=1, max_steps=n, n_regions=nreg, link=link)
+    gpu.set_regions(region)
+    gpu.step(n)
+    orc = oracle_mod.Oracle.from_lattice(lat, n_moments=3, max_steps=n, link=link)
+    Zr_o, w = orc.step_with_regional_moments(region, nreg, n)
+    for r in range(nreg):
+        Z_g, D_g = gpu.moments_region(r)
+        assert np.max(np.abs(Z_g - Zr_o[r]) / np.abs(Zr_o[r][:, :1])) <= 1e-9
+    # the confined half diffuses more slowly along y and z
+    assert gpu.moments_region(0)[1][1] < 0.5 * gpu.moments_region(1)[1][1]
+    # equilibration loop with the scaled hop probabilities
+    rng = np.random.default_rng(8)
+    rho0 = rng.random(lat.shape) * (lat.blocked == 0)
+    rho0 /= rho0.sum()
+    eq = lpc.Lattice.from_inputs(lat, n_moments=0, n_density=1, max_steps=4, link=link)
+    eq.set_state(lpc.LPC_FIELD_RHO, rho0)
+    it_g, d_g = eq.equilibrate(0.0, 25, 5)
+    orc2 = oracle_mod.Oracle.from_lattice(lat, n_moments=0, max_steps=4, link=link)
+    rho_o, it_o, dl = orc2.equilibrate(rho0, 0.0, 25)
+    assert it_g == it_o == 25 and abs(d_g - dl[-1]) <= 1e-10 * rho0.max()
+    assert np.max(np.abs(eq.field(lpc.LPC_FIELD_RHO) - rho_o)) <= 1e-10 * rho0.max()
+    # NULL removes the factors: bit-identical to a lattice that never had them
+    eq2 = lpc.Lattice.from_inputs(lat, n_moments=3, max_steps=6, link=link)
+    eq2.set_link_mobility(None)
+    assert eq2.bytes_per_site_step == 8 * (2 * 5 + 3)
+    ref = lpc.Lattice.from_inputs(lat, n_moments=3, max_steps=6)
+    eq2.set_kernel(1); ref.set_kernel(1)
+    eq2.step(6); ref.step(6)
+    assert np.array_equal(eq2.fid(), ref.fid()) and np.array_equal(eq2.field(lpc.LPC_FIELD_G), ref.field(lpc.LPC_FIELD_G))
+    assert np.array_equal(eq2.moments()[0], ref.moments()[0])
+    # errors: no room reserved, after the first step, factor out of range
+    with pytest.raises(lpc.LpcError) as e:
+        ref.set_link_mobility(link)
+    assert e.value.code == lpc.LPC_ESTATE
+    with pytest.raises(lpc.LpcError) as e:
+        eq2.set_link_mobility(link)
+    assert e.value.code == lpc.LPC_ESTATE
+    bad = link.copy()
+    bad[2, 3, 3, 3] = 1.0000001
+    with pytest.raises(lpc.LpcError) as e:
+        lpc.Lattice.from_inputs(lat, n_moments=0, max_steps=2, link=bad)
+    assert e.value.code == lpc.LPC_EINVAL
+    # device-resident factors
+    import torch
+    dev = lpc.Lattice.from_inputs(lat, n_moments=3, n_density=1, max_steps=n, n_regions=nreg, link=torch.from_numpy(link).cuda())
+    dev.set_regions(region)   # same launch sequence as `gpu`, hence the same summation order
+    dev.step(n)
+    assert np.array_equal(dev.fid(), gpu.fid())
+
+
+# ---------------------------------------------------------------------------------------------
+# f4: the film-electrode cell of PAPER.md:236-248 (100 x 100 x 300, no periodic boundary in z)
+# ---------------------------------------------------------------------------------------------
+def test_film_electrode_cell(lpc, oracle_mod):
+    n = 50000 if FULL else 150
+    lat = lpc_inputs.film(n_steps=n, n_moments=3)
+    assert lat.shape == (100, 100, 300) and lat.bc == (0, 0, 1) and abs(lat.notes["fraction"] - 0.38) < 0.01
+    label = lat.notes["particle"]
+    region = np.where(label > 0, 0, np.where((np.arange(300) >= 100) & (np.arange(300) < 200), 1, 2))[...].astype(np.uint8)
+    gpu = lpc.Lattice.from_inputs(lat, n_moments=3, max_steps=n, n_regions=3)
+    gpu.set_regions(region)
+    orc = oracle_mod.Oracle.from_lattice(lat, n_moments=3, max_steps=n)
+    gpu.step(n)
+    orc.step(n)
+    print(_check(lpc, lat, gpu, orc, n, what="film"))
+    # in-particle + bulk between the electrodes + bulk between the particles make up the whole signal
+    G = gpu.fid()
+    assert np.max(np.abs(sum(gpu.fid_region(r) for r in range(3)) - G)) < 1e-12
+    # the bulk gap between the electrodes keeps its line at delta = 0: a real, slowly shrinking signal
+    G1 = gpu.fid_region(1)
+    assert np.all(np.abs(G1.imag) < 0.02 * np.abs(G1.real)) and G1.real[-1] > 0.8 * G1.real[0]
+
+
 def test_regional_fid_large_spectrum_batches_and_errors(lpc):
     lat = lpc_inputs.random_small((12, 10, 20), seed=43, p_block=0.1)
     lat.omega[...] = -2 * np.pi * 2500.0
