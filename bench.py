@@ -55,6 +55,9 @@ def parse():
     p.add_argument("--moments", type=int, default=0, choices=[0, 3], help="also propagate the 3 VACF fields")
     p.add_argument("--precision", type=int, default=0, choices=[0, 1])
     p.add_argument("--kernel", type=int, default=0, choices=[0, 1, 2, 3])
+    p.add_argument("--slabs", type=int, default=0, metavar="S",
+                   help="run the workload as ONE lattice cut into x-slabs, S per rank (SURVEY 8(e)): a plane exchange after every step, "
+                        "strong scaling over --gpus; 0 (default) = independent replicas")
     p.add_argument("--no-cpu-baseline", action="store_true")
     p.add_argument("--no-e2e", action="store_true")
     p.add_argument("--ref-sample-size", type=int, default=int(os.environ.get("LPC_REF_SAMPLE_L", "256")),
@@ -200,6 +203,8 @@ def run_ours(args):
 
     L, K, W = args.size, args.steps, args.warmup
     lat = make_workload(args)
+    if args.slabs:
+        return run_slabs(args, lat, lpc, world, rank, local, dev)
     n_sites = lat.n_sites
     # pinned host buffers: the inputs of the end-to-end job
     host = [torch.from_numpy(a).pin_memory() for a in (lat.dF, lat.blocked, lat.omega)]
@@ -314,6 +319,77 @@ def run_ours(args):
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = oracle_sample(args.moments, L=args.ref_sample_size)[0]
         print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def run_slabs(args, lat, lpc, world, rank, local, dev):
+    """One lattice over all ranks as x-slabs: per step one sweep per slab and the exchange of the boundary planes
+    (device copies inside a process, NCCL send/recv between ranks).  value = sites x steps / slowest rank's time."""
+    import torch
+    import torch.distributed as dist
+
+    from paper_2603_22553_b200 import slab
+
+    K, W = args.steps, args.warmup
+
+    def factory(shape, bc, **cfg):
+        m = lpc.Lattice(shape, bc=bc, device=dev, **cfg)
+        m.set_kernel(args.kernel)
+        return m
+
+    ss = slab.SlabSet(lat.shape, bc=lat.bc, slabs_per_rank=args.slabs, lattice_factory=factory, precision=args.precision,
+                      n_moments=args.moments, dt=lat.dt, a=lat.a, alpha=lat.alpha, max_steps=K + W + 8)
+    ss.set_site_params(lat.dF, lat.blocked, lat.omega)
+    ss.step(W)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.25)
+    l0 = sum(m.launch_count for m in ss.lat.values())
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    tw0 = time.perf_counter()
+    ev0.record()
+    ss.step(K)
+    ev1.record()
+    barrier()
+    tw1 = time.perf_counter()
+    clocks = sampler.stop(tw0, tw1)
+    ms = ev0.elapsed_time(ev1)
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    launches = sum(m.launch_count for m in ss.lat.values()) - l0
+    fid = ss.fid()
+    assert np.isfinite(fid).all() and abs(fid[0] - 1.0) < (1e-4 if args.precision else 1e-12), "FID series is not sane"
+    if rank == 0:
+        peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+        peak = float(json.load(open(peaks_path))["hbm_gbs"]) if os.path.exists(peaks_path) else FALLBACK_HBM_GBS
+        m0 = next(iter(ss.lat.values()))
+        bps = m0.bytes_per_site_step
+        own = sum(hi - lo for s, (lo, hi) in ss.ranges.items() if s in ss.lat) * lat.ny * lat.nz
+        achieved = bps * own / (ms / K * 1e-3) / 1e9      # this rank's sites over this rank's time
+        plane_bytes = (lat.ny + 2) * m0.halo_planes(lpc.LPC_HALO_STATE, 0, lpc.LPC_HALO_SEND).shape[1] // (lat.ny + 2) * (4 if args.precision else 8)
+        print(json.dumps({
+            "metric": METRIC, "value": lat.n_sites * K / (ms_max * 1e-3) / 1e9, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": "f32" if args.precision else "f64", "data": "synthetic",
+            "config": {"workload": workload_name(args.size, args.moments, args.precision, args.workload), "lattice": list(lat.shape),
+                       "sites": lat.n_sites, "parallelism": f"x-slabs: {ss.n_slabs} slabs over {world} rank(s), one plane exchange per step "
+                                                           f"({2 + args.moments} channel planes of {plane_bytes} B per face)",
+                       "l2": "per-rank working set >> 126 MB L2" if bps * own > 4 * 126e6 else "per-rank working set is L2-sized"},
+            "clocks": clocks, "e2e": None, "gpu_launches": int(launches),
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                         "bytes_per_site_step": bps, "kernel_ms": ms / K, "launches_per_step": launches / K},
+        }))
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()

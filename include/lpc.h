@@ -50,6 +50,13 @@ extern "C" {
 #define LPC_FIELD_PZ 4
 #define LPC_FIELD_RHO 5 /* real density rho_i (needs n_density = 1): N doubles            */
 
+/* bc[0] value and lpc_halo_view selectors (slab decomposition along x) */
+#define LPC_BC_HALO 2
+#define LPC_HALO_PARAMS 0 /* the equilibrium density pi: 1 channel plane                      */
+#define LPC_HALO_STATE 1  /* the current state: 2 + n_density + n_moments channel planes      */
+#define LPC_HALO_SEND 0   /* the outermost owned plane on that side                           */
+#define LPC_HALO_RECV 1   /* the ghost plane beyond it                                        */
+
 /* lpc_set_kernel selectors */
 #define LPC_KERNEL_AUTO 0
 #define LPC_KERNEL_DIRECT 1 /* one thread per site pair, neighbours straight from global memory */
@@ -61,7 +68,9 @@ typedef struct lpc_lattice lpc_lattice; /* opaque, host struct owned by the libr
 
 typedef struct lpc_config {
   int32_t nx, ny, nz;  /* lattice size, each >= 1 ("system dimensions")            */
-  int32_t bc[3];       /* per axis: 0 periodic, 1 reflective zero-flux wall      */
+  int32_t bc[3];       /* per axis: 0 periodic, 1 reflective zero-flux wall;     */
+                       /* bc[0] may also be LPC_BC_HALO: this lattice is one x-slab of a larger */
+                       /* one and the caller supplies its two x ghost planes (see "Slabs")      */
   int32_t precision;   /* 0: fp64 storage and arithmetic; 1: fp32 storage and arithmetic with   */
                        /*    fp64 reductions                                                    */
   int32_t n_moments;   /* 0, or 3 to propagate P^x, P^y, P^z for the VACF / D (Eq. 4)           */
@@ -193,6 +202,44 @@ int lpc_moments_region(lpc_lattice* lat, int32_t region, int64_t count, double* 
  * Errors: LPC_ESTATE, LPC_EINVAL, LPC_ECUDA.                                                    */
 int lpc_spectrum(lpc_lattice* lat, int32_t region, int64_t count, double f0_hz, double df_hz, int64_t n_freq,
                  double lb_hz, double* out_re_im_host);
+
+/* ---- Slabs: one lattice split along x over several GPUs --------------------------------
+ * Each rank owns a contiguous range of x planes and creates a lattice of that size with bc[0] = LPC_BC_HALO.
+ * The library then leaves the two x ghost planes to the caller, who copies the neighbour's outermost owned
+ * plane into them (NCCL send/recv, a peer-to-peer copy, or a plain device copy on one GPU); at a reflective end
+ * of the whole lattice the ghost plane is simply left alone (it holds zeros = a wall).  Order of calls:
+ *   lpc_partition_sum            -> Z_local; the caller adds the ranks' values (Eq. 2 normalises over the
+ *   lpc_set_partition_sum(Z)        whole lattice) and hands the total back
+ *   lpc_set_site_params          pi, phase factors of the owned sites
+ *   exchange LPC_HALO_PARAMS     pi of the neighbours' boundary planes
+ *   lpc_slab_finish              initial state with the neighbours' pi (P^d(1), Z_d[1], G[0])
+ *   [lpc_set_state]              optional
+ *   exchange LPC_HALO_STATE
+ *   repeat: lpc_step_n(lat, 1); exchange LPC_HALO_STATE
+ * G[n], Z_d[m] of a slab are the sums over its own sites: the caller adds the ranks' series (one reduction
+ * when the series is read, none per step); D follows from the summed Z_d as in lpc_moments.  Not available in
+ * slab mode (LPC_ESTATE): lpc_step_n with n > 1, the persistent kernel, lpc_equilibrate, link factors.       */
+
+/* Z_local = sum of exp(-dF_i) over the open sites of this lattice (Eq. 2).  dF_kT, blocked: host
+ * or device, as lpc_set_site_params.  out: host.  Synchronises.  Errors: LPC_EINVAL, LPC_ECUDA.              */
+int lpc_partition_sum(lpc_lattice* lat, const double* dF_kT, const uint8_t* blocked, double* out);
+
+/* Normalise pi by Z instead of the lattice's own sum in every later lpc_set_site_params (Z <= 0 restores the
+ * default).  Errors: LPC_EINVAL (not finite).                                                                */
+int lpc_set_partition_sum(lpc_lattice* lat, double Z);
+
+/* Where a halo plane lives in the workspace.  set: LPC_HALO_PARAMS / LPC_HALO_STATE; side: 0 low x, 1 high x;
+ * role: LPC_HALO_SEND / LPC_HALO_RECV.  Returns the device address of channel 0's plane, the bytes of one
+ * plane (contiguous: (ny+2) x padded nz elements of the lattice's precision, ghost rows and columns included),
+ * the byte stride between channels and the number of channels.  STATE refers to the buffer that holds the
+ * current state, so ask again after every step.  Works for any bc (tests use it to inspect planes).
+ * Errors: LPC_EINVAL, LPC_ESTATE (no site parameters yet).                                                    */
+int lpc_halo_view(lpc_lattice* lat, int32_t set, int32_t side, int32_t role, void** plane_dev, size_t* plane_bytes,
+                  size_t* channel_stride_bytes, int32_t* n_channels);
+
+/* Slab mode: build the initial state once the pi ghost planes are in place (see the order above).  Resets the
+ * step counter and the series.  Synchronises.  Errors: LPC_ESTATE (not a slab, or no site parameters).         */
+int lpc_slab_finish(lpc_lattice* lat);
 
 /* Choose the step kernel (LPC_KERNEL_*).  AUTO picks PERSIST when one step's state and parameters
  * stay in L2 (<= 48 MB) and no region labels are set, else TMA.  Errors: LPC_EINVAL.             */

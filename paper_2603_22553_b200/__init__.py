@@ -20,12 +20,15 @@ LIB_PATH = os.path.join(_HERE, "liblpc.so")
 
 LPC_OK, LPC_EINVAL, LPC_ESTATE, LPC_ENOMEM, LPC_ECUDA = 0, -1, -2, -3, -4
 LPC_FIELD_G, LPC_FIELD_PI, LPC_FIELD_PX, LPC_FIELD_PY, LPC_FIELD_PZ, LPC_FIELD_RHO = range(6)
+LPC_BC_HALO = 2
+LPC_HALO_PARAMS, LPC_HALO_STATE = 0, 1
+LPC_HALO_SEND, LPC_HALO_RECV = 0, 1
 LPC_KERNEL_AUTO, LPC_KERNEL_DIRECT, LPC_KERNEL_TMA, LPC_KERNEL_PERSIST = range(4)
 
 EXPORTS = (
     "lpc_workspace_bytes", "lpc_create_lattice", "lpc_set_site_params", "lpc_set_link_mobility", "lpc_step_n", "lpc_read_fid",
     "lpc_moments", "lpc_read_field", "lpc_set_state", "lpc_equilibrate", "lpc_seed_from_density", "lpc_set_regions", "lpc_read_fid_region", "lpc_moments_region", "lpc_spectrum", "lpc_set_kernel",
-    "lpc_steps_done",
+    "lpc_steps_done", "lpc_partition_sum", "lpc_set_partition_sum", "lpc_halo_view", "lpc_slab_finish",
     "lpc_launch_count", "lpc_bytes_per_site_step", "lpc_destroy", "lpc_last_error",
 )
 
@@ -63,6 +66,11 @@ def _load():
     lib.lpc_create_lattice.argtypes = [C.POINTER(lpc_config), C.c_void_p, C.c_size_t, C.POINTER(C.c_void_p)]
     lib.lpc_set_site_params.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.lpc_set_link_mobility.argtypes = [C.c_void_p, C.c_void_p]
+    lib.lpc_partition_sum.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_double)]
+    lib.lpc_set_partition_sum.argtypes = [C.c_void_p, C.c_double]
+    lib.lpc_halo_view.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_void_p), C.POINTER(C.c_size_t),
+                                  C.POINTER(C.c_size_t), C.POINTER(C.c_int32)]
+    lib.lpc_slab_finish.argtypes = [C.c_void_p]
     lib.lpc_step_n.argtypes = [C.c_void_p, C.c_int64]
     lib.lpc_read_fid.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_void_p]
     lib.lpc_moments.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
@@ -157,6 +165,27 @@ def lpc_set_site_params(handle, dF, blocked, omega, g0=None):
 def lpc_set_link_mobility(handle, alpha_link):
     """alpha_link: [3, nx, ny, nz] float64 (host numpy or CUDA tensor), or None to remove the factors."""
     _check(_lib.lpc_set_link_mobility(handle, _ptr(alpha_link)))
+
+
+def lpc_partition_sum(handle, dF, blocked) -> float:
+    out = C.c_double(0.0)
+    _check(_lib.lpc_partition_sum(handle, _ptr(dF), _ptr(blocked), C.byref(out)))
+    return float(out.value)
+
+
+def lpc_set_partition_sum(handle, Z):
+    _check(_lib.lpc_set_partition_sum(handle, float(Z)))
+
+
+def lpc_halo_view(handle, which, side, role):
+    """(device address of channel 0's plane, bytes per plane, byte stride between channels, channels)."""
+    ptr, nb, st, nc = C.c_void_p(), C.c_size_t(), C.c_size_t(), C.c_int32()
+    _check(_lib.lpc_halo_view(handle, int(which), int(side), int(role), C.byref(ptr), C.byref(nb), C.byref(st), C.byref(nc)))
+    return int(ptr.value), int(nb.value), int(st.value), int(nc.value)
+
+
+def lpc_slab_finish(handle):
+    _check(_lib.lpc_slab_finish(handle))
 
 
 def lpc_step_n(handle, n):
@@ -315,6 +344,25 @@ class Lattice:
         if isinstance(alpha_link, np.ndarray):
             alpha_link = np.ascontiguousarray(alpha_link, dtype=np.float64)
         lpc_set_link_mobility(self.handle, alpha_link)
+
+    def partition_sum(self, dF, blocked):
+        return lpc_partition_sum(self.handle, np.ascontiguousarray(dF, dtype=np.float64), np.ascontiguousarray(blocked, dtype=np.uint8))
+
+    def set_partition_sum(self, Z):
+        lpc_set_partition_sum(self.handle, Z)
+
+    def slab_finish(self):
+        lpc_slab_finish(self.handle)
+
+    def halo_planes(self, which, side, role):
+        """The halo plane(s) as a [channels, plane_elements] strided view of the workspace tensor (no copy)."""
+        import torch
+
+        ptr, nb, st, nc = lpc_halo_view(self.handle, which, side, role)
+        off = ptr - self.workspace.data_ptr()
+        esz = 4 if self.cfg.precision else 8
+        flat = self.workspace.view(torch.float32 if self.cfg.precision else torch.float64)
+        return flat.as_strided((nc, nb // esz), (st // esz, 1), off // esz)
 
     def step(self, n=1):
         lpc_step_n(self.handle, n)

@@ -69,6 +69,9 @@ struct lpc_lattice {
   long long region_first;  // first sample of the regional series
   bool region_moments;     // the regional VACF is being recorded (labels were set at step 0)
   bool have_links;         // per-link mobility factors are set: the sweeps read the stored link weights
+  bool halo;               // bc[0] = LPC_BC_HALO: an x-slab whose x ghost planes the caller fills
+  bool halo_ready;         // lpc_slab_finish has run
+  double z_override;       // > 0: normalise pi by this partition sum (slab mode)
   int cur;  // index of the buffer holding the current state
   long long steps;
   long long launches;
@@ -87,7 +90,9 @@ int check_cfg(const lpc_config* c) {
   if (c->nx < 1 || c->ny < 1 || c->nz < 1) return fail(LPC_EINVAL, "lattice dimensions must be >= 1 (got %d %d %d)", c->nx, c->ny, c->nz);
   if ((long long)c->nx * c->ny * c->nz > (1ll << 40)) return fail(LPC_EINVAL, "lattice too large");
   for (int d = 0; d < 3; ++d)
-    if (c->bc[d] != 0 && c->bc[d] != 1) return fail(LPC_EINVAL, "bc[%d] must be 0 (periodic) or 1 (reflective)", d);
+    if (c->bc[d] != 0 && c->bc[d] != 1 && !(d == 0 && c->bc[d] == LPC_BC_HALO))
+      return fail(LPC_EINVAL, "bc[%d] must be 0 (periodic) or 1 (reflective)%s", d, d == 0 ? " or LPC_BC_HALO" : "");
+  if (c->bc[0] == LPC_BC_HALO && c->link_mobility) return fail(LPC_EINVAL, "link factors are not available in slab mode");
   if (c->precision != 0 && c->precision != 1) return fail(LPC_EINVAL, "precision must be 0 (fp64) or 1 (fp32)");
   if (c->n_moments != 0 && c->n_moments != 3) return fail(LPC_EINVAL, "n_moments must be 0 or 3");
   if (c->n_density != 0 && c->n_density != 1) return fail(LPC_EINVAL, "n_density must be 0 or 1");
@@ -441,11 +446,14 @@ int region_moment(lpc_lattice* h) {
   return h->cfg.precision ? region_moment_t<float, INIT>(h) : region_moment_t<double, INIT>(h);
 }
 
+// x ghost planes: 1 wrap (periodic), 0 zero (wall), 2 leave to the caller (slab)
+int xghost_mode(const lpc_lattice* h) { return h->halo ? 2 : (h->cfg.bc[0] == 0 ? 1 : 0); }
+
 template <typename T>
 int fill_state_ghosts(lpc_lattice* h) {
   const Layout& L = h->L;
   const long long cells = 2ll * ((long long)L.nx * L.ny + (long long)L.nx * L.nz + (long long)L.ny * L.nz) * h->C;
-  fill_ghosts_kernel<T><<<aux_grid(cells), 256, 0, h->stream>>>(wsp<T>(h, h->cur ? h->off.f1 : h->off.f0), h->C, L, h->cfg.bc[0] == 0,
+  fill_ghosts_kernel<T><<<aux_grid(cells), 256, 0, h->stream>>>(wsp<T>(h, h->cur ? h->off.f1 : h->off.f0), h->C, L, xghost_mode(h),
                                                                  h->cfg.bc[1] == 0, h->cfg.bc[2] == 0);
   CUDA_TRY(cudaGetLastError());
   h->launches++;
@@ -466,6 +474,39 @@ int set_g_from(lpc_lattice* h, const void* g) {
                                                              wsp<Ctl>(h, h->off.ctl), wsp<double2>(h, h->off.fid));
   CUDA_TRY(cudaGetLastError());
   h->launches++;
+  return LPC_OK;
+}
+
+// Pass 1 of the precompute: e_i = exp(-dF_i) on open sites into the dense scratch (which aliases the back
+// buffer) and their fixed-order sum into ctl->zsum.  dF and blocked travel through the staging buffer together.
+int boltzmann_pass(lpc_lattice* h, const double* dF, const uint8_t* blocked, Ctl* hc) {
+  Ctl* ctl = wsp<Ctl>(h, h->off.ctl);
+  double* e = wsp<double>(h, h->off.f1);
+  const bool dev_in = is_device_ptr(dF) && is_device_ptr(blocked);
+  if (dev_in) {
+    boltzmann_factor_kernel<<<aux_grid(h->N), 256, 0, h->stream>>>(dF, blocked, 0, h->N, e, ctl);
+    CUDA_TRY(cudaGetLastError());
+    h->launches++;
+  } else {
+    const long long chunk = std::min<long long>(h->N, STAGE_SITES);
+    unsigned char* stg = h->ws + h->off.staging;
+    for (long long i0 = 0; i0 < h->N; i0 += chunk) {
+      const long long n = std::min(chunk, h->N - i0);
+      CUDA_TRY(cudaMemcpyAsync(stg, dF + i0, (size_t)n * 8, cudaMemcpyDefault, h->stream));
+      CUDA_TRY(cudaMemcpyAsync(stg + (size_t)chunk * 8, blocked + i0, (size_t)n, cudaMemcpyDefault, h->stream));
+      boltzmann_factor_kernel<<<aux_grid(n), 256, 0, h->stream>>>(reinterpret_cast<const double*>(stg), stg + (size_t)chunk * 8, i0, n, e,
+                                                                   ctl);
+      CUDA_TRY(cudaGetLastError());
+      h->launches++;
+      CUDA_TRY(cudaStreamSynchronize(h->stream));
+    }
+  }
+  sum_kernel<<<aux_grid(h->N), 256, 0, h->stream>>>(e, h->N, wsp<double>(h, h->off.partials), ctl);
+  CUDA_TRY(cudaGetLastError());
+  h->launches++;
+  CUDA_TRY(cudaMemcpyAsync(hc, ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  if (hc->bad != 0) return fail(LPC_EINVAL, "exp(-dF) under- or overflows on %llu open sites: the spread of dF is too wide", hc->bad);
   return LPC_OK;
 }
 
@@ -497,34 +538,14 @@ int set_site_params_t(lpc_lattice* h, const double* dF, const uint8_t* blocked, 
   Ctl* ctl = wsp<Ctl>(h, h->off.ctl);
   CUDA_TRY(cudaMemsetAsync(h->ws, 0, h->off.staging, h->stream));  // ghosts, series, control block, state: all zero
   double* e = wsp<double>(h, h->off.f1);                            // dense scratch for exp(-dF), aliases the back buffer
-  int rc;
-  // pass 1: Boltzmann factors.  dF and blocked travel through the staging buffer together.
-  const bool dev_in = is_device_ptr(dF) && is_device_ptr(blocked);
-  if (dev_in) {
-    boltzmann_factor_kernel<<<aux_grid(h->N), 256, 0, h->stream>>>(dF, blocked, 0, h->N, e, ctl);
-    CUDA_TRY(cudaGetLastError());
-    h->launches++;
-  } else {
-    const long long chunk = std::min<long long>(h->N, STAGE_SITES);
-    unsigned char* stg = h->ws + h->off.staging;
-    for (long long i0 = 0; i0 < h->N; i0 += chunk) {
-      const long long n = std::min(chunk, h->N - i0);
-      CUDA_TRY(cudaMemcpyAsync(stg, dF + i0, (size_t)n * 8, cudaMemcpyDefault, h->stream));
-      CUDA_TRY(cudaMemcpyAsync(stg + (size_t)chunk * 8, blocked + i0, (size_t)n, cudaMemcpyDefault, h->stream));
-      boltzmann_factor_kernel<<<aux_grid(n), 256, 0, h->stream>>>(reinterpret_cast<const double*>(stg), stg + (size_t)chunk * 8, i0, n, e,
-                                                                   ctl);
-      CUDA_TRY(cudaGetLastError());
-      h->launches++;
-      CUDA_TRY(cudaStreamSynchronize(h->stream));
-    }
-  }
-  sum_kernel<<<aux_grid(h->N), 256, 0, h->stream>>>(e, h->N, wsp<double>(h, h->off.partials), ctl);
-  CUDA_TRY(cudaGetLastError());
-  h->launches++;
   Ctl hc;
-  CUDA_TRY(cudaMemcpyAsync(&hc, ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, h->stream));
-  CUDA_TRY(cudaStreamSynchronize(h->stream));
-  if (hc.bad != 0) return fail(LPC_EINVAL, "exp(-dF) under- or overflows on %llu open sites: the spread of dF is too wide", hc.bad);
+  int rc = boltzmann_pass(h, dF, blocked, &hc);
+  if (rc) return rc;
+  if (h->z_override > 0.0) {
+    // slab mode: Eq. 2 normalises over the whole lattice, the caller supplies that sum
+    hc.zsum = h->z_override;
+    CUDA_TRY(cudaMemcpyAsync(&ctl->zsum, &h->z_override, sizeof(double), cudaMemcpyHostToDevice, h->stream));
+  }
   if (!(hc.zsum > 0.0) || !std::isfinite(hc.zsum)) return fail(LPC_EINVAL, "every site is blocked (sum of Boltzmann factors = %g)", hc.zsum);
 
   // pass 2: pi, kappa, phase factors
@@ -543,7 +564,7 @@ int set_site_params_t(lpc_lattice* h, const double* dF, const uint8_t* blocked, 
                 h->cfg.precision ? "fp32" : "fp64");
   {
     const long long cells = 2ll * ((long long)L.nx * L.ny + (long long)L.nx * L.nz + (long long)L.ny * L.nz);
-    fill_ghosts_kernel<T><<<aux_grid(cells), 256, 0, h->stream>>>(wsp<T>(h, h->off.pi), 1, L, h->cfg.bc[0] == 0, h->cfg.bc[1] == 0,
+    fill_ghosts_kernel<T><<<aux_grid(cells), 256, 0, h->stream>>>(wsp<T>(h, h->off.pi), 1, L, xghost_mode(h), h->cfg.bc[1] == 0,
                                                                    h->cfg.bc[2] == 0);
     CUDA_TRY(cudaGetLastError());
     h->launches++;
@@ -793,6 +814,9 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
   h->have_regions = false;
   h->region_moments = false;
   h->have_links = false;
+  h->halo = cfg->bc[0] == LPC_BC_HALO;
+  h->halo_ready = false;
+  h->z_override = 0.0;
   h->region_first = 0;
   h->cur = 0;
   h->steps = 0;
@@ -848,6 +872,7 @@ int lpc_set_site_params(lpc_lattice* h, const double* dF, const uint8_t* blocked
   h->have_regions = false;
   h->region_moments = false;
   h->have_links = false;
+  h->halo_ready = false;
   return h->cfg.precision ? set_site_params_t<float>(h, dF, blocked, omega, g0) : set_site_params_t<double>(h, dF, blocked, omega, g0);
 }
 
@@ -861,11 +886,70 @@ int lpc_set_link_mobility(lpc_lattice* h, const double* alpha_link) {
   return h->cfg.precision ? set_link_mobility_t<float>(h, alpha_link) : set_link_mobility_t<double>(h, alpha_link);
 }
 
+int lpc_partition_sum(lpc_lattice* h, const double* dF, const uint8_t* blocked, double* out) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (!dF || !blocked || !out) return fail(LPC_EINVAL, "dF, blocked and out must not be NULL");
+  // the pass uses the back buffer as scratch: whatever the lattice held is gone
+  h->have_params = false;
+  h->halo_ready = false;
+  CUDA_TRY(cudaMemsetAsync(h->ws, 0, h->off.staging, h->stream));
+  Ctl hc;
+  int rc = boltzmann_pass(h, dF, blocked, &hc);
+  if (rc) return rc;
+  *out = hc.zsum;
+  return LPC_OK;
+}
+
+int lpc_set_partition_sum(lpc_lattice* h, double Z) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (!std::isfinite(Z)) return fail(LPC_EINVAL, "Z is not finite");
+  h->z_override = Z > 0.0 ? Z : 0.0;
+  return LPC_OK;
+}
+
+int lpc_halo_view(lpc_lattice* h, int32_t set, int32_t side, int32_t role, void** plane, size_t* plane_bytes, size_t* stride_bytes,
+                  int32_t* n_channels) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
+  if ((set != LPC_HALO_PARAMS && set != LPC_HALO_STATE) || (side != 0 && side != 1) || (role != LPC_HALO_SEND && role != LPC_HALO_RECV))
+    return fail(LPC_EINVAL, "bad selector (set %d, side %d, role %d)", set, side, role);
+  if (!plane || !plane_bytes || !stride_bytes || !n_channels) return fail(LPC_EINVAL, "output pointers must not be NULL");
+  const Layout& L = h->L;
+  // padded x index: ghost 0, owned 1 .. nx, ghost nx + 1
+  const long long xp = side == 0 ? (role == LPC_HALO_SEND ? 1 : 0) : (role == LPC_HALO_SEND ? L.nx : L.nx + 1);
+  const size_t base = set == LPC_HALO_PARAMS ? h->off.pi : (h->cur ? h->off.f1 : h->off.f0);
+  *plane = h->ws + base + (size_t)xp * L.sx * h->sT;
+  *plane_bytes = (size_t)L.sx * h->sT;
+  *stride_bytes = (size_t)L.np * h->sT;
+  *n_channels = set == LPC_HALO_PARAMS ? 1 : h->C;
+  return LPC_OK;
+}
+
+int lpc_slab_finish(lpc_lattice* h) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (!h->halo) return fail(LPC_ESTATE, "the lattice was not created with bc[0] = LPC_BC_HALO");
+  if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
+  h->have_regions = false;
+  h->region_moments = false;
+  CUDA_TRY(cudaMemsetAsync(h->ws + h->off.f0, 0, (size_t)h->C * h->L.np * h->sT, h->stream));
+  CUDA_TRY(cudaMemsetAsync(h->ws + h->off.f1, 0, (size_t)h->C * h->L.np * h->sT, h->stream));
+  int rc = h->cfg.precision ? init_state_t<float>(h) : init_state_t<double>(h);
+  if (rc) return rc;
+  rc = h->cfg.precision ? fill_state_ghosts<float>(h) : fill_state_ghosts<double>(h);
+  if (rc) return rc;
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  h->steps = 0;
+  h->halo_ready = true;
+  return LPC_OK;
+}
+
 int lpc_step_n(lpc_lattice* h, int64_t n) {
   if (!h) return fail(LPC_EINVAL, "lattice is NULL");
   if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
   if (n < 0) return fail(LPC_EINVAL, "n must be >= 0");
   if (h->steps + n > h->cfg.max_steps) return fail(LPC_EINVAL, "steps_done + n = %lld exceeds max_steps = %lld", (long long)(h->steps + n), (long long)h->cfg.max_steps);
+  if (h->halo && !h->halo_ready) return fail(LPC_ESTATE, "slab mode: lpc_slab_finish has not been called");
+  if (h->halo && n > 1) return fail(LPC_ESTATE, "slab mode: the x ghost planes must be exchanged after every step (n <= 1)");
   const bool persist = !h->have_regions && n >= 2 &&
                        (h->kernel == LPC_KERNEL_PERSIST || (h->kernel == LPC_KERNEL_AUTO && persist_by_default(h)));
   if (persist) return h->cfg.precision ? launch_persist<float>(h, n) : launch_persist<double>(h, n);
@@ -935,6 +1019,7 @@ int lpc_equilibrate(lpc_lattice* h, double threshold, int64_t max_iters, int64_t
   if (!h) return fail(LPC_EINVAL, "lattice is NULL");
   if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
   if (h->nrho != 1) return fail(LPC_ESTATE, "the density field is not propagated (n_density = 0)");
+  if (h->halo) return fail(LPC_ESTATE, "the equilibration loop is not available in slab mode");
   if (max_iters < 0) return fail(LPC_EINVAL, "max_iters must be >= 0");
   if (check_every < 1) return fail(LPC_EINVAL, "check_every must be >= 1");
   if (!(threshold == threshold)) return fail(LPC_EINVAL, "threshold is NaN");

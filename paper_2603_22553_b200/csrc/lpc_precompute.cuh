@@ -86,7 +86,8 @@ __global__ void site_params_kernel(const double* __restrict__ e, const double* _
   if (bad) atomicAdd(&ctl->bad, bad);
 }
 
-// Ghost layers of nch channel planes: periodic axis -> wrapped interior value, reflective -> 0.
+// Ghost layers of nch channel planes: periodic axis (1) -> wrapped interior value, reflective (0) -> 0;
+// perx = 2 (slab mode): the x ghost planes belong to the caller and are left alone.
 template <typename T>
 __global__ void fill_ghosts_kernel(T* __restrict__ f, int nch, Layout L, int perx, int pery, int perz) {
   const long long fz = (long long)L.nx * L.ny, fy = (long long)L.nx * L.nz, fx = (long long)L.ny * L.nz;
@@ -107,7 +108,7 @@ __global__ void fill_ghosts_kernel(T* __restrict__ f, int nch, Layout L, int per
     } else {
       r -= fz + fy;
       const int y = (int)(r / L.nz), z = (int)(r % L.nz);
-      g[L.idx(side ? L.nx : -1, y, z)] = perx ? g[L.idx(side ? 0 : L.nx - 1, y, z)] : (T)0;
+      if (perx != 2) g[L.idx(side ? L.nx : -1, y, z)] = perx ? g[L.idx(side ? 0 : L.nx - 1, y, z)] : (T)0;
     }
   }
 }

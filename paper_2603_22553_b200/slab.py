@@ -1,0 +1,191 @@
+"""One lattice split into x-slabs over several GPUs (include/lpc.h "Slabs").
+
+The lattice is cut along x into ``n_slabs = world * slabs_per_rank`` contiguous ranges; slab ``s`` lives on rank
+``s // slabs_per_rank``.  Every slab is an ordinary ``liblpc`` lattice created with ``bc[0] = LPC_BC_HALO``: the
+library leaves its two x ghost planes alone and this module fills them after every step with the neighbour's
+outermost owned plane -- a device copy when the neighbour lives in the same process, ``torch.distributed``
+send/recv (NCCL over NVLink between GPUs) otherwise.  That plane exchange is the only data-path communication per
+step.  G[n] and Z_d[m] stay per-slab partial series and are added once, when they are read.
+
+This module holds routing only; every number is computed by the kernels behind the C ABI.  The same driver code
+runs with all slabs in one process (how the GPU tests check it against the unsplit lattice on one B200) and with
+one process per GPU.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+LPC_BC_HALO = 2
+HALO_PARAMS, HALO_STATE = 0, 1
+SEND, RECV = 0, 1
+
+
+def slab_range(nx: int, n_slabs: int, s: int):
+    """Planes [lo, hi) of slab s: contiguous, sizes differ by at most one."""
+    base, rem = divmod(int(nx), int(n_slabs))
+    lo = s * base + min(s, rem)
+    return lo, lo + base + (1 if s < rem else 0)
+
+
+def neighbour(n_slabs: int, s: int, side: int, periodic: bool):
+    """Slab beyond the low (side 0) or high (side 1) face of slab s; None at a wall of the whole lattice."""
+    t = s - 1 if side == 0 else s + 1
+    if 0 <= t < n_slabs:
+        return t
+    return (t % n_slabs) if periodic else None
+
+
+def messages(n_slabs: int, periodic: bool):
+    """Every plane transfer of one exchange as (src_slab, src_side, dst_slab, dst_side), in the one global order
+    both ends of a pair of ranks use to match their sends and receives."""
+    out = []
+    for s in range(n_slabs):
+        for side in (0, 1):
+            t = neighbour(n_slabs, s, side, periodic)
+            if t is not None:
+                out.append((s, side, t, 1 - side))   # my low plane is the neighbour's high ghost and vice versa
+    return out
+
+
+class SlabSet:
+    """The slabs this process owns, and the routing between all of them.
+
+    lattice_factory(shape, bc, **cfg) builds one slab (default: ``paper_2603_22553_b200.Lattice``); it must offer
+    partition_sum / set_partition_sum / set_site_params / halo_planes / slab_finish / step / fid / moments /
+    field / set_state.  ``group`` is a torch.distributed process group (None: the default group if
+    torch.distributed is initialised, else a single process).
+    """
+
+    def __init__(self, global_shape, bc=(0, 0, 0), slabs_per_rank=1, lattice_factory=None, group=None, **cfg):
+        self.dist = None
+        self.rank, self.world = 0, 1
+        try:
+            import torch.distributed as dist
+
+            if dist.is_available() and dist.is_initialized():
+                self.dist = dist
+                self.group = group
+                self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
+        except ImportError:  # pragma: no cover
+            pass
+        self.global_shape = tuple(int(v) for v in global_shape)
+        self.bc = tuple(int(b) for b in bc)
+        if self.bc[0] not in (0, 1):
+            raise ValueError("bc[0] of the whole lattice must be 0 (periodic) or 1 (reflective)")
+        self.spr = int(slabs_per_rank)
+        self.n_slabs = self.world * self.spr
+        if self.n_slabs > self.global_shape[0]:
+            raise ValueError("more slabs than x planes")
+        self.periodic = self.bc[0] == 0
+        self.owned = list(range(self.rank * self.spr, (self.rank + 1) * self.spr))
+        if lattice_factory is None:
+            from . import Lattice as lattice_factory
+        self.ranges = {s: slab_range(self.global_shape[0], self.n_slabs, s) for s in range(self.n_slabs)}
+        self.lat = {}
+        for s in self.owned:
+            lo, hi = self.ranges[s]
+            self.lat[s] = lattice_factory((hi - lo,) + self.global_shape[1:], bc=(LPC_BC_HALO, self.bc[1], self.bc[2]), **cfg)
+        self.steps = 0
+
+    def owner(self, s: int) -> int:
+        return s // self.spr
+
+    def local_part(self, arr, s):
+        """The planes of slab s of an array over the whole lattice (leading axes before x are kept)."""
+        lo, hi = self.ranges[s]
+        a = np.asarray(arr)
+        lead = a.ndim - 3
+        return np.ascontiguousarray(a[(slice(None),) * lead + (slice(lo, hi),)])
+
+    # ---- reductions over all slabs -------------------------------------------------------------
+    def _allreduce(self, x: np.ndarray) -> np.ndarray:
+        """Sum over ranks of a float64 / complex128 host array (plumbing: the series are added once per read)."""
+        if self.dist is None or self.world == 1:
+            return x
+        import torch
+
+        t = torch.from_numpy(np.ascontiguousarray(x).view(np.float64).copy())
+        if self.dist.get_backend(self.group) == "nccl":
+            t = t.cuda()
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM, group=self.group)
+        return t.cpu().numpy().view(x.dtype).reshape(x.shape)
+
+    # ---- the plane exchange -------------------------------------------------------------------
+    def exchange(self, which):
+        """Fill every x ghost plane of `which` (HALO_PARAMS or HALO_STATE) from the neighbour's outermost owned
+        plane.  Same process: one device copy per plane.  Other rank: one send / recv per channel plane, all of one
+        exchange batched into a single group; both ends enumerate `messages()` in the same order, which is what
+        matches the two planes a pair of ranks swaps in each direction on a periodic ring of two."""
+        ops, keep = [], []
+        for src, sside, dst, dside in messages(self.n_slabs, self.periodic):
+            so, do = self.owner(src), self.owner(dst)
+            if so != self.rank and do != self.rank:
+                continue
+            if so == self.rank and do == self.rank:
+                self.lat[dst].halo_planes(which, dside, RECV).copy_(self.lat[src].halo_planes(which, sside, SEND))
+                continue
+            if so == self.rank:
+                planes = self.lat[src].halo_planes(which, sside, SEND)
+                for c in range(planes.shape[0]):
+                    ops.append(self.dist.P2POp(self.dist.isend, planes[c], self._global_rank(do), group=self.group))
+            else:
+                planes = self.lat[dst].halo_planes(which, dside, RECV)
+                for c in range(planes.shape[0]):
+                    ops.append(self.dist.P2POp(self.dist.irecv, planes[c], self._global_rank(so), group=self.group))
+            keep.append(planes)
+        if ops:
+            for req in self.dist.batch_isend_irecv(ops):
+                req.wait()
+
+    def _global_rank(self, r):
+        return r if self.group is None else self.dist.get_global_rank(self.group, r)
+
+    # ---- the call sequence of include/lpc.h "Slabs" ---------------------------------------------
+    def set_site_params(self, dF, blocked, omega, g0=None):
+        """dF, blocked, omega (and g0) are arrays over the WHOLE lattice (host); every rank cuts out its planes."""
+        parts = {s: (self.local_part(dF, s), self.local_part(blocked, s).astype(np.uint8), self.local_part(omega, s)) for s in self.owned}
+        z_local = np.array([sum(self.lat[s].partition_sum(parts[s][0], parts[s][1]) for s in self.owned)], dtype=np.float64)
+        Z = float(self._allreduce(z_local)[0])
+        for s in self.owned:
+            self.lat[s].set_partition_sum(Z)
+            self.lat[s].set_site_params(*parts[s])
+        self.exchange(HALO_PARAMS)
+        for s in self.owned:
+            self.lat[s].slab_finish()
+        if g0 is not None:
+            for s in self.owned:
+                self.lat[s].set_state(0, self.local_part(g0, s))
+        self.exchange(HALO_STATE)
+        self.steps = 0
+        return Z
+
+    def step(self, n=1):
+        """n time steps: per step one sweep per slab, then the plane exchange."""
+        for _ in range(int(n)):
+            for s in self.owned:
+                self.lat[s].step(1)
+            self.exchange(HALO_STATE)
+            self.steps += 1
+
+    def fid(self):
+        """G[0..steps] of the whole lattice: the slabs' partial series added in slab order, then over ranks."""
+        part = sum(self.lat[s].fid() for s in self.owned)
+        return self._allreduce(np.asarray(part, dtype=np.complex128))
+
+    def moments(self):
+        """(Z_d[1..steps+1], D_d) of the whole lattice; both are linear in the per-slab sums."""
+        zs, ds = zip(*(self.lat[s].moments() for s in self.owned))
+        z = self._allreduce(np.asarray(sum(zs), dtype=np.float64))
+        d = self._allreduce(np.asarray(sum(ds), dtype=np.float64))
+        return z, d
+
+    def field(self, which):
+        """Owned planes of a field, as {slab: array}; use ``gather_field`` for the whole lattice on every rank."""
+        return {s: self.lat[s].field(which) for s in self.owned}
+
+    def gather_field(self, which, dtype=np.float64):
+        out = np.zeros(self.global_shape, dtype=dtype)
+        for s, a in self.field(which).items():
+            lo, hi = self.ranges[s]
+            out[lo:hi] = a
+        return self._allreduce(out)

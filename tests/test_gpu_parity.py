@@ -720,3 +720,85 @@ def test_error_codes(lpc):
     assert lpc.lpc_read_fid(h).shape == (4,)
     assert lpc.lpc_steps_done(h) == 3 and lpc.lpc_launch_count(h) > 3
     lpc.lpc_destroy(h)
+
+
+# ---------------------------------------------------------------------------------------------
+# x-slab decomposition.  All slabs live on the one GPU here; the plane exchange is a device copy,
+# the driver code (paper_2603_22553_b200/slab.py) is the one a multi-GPU run executes.
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bc,n_slabs,kernel,precision", [((0, 0, 0), 2, 2, 0), ((1, 0, 0), 3, 2, 0), ((0, 1, 0), 1, 1, 0),
+                                                         ((1, 0, 1), 4, 0, 0), ((0, 0, 0), 3, 2, 1)])
+def test_slabs_match_unsplit_lattice_and_oracle(lpc, oracle_mod, bc, n_slabs, kernel, precision):
+    from paper_2603_22553_b200 import slab
+
+    n = 40
+    lat = lpc_inputs.random_small((50, 18, 70), bc=bc, p_block=0.25, alpha=0.9, seed=81, n_steps=n, n_moments=3)
+    rng = np.random.default_rng(3)
+    g0 = (rng.random(lat.shape) + 1j * rng.random(lat.shape)) * (lat.blocked == 0)
+    tol_site, tol_sum = (1e-5, 1e-5) if precision else (1e-10, 1e-9)
+
+    def factory(shape, bc, **cfg):
+        m = lpc.Lattice(shape, bc=bc, **cfg)
+        m.set_kernel(kernel)
+        return m
+
+    ss = slab.SlabSet(lat.shape, bc=lat.bc, slabs_per_rank=n_slabs, lattice_factory=factory, precision=precision, n_moments=3,
+                      n_density=1, dt=lat.dt, a=lat.a, alpha=lat.alpha, max_steps=n)
+    assert sorted(ss.lat) == list(range(n_slabs)) and sum(hi - lo for lo, hi in ss.ranges.values()) == lat.nx
+    ss.set_site_params(lat.dF, lat.blocked, lat.omega, g0)
+    orc = oracle_mod.Oracle.from_lattice(lat, n_moments=3, max_steps=n)
+    orc.set_g(g0)
+    assert abs(ss.fid()[0] - orc.fid()[0]) <= tol_sum * np.abs(g0).sum()
+    ss.step(n)
+    orc.step(n)
+    pi = orc.pi()
+    opn = lat.blocked == 0
+    G_o, sabs = orc.fid(with_scale=True)
+    assert np.max(np.abs(ss.fid() - G_o) / sabs) <= tol_sum
+    g = ss.gather_field(lpc.LPC_FIELD_G, dtype=np.complex128)
+    hmax = np.max(np.abs(g0)[opn] / pi[opn])   # |g_i(n)| <= max_j |g_j(0)| / pi_j * pi_i (detailed balance), the scale of Q13
+    assert np.max(np.abs(g - orc.g())[opn] / pi[opn]) <= tol_site * hmax
+    Z_o, D_o = orc.moments()
+    Z_g, D_g = ss.moments()
+    assert np.max(np.abs(Z_g - Z_o) / np.abs(Z_o[:, :1])) <= tol_sum
+    assert np.max(np.abs(D_g - D_o) / (np.abs(Z_o[:, 0]) / (2 * lat.dt))) <= tol_sum
+    for d in range(3):
+        P = ss.gather_field(lpc.LPC_FIELD_PX + d)
+        assert np.max(np.abs(P - orc.P(d))[opn] / (lat.a * pi[opn])) <= tol_site
+    # the density channel started at pi and stays there across the slab faces
+    rho = ss.gather_field(lpc.LPC_FIELD_RHO)
+    assert np.max(np.abs(rho - pi)[opn] / pi[opn]) <= (1e-4 if precision else 1e-12)
+    if precision == 0:
+        # against the unsplit lattice on the same kernel: same arithmetic per site, pi differs only through the
+        # order in which the partition sum was added up
+        whole = lpc.Lattice.from_inputs(lat, n_moments=3, n_density=1, max_steps=n, g0=g0)
+        whole.set_kernel(kernel)
+        whole.step(n)
+        assert np.max(np.abs(g - whole.field(lpc.LPC_FIELD_G))[opn] / pi[opn]) <= 1e-12 * hmax
+        assert np.max(np.abs(ss.fid() - whole.fid())) <= 1e-12 * np.abs(g0).sum()
+
+
+def test_slab_mode_errors(lpc):
+    lat = lpc_inputs.random_small((12, 10, 20), seed=82)
+    m = lpc.Lattice((12, 10, 20), bc=(lpc.LPC_BC_HALO, 0, 0), n_density=1, max_steps=5)
+    assert m.partition_sum(lat.dF, lat.blocked) == pytest.approx(np.exp(-lat.dF)[lat.blocked == 0].sum(), rel=1e-13)
+    m.set_site_params(lat.dF, lat.blocked, lat.omega)
+    with pytest.raises(lpc.LpcError) as e:
+        m.step(1)                      # lpc_slab_finish first
+    assert e.value.code == lpc.LPC_ESTATE
+    m.slab_finish()
+    m.step(1)
+    for bad in (lambda: m.step(2), lambda: m.equilibrate(1e-3, 5)):
+        with pytest.raises(lpc.LpcError) as e:
+            bad()
+        assert e.value.code == lpc.LPC_ESTATE
+    with pytest.raises(lpc.LpcError) as e:
+        lpc.Lattice((12, 10, 20), bc=(0, lpc.LPC_BC_HALO, 0))
+    assert e.value.code == lpc.LPC_EINVAL
+    plain = lpc.Lattice.from_inputs(lat, max_steps=2)
+    with pytest.raises(lpc.LpcError) as e:
+        plain.slab_finish()
+    assert e.value.code == lpc.LPC_ESTATE
+    # the plane views address the workspace: shape [channels, (ny+2) * padded nz]
+    v = plain.halo_planes(lpc.LPC_HALO_STATE, 0, lpc.LPC_HALO_SEND)
+    assert v.shape[0] == 2 + lat.n_moments and v.shape[1] % 12 == 0 and float(v[0].max()) == 1.0
