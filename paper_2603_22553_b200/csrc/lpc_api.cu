@@ -124,8 +124,8 @@ Layout make_layout(const lpc_config* c) {
 // and slightly worse at 256^3, so there is one tile shape.)
 constexpr int SM_COUNT = 148;
 
-void tma_geometry(int C, int nx, int ny, int nz, int* ty, int* tz, int* nstage, int* xc, int* tiles_z, int* tiles_y, int* chunks_x) {
-  *ty = 8; *tz = 64;
+void tma_geometry(int C, bool f32, int nx, int ny, int nz, int* ty, int* tz, int* nstage, int* xc, int* tiles_z, int* tiles_y, int* chunks_x) {
+  *ty = f32 ? 16 : 8; *tz = 64;   // fp32: a thread owns a z-quad (lpc_step_vec.cuh), 256 threads cover 16 rows
   *nstage = 4;   // 3 when the density rides along (3 channels); informational, the kernels fix it
   *tiles_z = (nz + *tz - 1) / *tz;
   *tiles_y = (ny + *ty - 1) / *ty;
@@ -168,7 +168,7 @@ Offsets make_offsets(const lpc_config* c, const Layout& L) {
   const size_t sT = c->precision ? 4 : 8;
   const int C = 2 + c->n_density + c->n_moments;
   int ty, tz, ns, xc, tzs, tys, cxs;
-  tma_geometry(C, c->nx, c->ny, c->nz, &ty, &tz, &ns, &xc, &tzs, &tys, &cxs);
+  tma_geometry(C, c->precision == 1, c->nx, c->ny, c->nz, &ty, &tz, &ns, &xc, &tzs, &tys, &cxs);
   // the LPC_XC override may only shrink chunks at run time; size for the worst case (one plane per chunk)
   const size_t tma_blocks = (size_t)tzs * tys * (size_t)c->nx;
   o.partial_slots = std::max<size_t>(std::max<size_t>(DIRECT_MAX_BLOCKS, AUX_BLOCKS), std::min<size_t>(tma_blocks, 1u << 20));
@@ -297,19 +297,30 @@ int launch_step_t(lpc_lattice* h) {
       h->launches++;
       return LPC_OK;
     };
+    constexpr bool F32 = sizeof(T) == 4;   // fp32 runs the z-quad march on 16 x 64 tiles, fp64 the z-pair march on 8 x 64
+    constexpr int NS = (NRHO == 0) ? 4 : 3;   // two CTAs per SM must fit in shared memory
+    constexpr int NSL = (NRHO == 0) ? 3 : 2;
     if constexpr (NMOM == 3) {
       StepArgs<T> am = a;
       am.c0 = 2 + NRHO;
       am.fout = a.fout + (long long)am.c0 * h->L.np;
-      int rc = h->have_links ? launch_links(step_tma_links_kernel<T, 0, 0, 3, 8, 64, 3>, TmaCfg<T, 0, 0, 3, 8, 64, 3, 1>(), h->tm_m[h->cur], am)
-                             : launch(step_tma_kernel<T, 0, 0, 3, 8, 64, 4>, TmaCfg<T, 0, 0, 3, 8, 64, 4>(), h->tm_m[h->cur], am);
+      int rc;
+      if constexpr (F32)
+        rc = h->have_links ? launch_links(step_tma_vec_links_kernel<T, 4, 0, 0, 3, 16, 64, 3>, TmaCfg<T, 0, 0, 3, 16, 64, 3, 1, 4>(), h->tm_m[h->cur], am)
+                           : launch(step_tma_vec_kernel<T, 4, 0, 0, 3, 16, 64, 4>, TmaCfg<T, 0, 0, 3, 16, 64, 4, 0, 4>(), h->tm_m[h->cur], am);
+      else
+        rc = h->have_links ? launch_links(step_tma_links_kernel<T, 0, 0, 3, 8, 64, 3>, TmaCfg<T, 0, 0, 3, 8, 64, 3, 1>(), h->tm_m[h->cur], am)
+                           : launch(step_tma_kernel<T, 0, 0, 3, 8, 64, 4>, TmaCfg<T, 0, 0, 3, 8, 64, 4>(), h->tm_m[h->cur], am);
       if (rc) return rc;
     }
     a.c0 = 0;
-    constexpr int NS = (NRHO == 0) ? 4 : 3;   // two CTAs per SM must fit in shared memory
-    constexpr int NSL = (NRHO == 0) ? 3 : 2;
-    int rc = h->have_links ? launch_links(step_tma_links_kernel<T, 2, NRHO, 0, 8, 64, NSL>, TmaCfg<T, 2, NRHO, 0, 8, 64, NSL, 1>(), h->tm_f[h->cur], a)
-                           : launch(step_tma_kernel<T, 2, NRHO, 0, 8, 64, NS>, TmaCfg<T, 2, NRHO, 0, 8, 64, NS>(), h->tm_f[h->cur], a);
+    int rc;
+    if constexpr (F32)
+      rc = h->have_links ? launch_links(step_tma_vec_links_kernel<T, 4, 2, NRHO, 0, 16, 64, NSL>, TmaCfg<T, 2, NRHO, 0, 16, 64, NSL, 1, 4>(), h->tm_f[h->cur], a)
+                         : launch(step_tma_vec_kernel<T, 4, 2, NRHO, 0, 16, 64, NS>, TmaCfg<T, 2, NRHO, 0, 16, 64, NS, 0, 4>(), h->tm_f[h->cur], a);
+    else
+      rc = h->have_links ? launch_links(step_tma_links_kernel<T, 2, NRHO, 0, 8, 64, NSL>, TmaCfg<T, 2, NRHO, 0, 8, 64, NSL, 1>(), h->tm_f[h->cur], a)
+                         : launch(step_tma_kernel<T, 2, NRHO, 0, 8, 64, NS>, TmaCfg<T, 2, NRHO, 0, 8, 64, NS>(), h->tm_f[h->cur], a);
     if (rc) return rc;
     h->cur ^= 1;
     return LPC_OK;
@@ -827,7 +838,7 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
     if (!strcmp(e, "tma")) h->kernel = LPC_KERNEL_TMA;
     if (!strcmp(e, "persist")) h->kernel = LPC_KERNEL_PERSIST;
   }
-  tma_geometry(h->C, cfg->nx, cfg->ny, cfg->nz, &h->ty, &h->tz, &h->nstage, &h->xc, &h->tiles_z, &h->tiles_y, &h->chunks_x);
+  tma_geometry(h->C, cfg->precision == 1, cfg->nx, cfg->ny, cfg->nz, &h->ty, &h->tz, &h->nstage, &h->xc, &h->tiles_z, &h->tiles_y, &h->chunks_x);
   h->tma_ok = (size_t)h->tiles_z * h->tiles_y * h->chunks_x <= h->off.partial_slots;
   if (h->tma_ok) {
     const Layout& L = h->L;

@@ -240,14 +240,15 @@ struct TmaLinkMaps {
   CUtensorMap pic, mx, my, mz;   // pi centres, the three link channels
 };
 
-template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int LK = 0>
+// VW: sites per thread along z (one 16-byte vector: 2 in fp64, 4 in the fp32 march of lpc_step_vec.cuh).
+template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int LK = 0, int VW = 2>
 struct TmaCfg {
   static constexpr int C = NH + NRHO + NMOM;
   static constexpr int NRED = 2 + NMOM;
   static constexpr int HZ = 16 / (int)sizeof(T);  // z halo of 16 bytes on each side keeps the centre pairs 16-byte aligned
   static constexpr int TZW = TZ + 2 * HZ;
   static constexpr int TYH = TY + 2;
-  static constexpr int NCONS = TY * TZ / 2;  // consumer threads, one per z-pair
+  static constexpr int NCONS = TY * TZ / VW;  // consumer threads, one per z-pair (z-quad with VW = 4)
   static constexpr int NCW = NCONS / 32;
   static constexpr int NTHREADS = NCONS;      // no producer warp: thread 0 issues the TMA loads between planes
   static constexpr int F_RAW = C * TYH * TZW * (int)sizeof(T);
@@ -273,10 +274,10 @@ struct TmaCfg {
   static constexpr int SMEM_BYTES = RED_OFF + ((NTHREADS / 32) * NRED + 1) * 8 + 128;  // +128: manual alignment slack
   // Resident CTAs per SM the registers are budgeted for: two 8-warp CTAs (TY = 8, up to 3 channels) or
   // one.  16 warps per SM are 4 per scheduler, i.e. up to 128 registers per thread.
-  static constexpr int LB_CTAS = (TY == 8 && C <= 3) ? 2 : 1;
+  static constexpr int LB_CTAS = (NCONS == 256 && C <= 3) ? 2 : 1;
   static constexpr int LB_THREADS = NTHREADS;
   static_assert(NCONS % 32 == 0, "consumer threads must fill whole warps");
-  static_assert(TZ % 2 == 0, "TZ must be even");
+  static_assert(TZ % VW == 0, "TZ must be a multiple of the vector width");
 };
 
 template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int LK, typename LM>
@@ -529,3 +530,5 @@ __global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1>::
 }
 
 }  // namespace lpc
+
+#include "lpc_step_vec.cuh"

@@ -1,0 +1,314 @@
+// lpc_step_vec.cuh -- the TMA march of lpc_step.cuh with VW sites per thread along z (included by lpc_step.cuh).
+//
+// The fp64 march gives a thread one 16-byte z-pair.  In fp32 a pair is only 8 bytes: the same instruction count
+// per site moves half the bytes and the sweep becomes issue-bound (ncu, profiles/: 532 M warp instructions per
+// 512^3 launch in fp32 against 555 M in fp64, DRAM at 57% of peak).  Here a thread owns a 16-byte z-QUAD in fp32
+// (VW = 4) on a 16 x 64 tile, so that barrier waits, address arithmetic, the TMA issue and the y-halo loads are
+// paid once per four sites.  Same per-site arithmetic (SiteUpdate::gather), same staging, pipeline and reduction
+// as step_tma_body; the state agrees bit for bit with the direct and persistent kernels.
+#pragma once
+
+namespace lpc {
+
+template <typename T, int VW> struct VecN;
+template <> struct VecN<double, 2> { using type = double2; };
+template <> struct VecN<float, 2> { using type = float2; };
+template <> struct VecN<float, 4> { using type = float4; };
+
+template <typename T, int VW>
+__device__ __forceinline__ void ldv(const T* p, T (&o)[VW]) {
+  const typename VecN<T, VW>::type v = *reinterpret_cast<const typename VecN<T, VW>::type*>(p);
+  o[0] = v.x; o[1] = v.y;
+  if constexpr (VW == 4) { o[2] = v.z; o[3] = v.w; }
+}
+template <typename T, int VW>
+__device__ __forceinline__ typename VecN<T, VW>::type packv(const T (&o)[VW]) {
+  typename VecN<T, VW>::type v;
+  v.x = o[0]; v.y = o[1];
+  if constexpr (VW == 4) { v.z = o[2]; v.w = o[3]; }
+  return v;
+}
+// the first nvalid of VW consecutive sites
+template <typename T, int VW>
+__device__ __forceinline__ void store_vec(T* __restrict__ p, typename VecN<T, VW>::type v, int nvalid) {
+  if (nvalid == VW) {
+    *reinterpret_cast<typename VecN<T, VW>::type*>(p) = v;
+  } else {
+    T o[VW];
+    o[0] = v.x; o[1] = v.y;
+    if constexpr (VW == 4) { o[2] = v.z; o[3] = v.w; }
+#pragma unroll
+    for (int k = 0; k < VW; ++k)
+      if (k < nvalid) p[k] = o[k];
+  }
+}
+// one channel of a group that lies on a periodic face: the sites and their ghost copies (rare, out of line)
+template <typename T, int VW>
+__device__ __noinline__ void store_face_vec(T* __restrict__ base, long long i, int nx, int ny, int nz, long long sy, long long sx,
+                                            int permask, int x, int y, int z, typename VecN<T, VW>::type v, int nvalid) {
+  store_vec<T, VW>(base + i, v, nvalid);
+  if (permask & 4) {
+    T o[VW];
+    o[0] = v.x; o[1] = v.y;
+    if constexpr (VW == 4) { o[2] = v.z; o[3] = v.w; }
+#pragma unroll
+    for (int k = 0; k < VW; ++k) {
+      if (k < nvalid && z + k == 0) base[i + k + nz] = o[k];        // ghost column z = nz
+      if (k < nvalid && z + k == nz - 1) base[i + k - nz] = o[k];   // ghost column z = -1
+    }
+  }
+  if (permask & 2) {
+    if (y == 0) store_vec<T, VW>(base + i + (long long)ny * sy, v, nvalid);
+    if (y == ny - 1) store_vec<T, VW>(base + i - (long long)ny * sy, v, nvalid);
+  }
+  if (permask & 1) {
+    if (x == 0) store_vec<T, VW>(base + i + (long long)nx * sx, v, nvalid);
+    if (x == nx - 1) store_vec<T, VW>(base + i - (long long)nx * sx, v, nvalid);
+  }
+}
+
+template <typename T, int VW, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int LK, typename LM>
+__device__ __forceinline__ void step_tma_body_v(const CUtensorMap& tm_f, const CUtensorMap& tm_pi, const CUtensorMap& tm_cs, const LM& lm,
+                                                const StepArgs<T>& a) {
+  using K = TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, LK, VW>;
+  using V = typename VecN<T, VW>::type;
+  constexpr int C = K::C, NRED = K::NRED, TZW = K::TZW, TYH = K::TYH, HZ = K::HZ;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  unsigned char* smem = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem + K::BAR_OFF);
+  uint64_t* empty = full + NSTAGE;
+  double* red = reinterpret_cast<double*>(smem + K::RED_OFF);
+
+  const Layout& L = a.L;
+  const int bz = blockIdx.x % a.tiles_z;
+  const int by = (blockIdx.x / a.tiles_z) % a.tiles_y;
+  const int bx = blockIdx.x / (a.tiles_z * a.tiles_y);
+  const int z0 = bz * TZ, y0 = by * TY, x0 = bx * a.xc;
+  const int nplanes = min(a.xc, L.nx - x0);
+  const int nloads = nplanes + 2;
+  const int lane = threadIdx.x & 31;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < NSTAGE; ++s) {
+      mbar_init(&full[s], 1);
+      mbar_init(&empty[s], K::NCW);
+    }
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  double acc[NRED];
+#pragma unroll
+  for (int r = 0; r < NRED; ++r) acc[r] = 0.0;
+
+  // ----- TMA issue (thread 0): load j brings plane x0-1+j into stage j % NSTAGE (as in step_tma_body) -----
+  int jl = 0;
+  auto issue_load = [&]() {
+    const int s = jl % NSTAGE;
+    if (jl >= NSTAGE) mbar_wait(&empty[s], ((jl / NSTAGE) - 1) & 1);
+    unsigned char* st = smem + s * K::STAGE_BYTES;
+    const bool need_kcs = (NH == 2) && (jl >= 1 && jl <= nplanes);
+    mbar_expect_tx(&full[s], K::TX_BYTES + (need_kcs ? K::KCS_RAW : 0));
+    tma_load_4d(st, &tm_f, &full[s], L.padz + z0 - HZ, y0, x0 + jl, a.c0);
+    if constexpr (LK) {
+      tma_load_3d(st + K::F_BYTES, &lm.pic, &full[s], L.padz + z0, y0 + 1, x0 + jl);
+      tma_load_3d(st + K::MX_OFF, &lm.mx, &full[s], L.padz + z0, y0 + 1, x0 + jl);
+      tma_load_3d(st + K::MY_OFF, &lm.my, &full[s], L.padz + z0, y0, x0 + jl);
+      tma_load_3d(st + K::MZ_OFF, &lm.mz, &full[s], L.padz + z0 - HZ, y0 + 1, x0 + jl);
+    } else {
+      tma_load_3d(st + K::F_BYTES, &tm_pi, &full[s], L.padz + z0 - HZ, y0, x0 + jl);
+    }
+    if (need_kcs) tma_load_4d(st + K::F_BYTES + K::PI_BYTES, &tm_cs, &full[s], L.padz + z0, y0 + 1, x0 + jl, 0);
+    ++jl;
+  };
+  if (threadIdx.x == 0) {
+    tma_prefetch_desc(&tm_f);
+    if constexpr (LK) {
+      tma_prefetch_desc(&lm.pic);
+      tma_prefetch_desc(&lm.mx);
+      tma_prefetch_desc(&lm.my);
+      tma_prefetch_desc(&lm.mz);
+    } else {
+      tma_prefetch_desc(&tm_pi);
+    }
+    tma_prefetch_desc(&tm_cs);
+    for (int j = 0; j < NSTAGE && j < nloads; ++j) issue_load();
+  }
+
+  const int ty = threadIdx.x / (TZ / VW);   // row inside the tile
+  const int tp = threadIdx.x % (TZ / VW);   // group inside the row
+  const int y = y0 + ty, z = z0 + VW * tp;
+  const int nvalid = (y < L.ny) ? max(0, min(VW, L.nz - z)) : 0;   // the first nvalid sites of the group exist
+  const int ec = (ty + 1) * TZW + VW * tp + HZ;  // element offset of the group in a halo'd tile
+  const int ek = ty * TZ + VW * tp;              // and in a tile without halo
+  const bool edge_yz = (a.per[1] && (y == 0 || y == L.ny - 1)) || (a.per[2] && (z == 0 || z + VW >= L.nz));
+  const int permask = (a.per[0] ? 1 : 0) | (a.per[1] ? 2 : 0) | (a.per[2] ? 4 : 0);
+  T* outp = a.fout + L.idx(x0, y, z);
+
+  // one x-plane as a thread holds it: the group's values of every channel and of pi, kappa, and mlo = the link
+  // weight towards the plane below (LK: the plane's own +x link weight, i.e. the -x weight of the plane above)
+  struct Plane {
+    T f[C][VW];
+    T pi[VW], kap[VW], mlo[VW];
+  };
+  Plane P0, P1, P2;
+  int sj = 0;
+  uint32_t phj = 0;
+  auto take = [&](Plane& n, const Plane* below) {
+    mbar_wait(&full[sj], phj);
+    const T* sf = reinterpret_cast<const T*>(smem + sj * K::STAGE_BYTES);
+    const T* sp = reinterpret_cast<const T*>(smem + sj * K::STAGE_BYTES + K::F_BYTES);
+#pragma unroll
+    for (int c = 0; c < C; ++c) ldv<T, VW>(sf + c * TYH * TZW + ec, n.f[c]);
+    ldv<T, VW>(sp + (LK ? ek : ec), n.pi);
+#pragma unroll
+    for (int k = 0; k < VW; ++k) n.kap[k] = kappa_of(n.pi[k], a.a6);
+    if constexpr (LK) {
+      ldv<T, VW>(reinterpret_cast<const T*>(smem + sj * K::STAGE_BYTES + K::MX_OFF) + ek, n.mlo);
+    } else if (below) {
+#pragma unroll
+      for (int k = 0; k < VW; ++k) n.mlo[k] = tmin(n.pi[k], below->pi[k]);
+    }
+    if (++sj == NSTAGE) {
+      sj = 0;
+      phj ^= 1u;
+    }
+  };
+
+  auto plane = [&](int x, int sc, const Plane& prv, const Plane& ctr, Plane& nxt) {
+    if (threadIdx.x == 0 && jl < nloads) issue_load();
+    take(nxt, &ctr);
+    const T* sf = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES);
+    const T* sk = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES + K::F_BYTES + K::PI_BYTES);
+    T csv[VW], snv[VW];
+    if (NH == 2) {
+      ldv<T, VW>(sk + ek, csv);
+      ldv<T, VW>(sk + TY * TZ + ek, snv);
+    }
+    SiteUpdate<T, NRHO, NMOM> u[VW];
+    if constexpr (LK) {
+      const T* smy = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES + K::MY_OFF) + ek;   // row y-1 of the box
+      const T* smz = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES + K::MZ_OFF) + ty * K::TZM + HZ + VW * tp;
+      T mym[VW], myp[VW], mzp[VW];
+      ldv<T, VW>(smy, mym);
+      ldv<T, VW>(smy + TZ, myp);
+      ldv<T, VW>(smz, mzp);
+      const T mz0 = smz[-1];
+#pragma unroll
+      for (int k = 0; k < VW; ++k) {
+        u[k].mxm = prv.mlo[k]; u[k].mxp = ctr.mlo[k];
+        u[k].mym = mym[k]; u[k].myp = myp[k];
+        u[k].mzm = k == 0 ? mz0 : mzp[k ? k - 1 : 0];
+        u[k].mzp = mzp[k];
+      }
+    } else {
+      const T* sp = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES + K::F_BYTES);
+      T pym[VW], pyp[VW];
+      ldv<T, VW>(sp + ec - TZW, pym);
+      ldv<T, VW>(sp + ec + TZW, pyp);
+      const T pzm = sp[ec - 1], pzp = sp[ec + VW];
+#pragma unroll
+      for (int k = 0; k < VW; ++k) {
+        u[k].mxm = ctr.mlo[k]; u[k].mxp = nxt.mlo[k];
+        u[k].mym = tmin(ctr.pi[k], pym[k]); u[k].myp = tmin(ctr.pi[k], pyp[k]);
+        u[k].mzp = tmin(ctr.pi[k], k == VW - 1 ? pzp : ctr.pi[k == VW - 1 ? k : k + 1]);
+      }
+      u[0].mzm = tmin(ctr.pi[0], pzm);
+#pragma unroll
+      for (int k = 1; k < VW; ++k) u[k].mzm = u[k - 1].mzp;
+    }
+#pragma unroll
+    for (int k = 0; k < VW; ++k) {
+      u[k].pc = ctr.pi[k];
+      u[k].kap = ctr.kap[k];
+    }
+
+    T o[C][VW];
+#pragma unroll
+    for (int c = 0; c < C; ++c) {
+      const T* fcn = sf + c * TYH * TZW;
+      T fym[VW], fyp[VW];
+      ldv<T, VW>(fcn + ec - TZW, fym);
+      ldv<T, VW>(fcn + ec + TZW, fyp);
+      const T fzm = fcn[ec - 1], fzp = fcn[ec + VW];
+      if (NMOM == 3 && c >= NH + NRHO) {
+        const int d = c - NH - NRHO;
+        double t = 0.0;
+#pragma unroll
+        for (int k = 0; k < VW; ++k) {
+          const T dm = (d == 0) ? (u[k].mxp - u[k].mxm) : (d == 1) ? (u[k].myp - u[k].mym) : (u[k].mzp - u[k].mzm);
+          if (k < nvalid) t += (double)ctr.f[c][k] * (double)dm;
+        }
+        acc[2 + d] += t;
+      }
+#pragma unroll
+      for (int k = 0; k < VW; ++k)
+        o[c][k] = u[k].gather(ctr.f[c][k], prv.f[c][k], nxt.f[c][k], fym[k], fyp[k], k == 0 ? fzm : ctr.f[c][k ? k - 1 : 0],
+                              k == VW - 1 ? fzp : ctr.f[c][k == VW - 1 ? k : k + 1]);
+    }
+    // every shared-memory read of stage sc is done: hand it back to the producer
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty[sc]);
+
+    if (NH == 2) {
+#pragma unroll
+      for (int k = 0; k < VW; ++k) {
+        const T hr = o[0][k], hi = o[1][k];
+        o[0][k] = csv[k] * hr - snv[k] * hi;
+        o[1][k] = csv[k] * hi + snv[k] * hr;
+        if (k < nvalid) {
+          acc[0] += (double)ctr.pi[k] * (double)o[0][k];
+          acc[1] += (double)ctr.pi[k] * (double)o[1][k];
+        }
+      }
+    }
+    if (nvalid > 0) {
+      if (edge_yz || (a.per[0] && (x == 0 || x == L.nx - 1))) {
+        const long long i = L.idx(x, y, z);
+#pragma unroll
+        for (int c = 0; c < C; ++c)
+          store_face_vec<T, VW>(a.fout + (long long)c * L.np, i, L.nx, L.ny, L.nz, L.sy, L.sx, permask, x, y, z, packv<T, VW>(o[c]), nvalid);
+      } else {
+#pragma unroll
+        for (int c = 0; c < C; ++c) store_vec<T, VW>(outp + (long long)c * L.np, packv<T, VW>(o[c]), nvalid);
+      }
+    }
+    outp += L.sx;
+  };
+
+  take(P0, nullptr);
+  __syncwarp();
+  if (lane == 0) mbar_arrive(&empty[0]);   // the plane below the chunk is only needed for its centres
+  take(P1, &P0);
+
+  // the march, unrolled by three so that the planes keep their registers while their roles rotate
+  int sc = 1 % NSTAGE;
+  auto next_stage = [&]() { if (++sc == NSTAGE) sc = 0; };
+  int p = 0;
+  for (; p + 3 <= nplanes; p += 3) {
+    plane(x0 + p, sc, P0, P1, P2); next_stage();
+    plane(x0 + p + 1, sc, P1, P2, P0); next_stage();
+    plane(x0 + p + 2, sc, P2, P0, P1); next_stage();
+  }
+  if (p < nplanes) { plane(x0 + p, sc, P0, P1, P2); next_stage(); ++p; }
+  if (p < nplanes) { plane(x0 + p, sc, P1, P2, P0); next_stage(); ++p; }
+
+  block_reduce_finalize<NRED, (NH == 2) ? FIN_STEP : FIN_MOM, NMOM>(acc, red, a.partials, a.ctl, a.fid, a.vacf, a.vacf_stride, a.zscale,
+                                                                    gridDim.x, blockIdx.x);
+}
+
+template <typename T, int VW, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE>
+__global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 0, VW>::LB_THREADS, TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 0, VW>::LB_CTAS)
+    step_tma_vec_kernel(const __grid_constant__ CUtensorMap tm_f, const __grid_constant__ CUtensorMap tm_pi,
+                        const __grid_constant__ CUtensorMap tm_cs, StepArgs<T> a) {
+  step_tma_body_v<T, VW, NH, NRHO, NMOM, TY, TZ, NSTAGE, 0>(tm_f, tm_pi, tm_cs, NoLinkMaps(), a);
+}
+
+template <typename T, int VW, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE>
+__global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1, VW>::LB_THREADS, TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1, VW>::LB_CTAS)
+    step_tma_vec_links_kernel(const __grid_constant__ CUtensorMap tm_f, const __grid_constant__ CUtensorMap tm_cs,
+                              const __grid_constant__ TmaLinkMaps lm, StepArgs<T> a) {
+  step_tma_body_v<T, VW, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1>(tm_f, tm_f, tm_cs, lm, a);
+}
+
+}  // namespace lpc
