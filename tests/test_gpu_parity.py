@@ -504,7 +504,7 @@ def test_link_mobility_regions_equilibration_and_errors(lpc, oracle_mod):
 # f4: the film-electrode cell of PAPER.md:236-248 (100 x 100 x 300, no periodic boundary in z)
 # ---------------------------------------------------------------------------------------------
 def test_film_electrode_cell(lpc, oracle_mod):
-    n = 50000 if FULL else 150
+    n = 2000 if FULL else 150
     lat = lpc_inputs.film(n_steps=n, n_moments=3)
     assert lat.shape == (100, 100, 300) and lat.bc == (0, 0, 1) and abs(lat.notes["fraction"] - 0.38) < 0.01
     label = lat.notes["particle"]
