@@ -297,30 +297,21 @@ int launch_step_t(lpc_lattice* h) {
       h->launches++;
       return LPC_OK;
     };
-    constexpr bool F32 = sizeof(T) == 4;   // fp32 runs the z-quad march on 16 x 64 tiles, fp64 the z-pair march on 8 x 64
+    // fp64: a thread owns a z-pair on 8 x 64 tiles; fp32: a z-quad on 16 x 64 tiles (one 16-byte group either way)
+    constexpr int VW = 16 / (int)sizeof(T), TY = 4 * VW;
     constexpr int NS = (NRHO == 0) ? 4 : 3;   // two CTAs per SM must fit in shared memory
-    constexpr int NSL = (NRHO == 0) ? 3 : 2;
+    constexpr int NSL = (NRHO == 0) ? 3 : 2;  // with the link-weight boxes
     if constexpr (NMOM == 3) {
       StepArgs<T> am = a;
       am.c0 = 2 + NRHO;
       am.fout = a.fout + (long long)am.c0 * h->L.np;
-      int rc;
-      if constexpr (F32)
-        rc = h->have_links ? launch_links(step_tma_vec_links_kernel<T, 4, 0, 0, 3, 16, 64, 3>, TmaCfg<T, 0, 0, 3, 16, 64, 3, 1, 4>(), h->tm_m[h->cur], am)
-                           : launch(step_tma_vec_kernel<T, 4, 0, 0, 3, 16, 64, 4>, TmaCfg<T, 0, 0, 3, 16, 64, 4, 0, 4>(), h->tm_m[h->cur], am);
-      else
-        rc = h->have_links ? launch_links(step_tma_links_kernel<T, 0, 0, 3, 8, 64, 3>, TmaCfg<T, 0, 0, 3, 8, 64, 3, 1>(), h->tm_m[h->cur], am)
-                           : launch(step_tma_kernel<T, 0, 0, 3, 8, 64, 4>, TmaCfg<T, 0, 0, 3, 8, 64, 4>(), h->tm_m[h->cur], am);
+      int rc = h->have_links ? launch_links(step_tma_links_kernel<T, 0, 0, 3, TY, 64, 3, VW>, TmaCfg<T, 0, 0, 3, TY, 64, 3, 1, VW>(), h->tm_m[h->cur], am)
+                             : launch(step_tma_kernel<T, 0, 0, 3, TY, 64, 4, VW>, TmaCfg<T, 0, 0, 3, TY, 64, 4, 0, VW>(), h->tm_m[h->cur], am);
       if (rc) return rc;
     }
     a.c0 = 0;
-    int rc;
-    if constexpr (F32)
-      rc = h->have_links ? launch_links(step_tma_vec_links_kernel<T, 4, 2, NRHO, 0, 16, 64, NSL>, TmaCfg<T, 2, NRHO, 0, 16, 64, NSL, 1, 4>(), h->tm_f[h->cur], a)
-                         : launch(step_tma_vec_kernel<T, 4, 2, NRHO, 0, 16, 64, NS>, TmaCfg<T, 2, NRHO, 0, 16, 64, NS, 0, 4>(), h->tm_f[h->cur], a);
-    else
-      rc = h->have_links ? launch_links(step_tma_links_kernel<T, 2, NRHO, 0, 8, 64, NSL>, TmaCfg<T, 2, NRHO, 0, 8, 64, NSL, 1>(), h->tm_f[h->cur], a)
-                         : launch(step_tma_kernel<T, 2, NRHO, 0, 8, 64, NS>, TmaCfg<T, 2, NRHO, 0, 8, 64, NS>(), h->tm_f[h->cur], a);
+    int rc = h->have_links ? launch_links(step_tma_links_kernel<T, 2, NRHO, 0, TY, 64, NSL, VW>, TmaCfg<T, 2, NRHO, 0, TY, 64, NSL, 1, VW>(), h->tm_f[h->cur], a)
+                           : launch(step_tma_kernel<T, 2, NRHO, 0, TY, 64, NS, VW>, TmaCfg<T, 2, NRHO, 0, TY, 64, NS, 0, VW>(), h->tm_f[h->cur], a);
     if (rc) return rc;
     h->cur ^= 1;
     return LPC_OK;

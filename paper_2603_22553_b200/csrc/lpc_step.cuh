@@ -3,7 +3,7 @@
 // Two kernels compute the same thing with the same per-site arithmetic (SiteUpdate):
 //   step_direct_kernel : one thread per z-pair of sites, neighbours read straight from global
 //                        memory (L1/L2 serve the reuse).  Works for every size; the fallback.
-//   step_tma_kernel    : a CTA owns a (TY x TZ) tile of the y-z plane and marches along x.  One
+//   step_tma_kernel    : (lpc_step_vec.cuh) a CTA owns a (TY x TZ) tile of the y-z plane and marches along x.  One
 //                        x-plane per stage is streamed into shared memory with cp.async.bulk.tensor
 //                        (TMA, halo included) behind a full/empty mbarrier ring; thread 0 issues the
 //                        loads between planes (no producer warp: 16 warps per SM leave 128 registers
@@ -44,28 +44,6 @@ __device__ __forceinline__ void store_with_ghosts(T* __restrict__ base, const La
   if (per[0]) {
     if (x == 0) store_pair(base, i + (long long)L.nx * L.sx, oa, ob, vb);
     if (x == L.nx - 1) store_pair(base, i - (long long)L.nx * L.sx, oa, ob, vb);
-  }
-}
-
-// One channel of a pair that lies on a periodic face (rare; kept out of line, with scalar arguments
-// only, so that the march of the TMA kernel stays small and the kernel parameters stay in the
-// constant bank).  i is the padded index of (x, y, z); permask bit d = axis d is periodic.
-template <typename T>
-__device__ __noinline__ void store_face_pair(T* __restrict__ base, long long i, int nx, int ny, int nz, long long sy, long long sx,
-                                             int permask, int x, int y, int z, T oa, T ob, bool vb) {
-  store_pair(base, i, oa, ob, vb);
-  if (permask & 4) {
-    if (z == 0) base[i + nz] = oa;
-    if (z == nz - 1) base[i - nz] = oa;
-    if (vb && z + 1 == nz - 1) base[i + 1 - nz] = ob;
-  }
-  if (permask & 2) {
-    if (y == 0) store_pair(base, i + (long long)ny * sy, oa, ob, vb);
-    if (y == ny - 1) store_pair(base, i - (long long)ny * sy, oa, ob, vb);
-  }
-  if (permask & 1) {
-    if (x == 0) store_pair(base, i + (long long)nx * sx, oa, ob, vb);
-    if (x == nx - 1) store_pair(base, i - (long long)nx * sx, oa, ob, vb);
   }
 }
 
@@ -280,254 +258,7 @@ struct TmaCfg {
   static_assert(TZ % VW == 0, "TZ must be a multiple of the vector width");
 };
 
-template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int LK, typename LM>
-__device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUtensorMap& tm_pi, const CUtensorMap& tm_cs, const LM& lm,
-                                              const StepArgs<T>& a) {
-  using K = TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, LK>;
-  using V2 = typename Vec2<T>::type;
-  constexpr int C = K::C, NRED = K::NRED, TZW = K::TZW, TYH = K::TYH, HZ = K::HZ;
-  extern __shared__ __align__(128) unsigned char smem_raw[];
-  // round the base up to 128 bytes by offset arithmetic so that the pointer stays in the shared window
-  unsigned char* smem = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
-  uint64_t* full = reinterpret_cast<uint64_t*>(smem + K::BAR_OFF);
-  uint64_t* empty = full + NSTAGE;
-  double* red = reinterpret_cast<double*>(smem + K::RED_OFF);
-
-  const Layout& L = a.L;
-  const int bz = blockIdx.x % a.tiles_z;
-  const int by = (blockIdx.x / a.tiles_z) % a.tiles_y;
-  const int bx = blockIdx.x / (a.tiles_z * a.tiles_y);
-  const int z0 = bz * TZ, y0 = by * TY, x0 = bx * a.xc;
-  const int nplanes = min(a.xc, L.nx - x0);
-  const int nloads = nplanes + 2;
-  const int lane = threadIdx.x & 31;
-
-  if (threadIdx.x == 0) {
-    for (int s = 0; s < NSTAGE; ++s) {
-      mbar_init(&full[s], 1);
-      mbar_init(&empty[s], K::NCW);
-    }
-    mbar_fence_init();
-  }
-  __syncthreads();
-
-  double acc[NRED];
-#pragma unroll
-  for (int r = 0; r < NRED; ++r) acc[r] = 0.0;
-
-  // ----- TMA issue (thread 0): load j brings plane x0-1+j into stage j % NSTAGE -----
-  int jl = 0;  // next load to issue (thread 0 only)
-  auto issue_load = [&]() {
-    const int s = jl % NSTAGE;
-    if (jl >= NSTAGE) mbar_wait(&empty[s], ((jl / NSTAGE) - 1) & 1);   // every warp is done with the plane it held
-    unsigned char* st = smem + s * K::STAGE_BYTES;
-    const bool need_kcs = (NH == 2) && (jl >= 1 && jl <= nplanes);
-    mbar_expect_tx(&full[s], K::TX_BYTES + (need_kcs ? K::KCS_RAW : 0));
-    // plane x0-1+j lives at padded x coordinate x0+j; box starts HZ columns / 1 row before the tile
-    tma_load_4d(st, &tm_f, &full[s], L.padz + z0 - HZ, y0, x0 + jl, a.c0);
-    if constexpr (LK) {
-      tma_load_3d(st + K::F_BYTES, &lm.pic, &full[s], L.padz + z0, y0 + 1, x0 + jl);
-      tma_load_3d(st + K::MX_OFF, &lm.mx, &full[s], L.padz + z0, y0 + 1, x0 + jl);
-      tma_load_3d(st + K::MY_OFF, &lm.my, &full[s], L.padz + z0, y0, x0 + jl);           // rows y0-1 .. y0+TY-1
-      tma_load_3d(st + K::MZ_OFF, &lm.mz, &full[s], L.padz + z0 - HZ, y0 + 1, x0 + jl);  // columns z0-HZ .. z0+TZ-1
-    } else {
-      tma_load_3d(st + K::F_BYTES, &tm_pi, &full[s], L.padz + z0 - HZ, y0, x0 + jl);
-    }
-    if (need_kcs) tma_load_4d(st + K::F_BYTES + K::PI_BYTES, &tm_cs, &full[s], L.padz + z0, y0 + 1, x0 + jl, 0);
-    ++jl;
-  };
-  if (threadIdx.x == 0) {
-    tma_prefetch_desc(&tm_f);
-    if constexpr (LK) {
-      tma_prefetch_desc(&lm.pic);
-      tma_prefetch_desc(&lm.mx);
-      tma_prefetch_desc(&lm.my);
-      tma_prefetch_desc(&lm.mz);
-    } else {
-      tma_prefetch_desc(&tm_pi);
-    }
-    tma_prefetch_desc(&tm_cs);
-    for (int j = 0; j < NSTAGE && j < nloads; ++j) issue_load();
-  }
-  {
-    // ===== consumer warps =====
-    const int ty = threadIdx.x / (TZ / 2);   // row inside the tile
-    const int tp = threadIdx.x % (TZ / 2);   // pair inside the row
-    const int y = y0 + ty, z = z0 + 2 * tp;
-    const bool va = (y < L.ny) && (z < L.nz);
-    const bool vb = (y < L.ny) && (z + 1 < L.nz);
-    const int ec = (ty + 1) * TZW + 2 * tp + HZ;  // element offset of the centre pair in a halo'd tile
-    const int ek = ty * TZ + 2 * tp;              // element offset of the pair in a tile without halo
-    // sites on a periodic face also write their ghost copies: rare, so it is a separate path
-    const bool edge_yz = (a.per[1] && (y == 0 || y == L.ny - 1)) || (a.per[2] && (z == 0 || z + 2 >= L.nz - 1));
-    const int permask = (a.per[0] ? 1 : 0) | (a.per[1] ? 2 : 0) | (a.per[2] ? 4 : 0);
-    T* outp = a.fout + L.idx(x0, y, z);
-
-    // One x-plane as a consumer thread holds it: the centre pair of every channel and of pi, kappa of
-    // the pair, and mlo = min(pi, pi of the plane below) -- the symmetric link weight m_ij of the -x
-    // link (which is the +x link of the plane below).  With stored link weights (LK) mlo holds the plane's
-    // own +x link weight instead, which is the -x link of the plane above.
-    struct Plane {
-      V2 f[C];
-      V2 pi, kap, mlo;
-    };
-    Plane P0, P1, P2;
-    int sj = 0;            // stage of the next plane to take from the ring
-    uint32_t phj = 0;      // and its phase bit
-    auto take = [&](Plane& n, const Plane* below) {
-      mbar_wait(&full[sj], phj);
-      const T* sf = reinterpret_cast<const T*>(smem + sj * K::STAGE_BYTES);
-      const T* sp = reinterpret_cast<const T*>(smem + sj * K::STAGE_BYTES + K::F_BYTES);
-#pragma unroll
-      for (int c = 0; c < C; ++c) n.f[c] = *reinterpret_cast<const V2*>(sf + c * TYH * TZW + ec);
-      n.pi = *reinterpret_cast<const V2*>(sp + (LK ? ek : ec));
-      n.kap.x = kappa_of(n.pi.x, a.a6);
-      n.kap.y = kappa_of(n.pi.y, a.a6);
-      if constexpr (LK) {
-        n.mlo = *reinterpret_cast<const V2*>(reinterpret_cast<const T*>(smem + sj * K::STAGE_BYTES + K::MX_OFF) + ek);
-      } else if (below) {
-        n.mlo.x = tmin(n.pi.x, below->pi.x);
-        n.mlo.y = tmin(n.pi.y, below->pi.y);
-      }
-      if (++sj == NSTAGE) {
-        sj = 0;
-        phj ^= 1u;
-      }
-    };
-
-    // one plane of the march: prv / ctr / nxt are the planes x-1 / x / x+1, sc the stage that holds x
-    auto plane = [&](int x, int sc, const Plane& prv, const Plane& ctr, Plane& nxt) {
-      // refill the stage that held plane x-1 (released when the previous plane was finished)
-      if (threadIdx.x == 0 && jl < nloads) issue_load();
-      take(nxt, &ctr);
-      const T* sf = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES);
-      const T* sp = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES + K::F_BYTES);
-      const T* sk = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES + K::F_BYTES + K::PI_BYTES);
-      V2 csv, snv;
-      if (NH == 2) {
-        csv = *reinterpret_cast<const V2*>(sk + ek);
-        snv = *reinterpret_cast<const V2*>(sk + TY * TZ + ek);
-      }
-      SiteUpdate<T, NRHO, NMOM> ua, ub;
-      ua.pc = ctr.pi.x; ub.pc = ctr.pi.y;
-      ua.kap = ctr.kap.x; ub.kap = ctr.kap.y;
-      if constexpr (LK) {
-        const T* smy = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES + K::MY_OFF) + ek;          // row y-1 of the box
-        const T* smz = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES + K::MZ_OFF) + ty * K::TZM + HZ + 2 * tp;
-        const V2 mym = *reinterpret_cast<const V2*>(smy);
-        const V2 myp = *reinterpret_cast<const V2*>(smy + TZ);
-        const V2 mzp = *reinterpret_cast<const V2*>(smz);
-        ua.mxm = prv.mlo.x; ub.mxm = prv.mlo.y;
-        ua.mxp = ctr.mlo.x; ub.mxp = ctr.mlo.y;
-        ua.mym = mym.x; ub.mym = mym.y;
-        ua.myp = myp.x; ub.myp = myp.y;
-        ua.mzm = smz[-1];
-        ua.mzp = mzp.x;
-        ub.mzm = mzp.x;
-        ub.mzp = mzp.y;
-      } else {
-        const V2 pym = *reinterpret_cast<const V2*>(sp + ec - TZW);
-        const V2 pyp = *reinterpret_cast<const V2*>(sp + ec + TZW);
-        const T pzm = sp[ec - 1], pzp = sp[ec + 2];
-        ua.mxm = ctr.mlo.x; ub.mxm = ctr.mlo.y;
-        ua.mxp = nxt.mlo.x; ub.mxp = nxt.mlo.y;
-        ua.mym = tmin(ctr.pi.x, pym.x); ub.mym = tmin(ctr.pi.y, pym.y);
-        ua.myp = tmin(ctr.pi.x, pyp.x); ub.myp = tmin(ctr.pi.y, pyp.y);
-        ua.mzm = tmin(ctr.pi.x, pzm);
-        ua.mzp = tmin(ctr.pi.x, ctr.pi.y);
-        ub.mzm = ua.mzp;
-        ub.mzp = tmin(ctr.pi.y, pzp);
-      }
-
-      T oa[C], ob[C];
-#pragma unroll
-      for (int c = 0; c < C; ++c) {
-        const T* fcn = sf + c * TYH * TZW;
-        const V2 fym = *reinterpret_cast<const V2*>(fcn + ec - TZW);
-        const V2 fyp = *reinterpret_cast<const V2*>(fcn + ec + TZW);
-        const T fzm = fcn[ec - 1], fzp = fcn[ec + 2];
-        if (NMOM == 3 && c >= NH + NRHO) {
-          const int d = c - NH - NRHO;
-          const T dma = (d == 0) ? (ua.mxp - ua.mxm) : (d == 1) ? (ua.myp - ua.mym) : (ua.mzp - ua.mzm);
-          const T dmb = (d == 0) ? (ub.mxp - ub.mxm) : (d == 1) ? (ub.myp - ub.mym) : (ub.mzp - ub.mzm);
-          double t = 0.0;
-          if (va) t += (double)ctr.f[c].x * (double)dma;
-          if (vb) t += (double)ctr.f[c].y * (double)dmb;
-          acc[2 + d] += t;
-        }
-        oa[c] = ua.gather(ctr.f[c].x, prv.f[c].x, nxt.f[c].x, fym.x, fyp.x, fzm, ctr.f[c].y);
-        ob[c] = ub.gather(ctr.f[c].y, prv.f[c].y, nxt.f[c].y, fym.y, fyp.y, ctr.f[c].x, fzp);
-      }
-      // every shared-memory read of stage sc is done: hand it back to the producer
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&empty[sc]);
-
-      if (NH == 2) {
-        const T ar = oa[0], ai = oa[1], br = ob[0], bi = ob[1];
-        oa[0] = csv.x * ar - snv.x * ai;
-        oa[1] = csv.x * ai + snv.x * ar;
-        ob[0] = csv.y * br - snv.y * bi;
-        ob[1] = csv.y * bi + snv.y * br;
-      }
-      if (va) {
-        if (NH == 2) {
-          acc[0] += (double)ctr.pi.x * (double)oa[0];
-          acc[1] += (double)ctr.pi.x * (double)oa[1];
-          if (vb) {
-            acc[0] += (double)ctr.pi.y * (double)ob[0];
-            acc[1] += (double)ctr.pi.y * (double)ob[1];
-          }
-        }
-        if (edge_yz || (a.per[0] && (x == 0 || x == L.nx - 1))) {
-          const long long i = L.idx(x, y, z);
-#pragma unroll
-          for (int c = 0; c < C; ++c)
-            store_face_pair<T>(a.fout + (long long)c * L.np, i, L.nx, L.ny, L.nz, L.sy, L.sx, permask, x, y, z, oa[c], ob[c], vb);
-        } else {
-#pragma unroll
-          for (int c = 0; c < C; ++c) store_pair(outp + (long long)c * L.np, 0, oa[c], ob[c], vb);
-        }
-      }
-      outp += L.sx;
-    };
-
-    take(P0, nullptr);
-    __syncwarp();
-    if (lane == 0) mbar_arrive(&empty[0]);   // the plane below the chunk is only needed for its centres
-    take(P1, &P0);
-
-    // the march, unrolled by three so that the planes keep their registers while their roles rotate
-    int sc = 1 % NSTAGE;
-    auto next_stage = [&]() { if (++sc == NSTAGE) sc = 0; };
-    int p = 0;
-    for (; p + 3 <= nplanes; p += 3) {
-      plane(x0 + p, sc, P0, P1, P2); next_stage();
-      plane(x0 + p + 1, sc, P1, P2, P0); next_stage();
-      plane(x0 + p + 2, sc, P2, P0, P1); next_stage();
-    }
-    if (p < nplanes) { plane(x0 + p, sc, P0, P1, P2); next_stage(); ++p; }
-    if (p < nplanes) { plane(x0 + p, sc, P1, P2, P0); next_stage(); ++p; }
-  }
-  block_reduce_finalize<NRED, (NH == 2) ? FIN_STEP : FIN_MOM, NMOM>(acc, red, a.partials, a.ctl, a.fid, a.vacf, a.vacf_stride, a.zscale, gridDim.x,
-                                              blockIdx.x);
-}
-
 struct NoLinkMaps {};
-
-template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE>
-__global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE>::LB_THREADS, TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE>::LB_CTAS)
-    step_tma_kernel(const __grid_constant__ CUtensorMap tm_f, const __grid_constant__ CUtensorMap tm_pi,
-                    const __grid_constant__ CUtensorMap tm_cs, StepArgs<T> a) {
-  step_tma_body<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 0>(tm_f, tm_pi, tm_cs, NoLinkMaps(), a);
-}
-
-// the same sweep with stored link weights (per-link mobility factors)
-template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE>
-__global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1>::LB_THREADS, TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1>::LB_CTAS)
-    step_tma_links_kernel(const __grid_constant__ CUtensorMap tm_f, const __grid_constant__ CUtensorMap tm_cs,
-                          const __grid_constant__ TmaLinkMaps lm, StepArgs<T> a) {
-  step_tma_body<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1>(tm_f, tm_f, tm_cs, lm, a);
-}
 
 }  // namespace lpc
 

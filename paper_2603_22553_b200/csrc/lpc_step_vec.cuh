@@ -1,11 +1,14 @@
-// lpc_step_vec.cuh -- the TMA march of lpc_step.cuh with VW sites per thread along z (included by lpc_step.cuh).
+// lpc_step_vec.cuh -- the TMA march (step_tma_kernel, step_tma_links_kernel); included by lpc_step.cuh.
 //
-// The fp64 march gives a thread one 16-byte z-pair.  In fp32 a pair is only 8 bytes: the same instruction count
-// per site moves half the bytes and the sweep becomes issue-bound (ncu, profiles/: 532 M warp instructions per
-// 512^3 launch in fp32 against 555 M in fp64, DRAM at 57% of peak).  Here a thread owns a 16-byte z-QUAD in fp32
-// (VW = 4) on a 16 x 64 tile, so that barrier waits, address arithmetic, the TMA issue and the y-halo loads are
-// paid once per four sites.  Same per-site arithmetic (SiteUpdate::gather), same staging, pipeline and reduction
-// as step_tma_body; the state agrees bit for bit with the direct and persistent kernels.
+// A CTA owns a (TY x TZ) tile of the y-z plane and marches along x.  One x-plane per stage is streamed into shared
+// memory with cp.async.bulk.tensor (TMA, halo included) behind a full/empty mbarrier ring; thread 0 issues the loads
+// between planes (no producer warp: 16 warps per SM leave 128 registers per thread).  A thread owns ONE 16-BYTE GROUP
+// of VW consecutive z sites -- a pair in fp64 (8 x 64 tiles), a quad in fp32 (16 x 64 tiles) -- keeps the x-1 / x / x+1
+// values of its group in registers and reads the in-plane neighbours from shared memory, all with 16-byte loads.
+// (fp32 first ran with pairs: the same instruction count per site for half the bytes made it issue-bound, 532 M warp
+// instructions per 512^3 launch and DRAM at 57% of peak; with quads 410 M and 0.914 -> 0.715 ms.  The fp64 sweep
+// measures the same with this body as with the pair-only code it replaced.)
+// Per-site arithmetic is SiteUpdate::gather, so the state agrees bit for bit with the direct and persistent kernels.
 #pragma once
 
 namespace lpc {
@@ -68,7 +71,7 @@ __device__ __noinline__ void store_face_vec(T* __restrict__ base, long long i, i
 }
 
 template <typename T, int VW, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int LK, typename LM>
-__device__ __forceinline__ void step_tma_body_v(const CUtensorMap& tm_f, const CUtensorMap& tm_pi, const CUtensorMap& tm_cs, const LM& lm,
+__device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUtensorMap& tm_pi, const CUtensorMap& tm_cs, const LM& lm,
                                                 const StepArgs<T>& a) {
   using K = TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, LK, VW>;
   using V = typename VecN<T, VW>::type;
@@ -297,18 +300,19 @@ __device__ __forceinline__ void step_tma_body_v(const CUtensorMap& tm_f, const C
                                                                     gridDim.x, blockIdx.x);
 }
 
-template <typename T, int VW, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE>
+template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int VW>
 __global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 0, VW>::LB_THREADS, TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 0, VW>::LB_CTAS)
-    step_tma_vec_kernel(const __grid_constant__ CUtensorMap tm_f, const __grid_constant__ CUtensorMap tm_pi,
-                        const __grid_constant__ CUtensorMap tm_cs, StepArgs<T> a) {
-  step_tma_body_v<T, VW, NH, NRHO, NMOM, TY, TZ, NSTAGE, 0>(tm_f, tm_pi, tm_cs, NoLinkMaps(), a);
+    step_tma_kernel(const __grid_constant__ CUtensorMap tm_f, const __grid_constant__ CUtensorMap tm_pi,
+                    const __grid_constant__ CUtensorMap tm_cs, StepArgs<T> a) {
+  step_tma_body<T, VW, NH, NRHO, NMOM, TY, TZ, NSTAGE, 0>(tm_f, tm_pi, tm_cs, NoLinkMaps(), a);
 }
 
-template <typename T, int VW, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE>
+// the same sweep with stored link weights (per-link mobility factors)
+template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int VW>
 __global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1, VW>::LB_THREADS, TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1, VW>::LB_CTAS)
-    step_tma_vec_links_kernel(const __grid_constant__ CUtensorMap tm_f, const __grid_constant__ CUtensorMap tm_cs,
-                              const __grid_constant__ TmaLinkMaps lm, StepArgs<T> a) {
-  step_tma_body_v<T, VW, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1>(tm_f, tm_f, tm_cs, lm, a);
+    step_tma_links_kernel(const __grid_constant__ CUtensorMap tm_f, const __grid_constant__ CUtensorMap tm_cs,
+                          const __grid_constant__ TmaLinkMaps lm, StepArgs<T> a) {
+  step_tma_body<T, VW, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1>(tm_f, tm_f, tm_cs, lm, a);
 }
 
 }  // namespace lpc
