@@ -68,6 +68,7 @@ struct lpc_lattice {
   bool have_regions;
   long long region_first;  // first sample of the regional series
   bool region_moments;     // the regional VACF is being recorded (labels were set at step 0)
+  bool regions_fused;      // the last launch_step accumulated the regional FID inside the sweep
   bool have_links;         // per-link mobility factors are set: the sweeps read the stored link weights
   bool halo;               // bc[0] = LPC_BC_HALO: an x-slab whose x ghost planes the caller fills
   bool halo_ready;         // lpc_slab_finish has run
@@ -187,7 +188,7 @@ Offsets make_offsets(const lpc_config* c, const Layout& L) {
   o.fidr = p; p += align_up((size_t)c->n_regions * (c->max_steps + 1) * sizeof(double2));
   o.vacfr = p; p += align_up((c->n_regions && c->n_moments) ? (size_t)c->n_regions * 3 * (c->max_steps + 2) * sizeof(double) : 0);
   o.wr = p; p += align_up(c->n_regions ? MAX_REGIONS * sizeof(double) : 0);
-  o.rpartials = p; p += align_up(c->n_regions ? (size_t)AUX_BLOCKS * 4 * MAX_REGIONS * sizeof(double) : 0);
+  o.rpartials = p; p += align_up(c->n_regions ? std::max<size_t>((size_t)AUX_BLOCKS * 4, o.partial_slots * 2) * MAX_REGIONS * sizeof(double) : 0);
   o.spec = p; p += align_up((size_t)SPEC_BATCH * sizeof(double2));
   o.staging = p; p += align_up((size_t)std::min<long long>(N, STAGE_SITES) * 16);
   o.total = p;
@@ -244,6 +245,11 @@ bool is_device_ptr(const void* p) {
 
 int aux_grid(long long n) { return (int)std::max<long long>(1, std::min<long long>((n + 255) / 256, AUX_BLOCKS)); }
 
+// the regional FID can ride on the TMA magnetisation sweep when there is no density channel next to it
+bool regions_fusable(const lpc_lattice* h) {
+  return h->have_regions && h->nrho == 0 && h->tma_ok && h->kernel != LPC_KERNEL_DIRECT && !getenv("LPC_NO_REGION_FUSION");
+}
+
 // ---- launch of one sweep ---------------------------------------------------------------------
 template <typename T, int NRHO, int NMOM>
 int launch_step_t(lpc_lattice* h) {
@@ -265,6 +271,15 @@ int launch_step_t(lpc_lattice* h) {
   a.xc = h->xc; a.tiles_z = h->tiles_z; a.tiles_y = h->tiles_y; a.chunks_x = h->chunks_x;
 
   const bool use_tma = h->tma_ok && h->kernel != LPC_KERNEL_DIRECT;
+  // region-resolved FID inside the magnetisation sweep (no separate pass over the state): TMA kernel, no density channel
+  const bool fuse_regions = use_tma && regions_fusable(h);
+  h->regions_fused = fuse_regions;
+  a.label = fuse_regions ? h->ws + h->off.regions : nullptr;
+  a.rpartials = wsp<double>(h, h->off.rpartials);
+  a.fidr = wsp<double2>(h, h->off.fidr);
+  a.fidr_stride = h->cfg.max_steps + 1;
+  a.region_sample = h->steps + 1;
+  a.n_regions = h->cfg.n_regions;
   if (use_tma) {
     const unsigned grid = (unsigned)(h->tiles_z * h->tiles_y * h->chunks_x);
     auto launch = [&](auto kern, auto cfg, const CUtensorMap& tm, const StepArgs<T>& args) -> int {
@@ -310,8 +325,18 @@ int launch_step_t(lpc_lattice* h) {
       if (rc) return rc;
     }
     a.c0 = 0;
-    int rc = h->have_links ? launch_links(step_tma_links_kernel<T, 2, NRHO, 0, TY, 64, NSL, VW>, TmaCfg<T, 2, NRHO, 0, TY, 64, NSL, 1, VW>(), h->tm_f[h->cur], a)
-                           : launch(step_tma_kernel<T, 2, NRHO, 0, TY, 64, NS, VW>, TmaCfg<T, 2, NRHO, 0, TY, 64, NS, 0, VW>(), h->tm_f[h->cur], a);
+    int rc;
+    if constexpr (NRHO == 0) {
+      if (fuse_regions)   // one stage less: the per-thread region slots take 32 KB of shared memory
+        rc = h->have_links ? launch_links(step_tma_links_kernel<T, 2, 0, 0, TY, 64, 2, VW, 1>, TmaCfg<T, 2, 0, 0, TY, 64, 2, 1, VW, 1>(), h->tm_f[h->cur], a)
+                           : launch(step_tma_kernel<T, 2, 0, 0, TY, 64, 3, VW, 1>, TmaCfg<T, 2, 0, 0, TY, 64, 3, 0, VW, 1>(), h->tm_f[h->cur], a);
+      else
+        rc = h->have_links ? launch_links(step_tma_links_kernel<T, 2, 0, 0, TY, 64, NSL, VW>, TmaCfg<T, 2, 0, 0, TY, 64, NSL, 1, VW>(), h->tm_f[h->cur], a)
+                           : launch(step_tma_kernel<T, 2, 0, 0, TY, 64, NS, VW>, TmaCfg<T, 2, 0, 0, TY, 64, NS, 0, VW>(), h->tm_f[h->cur], a);
+    } else {
+      rc = h->have_links ? launch_links(step_tma_links_kernel<T, 2, NRHO, 0, TY, 64, NSL, VW>, TmaCfg<T, 2, NRHO, 0, TY, 64, NSL, 1, VW>(), h->tm_f[h->cur], a)
+                         : launch(step_tma_kernel<T, 2, NRHO, 0, TY, 64, NS, VW>, TmaCfg<T, 2, NRHO, 0, TY, 64, NS, 0, VW>(), h->tm_f[h->cur], a);
+    }
     if (rc) return rc;
     h->cur ^= 1;
     return LPC_OK;
@@ -816,6 +841,7 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
   h->have_regions = false;
   h->region_moments = false;
   h->have_links = false;
+  h->regions_fused = false;
   h->halo = cfg->bc[0] == LPC_BC_HALO;
   h->halo_ready = false;
   h->z_override = 0.0;
@@ -963,7 +989,7 @@ int lpc_step_n(lpc_lattice* h, int64_t n) {
     int rc = h->cfg.precision ? launch_step<float>(h) : launch_step<double>(h);
     if (rc) return rc;
     h->steps++;
-    if (h->have_regions) {
+    if (h->have_regions && !h->regions_fused) {
       rc = region_reduce(h, h->steps);
       if (rc) return rc;
     }
@@ -1140,7 +1166,9 @@ double lpc_bytes_per_site_step(const lpc_lattice* h) {
   // read C state channels + pi + cos + sin, write C state channels; with region labels one more pass
   // reads h (2 channels), pi and the label
   // with per-link mobility factors the sweep also reads three stored link weights per site
-  return (double)h->sT * (2.0 * h->C + 3.0 + (h->have_links ? 3.0 : 0.0)) + (h->have_regions ? 3.0 * h->sT + 1.0 : 0.0);
+  // region labels: one byte per site inside the sweep, or one more pass over h (2 channels), pi and the label
+  const double regions = !h->have_regions ? 0.0 : regions_fusable(h) ? 1.0 : 3.0 * h->sT + 1.0;
+  return (double)h->sT * (2.0 * h->C + 3.0 + (h->have_links ? 3.0 : 0.0)) + regions;
 }
 
 void lpc_destroy(lpc_lattice* h) { delete h; }

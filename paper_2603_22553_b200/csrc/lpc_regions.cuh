@@ -12,7 +12,6 @@
 
 namespace lpc {
 
-constexpr int MAX_REGIONS = 8;
 
 // G_r[sample] for all regions: one pass over the current state (16 B) + pi (8 B) + label (1 B) per site.
 // Per-thread accumulators are selected by predicate (no indexed registers), reduced per warp and block,

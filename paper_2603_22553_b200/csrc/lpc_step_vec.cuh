@@ -70,10 +70,11 @@ __device__ __noinline__ void store_face_vec(T* __restrict__ base, long long i, i
   }
 }
 
-template <typename T, int VW, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int LK, typename LM>
+template <typename T, int VW, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int LK, int REG, typename LM>
 __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUtensorMap& tm_pi, const CUtensorMap& tm_cs, const LM& lm,
                                                 const StepArgs<T>& a) {
-  using K = TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, LK, VW>;
+  using K = TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, LK, VW, REG>;
+  static_assert(!REG || NH == 2, "the regional FID rides on the magnetisation sweep");
   using V = typename VecN<T, VW>::type;
   constexpr int C = K::C, NRED = K::NRED, TZW = K::TZW, TYH = K::TYH, HZ = K::HZ;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -81,6 +82,12 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
   uint64_t* full = reinterpret_cast<uint64_t*>(smem + K::BAR_OFF);
   uint64_t* empty = full + NSTAGE;
   double* red = reinterpret_cast<double*>(smem + K::RED_OFF);
+  // REG: thread t owns the slots rslot[(2 r + c) * NTHREADS + t] of region r, component c (no atomics, fixed order)
+  double* rslot = reinterpret_cast<double*>(smem + K::RSLOT_OFF);
+  if constexpr (REG) {
+#pragma unroll
+    for (int q = 0; q < 2 * MAX_REGIONS; ++q) rslot[q * K::NTHREADS + threadIdx.x] = 0.0;
+  }
 
   const Layout& L = a.L;
   const int bz = blockIdx.x % a.tiles_z;
@@ -147,6 +154,18 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
   const bool edge_yz = (a.per[1] && (y == 0 || y == L.ny - 1)) || (a.per[2] && (z == 0 || z + VW >= L.nz));
   const int permask = (a.per[0] ? 1 : 0) | (a.per[1] ? 2 : 0) | (a.per[2] ? 4 : 0);
   T* outp = a.fout + L.idx(x0, y, z);
+  // REG: the running sum of the region the thread is in; it moves to the thread's slot when the label changes
+  const uint8_t* labp = REG ? a.label + ((long long)x0 * L.ny + y) * L.nz + z : nullptr;
+  int rcur = 255;
+  double racc0 = 0.0, racc1 = 0.0;
+  auto rflush = [&](int next) {
+    if (rcur < MAX_REGIONS) {
+      rslot[(2 * rcur) * K::NTHREADS + threadIdx.x] += racc0;
+      rslot[(2 * rcur + 1) * K::NTHREADS + threadIdx.x] += racc1;
+    }
+    racc0 = racc1 = 0.0;
+    rcur = next;
+  };
 
   // one x-plane as a thread holds it: the group's values of every channel and of pi, kappa, and mlo = the link
   // weight towards the plane below (LK: the plane's own +x link weight, i.e. the -x weight of the plane above)
@@ -180,6 +199,12 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
 
   auto plane = [&](int x, int sc, const Plane& prv, const Plane& ctr, Plane& nxt) {
     if (threadIdx.x == 0 && jl < nloads) issue_load();
+    int labs[VW];
+    if constexpr (REG) {
+#pragma unroll
+      for (int k = 0; k < VW; ++k) labs[k] = (k < nvalid) ? (int)__ldg(labp + k) : 255;
+      labp += (long long)L.ny * L.nz;
+    }
     take(nxt, &ctr);
     const T* sf = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES);
     const T* sk = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES + K::F_BYTES + K::PI_BYTES);
@@ -262,6 +287,11 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
         if (k < nvalid) {
           acc[0] += (double)ctr.pi[k] * (double)o[0][k];
           acc[1] += (double)ctr.pi[k] * (double)o[1][k];
+          if constexpr (REG) {
+            if (labs[k] != rcur) rflush(labs[k]);
+            racc0 += (double)ctr.pi[k] * (double)o[0][k];
+            racc1 += (double)ctr.pi[k] * (double)o[1][k];
+          }
         }
       }
     }
@@ -296,23 +326,53 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
   if (p < nplanes) { plane(x0 + p, sc, P0, P1, P2); next_stage(); ++p; }
   if (p < nplanes) { plane(x0 + p, sc, P1, P2, P0); next_stage(); ++p; }
 
-  block_reduce_finalize<NRED, (NH == 2) ? FIN_STEP : FIN_MOM, NMOM>(acc, red, a.partials, a.ctl, a.fid, a.vacf, a.vacf_stride, a.zscale,
-                                                                    gridDim.x, blockIdx.x);
+  if constexpr (REG) {
+    // block partial of every (region, component) column: warp w adds the slots of columns 2w, 2w+1 in a fixed order
+    rflush(255);
+    __syncthreads();
+    const int warp = threadIdx.x >> 5;
+    for (int q = warp; q < 2 * MAX_REGIONS; q += K::NTHREADS / 32) {
+      double v = 0.0;
+      for (int t = lane; t < K::NTHREADS; t += 32) v += rslot[q * K::NTHREADS + t];
+      v = warp_sum(v);
+      if (lane == 0) a.rpartials[(size_t)blockIdx.x * 2 * MAX_REGIONS + q] = v;
+    }
+    __threadfence();
+  }
+  const bool last = block_reduce_finalize<NRED, (NH == 2) ? FIN_STEP : FIN_MOM, NMOM>(acc, red, a.partials, a.ctl, a.fid, a.vacf,
+                                                                                      a.vacf_stride, a.zscale, gridDim.x, blockIdx.x);
+  if constexpr (REG) {
+    if (!last) return;
+    // the last CTA adds the block partials: thread t takes column t % 16 over the blocks t/16, t/16 + P, ...
+    __threadfence();
+    constexpr int NC = 2 * MAX_REGIONS, P = K::NTHREADS / NC;
+    const int col = threadIdx.x % NC, part = threadIdx.x / NC;
+    double v = 0.0;
+    for (unsigned int b = part; b < gridDim.x; b += P) v += __ldcg(&a.rpartials[(size_t)b * NC + col]);
+    __syncthreads();
+    rslot[part * NC + col] = v;
+    __syncthreads();
+    if (threadIdx.x < NC && (threadIdx.x >> 1) < a.n_regions) {
+      double t = 0.0;
+      for (int q = 0; q < P; ++q) t += rslot[q * NC + threadIdx.x];
+      reinterpret_cast<double*>(a.fidr + (threadIdx.x >> 1) * a.fidr_stride + a.region_sample)[threadIdx.x & 1] = t;
+    }
+  }
 }
 
-template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int VW>
-__global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 0, VW>::LB_THREADS, TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 0, VW>::LB_CTAS)
+template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int VW, int REG = 0>
+__global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 0, VW, REG>::LB_THREADS, TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 0, VW, REG>::LB_CTAS)
     step_tma_kernel(const __grid_constant__ CUtensorMap tm_f, const __grid_constant__ CUtensorMap tm_pi,
                     const __grid_constant__ CUtensorMap tm_cs, StepArgs<T> a) {
-  step_tma_body<T, VW, NH, NRHO, NMOM, TY, TZ, NSTAGE, 0>(tm_f, tm_pi, tm_cs, NoLinkMaps(), a);
+  step_tma_body<T, VW, NH, NRHO, NMOM, TY, TZ, NSTAGE, 0, REG>(tm_f, tm_pi, tm_cs, NoLinkMaps(), a);
 }
 
 // the same sweep with stored link weights (per-link mobility factors)
-template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int VW>
-__global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1, VW>::LB_THREADS, TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1, VW>::LB_CTAS)
+template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int VW, int REG = 0>
+__global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1, VW, REG>::LB_THREADS, TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1, VW, REG>::LB_CTAS)
     step_tma_links_kernel(const __grid_constant__ CUtensorMap tm_f, const __grid_constant__ CUtensorMap tm_cs,
                           const __grid_constant__ TmaLinkMaps lm, StepArgs<T> a) {
-  step_tma_body<T, VW, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1>(tm_f, tm_f, tm_cs, lm, a);
+  step_tma_body<T, VW, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1, REG>(tm_f, tm_f, tm_cs, lm, a);
 }
 
 }  // namespace lpc

@@ -317,7 +317,8 @@ def test_regional_fid_and_spectrum_match_oracle(lpc, oracle_mod, kernel, precisi
     gpu = lpc.Lattice.from_inputs(lat, precision=precision, max_steps=n, n_regions=nreg)
     gpu.set_kernel(kernel)
     gpu.set_regions(region)
-    assert gpu.bytes_per_site_step == (4 if precision else 8) * 10 + 1
+    # the TMA sweep reads the labels itself (+1 B); the direct kernel is followed by a pass over h, pi and the labels
+    assert gpu.bytes_per_site_step == (4 if precision else 8) * (7 if kernel == 2 else 10) + 1
     gpu.step(n)
     orc = oracle_mod.Oracle.from_lattice(lat, n_moments=0, max_steps=n)
     Gr_o = orc.step_with_regions(region, nreg, n)
@@ -802,3 +803,43 @@ def test_slab_mode_errors(lpc):
     # the plane views address the workspace: shape [channels, (ny+2) * padded nz]
     v = plain.halo_planes(lpc.LPC_HALO_STATE, 0, lpc.LPC_HALO_SEND)
     assert v.shape[0] == 2 + lat.n_moments and v.shape[1] % 12 == 0 and float(v[0].max()) == 1.0
+
+
+def test_regional_fid_fused_sweep_matches_separate_pass(lpc, oracle_mod):
+    """The TMA sweep accumulates G_r itself (per-thread slots, label changes inside a thread's column, ragged tiles,
+    labels outside 0..n_regions-1); the separate reduction pass gives the same series up to summation order."""
+    n, nreg = 30, 5
+    lat = lpc_inputs.random_small((37, 21, 131), bc=(0, 1, 0), p_block=0.2, alpha=0.9, seed=91, n_steps=n, n_moments=0)
+    rng = np.random.default_rng(9)
+    region = rng.integers(0, 7, size=lat.shape).astype(np.uint8)          # iid labels 0..6: 5 and 6 are in no region
+    region[:, :, 40:90] = 2                                                # and a blob
+    link = lpc_inputs.random_links(lat.shape, seed=5)
+    orc = oracle_mod.Oracle.from_lattice(lat, n_moments=0, max_steps=n)
+    Gr_o = orc.step_with_regions(region, nreg, n)
+    _, sabs = orc.fid(with_scale=True)
+    for precision, tol in ((0, 1e-9), (1, 1e-5)):
+        out = {}
+        for fused in (True, False):
+            if not fused:
+                os.environ["LPC_NO_REGION_FUSION"] = "1"
+            try:
+                gpu = lpc.Lattice.from_inputs(lat, precision=precision, max_steps=n, n_regions=nreg)
+                gpu.set_kernel(2)
+                gpu.set_regions(region)
+                assert gpu.bytes_per_site_step == (4 if precision else 8) * 7 + (1 if fused else (4 if precision else 8) * 3 + 1)
+                l0 = gpu.launch_count
+                gpu.step(n)
+                assert gpu.launch_count - l0 == (n if fused else 2 * n)
+                out[fused] = np.array([gpu.fid_region(r) for r in range(nreg)])
+            finally:
+                os.environ.pop("LPC_NO_REGION_FUSION", None)
+        assert np.max(np.abs(out[True] - Gr_o) / sabs) <= tol
+        assert np.max(np.abs(out[True] - out[False]) / sabs) <= (1e-5 if precision else 1e-13)
+    # with stored link weights the fused sweep is the links kernel
+    gpu = lpc.Lattice.from_inputs(lat, max_steps=n, n_regions=nreg, link=link)
+    gpu.set_regions(region)
+    orc = oracle_mod.Oracle.from_lattice(lat, n_moments=0, max_steps=n, link=link)
+    Gr_o = orc.step_with_regions(region, nreg, n)
+    _, sabs = orc.fid(with_scale=True)
+    gpu.step(n)
+    assert np.max(np.abs(np.array([gpu.fid_region(r) for r in range(nreg)]) - Gr_o) / sabs) <= 1e-9
