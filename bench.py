@@ -55,6 +55,8 @@ def parse():
     p.add_argument("--moments", type=int, default=0, choices=[0, 3], help="also propagate the 3 VACF fields")
     p.add_argument("--precision", type=int, default=0, choices=[0, 1])
     p.add_argument("--kernel", type=int, default=0, choices=[0, 1, 2, 3])
+    p.add_argument("--regions", type=int, default=0, metavar="R",
+                   help="label R (1..8) equal x-ranges as regions and record the region-resolved FID G_r[n] as well")
     p.add_argument("--slabs", type=int, default=0, metavar="S",
                    help="run the workload as ONE lattice cut into x-slabs, S per rank (SURVEY 8(e)): a plane exchange after every step, "
                         "strong scaling over --gpus; 0 (default) = independent replicas")
@@ -211,7 +213,8 @@ def run_ours(args):
     h2d_job = sum(t.numel() * t.element_size() for t in host)
 
     sim = lpc.Lattice(lat.shape, bc=lat.bc, precision=args.precision, n_moments=args.moments, dt=lat.dt, a=lat.a,
-                      alpha=lat.alpha, max_steps=2 * K + W + 8, device=dev, link_mobility=1 if args.links else 0)
+                      alpha=lat.alpha, max_steps=2 * K + W + 8, device=dev, link_mobility=1 if args.links else 0,
+                      n_regions=args.regions)
     sim.set_kernel(args.kernel)
     link = None
     if args.links:
@@ -219,10 +222,18 @@ def run_ours(args):
         link = torch.from_numpy(lpc_inputs.confined_links(lat.dF != 0.0, 0.25)).pin_memory()
         h2d_job += link.numel() * link.element_size()
 
+    labels = None
+    if args.regions:
+        x = np.arange(lat.nx, dtype=np.int64)[:, None, None] * np.ones(lat.shape, dtype=np.int64)
+        labels = torch.from_numpy((x * args.regions // lat.nx).astype(np.uint8)).pin_memory()
+        h2d_job += labels.numel()
+
     def set_params():
         sim.set_site_params(*host)
         if link is not None:
             sim.set_link_mobility(link)
+        if labels is not None:
+            sim.set_regions(labels)
 
     def barrier():
         if world > 1:
@@ -294,6 +305,8 @@ def run_ours(args):
             key = f"{L}^3/m{args.moments}/p{args.precision}" if args.workload == "sweep" else f"{args.workload}/m{args.moments}/p{args.precision}"
             if args.links:
                 key += "/links"
+            if args.regions:
+                key += "/regions"
             for row in open(tpath):
                 cols = row.strip().split(",")
                 if cols and cols[0] == key:
@@ -307,7 +320,8 @@ def run_ours(args):
                        "l2": (f"working set {bps * n_sites / 1e9:.2f} GB per step >> 126 MB L2, no flush needed"
                               if bps * n_sites > 4 * 126e6 else "working set is L2-sized: not an HBM measurement"),
                        "kernel": {0: "auto", 1: "direct", 2: "tma", 3: "persistent"}[args.kernel],
-                       "links": "alpha_ij = 0.25 on links that touch a porous site" if args.links else "none"},
+                       "links": "alpha_ij = 0.25 on links that touch a porous site" if args.links else "none",
+                       "regions": args.regions},
             "clocks": clocks,
             "e2e": e2e,
             "gpu_launches": int(launches),
