@@ -81,7 +81,7 @@ struct lpc_lattice {
   int ty, tz, nstage, xc, tiles_z, tiles_y, chunks_x;
   bool tma_ok;
   TmaLinkMaps tm_l;  // pi centres and the three link-weight channels (link_mobility = 1)
-  CUtensorMap tm_f[2], tm_m[2], tm_pi, tm_cs;  // tm_f: magnetisation (+ density) channels, tm_m: the 3 moment channels
+  CUtensorMap tm_f[2], tm_m[2], tm_r[2], tm_pi, tm_cs;  // tm_r: one channel per box (the density channel alone, equilibration)  // tm_f: magnetisation (+ density) channels, tm_m: the 3 moment channels
 };
 
 namespace {
@@ -742,14 +742,42 @@ int equilibrate_t(lpc_lattice* h, double threshold, int64_t max_iters, int64_t c
   for (int d = 0; d < 3; ++d) a.per[d] = h->cfg.bc[d] == 0;
   const long long npairs = (long long)((L.nz + 1) / 2) * L.ny * L.nx;
   const int grid = (int)std::max<long long>(1, std::min<long long>((npairs + 255) / 256, DIRECT_MAX_BLOCKS));
+  // The same sweep on the TMA march (the density channel alone: NH = 0, NRHO = 1), unless the direct kernel is asked for
+  const bool use_tma = h->tma_ok && h->kernel != LPC_KERNEL_DIRECT;
+  StepArgs<T> sa;
+  sa.L = L; sa.fin = nullptr; sa.pi = a.pi; sa.cs = wsp<T>(h, h->off.cs); sa.mlink = a.mlink; sa.a6 = a.a6;
+  sa.partials = a.partials; sa.ctl = ctl; sa.fid = nullptr; sa.vacf = nullptr; sa.vacf_stride = 0; sa.zscale = 0.0;
+  for (int d = 0; d < 3; ++d) sa.per[d] = a.per[d];
+  sa.label = nullptr; sa.rpartials = nullptr; sa.fidr = nullptr; sa.fidr_stride = 0; sa.region_sample = 0; sa.n_regions = 0;
+  sa.c0 = 2; sa.xc = h->xc; sa.tiles_z = h->tiles_z; sa.tiles_y = h->tiles_y; sa.chunks_x = h->chunks_x;
+  constexpr int VW = 16 / (int)sizeof(T), TY = 4 * VW;
+  using KP = TmaCfg<T, 0, 1, 0, TY, 64, 4, 0, VW>;
+  using KL = TmaCfg<T, 0, 1, 0, TY, 64, 4, 1, VW>;
+  if (use_tma) {
+    static bool attr_set = false;
+    if (!attr_set) {
+      CUDA_TRY(cudaFuncSetAttribute(step_tma_kernel<T, 0, 1, 0, TY, 64, 4, VW>, cudaFuncAttributeMaxDynamicSharedMemorySize, KP::SMEM_BYTES));
+      CUDA_TRY(cudaFuncSetAttribute(step_tma_links_kernel<T, 0, 1, 0, TY, 64, 4, VW>, cudaFuncAttributeMaxDynamicSharedMemorySize, KL::SMEM_BYTES));
+      attr_set = true;
+    }
+  }
+  const unsigned tgrid = (unsigned)(h->tiles_z * h->tiles_y * h->chunks_x);
   int64_t done = 0;
   double delta = 0.0;
   while (done < max_iters) {
     const int64_t batch = std::min<int64_t>(check_every, max_iters - done);
     for (int64_t k = 0; k < batch; ++k) {
-      a.rin = ch[src];
-      a.rout = ch[src ^ 1];
-      equil_kernel<T><<<grid, 256, 0, h->stream>>>(a);
+      if (use_tma) {
+        sa.fout = ch[src ^ 1];
+        if (h->have_links)
+          step_tma_links_kernel<T, 0, 1, 0, TY, 64, 4, VW><<<tgrid, KL::NTHREADS, KL::SMEM_BYTES, h->stream>>>(h->tm_r[src], h->tm_cs, h->tm_l, sa);
+        else
+          step_tma_kernel<T, 0, 1, 0, TY, 64, 4, VW><<<tgrid, KP::NTHREADS, KP::SMEM_BYTES, h->stream>>>(h->tm_r[src], h->tm_pi, h->tm_cs, sa);
+      } else {
+        a.rin = ch[src];
+        a.rout = ch[src ^ 1];
+        equil_kernel<T><<<grid, 256, 0, h->stream>>>(a);
+      }
       CUDA_TRY(cudaGetLastError());
       h->launches++;
       src ^= 1;
@@ -871,6 +899,9 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
     if (!rc) rc = encode_map(&h->tm_f[1], f32, h->ws + h->off.f1, 4, d4, bf);
     if (!rc && h->nmom == 3) rc = encode_map(&h->tm_m[0], f32, h->ws + h->off.f0, 4, d4, bm);
     if (!rc && h->nmom == 3) rc = encode_map(&h->tm_m[1], f32, h->ws + h->off.f1, 4, d4, bm);
+    const cuuint32_t br[4] = {b4[0], b4[1], 1, 1};
+    if (!rc && h->nrho == 1) rc = encode_map(&h->tm_r[0], f32, h->ws + h->off.f0, 4, d4, br);
+    if (!rc && h->nrho == 1) rc = encode_map(&h->tm_r[1], f32, h->ws + h->off.f1, 4, d4, br);
     if (!rc) rc = encode_map(&h->tm_pi, f32, h->ws + h->off.pi, 3, d4, b4);
     if (!rc) rc = encode_map(&h->tm_cs, f32, h->ws + h->off.cs, 4, dk, bk);
     if (!rc && cfg->link_mobility) {

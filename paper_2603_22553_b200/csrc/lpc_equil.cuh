@@ -60,39 +60,8 @@ __global__ void __launch_bounds__(256) equil_kernel(EquilArgs<T> a) {
     }
     store_with_ghosts(a.rout, L, a.per, i, x, y, z, out[0], out[1], vb);
   }
-  // block max -> partial -> the last block reduces the partials
-  __shared__ double red[8];
-  __shared__ unsigned int s_last;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) dmax = fmax(dmax, __shfl_down_sync(0xffffffffu, dmax, o));
-  if (lane == 0) red[warp] = dmax;
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    double v = 0.0;
-    for (int w = 0; w < 8; ++w) v = fmax(v, red[w]);
-    a.partials[blockIdx.x] = v;
-    __threadfence();
-    s_last = (atomicAdd(&a.ctl->ticket, 1u) == gridDim.x - 1);
-  }
-  __syncthreads();
-  if (!s_last) return;
-  __threadfence();
-  double v = 0.0;
-  for (unsigned int b = threadIdx.x; b < gridDim.x; b += blockDim.x) v = fmax(v, __ldcg(&a.partials[b]));
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
-  __syncthreads();
-  if (lane == 0) red[warp] = v;
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    double t = 0.0;
-    for (int w = 0; w < 8; ++w) t = fmax(t, red[w]);
-    a.ctl->scratch[4] = t;
-    a.ctl->scratch[5] += 1.0;
-    a.ctl->ticket = 0;
-    __threadfence();
-  }
+  __shared__ double red[8 + 1];
+  block_max_finalize(dmax, red, a.partials, a.ctl, gridDim.x, blockIdx.x);
 }
 
 // g(0) <- rho: h = r (real) on every site, ghosts included (they already mirror r).

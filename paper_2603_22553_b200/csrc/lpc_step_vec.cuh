@@ -75,6 +75,10 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
                                                 const StepArgs<T>& a) {
   using K = TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, LK, VW, REG>;
   static_assert(!REG || NH == 2, "the regional FID rides on the magnetisation sweep");
+  // NH = 0 without moment fields is the density channel alone: one sweep of the equilibration loop,
+  // rho <- W rho with delta = max_i |rho_i(t+1) - rho_i(t)| = max_i pi_i |r'_i - r_i| in acc[0] (a maximum, not a sum)
+  constexpr bool EQ = (NH == 0 && NMOM == 0);
+  static_assert(!EQ || NRHO == 1, "a sweep needs channels");
   using V = typename VecN<T, VW>::type;
   constexpr int C = K::C, NRED = K::NRED, TZW = K::TZW, TYH = K::TYH, HZ = K::HZ;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -278,6 +282,11 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
     __syncwarp();
     if (lane == 0) mbar_arrive(&empty[sc]);
 
+    if constexpr (EQ) {
+#pragma unroll
+      for (int k = 0; k < VW; ++k)
+        if (k < nvalid) acc[0] = fmax(acc[0], (double)ctr.pi[k] * fabs((double)o[0][k] - (double)ctr.f[0][k]));
+    }
     if (NH == 2) {
 #pragma unroll
       for (int k = 0; k < VW; ++k) {
@@ -338,6 +347,10 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
       if (lane == 0) a.rpartials[(size_t)blockIdx.x * 2 * MAX_REGIONS + q] = v;
     }
     __threadfence();
+  }
+  if constexpr (EQ) {
+    block_max_finalize(acc[0], red, a.partials, a.ctl, gridDim.x, blockIdx.x);
+    return;
   }
   const bool last = block_reduce_finalize<NRED, (NH == 2) ? FIN_STEP : FIN_MOM, NMOM>(acc, red, a.partials, a.ctl, a.fid, a.vacf,
                                                                                       a.vacf_stride, a.zscale, gridDim.x, blockIdx.x);

@@ -843,3 +843,24 @@ def test_regional_fid_fused_sweep_matches_separate_pass(lpc, oracle_mod):
     _, sabs = orc.fid(with_scale=True)
     gpu.step(n)
     assert np.max(np.abs(np.array([gpu.fid_region(r) for r in range(nreg)]) - Gr_o) / sabs) <= 1e-9
+
+
+@pytest.mark.parametrize("precision", [0, 1])
+def test_equilibration_tma_sweep_agrees_bitwise_with_direct_sweep(lpc, precision):
+    """The equilibration sweep runs on the TMA march (density channel alone) or, with LPC_KERNEL_DIRECT, on the
+    per-pair kernel: same per-site arithmetic, and a maximum does not depend on the order it is taken in."""
+    lat = lpc_inputs.random_small((37, 21, 131), bc=(0, 1, 0), p_block=0.2, alpha=0.9, seed=92, n_moments=3)
+    rng = np.random.default_rng(10)
+    rho0 = rng.random(lat.shape) * (lat.blocked == 0)
+    rho0 /= rho0.sum()
+    link = lpc_inputs.random_links(lat.shape, seed=6)
+    for lk in (None, link):
+        res = []
+        for kernel in (0, 1):
+            gpu = lpc.Lattice.from_inputs(lat, precision=precision, n_moments=3, n_density=1, max_steps=4, link=lk)
+            gpu.set_kernel(kernel)
+            gpu.set_state(lpc.LPC_FIELD_RHO, rho0)
+            its, delta = gpu.equilibrate(0.0, 17, 17)
+            res.append((its, delta, gpu.field(lpc.LPC_FIELD_RHO), gpu.field(lpc.LPC_FIELD_G), gpu.field(lpc.LPC_FIELD_PX)))
+        assert res[0][0] == res[1][0] == 17 and res[0][1] == res[1][1] > 0
+        assert all(np.array_equal(x, y) for x, y in zip(res[0][2:], res[1][2:]))
