@@ -13,34 +13,75 @@
 namespace lpc {
 
 
+// Region accumulators of one thread.  Regions are blobs, so consecutive sites of a thread mostly carry the same
+// label: the running sums of the current region stay in registers (cur) and move to the per-region array only
+// when the label changes (that array is indexed at run time and lives in local memory; it is touched rarely).
+// Thread-private throughout, so the result does not depend on timing.
+template <int NV>
+struct RegionAcc {
+  double acc[MAX_REGIONS][NV];
+  double cur[NV];
+  int rcur;
+  __device__ __forceinline__ void init() {
+#pragma unroll
+    for (int r = 0; r < MAX_REGIONS; ++r)
+#pragma unroll
+      for (int v = 0; v < NV; ++v) acc[r][v] = 0.0;
+#pragma unroll
+    for (int v = 0; v < NV; ++v) cur[v] = 0.0;
+    rcur = 255;
+  }
+  __device__ __forceinline__ void flush(int next) {
+    if (rcur < MAX_REGIONS) {
+#pragma unroll
+      for (int v = 0; v < NV; ++v) acc[rcur][v] += cur[v];
+    }
+#pragma unroll
+    for (int v = 0; v < NV; ++v) cur[v] = 0.0;
+    rcur = next;
+  }
+  __device__ __forceinline__ void add(int lab, const double (&v)[NV]) {
+    if (lab != rcur) flush(lab);
+#pragma unroll
+    for (int k = 0; k < NV; ++k) cur[k] += v[k];
+  }
+};
+
+// Rows (x, y) are dealt to warps, the lanes of a warp stride along z: coalesced, and the index arithmetic is paid
+// once per row.  body(i_dense, j_padded) is called for every site.
+template <typename F>
+__device__ __forceinline__ void for_sites_by_rows(const Layout& L, F body) {
+  const long long rows = (long long)L.nx * L.ny;
+  const int lane = threadIdx.x & 31;
+  const long long warps = (long long)gridDim.x * (blockDim.x >> 5);
+  for (long long r = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); r < rows; r += warps) {
+    const int x = (int)(r / L.ny), y = (int)(r % L.ny);
+    const long long i0 = r * L.nz, j0 = L.idx(x, y, 0);
+    for (int z = lane; z < L.nz; z += 32) body(i0 + z, j0 + z);
+  }
+}
+
 // G_r[sample] for all regions: one pass over the current state (16 B) + pi (8 B) + label (1 B) per site.
-// Per-thread accumulators are selected by predicate (no indexed registers), reduced per warp and block,
+// Per-thread region accumulators (RegionAcc), reduced per warp and block,
 // and the last block sums the block partials in a fixed order.
 template <typename T>
 __global__ void __launch_bounds__(256)
     region_reduce_kernel(Layout L, const T* __restrict__ pi, const T* __restrict__ f, const uint8_t* __restrict__ label, int n_regions,
                          double* partials, Ctl* ctl, double2* fidr, long long stride, long long sample) {
-  double ar[MAX_REGIONS], ai[MAX_REGIONS];
-#pragma unroll
-  for (int r = 0; r < MAX_REGIONS; ++r) ar[r] = ai[r] = 0.0;
-  const long long n = (long long)L.nx * L.ny * L.nz;
-  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-    const long long j = dense_to_padded(L, i);
+  RegionAcc<2> ra;
+  ra.init();
+  for_sites_by_rows(L, [&](long long i, long long j) {
     const double p = (double)pi[j];
-    const double gr = p * (double)f[j], gi = p * (double)f[L.np + j];
-    const int lab = label[i];
-#pragma unroll
-    for (int r = 0; r < MAX_REGIONS; ++r) {
-      ar[r] += (lab == r) ? gr : 0.0;
-      ai[r] += (lab == r) ? gi : 0.0;
-    }
-  }
+    const double g[2] = {p * (double)f[j], p * (double)f[L.np + j]};
+    ra.add(label[i], g);
+  });
+  ra.flush(255);
   __shared__ double red[8][2 * MAX_REGIONS];
   __shared__ unsigned int s_last;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
   for (int r = 0; r < MAX_REGIONS; ++r) {
-    const double vr = warp_sum(ar[r]), vi = warp_sum(ai[r]);
+    const double vr = warp_sum(ra.acc[r][0]), vi = warp_sum(ra.acc[r][1]);
     if (lane == 0) {
       red[warp][2 * r] = vr;
       red[warp][2 * r + 1] = vi;
@@ -77,24 +118,18 @@ __global__ void __launch_bounds__(256)
 // starts, normalised by the region's equilibrium population w_r = sum_{i in r} pi_i (Q27):
 //   INIT: w_r, and Z^r_d[1]   = (a^2 alpha/6) sum_{i in r} (m_{i,+d} + m_{i,-d}) / w_r
 //   STEP: Z^r_d[k+1] = (a alpha/6) sum_{i in r} q^d_i(k) (m_{i,+d} - m_{i,-d}) / w_r     (q = P/pi before the sweep)
-// One pass over pi (with neighbours), the three moment channels and the labels; predicate-selected
-// accumulators, block partials, fixed-order sum by the last block.
+// One pass over pi (with neighbours), the three moment channels and the labels; per-thread region accumulators
+// (RegionAcc), block partials, fixed-order sum by the last block.
 template <typename T, bool INIT>
 __global__ void __launch_bounds__(256)
     region_moment_kernel(Layout L, const T* __restrict__ pi, const T* __restrict__ mlink, const T* __restrict__ q,
                          const uint8_t* __restrict__ label, int n_regions,
                          double* partials, Ctl* ctl, double* wr, double* vacfr, long long stride, long long index, double scale) {
   constexpr int NV = INIT ? 4 : 3;   // INIT also sums pi
-  double acc[MAX_REGIONS][NV];
-#pragma unroll
-  for (int r = 0; r < MAX_REGIONS; ++r)
-#pragma unroll
-    for (int v = 0; v < NV; ++v) acc[r][v] = 0.0;
-  const long long n = (long long)L.nx * L.ny * L.nz;
+  RegionAcc<NV> ra;
+  ra.init();
   const long long st[3] = {L.sx, L.sy, 1};
-  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-    const long long j = dense_to_padded(L, i);
-    const int lab = label[i];
+  for_sites_by_rows(L, [&](long long i, long long j) {
     const T p = pi[j];
     double v[NV];
 #pragma unroll
@@ -104,11 +139,9 @@ __global__ void __launch_bounds__(256)
       v[d] = INIT ? (double)mp + (double)mm : (double)q[(long long)d * L.np + j] * (double)(mp - mm);
     }
     if (INIT) v[NV - 1] = (double)p;
-#pragma unroll
-    for (int r = 0; r < MAX_REGIONS; ++r)
-#pragma unroll
-      for (int k = 0; k < NV; ++k) acc[r][k] += (lab == r) ? v[k] : 0.0;
-  }
+    ra.add(label[i], v);
+  });
+  ra.flush(255);
   constexpr int NC = MAX_REGIONS * NV;
   __shared__ double red[8][NC];
   __shared__ unsigned int s_last;
@@ -117,7 +150,7 @@ __global__ void __launch_bounds__(256)
   for (int r = 0; r < MAX_REGIONS; ++r)
 #pragma unroll
     for (int k = 0; k < NV; ++k) {
-      const double t = warp_sum(acc[r][k]);
+      const double t = warp_sum(ra.acc[r][k]);
       if (lane == 0) red[warp][r * NV + k] = t;
     }
   __syncthreads();
