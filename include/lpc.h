@@ -217,8 +217,11 @@ int lpc_spectrum(lpc_lattice* lat, int32_t region, int64_t count, double f0_hz, 
  *   exchange LPC_HALO_STATE
  *   repeat: lpc_step_n(lat, 1); exchange LPC_HALO_STATE
  * G[n], Z_d[m] of a slab are the sums over its own sites: the caller adds the ranks' series (one reduction
- * when the series is read, none per step); D follows from the summed Z_d as in lpc_moments.  Not available in
- * slab mode (LPC_ESTATE): lpc_step_n with n > 1, the persistent kernel, lpc_equilibrate, link factors.       */
+ * when the series is read, none per step); D follows from the summed Z_d as in lpc_moments.  The equilibration
+ * loop runs the same way: lpc_equilibrate(lat, threshold, 1, 1, ...) is one sweep, the caller exchanges
+ * LPC_HALO_STATE and takes the largest delta of all slabs.  Not available in slab mode: lpc_step_n with n > 1,
+ * lpc_equilibrate with max_iters > 1 (LPC_ESTATE), the persistent kernel (never chosen), link factors
+ * (LPC_EINVAL at creation).                                                                                  */
 
 /* Z_local = sum of exp(-dF_i) over the open sites of this lattice (Eq. 2).  dF_kT, blocked: host
  * or device, as lpc_set_site_params.  out: host.  Synchronises.  Errors: LPC_EINVAL, LPC_ECUDA.              */

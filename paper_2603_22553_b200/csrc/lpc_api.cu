@@ -1078,7 +1078,9 @@ int lpc_equilibrate(lpc_lattice* h, double threshold, int64_t max_iters, int64_t
   if (!h) return fail(LPC_EINVAL, "lattice is NULL");
   if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
   if (h->nrho != 1) return fail(LPC_ESTATE, "the density field is not propagated (n_density = 0)");
-  if (h->halo) return fail(LPC_ESTATE, "the equilibration loop is not available in slab mode");
+  if (h->halo && !h->halo_ready) return fail(LPC_ESTATE, "slab mode: lpc_slab_finish has not been called");
+  if (h->halo && max_iters > 1)
+    return fail(LPC_ESTATE, "slab mode: the x ghost planes must be exchanged after every sweep (max_iters <= 1)");
   if (max_iters < 0) return fail(LPC_EINVAL, "max_iters must be >= 0");
   if (check_every < 1) return fail(LPC_EINVAL, "check_every must be >= 1");
   if (!(threshold == threshold)) return fail(LPC_EINVAL, "threshold is NaN");

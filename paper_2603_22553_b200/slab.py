@@ -167,6 +167,39 @@ class SlabSet:
             self.exchange(HALO_STATE)
             self.steps += 1
 
+    def _allreduce_max(self, v: float) -> float:
+        if self.dist is None or self.world == 1:
+            return v
+        import torch
+
+        t = torch.tensor([v], dtype=torch.float64)
+        if self.dist.get_backend(self.group) == "nccl":
+            t = t.cuda()
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX, group=self.group)
+        return float(t.item())
+
+    def set_state(self, which, arr):
+        """arr over the WHOLE lattice (e.g. an initial density for the equilibration loop)."""
+        for s in self.owned:
+            self.lat[s].set_state(which, self.local_part(arr, s))
+        self.exchange(HALO_STATE)
+
+    def equilibrate(self, threshold, max_iters):
+        """The equilibration loop over all slabs: one sweep per slab, the plane exchange, and the
+        largest per-site change of all slabs compared with the threshold.  Returns (sweeps done, last delta)."""
+        done, delta = 0, 0.0
+        while done < max_iters:
+            delta = 0.0
+            for s in self.owned:
+                _, d = self.lat[s].equilibrate(0.0, 1, 1)
+                delta = max(delta, d)
+            self.exchange(HALO_STATE)
+            delta = self._allreduce_max(delta)
+            done += 1
+            if delta < threshold:
+                break
+        return done, delta
+
     def fid(self):
         """G[0..steps] of the whole lattice: the slabs' partial series added in slab order, then over ranks."""
         part = sum(self.lat[s].fid() for s in self.owned)

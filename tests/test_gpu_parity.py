@@ -789,6 +789,7 @@ def test_slab_mode_errors(lpc):
     assert e.value.code == lpc.LPC_ESTATE
     m.slab_finish()
     m.step(1)
+    assert m.equilibrate(0.0, 1, 1)[0] == 1          # one sweep at a time is what the slab driver runs
     for bad in (lambda: m.step(2), lambda: m.equilibrate(1e-3, 5)):
         with pytest.raises(lpc.LpcError) as e:
             bad()
@@ -864,3 +865,25 @@ def test_equilibration_tma_sweep_agrees_bitwise_with_direct_sweep(lpc, precision
             res.append((its, delta, gpu.field(lpc.LPC_FIELD_RHO), gpu.field(lpc.LPC_FIELD_G), gpu.field(lpc.LPC_FIELD_PX)))
         assert res[0][0] == res[1][0] == 17 and res[0][1] == res[1][1] > 0
         assert all(np.array_equal(x, y) for x, y in zip(res[0][2:], res[1][2:]))
+
+
+@pytest.mark.parametrize("bc,n_slabs", [((0, 0, 0), 2), ((1, 0, 0), 3)])
+def test_slab_equilibration_loop_matches_oracle(lpc, oracle_mod, bc, n_slabs):
+    from paper_2603_22553_b200 import slab
+
+    lat = lpc_inputs.random_small((30, 12, 40), bc=bc, p_block=0.25, alpha=0.9, seed=83)
+    rng = np.random.default_rng(12)
+    rho0 = rng.random(lat.shape) * (lat.blocked == 0)
+    rho0 /= rho0.sum()
+    orc = oracle_mod.Oracle.from_lattice(lat, n_moments=0, max_steps=4)
+    _, _, dl = orc.equilibrate(rho0, 0.0, 40)
+    k_stop = 27
+    thr = float(np.sqrt(dl[k_stop - 1] * dl[k_stop - 2]))
+    rho_o, it_o, deltas = orc.equilibrate(rho0, thr, 500)
+    assert it_o == k_stop
+    ss = slab.SlabSet(lat.shape, bc=lat.bc, slabs_per_rank=n_slabs, n_density=1, dt=lat.dt, a=lat.a, alpha=lat.alpha, max_steps=4)
+    ss.set_site_params(lat.dF, lat.blocked, lat.omega)
+    ss.set_state(lpc.LPC_FIELD_RHO, rho0)
+    it_g, d_g = ss.equilibrate(thr, 500)
+    assert it_g == it_o and abs(d_g - deltas[-1]) <= 1e-10 * rho0.max()
+    assert np.max(np.abs(ss.gather_field(lpc.LPC_FIELD_RHO) - rho_o)) <= 1e-10 * rho0.max()
