@@ -60,6 +60,9 @@ def parse():
     p.add_argument("--slabs", type=int, default=0, metavar="S",
                    help="run the workload as ONE lattice cut into x-slabs, S per rank (SURVEY 8(e)): a plane exchange after every step, "
                         "strong scaling over --gpus; 0 (default) = independent replicas")
+    p.add_argument("--slab-direct", action="store_true",
+                   help="with --slabs: let the sweeps store their outermost planes into the ghost planes of neighbour slabs of the "
+                        "same process (lpc_set_halo_peers) instead of copying them afterwards")
     p.add_argument("--no-cpu-baseline", action="store_true")
     p.add_argument("--no-e2e", action="store_true")
     p.add_argument("--ref-sample-size", type=int, default=int(os.environ.get("LPC_REF_SAMPLE_L", "256")),
@@ -356,6 +359,7 @@ def run_slabs(args, lat, lpc, world, rank, local, dev):
     ss = slab.SlabSet(lat.shape, bc=lat.bc, slabs_per_rank=args.slabs, lattice_factory=factory, precision=args.precision,
                       n_moments=args.moments, dt=lat.dt, a=lat.a, alpha=lat.alpha, max_steps=K + W + 8)
     ss.set_site_params(lat.dF, lat.blocked, lat.omega)
+    n_direct = ss.enable_direct_stores() if args.slab_direct else 0
     ss.step(W)
 
     def barrier():
@@ -398,7 +402,8 @@ def run_slabs(args, lat, lpc, world, rank, local, dev):
             "dtype": "f32" if args.precision else "f64", "data": "synthetic",
             "config": {"workload": workload_name(args.size, args.moments, args.precision, args.workload), "lattice": list(lat.shape),
                        "sites": lat.n_sites, "parallelism": f"x-slabs: {ss.n_slabs} slabs over {world} rank(s), one plane exchange per step "
-                                                           f"({2 + args.moments} channel planes of {plane_bytes} B per face)",
+                                                           f"({2 + args.moments} channel planes of {plane_bytes} B per face); "
+                                                           f"{n_direct} faces stored by the sweeps themselves, the rest copied / sent",
                        "l2": "per-rank working set >> 126 MB L2" if bps * own > 4 * 126e6 else "per-rank working set is L2-sized"},
             "clocks": clocks, "e2e": None, "gpu_launches": int(launches),
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,

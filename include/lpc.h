@@ -54,6 +54,8 @@ extern "C" {
 #define LPC_BC_HALO 2
 #define LPC_HALO_PARAMS 0 /* the equilibrium density pi: 1 channel plane                      */
 #define LPC_HALO_STATE 1  /* the current state: 2 + n_density + n_moments channel planes      */
+#define LPC_HALO_STATE0 2 /* the same planes of state buffer 0 / 1 explicitly (the two buffers  */
+#define LPC_HALO_STATE1 3 /* alternate from step to step; for lpc_set_halo_peers)               */
 #define LPC_HALO_SEND 0   /* the outermost owned plane on that side                           */
 #define LPC_HALO_RECV 1   /* the ghost plane beyond it                                        */
 
@@ -239,6 +241,20 @@ int lpc_set_partition_sum(lpc_lattice* lat, double Z);
  * Errors: LPC_EINVAL, LPC_ESTATE (no site parameters yet).                                                    */
 int lpc_halo_view(lpc_lattice* lat, int32_t set, int32_t side, int32_t role, void** plane_dev, size_t* plane_bytes,
                   size_t* channel_stride_bytes, int32_t* n_channels);
+
+/* Slab mode, direct halo stores: let the step kernel itself write this slab's outermost x planes into the
+ * neighbours' x ghost planes, so that no copy or send follows the sweep (the transfer rides on the sweep's own
+ * stores, plane by plane).  lo0 / lo1: device address of channel 0 of the ghost plane beyond x = 0 -- the
+ * neighbour's LPC_HALO_RECV plane on its HIGH side -- in the neighbour's state buffer 0 / 1 (lpc_halo_view with
+ * LPC_HALO_STATE0 / LPC_HALO_STATE1 on the neighbour), lo_channel_stride_bytes its channel stride; hi* likewise
+ * for the neighbour beyond x = nx-1.  NULL, NULL = no neighbour there or no direct stores.  The memory must be
+ * writable from this lattice's device (the same device, or a peer mapping) and all slabs must step together
+ * (same number of lpc_step_n(lat, 1) calls), with every slab's step n finished before any slab's step n+1
+ * starts (one stream, or an event per step).  Needs the TMA kernel.  The first exchange after lpc_slab_finish /
+ * lpc_set_state and the exchanges of the equilibration sweeps remain the caller's.
+ * Errors: LPC_ESTATE (not a slab, no TMA geometry), LPC_EINVAL.                                               */
+int lpc_set_halo_peers(lpc_lattice* lat, void* lo0, void* lo1, size_t lo_channel_stride_bytes, void* hi0, void* hi1,
+                       size_t hi_channel_stride_bytes);
 
 /* Slab mode: build the initial state once the pi ghost planes are in place (see the order above).  Resets the
  * step counter and the series.  Synchronises.  Errors: LPC_ESTATE (not a slab, or no site parameters).         */

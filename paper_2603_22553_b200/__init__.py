@@ -21,14 +21,14 @@ LIB_PATH = os.path.join(_HERE, "liblpc.so")
 LPC_OK, LPC_EINVAL, LPC_ESTATE, LPC_ENOMEM, LPC_ECUDA = 0, -1, -2, -3, -4
 LPC_FIELD_G, LPC_FIELD_PI, LPC_FIELD_PX, LPC_FIELD_PY, LPC_FIELD_PZ, LPC_FIELD_RHO = range(6)
 LPC_BC_HALO = 2
-LPC_HALO_PARAMS, LPC_HALO_STATE = 0, 1
+LPC_HALO_PARAMS, LPC_HALO_STATE, LPC_HALO_STATE0, LPC_HALO_STATE1 = 0, 1, 2, 3
 LPC_HALO_SEND, LPC_HALO_RECV = 0, 1
 LPC_KERNEL_AUTO, LPC_KERNEL_DIRECT, LPC_KERNEL_TMA, LPC_KERNEL_PERSIST = range(4)
 
 EXPORTS = (
     "lpc_workspace_bytes", "lpc_create_lattice", "lpc_set_site_params", "lpc_set_link_mobility", "lpc_step_n", "lpc_read_fid",
     "lpc_moments", "lpc_read_field", "lpc_set_state", "lpc_equilibrate", "lpc_seed_from_density", "lpc_set_regions", "lpc_read_fid_region", "lpc_moments_region", "lpc_spectrum", "lpc_set_kernel",
-    "lpc_steps_done", "lpc_partition_sum", "lpc_set_partition_sum", "lpc_halo_view", "lpc_slab_finish",
+    "lpc_steps_done", "lpc_partition_sum", "lpc_set_partition_sum", "lpc_halo_view", "lpc_set_halo_peers", "lpc_slab_finish",
     "lpc_launch_count", "lpc_bytes_per_site_step", "lpc_destroy", "lpc_last_error",
 )
 
@@ -71,6 +71,7 @@ def _load():
     lib.lpc_halo_view.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_void_p), C.POINTER(C.c_size_t),
                                   C.POINTER(C.c_size_t), C.POINTER(C.c_int32)]
     lib.lpc_slab_finish.argtypes = [C.c_void_p]
+    lib.lpc_set_halo_peers.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p, C.c_size_t]
     lib.lpc_step_n.argtypes = [C.c_void_p, C.c_int64]
     lib.lpc_read_fid.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_void_p]
     lib.lpc_moments.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
@@ -182,6 +183,14 @@ def lpc_halo_view(handle, which, side, role):
     ptr, nb, st, nc = C.c_void_p(), C.c_size_t(), C.c_size_t(), C.c_int32()
     _check(_lib.lpc_halo_view(handle, int(which), int(side), int(role), C.byref(ptr), C.byref(nb), C.byref(st), C.byref(nc)))
     return int(ptr.value), int(nb.value), int(st.value), int(nc.value)
+
+
+def lpc_set_halo_peers(handle, lo=None, hi=None):
+    """lo / hi: None or (address in buffer 0, address in buffer 1, channel stride in bytes) of the neighbour's ghost plane."""
+    lo = lo or (None, None, 0)
+    hi = hi or (None, None, 0)
+    _check(_lib.lpc_set_halo_peers(handle, C.c_void_p(lo[0]), C.c_void_p(lo[1]), C.c_size_t(lo[2]), C.c_void_p(hi[0]), C.c_void_p(hi[1]),
+                                   C.c_size_t(hi[2])))
 
 
 def lpc_slab_finish(handle):
@@ -353,6 +362,15 @@ class Lattice:
 
     def slab_finish(self):
         lpc_slab_finish(self.handle)
+
+    def ghost_plane_addresses(self, side):
+        """(address in state buffer 0, in buffer 1, channel stride in bytes) of this lattice's x ghost plane on `side`."""
+        p0, _, st, _ = lpc_halo_view(self.handle, LPC_HALO_STATE0, side, LPC_HALO_RECV)
+        p1, _, _, _ = lpc_halo_view(self.handle, LPC_HALO_STATE1, side, LPC_HALO_RECV)
+        return p0, p1, st
+
+    def set_halo_peers(self, lo=None, hi=None):
+        lpc_set_halo_peers(self.handle, lo, hi)
 
     def halo_planes(self, which, side, role):
         """The halo plane(s) as a [channels, plane_elements] strided view of the workspace tensor (no copy)."""

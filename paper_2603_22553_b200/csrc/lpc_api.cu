@@ -73,6 +73,8 @@ struct lpc_lattice {
   bool halo;               // bc[0] = LPC_BC_HALO: an x-slab whose x ghost planes the caller fills
   bool halo_ready;         // lpc_slab_finish has run
   double z_override;       // > 0: normalise pi by this partition sum (slab mode)
+  unsigned char* peer[2][2];  // [side][buffer]: channel 0 of the neighbour's x ghost plane in its state buffer 0 / 1, or nullptr
+  size_t peer_stride[2];      // that neighbour's channel stride in bytes
   int cur;  // index of the buffer holding the current state
   long long steps;
   long long launches;
@@ -271,8 +273,17 @@ int launch_step_t(lpc_lattice* h) {
   a.xc = h->xc; a.tiles_z = h->tiles_z; a.tiles_y = h->tiles_y; a.chunks_x = h->chunks_x;
 
   const bool use_tma = h->tma_ok && h->kernel != LPC_KERNEL_DIRECT;
+  // slab mode with direct halo stores: the sweep writes into the buffer the neighbours write in this step (all slabs
+  // step together, so that is their buffer cur ^ 1 as well)
+  for (int s = 0; s < 2; ++s) {
+    a.peer[s] = reinterpret_cast<T*>(h->peer[s][h->cur ^ 1]);
+    a.peer_stride[s] = (long long)(h->peer_stride[s] / sizeof(T));
+  }
+  const bool peers = a.peer[0] || a.peer[1];
+  if (peers && !use_tma) return fail(LPC_ESTATE, "direct halo stores need the TMA kernel");
   // region-resolved FID inside the magnetisation sweep (no separate pass over the state): TMA kernel, no density channel
-  const bool fuse_regions = use_tma && regions_fusable(h);
+  // (and not together with direct halo stores: that combination runs the separate pass)
+  const bool fuse_regions = use_tma && regions_fusable(h) && !peers;
   h->regions_fused = fuse_regions;
   a.label = fuse_regions ? h->ws + h->off.regions : nullptr;
   a.rpartials = wsp<double>(h, h->off.rpartials);
@@ -320,7 +331,10 @@ int launch_step_t(lpc_lattice* h) {
       StepArgs<T> am = a;
       am.c0 = 2 + NRHO;
       am.fout = a.fout + (long long)am.c0 * h->L.np;
+      for (int s = 0; s < 2; ++s)
+        if (am.peer[s]) am.peer[s] += (long long)am.c0 * am.peer_stride[s];
       int rc = h->have_links ? launch_links(step_tma_links_kernel<T, 0, 0, 3, TY, 64, 3, VW>, TmaCfg<T, 0, 0, 3, TY, 64, 3, 1, VW>(), h->tm_m[h->cur], am)
+               : peers       ? launch(step_tma_kernel<T, 0, 0, 3, TY, 64, 4, VW, 2>, TmaCfg<T, 0, 0, 3, TY, 64, 4, 0, VW, 2>(), h->tm_m[h->cur], am)
                              : launch(step_tma_kernel<T, 0, 0, 3, TY, 64, 4, VW>, TmaCfg<T, 0, 0, 3, TY, 64, 4, 0, VW>(), h->tm_m[h->cur], am);
       if (rc) return rc;
     }
@@ -332,9 +346,11 @@ int launch_step_t(lpc_lattice* h) {
                            : launch(step_tma_kernel<T, 2, 0, 0, TY, 64, 3, VW, 1>, TmaCfg<T, 2, 0, 0, TY, 64, 3, 0, VW, 1>(), h->tm_f[h->cur], a);
       else
         rc = h->have_links ? launch_links(step_tma_links_kernel<T, 2, 0, 0, TY, 64, NSL, VW>, TmaCfg<T, 2, 0, 0, TY, 64, NSL, 1, VW>(), h->tm_f[h->cur], a)
+             : peers       ? launch(step_tma_kernel<T, 2, 0, 0, TY, 64, NS, VW, 2>, TmaCfg<T, 2, 0, 0, TY, 64, NS, 0, VW, 2>(), h->tm_f[h->cur], a)
                            : launch(step_tma_kernel<T, 2, 0, 0, TY, 64, NS, VW>, TmaCfg<T, 2, 0, 0, TY, 64, NS, 0, VW>(), h->tm_f[h->cur], a);
     } else {
       rc = h->have_links ? launch_links(step_tma_links_kernel<T, 2, NRHO, 0, TY, 64, NSL, VW>, TmaCfg<T, 2, NRHO, 0, TY, 64, NSL, 1, VW>(), h->tm_f[h->cur], a)
+           : peers       ? launch(step_tma_kernel<T, 2, NRHO, 0, TY, 64, NS, VW, 2>, TmaCfg<T, 2, NRHO, 0, TY, 64, NS, 0, VW, 2>(), h->tm_f[h->cur], a)
                          : launch(step_tma_kernel<T, 2, NRHO, 0, TY, 64, NS, VW>, TmaCfg<T, 2, NRHO, 0, TY, 64, NS, 0, VW>(), h->tm_f[h->cur], a);
     }
     if (rc) return rc;
@@ -372,6 +388,8 @@ int launch_persist_t(lpc_lattice* h, int64_t n) {
   a.vacf_stride = h->cfg.max_steps + 2;
   a.zscale = h->cfg.a * h->cfg.alpha / 6.0;
   for (int d = 0; d < 3; ++d) a.per[d] = h->cfg.bc[d] == 0;
+  a.peer[0] = a.peer[1] = nullptr; a.peer_stride[0] = a.peer_stride[1] = 0;
+  a.label = nullptr; a.rpartials = nullptr; a.fidr = nullptr; a.fidr_stride = 0; a.region_sample = 0; a.n_regions = 0;
   a.c0 = 0; a.xc = 0; a.tiles_z = a.tiles_y = a.chunks_x = 0;
   auto kern = step_persist_kernel<T, NRHO, NMOM>;
   static int per_sm = 0;
@@ -748,6 +766,7 @@ int equilibrate_t(lpc_lattice* h, double threshold, int64_t max_iters, int64_t c
   sa.L = L; sa.fin = nullptr; sa.pi = a.pi; sa.cs = wsp<T>(h, h->off.cs); sa.mlink = a.mlink; sa.a6 = a.a6;
   sa.partials = a.partials; sa.ctl = ctl; sa.fid = nullptr; sa.vacf = nullptr; sa.vacf_stride = 0; sa.zscale = 0.0;
   for (int d = 0; d < 3; ++d) sa.per[d] = a.per[d];
+  sa.peer[0] = sa.peer[1] = nullptr; sa.peer_stride[0] = sa.peer_stride[1] = 0;
   sa.label = nullptr; sa.rpartials = nullptr; sa.fidr = nullptr; sa.fidr_stride = 0; sa.region_sample = 0; sa.n_regions = 0;
   sa.c0 = 2; sa.xc = h->xc; sa.tiles_z = h->tiles_z; sa.tiles_y = h->tiles_y; sa.chunks_x = h->chunks_x;
   constexpr int VW = 16 / (int)sizeof(T), TY = 4 * VW;
@@ -873,6 +892,7 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
   h->halo = cfg->bc[0] == LPC_BC_HALO;
   h->halo_ready = false;
   h->z_override = 0.0;
+  for (int s = 0; s < 2; ++s) h->peer[s][0] = h->peer[s][1] = nullptr, h->peer_stride[s] = 0;
   h->region_first = 0;
   h->cur = 0;
   h->steps = 0;
@@ -970,17 +990,32 @@ int lpc_halo_view(lpc_lattice* h, int32_t set, int32_t side, int32_t role, void*
                   int32_t* n_channels) {
   if (!h) return fail(LPC_EINVAL, "lattice is NULL");
   if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
-  if ((set != LPC_HALO_PARAMS && set != LPC_HALO_STATE) || (side != 0 && side != 1) || (role != LPC_HALO_SEND && role != LPC_HALO_RECV))
+  if ((set != LPC_HALO_PARAMS && set != LPC_HALO_STATE && set != LPC_HALO_STATE0 && set != LPC_HALO_STATE1) || (side != 0 && side != 1) || (role != LPC_HALO_SEND && role != LPC_HALO_RECV))
     return fail(LPC_EINVAL, "bad selector (set %d, side %d, role %d)", set, side, role);
   if (!plane || !plane_bytes || !stride_bytes || !n_channels) return fail(LPC_EINVAL, "output pointers must not be NULL");
   const Layout& L = h->L;
   // padded x index: ghost 0, owned 1 .. nx, ghost nx + 1
   const long long xp = side == 0 ? (role == LPC_HALO_SEND ? 1 : 0) : (role == LPC_HALO_SEND ? L.nx : L.nx + 1);
-  const size_t base = set == LPC_HALO_PARAMS ? h->off.pi : (h->cur ? h->off.f1 : h->off.f0);
+  const size_t base = set == LPC_HALO_PARAMS ? h->off.pi
+                    : set == LPC_HALO_STATE0 ? h->off.f0
+                    : set == LPC_HALO_STATE1 ? h->off.f1
+                                             : (h->cur ? h->off.f1 : h->off.f0);
   *plane = h->ws + base + (size_t)xp * L.sx * h->sT;
   *plane_bytes = (size_t)L.sx * h->sT;
   *stride_bytes = (size_t)L.np * h->sT;
   *n_channels = set == LPC_HALO_PARAMS ? 1 : h->C;
+  return LPC_OK;
+}
+
+int lpc_set_halo_peers(lpc_lattice* h, void* lo0, void* lo1, size_t lo_stride, void* hi0, void* hi1, size_t hi_stride) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (!h->halo) return fail(LPC_ESTATE, "the lattice was not created with bc[0] = LPC_BC_HALO");
+  if ((lo0 == nullptr) != (lo1 == nullptr) || (hi0 == nullptr) != (hi1 == nullptr))
+    return fail(LPC_EINVAL, "give both buffers of a neighbour or neither");
+  if ((lo0 && lo_stride % h->sT) || (hi0 && hi_stride % h->sT)) return fail(LPC_EINVAL, "channel stride is not a multiple of the element size");
+  if ((lo0 || hi0) && !h->tma_ok) return fail(LPC_ESTATE, "direct halo stores need the TMA kernel, which this lattice cannot run");
+  h->peer[0][0] = static_cast<unsigned char*>(lo0); h->peer[0][1] = static_cast<unsigned char*>(lo1); h->peer_stride[0] = lo_stride;
+  h->peer[1][0] = static_cast<unsigned char*>(hi0); h->peer[1][1] = static_cast<unsigned char*>(hi1); h->peer_stride[1] = hi_stride;
   return LPC_OK;
 }
 

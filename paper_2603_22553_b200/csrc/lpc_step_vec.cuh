@@ -46,6 +46,15 @@ __device__ __forceinline__ void store_vec(T* __restrict__ p, typename VecN<T, VW
   }
 }
 // one channel of a group that lies on a periodic face: the sites and their ghost copies (rare, out of line)
+// store_peer_vec: the same group into the same channel's ghost plane of the x neighbours (slab mode with direct halo
+// stores); peer_lo / peer_hi may be nullptr.
+template <typename T, int VW>
+__device__ __noinline__ void store_peer_vec(T* __restrict__ peer_lo, T* __restrict__ peer_hi, long long po, int nx, int x,
+                                            typename VecN<T, VW>::type v, int nvalid) {
+  if (peer_lo && x == 0) store_vec<T, VW>(peer_lo + po, v, nvalid);
+  if (peer_hi && x == nx - 1) store_vec<T, VW>(peer_hi + po, v, nvalid);
+}
+
 template <typename T, int VW>
 __device__ __noinline__ void store_face_vec(T* __restrict__ base, long long i, int nx, int ny, int nz, long long sy, long long sx,
                                             int permask, int x, int y, int z, typename VecN<T, VW>::type v, int nvalid) {
@@ -70,10 +79,13 @@ __device__ __noinline__ void store_face_vec(T* __restrict__ base, long long i, i
   }
 }
 
-template <typename T, int VW, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int LK, int REG, typename LM>
+// FEAT bit 0 (REG): region-resolved FID inside the sweep; bit 1 (PEER): slab mode with direct halo stores.
+template <typename T, int VW, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int LK, int FEAT, typename LM>
 __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUtensorMap& tm_pi, const CUtensorMap& tm_cs, const LM& lm,
                                                 const StepArgs<T>& a) {
-  using K = TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, LK, VW, REG>;
+  constexpr int REG = FEAT & 1;
+  constexpr bool PEER = (FEAT & 2) != 0;
+  using K = TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, LK, VW, FEAT>;
   static_assert(!REG || NH == 2, "the regional FID rides on the magnetisation sweep");
   // NH = 0 without moment fields is the density channel alone: one sweep of the equilibration loop,
   // rho <- W rho with delta = max_i |rho_i(t+1) - rho_i(t)| = max_i pi_i |r'_i - r_i| in acc[0] (a maximum, not a sum)
@@ -157,6 +169,7 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
   const int ek = ty * TZ + VW * tp;              // and in a tile without halo
   const bool edge_yz = (a.per[1] && (y == 0 || y == L.ny - 1)) || (a.per[2] && (z == 0 || z + VW >= L.nz));
   const int permask = (a.per[0] ? 1 : 0) | (a.per[1] ? 2 : 0) | (a.per[2] ? 4 : 0);
+  const bool xface = a.per[0] || PEER;   // the outermost x planes have copies to write
   T* outp = a.fout + L.idx(x0, y, z);
   // REG: the running sum of the region the thread is in; it moves to the thread's slot when the label changes
   const uint8_t* labp = REG ? a.label + ((long long)x0 * L.ny + y) * L.nz + z : nullptr;
@@ -305,11 +318,15 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
       }
     }
     if (nvalid > 0) {
-      if (edge_yz || (a.per[0] && (x == 0 || x == L.nx - 1))) {
+      if (edge_yz || (xface && (x == 0 || x == L.nx - 1))) {
         const long long i = L.idx(x, y, z);
 #pragma unroll
-        for (int c = 0; c < C; ++c)
+        for (int c = 0; c < C; ++c) {
           store_face_vec<T, VW>(a.fout + (long long)c * L.np, i, L.nx, L.ny, L.nz, L.sy, L.sx, permask, x, y, z, packv<T, VW>(o[c]), nvalid);
+          if constexpr (PEER)   // the neighbours' ghost planes: same offset inside the padded plane
+            store_peer_vec<T, VW>(a.peer[0] ? a.peer[0] + c * a.peer_stride[0] : nullptr, a.peer[1] ? a.peer[1] + c * a.peer_stride[1] : nullptr,
+                                  i - (long long)(x + 1) * L.sx, L.nx, x, packv<T, VW>(o[c]), nvalid);
+        }
       } else {
 #pragma unroll
         for (int c = 0; c < C; ++c) store_vec<T, VW>(outp + (long long)c * L.np, packv<T, VW>(o[c]), nvalid);
@@ -373,19 +390,19 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
   }
 }
 
-template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int VW, int REG = 0>
-__global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 0, VW, REG>::LB_THREADS, TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 0, VW, REG>::LB_CTAS)
+template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int VW, int FEAT = 0>
+__global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 0, VW, FEAT>::LB_THREADS, TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 0, VW, FEAT>::LB_CTAS)
     step_tma_kernel(const __grid_constant__ CUtensorMap tm_f, const __grid_constant__ CUtensorMap tm_pi,
                     const __grid_constant__ CUtensorMap tm_cs, StepArgs<T> a) {
-  step_tma_body<T, VW, NH, NRHO, NMOM, TY, TZ, NSTAGE, 0, REG>(tm_f, tm_pi, tm_cs, NoLinkMaps(), a);
+  step_tma_body<T, VW, NH, NRHO, NMOM, TY, TZ, NSTAGE, 0, FEAT>(tm_f, tm_pi, tm_cs, NoLinkMaps(), a);
 }
 
 // the same sweep with stored link weights (per-link mobility factors)
-template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int VW, int REG = 0>
-__global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1, VW, REG>::LB_THREADS, TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1, VW, REG>::LB_CTAS)
+template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int VW, int FEAT = 0>
+__global__ void __launch_bounds__(TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1, VW, FEAT>::LB_THREADS, TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1, VW, FEAT>::LB_CTAS)
     step_tma_links_kernel(const __grid_constant__ CUtensorMap tm_f, const __grid_constant__ CUtensorMap tm_cs,
                           const __grid_constant__ TmaLinkMaps lm, StepArgs<T> a) {
-  step_tma_body<T, VW, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1, REG>(tm_f, tm_f, tm_cs, lm, a);
+  step_tma_body<T, VW, NH, NRHO, NMOM, TY, TZ, NSTAGE, 1, FEAT>(tm_f, tm_f, tm_cs, lm, a);
 }
 
 }  // namespace lpc

@@ -86,6 +86,23 @@ class SlabSet:
             lo, hi = self.ranges[s]
             self.lat[s] = lattice_factory((hi - lo,) + self.global_shape[1:], bc=(LPC_BC_HALO, self.bc[1], self.bc[2]), **cfg)
         self.steps = 0
+        self.direct = set()   # (src slab, src side) whose plane the step kernel stores into the neighbour itself
+
+    def enable_direct_stores(self):
+        """Let the step kernel write a slab's outermost planes straight into the ghost planes of neighbours that live
+        in this process (same device: plain device addresses; several devices of one process: peer access must be
+        enabled) -- the transfer rides on the sweep's own stores and `exchange` has nothing left to do for those
+        faces.  Faces towards other ranks keep the send / recv.  Call after set_site_params."""
+        self.direct = set()
+        for s in self.owned:
+            peers = [None, None]
+            for side in (0, 1):
+                t = neighbour(self.n_slabs, s, side, self.periodic)
+                if t is not None and self.owner(t) == self.rank and hasattr(self.lat[t], "ghost_plane_addresses"):
+                    peers[side] = self.lat[t].ghost_plane_addresses(1 - side)
+                    self.direct.add((s, side))
+            self.lat[s].set_halo_peers(lo=peers[0], hi=peers[1])
+        return len(self.direct)
 
     def owner(self, s: int) -> int:
         return s // self.spr
@@ -111,7 +128,7 @@ class SlabSet:
         return t.cpu().numpy().view(x.dtype).reshape(x.shape)
 
     # ---- the plane exchange -------------------------------------------------------------------
-    def exchange(self, which):
+    def exchange(self, which, after_step=False):
         """Fill every x ghost plane of `which` (HALO_PARAMS or HALO_STATE) from the neighbour's outermost owned
         plane.  Same process: one device copy per plane.  Other rank: one send / recv per channel plane, all of one
         exchange batched into a single group; both ends enumerate `messages()` in the same order, which is what
@@ -121,6 +138,8 @@ class SlabSet:
             so, do = self.owner(src), self.owner(dst)
             if so != self.rank and do != self.rank:
                 continue
+            if after_step and (src, sside) in self.direct:
+                continue   # the sweep stored this plane into the neighbour's ghost plane already
             if so == self.rank and do == self.rank:
                 self.lat[dst].halo_planes(which, dside, RECV).copy_(self.lat[src].halo_planes(which, sside, SEND))
                 continue
@@ -164,7 +183,7 @@ class SlabSet:
         for _ in range(int(n)):
             for s in self.owned:
                 self.lat[s].step(1)
-            self.exchange(HALO_STATE)
+            self.exchange(HALO_STATE, after_step=True)
             self.steps += 1
 
     def _allreduce_max(self, v: float) -> float:

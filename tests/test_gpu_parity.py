@@ -727,9 +727,10 @@ def test_error_codes(lpc):
 # x-slab decomposition.  All slabs live on the one GPU here; the plane exchange is a device copy,
 # the driver code (paper_2603_22553_b200/slab.py) is the one a multi-GPU run executes.
 # ---------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("bc,n_slabs,kernel,precision", [((0, 0, 0), 2, 2, 0), ((1, 0, 0), 3, 2, 0), ((0, 1, 0), 1, 1, 0),
-                                                         ((1, 0, 1), 4, 0, 0), ((0, 0, 0), 3, 2, 1)])
-def test_slabs_match_unsplit_lattice_and_oracle(lpc, oracle_mod, bc, n_slabs, kernel, precision):
+@pytest.mark.parametrize("bc,n_slabs,kernel,precision,direct", [
+    ((0, 0, 0), 2, 2, 0, False), ((1, 0, 0), 3, 2, 0, False), ((0, 1, 0), 1, 1, 0, False), ((1, 0, 1), 4, 0, 0, False),
+    ((0, 0, 0), 3, 2, 1, False), ((0, 0, 0), 2, 2, 0, True), ((1, 0, 0), 3, 0, 0, True), ((0, 1, 0), 1, 2, 0, True), ((0, 0, 1), 4, 2, 1, True)])
+def test_slabs_match_unsplit_lattice_and_oracle(lpc, oracle_mod, bc, n_slabs, kernel, precision, direct):
     from paper_2603_22553_b200 import slab
 
     n = 40
@@ -747,6 +748,10 @@ def test_slabs_match_unsplit_lattice_and_oracle(lpc, oracle_mod, bc, n_slabs, ke
                       n_density=1, dt=lat.dt, a=lat.a, alpha=lat.alpha, max_steps=n)
     assert sorted(ss.lat) == list(range(n_slabs)) and sum(hi - lo for lo, hi in ss.ranges.values()) == lat.nx
     ss.set_site_params(lat.dF, lat.blocked, lat.omega, g0)
+    if direct:
+        # the sweeps store their outermost planes into the neighbours' ghost planes themselves: nothing is copied
+        assert ss.enable_direct_stores() == len(slab.messages(n_slabs, lat.bc[0] == 0))
+        ss.exchange = lambda which, after_step=False, _ex=ss.exchange: _ex(which, after_step) if not after_step else None
     orc = oracle_mod.Oracle.from_lattice(lat, n_moments=3, max_steps=n)
     orc.set_g(g0)
     assert abs(ss.fid()[0] - orc.fid()[0]) <= tol_sum * np.abs(g0).sum()
