@@ -266,6 +266,7 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
     for (int k = 0; k < VW; ++k) {
       u[k].pc = ctr.pi[k];
       u[k].kap = ctr.kap[k];
+      u[k].sum_weights();
     }
 
     T o[C][VW];
