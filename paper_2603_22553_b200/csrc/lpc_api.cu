@@ -252,6 +252,12 @@ bool regions_fusable(const lpc_lattice* h) {
   return h->have_regions && h->nrho == 0 && h->tma_ok && h->kernel != LPC_KERNEL_DIRECT && !getenv("LPC_NO_REGION_FUSION");
 }
 
+// what launch_step_t will decide for the next step: regional sums inside the TMA sweeps (not with direct halo stores)
+bool will_fuse_regions(const lpc_lattice* h) {
+  const bool peers = h->peer[0][h->cur ^ 1] || h->peer[1][h->cur ^ 1];
+  return regions_fusable(h) && !peers;
+}
+
 // ---- launch of one sweep ---------------------------------------------------------------------
 template <typename T, int NRHO, int NMOM>
 int launch_step_t(lpc_lattice* h) {
@@ -283,12 +289,15 @@ int launch_step_t(lpc_lattice* h) {
   if (peers && !use_tma) return fail(LPC_ESTATE, "direct halo stores need the TMA kernel");
   // region-resolved FID inside the magnetisation sweep (no separate pass over the state): TMA kernel, no density channel
   // (and not together with direct halo stores: that combination runs the separate pass)
-  const bool fuse_regions = use_tma && regions_fusable(h) && !peers;
+  const bool fuse_regions = use_tma && will_fuse_regions(h);
   h->regions_fused = fuse_regions;
   a.label = fuse_regions ? h->ws + h->off.regions : nullptr;
   a.rpartials = wsp<double>(h, h->off.rpartials);
   a.fidr = wsp<double2>(h, h->off.fidr);
   a.fidr_stride = h->cfg.max_steps + 1;
+  a.vacfr = wsp<double>(h, h->off.vacfr);
+  a.wr = wsp<double>(h, h->off.wr);
+  a.vacfr_stride = h->cfg.max_steps + 2;
   a.region_sample = h->steps + 1;
   a.n_regions = h->cfg.n_regions;
   if (use_tma) {
@@ -333,7 +342,11 @@ int launch_step_t(lpc_lattice* h) {
       am.fout = a.fout + (long long)am.c0 * h->L.np;
       for (int s = 0; s < 2; ++s)
         if (am.peer[s]) am.peer[s] += (long long)am.c0 * am.peer_stride[s];
-      int rc = h->have_links ? launch_links(step_tma_links_kernel<T, 0, 0, 3, TY, 64, 3, VW>, TmaCfg<T, 0, 0, 3, TY, 64, 3, 1, VW>(), h->tm_m[h->cur], am)
+      am.region_sample = h->steps + 2;   // Z_d[k+1] of the fields before this sweep
+      const bool fuse_vacf = fuse_regions && h->region_moments;
+      int rc = fuse_vacf ? (h->have_links ? launch_links(step_tma_links_kernel<T, 0, 0, 3, TY, 64, 3, VW, 1>, TmaCfg<T, 0, 0, 3, TY, 64, 3, 1, VW, 1>(), h->tm_m[h->cur], am)
+                                          : launch(step_tma_kernel<T, 0, 0, 3, TY, 64, 4, VW, 1>, TmaCfg<T, 0, 0, 3, TY, 64, 4, 0, VW, 1>(), h->tm_m[h->cur], am))
+               : h->have_links ? launch_links(step_tma_links_kernel<T, 0, 0, 3, TY, 64, 3, VW>, TmaCfg<T, 0, 0, 3, TY, 64, 3, 1, VW>(), h->tm_m[h->cur], am)
                : peers       ? launch(step_tma_kernel<T, 0, 0, 3, TY, 64, 4, VW, 2>, TmaCfg<T, 0, 0, 3, TY, 64, 4, 0, VW, 2>(), h->tm_m[h->cur], am)
                              : launch(step_tma_kernel<T, 0, 0, 3, TY, 64, 4, VW>, TmaCfg<T, 0, 0, 3, TY, 64, 4, 0, VW>(), h->tm_m[h->cur], am);
       if (rc) return rc;
@@ -341,9 +354,9 @@ int launch_step_t(lpc_lattice* h) {
     a.c0 = 0;
     int rc;
     if constexpr (NRHO == 0) {
-      if (fuse_regions)   // one stage less: the per-thread region slots take 32 KB of shared memory
-        rc = h->have_links ? launch_links(step_tma_links_kernel<T, 2, 0, 0, TY, 64, 2, VW, 1>, TmaCfg<T, 2, 0, 0, TY, 64, 2, 1, VW, 1>(), h->tm_f[h->cur], a)
-                           : launch(step_tma_kernel<T, 2, 0, 0, TY, 64, 3, VW, 1>, TmaCfg<T, 2, 0, 0, TY, 64, 3, 0, VW, 1>(), h->tm_f[h->cur], a);
+      if (fuse_regions)
+        rc = h->have_links ? launch_links(step_tma_links_kernel<T, 2, 0, 0, TY, 64, NSL, VW, 1>, TmaCfg<T, 2, 0, 0, TY, 64, NSL, 1, VW, 1>(), h->tm_f[h->cur], a)
+                           : launch(step_tma_kernel<T, 2, 0, 0, TY, 64, NS, VW, 1>, TmaCfg<T, 2, 0, 0, TY, 64, NS, 0, VW, 1>(), h->tm_f[h->cur], a);
       else
         rc = h->have_links ? launch_links(step_tma_links_kernel<T, 2, 0, 0, TY, 64, NSL, VW>, TmaCfg<T, 2, 0, 0, TY, 64, NSL, 1, VW>(), h->tm_f[h->cur], a)
              : peers       ? launch(step_tma_kernel<T, 2, 0, 0, TY, 64, NS, VW, 2>, TmaCfg<T, 2, 0, 0, TY, 64, NS, 0, VW, 2>(), h->tm_f[h->cur], a)
@@ -390,6 +403,7 @@ int launch_persist_t(lpc_lattice* h, int64_t n) {
   for (int d = 0; d < 3; ++d) a.per[d] = h->cfg.bc[d] == 0;
   a.peer[0] = a.peer[1] = nullptr; a.peer_stride[0] = a.peer_stride[1] = 0;
   a.label = nullptr; a.rpartials = nullptr; a.fidr = nullptr; a.fidr_stride = 0; a.region_sample = 0; a.n_regions = 0;
+  a.vacfr = nullptr; a.wr = nullptr; a.vacfr_stride = 0;
   a.c0 = 0; a.xc = 0; a.tiles_z = a.tiles_y = a.chunks_x = 0;
   auto kern = step_persist_kernel<T, NRHO, NMOM>;
   static int per_sm = 0;
@@ -768,6 +782,7 @@ int equilibrate_t(lpc_lattice* h, double threshold, int64_t max_iters, int64_t c
   for (int d = 0; d < 3; ++d) sa.per[d] = a.per[d];
   sa.peer[0] = sa.peer[1] = nullptr; sa.peer_stride[0] = sa.peer_stride[1] = 0;
   sa.label = nullptr; sa.rpartials = nullptr; sa.fidr = nullptr; sa.fidr_stride = 0; sa.region_sample = 0; sa.n_regions = 0;
+  sa.vacfr = nullptr; sa.wr = nullptr; sa.vacfr_stride = 0;
   sa.c0 = 2; sa.xc = h->xc; sa.tiles_z = h->tiles_z; sa.tiles_y = h->tiles_y; sa.chunks_x = h->chunks_x;
   constexpr int VW = 16 / (int)sizeof(T), TY = 4 * VW;
   using KP = TmaCfg<T, 0, 1, 0, TY, 64, 4, 0, VW>;
@@ -1048,7 +1063,7 @@ int lpc_step_n(lpc_lattice* h, int64_t n) {
                        (h->kernel == LPC_KERNEL_PERSIST || (h->kernel == LPC_KERNEL_AUTO && persist_by_default(h)));
   if (persist) return h->cfg.precision ? launch_persist<float>(h, n) : launch_persist<double>(h, n);
   for (int64_t k = 0; k < n; ++k) {
-    if (h->region_moments) {
+    if (h->region_moments && !will_fuse_regions(h)) {   // else the moment sweep books the regional VACF itself
       int rc = region_moment<false>(h);
       if (rc) return rc;
     }

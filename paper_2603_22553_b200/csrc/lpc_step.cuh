@@ -219,7 +219,7 @@ struct TmaLinkMaps {
 };
 
 // VW: sites per thread along z (one 16-byte vector: 2 in fp64, 4 in the fp32 march of lpc_step_vec.cuh).
-// FEAT bit 0: the region-resolved FID is accumulated in the same sweep (per-thread slots in shared memory);
+// FEAT bit 0: the region-resolved FID (magnetisation sweep) or VACF (moment sweep) is accumulated in the same sweep;
 // bit 1: slab mode with direct halo stores (no shared memory of its own).
 template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int LK = 0, int VW = 2, int FEAT = 0>
 struct TmaCfg {
@@ -252,7 +252,7 @@ struct TmaCfg {
   static constexpr int BAR_OFF = NSTAGE * STAGE_BYTES;
   static constexpr int RED_OFF = BAR_OFF + 2 * NSTAGE * 8;
   static constexpr int RSLOT_OFF = (RED_OFF + ((NTHREADS / 32) * NRED + 1) * 8 + 15) / 16 * 16;
-  static constexpr int RSLOT_BYTES = (FEAT & 1) ? NTHREADS * 2 * MAX_REGIONS * 8 : 0;   // [region][re,im][thread] doubles
+  static constexpr int RSLOT_BYTES = (FEAT & 1) ? NTHREADS * 8 : 0;   // scratch of the regional column sums (<= NTHREADS doubles)
   static constexpr int SMEM_BYTES = RSLOT_OFF + RSLOT_BYTES + 128;  // +128: manual alignment slack
   // Resident CTAs per SM the registers are budgeted for: two 8-warp CTAs (TY = 8, up to 3 channels) or
   // one.  16 warps per SM are 4 per scheduler, i.e. up to 128 registers per thread.

@@ -86,7 +86,9 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
   constexpr int REG = FEAT & 1;
   constexpr bool PEER = (FEAT & 2) != 0;
   using K = TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, LK, VW, FEAT>;
-  static_assert(!REG || NH == 2, "the regional FID rides on the magnetisation sweep");
+  // REG on the magnetisation sweep: G_r (2 values per site); on the moment sweep: the regional VACF (3 values per site)
+  static_assert(!REG || NH == 2 || NMOM == 3, "regional sums ride on the magnetisation or on the moment sweep");
+  constexpr int RNV = (NH == 2) ? 2 : 3;
   // NH = 0 without moment fields is the density channel alone: one sweep of the equilibration loop,
   // rho <- W rho with delta = max_i |rho_i(t+1) - rho_i(t)| = max_i pi_i |r'_i - r_i| in acc[0] (a maximum, not a sum)
   constexpr bool EQ = (NH == 0 && NMOM == 0);
@@ -98,12 +100,7 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
   uint64_t* full = reinterpret_cast<uint64_t*>(smem + K::BAR_OFF);
   uint64_t* empty = full + NSTAGE;
   double* red = reinterpret_cast<double*>(smem + K::RED_OFF);
-  // REG: thread t owns the slots rslot[(2 r + c) * NTHREADS + t] of region r, component c (no atomics, fixed order)
-  double* rslot = reinterpret_cast<double*>(smem + K::RSLOT_OFF);
-  if constexpr (REG) {
-#pragma unroll
-    for (int q = 0; q < 2 * MAX_REGIONS; ++q) rslot[q * K::NTHREADS + threadIdx.x] = 0.0;
-  }
+  double* rred = reinterpret_cast<double*>(smem + K::RSLOT_OFF);   // REG: warp partials of the regional columns
 
   const Layout& L = a.L;
   const int bz = blockIdx.x % a.tiles_z;
@@ -173,14 +170,32 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
   T* outp = a.fout + L.idx(x0, y, z);
   // REG: the running sum of the region the thread is in; it moves to the thread's slot when the label changes
   const uint8_t* labp = REG ? a.label + ((long long)x0 * L.ny + y) * L.nz + z : nullptr;
+  // running sums of the region the thread is in (registers); they move to the thread's own per-region array -- indexed at
+  // run time, hence in local memory, touched only when the label changes along the thread's column -- on a change
+  // the magnetisation sweep has the registers to request the labels a plane ahead; the moment sweep (at the 128-register
+  // cap) reads them at the top of the plane they belong to
+  constexpr bool LABEL_AHEAD = (NH == 2);
+  int labn[VW];
+  if constexpr (REG && LABEL_AHEAD) {
+#pragma unroll
+    for (int k = 0; k < VW; ++k) labn[k] = (k < nvalid) ? (int)__ldg(labp + k) : 255;
+  }
   int rcur = 255;
-  double racc0 = 0.0, racc1 = 0.0;
+  double racc[RNV];
+  double rall[REG ? MAX_REGIONS * RNV : 1];
+  if constexpr (REG) {
+#pragma unroll
+    for (int q = 0; q < MAX_REGIONS * RNV; ++q) rall[q] = 0.0;
+#pragma unroll
+    for (int v = 0; v < RNV; ++v) racc[v] = 0.0;
+  }
   auto rflush = [&](int next) {
     if (rcur < MAX_REGIONS) {
-      rslot[(2 * rcur) * K::NTHREADS + threadIdx.x] += racc0;
-      rslot[(2 * rcur + 1) * K::NTHREADS + threadIdx.x] += racc1;
+#pragma unroll
+      for (int v = 0; v < RNV; ++v) rall[rcur * RNV + v] += racc[v];
     }
-    racc0 = racc1 = 0.0;
+#pragma unroll
+    for (int v = 0; v < RNV; ++v) racc[v] = 0.0;
     rcur = next;
   };
 
@@ -217,7 +232,16 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
   auto plane = [&](int x, int sc, const Plane& prv, const Plane& ctr, Plane& nxt) {
     if (threadIdx.x == 0 && jl < nloads) issue_load();
     int labs[VW];
-    if constexpr (REG) {
+    if constexpr (REG && LABEL_AHEAD) {
+      // the labels of this plane were requested one plane ago; request the next plane's now
+#pragma unroll
+      for (int k = 0; k < VW; ++k) labs[k] = labn[k];
+      labp += (long long)L.ny * L.nz;
+      if (x + 1 < x0 + nplanes) {
+#pragma unroll
+        for (int k = 0; k < VW; ++k) labn[k] = (k < nvalid) ? (int)__ldg(labp + k) : 255;
+      }
+    } else if constexpr (REG) {
 #pragma unroll
       for (int k = 0; k < VW; ++k) labs[k] = (k < nvalid) ? (int)__ldg(labp + k) : 255;
       labp += (long long)L.ny * L.nz;
@@ -283,7 +307,16 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
 #pragma unroll
         for (int k = 0; k < VW; ++k) {
           const T dm = (d == 0) ? (u[k].mxp - u[k].mxm) : (d == 1) ? (u[k].myp - u[k].mym) : (u[k].mzp - u[k].mzm);
-          if (k < nvalid) t += (double)ctr.f[c][k] * (double)dm;
+          const double qd = (double)ctr.f[c][k] * (double)dm;
+          if (k < nvalid) t += qd;
+          if constexpr (REG && NMOM == 3) {
+            // regional VACF: the same product, booked under the label of the site (labels of a group are visited in
+            // d-major order, so a group that straddles two regions flushes more often, never wrongly)
+            if (k < nvalid) {
+              if (labs[k] != rcur) rflush(labs[k]);
+              racc[d] += qd;
+            }
+          }
         }
         acc[2 + d] += t;
       }
@@ -312,8 +345,8 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
           acc[1] += (double)ctr.pi[k] * (double)o[1][k];
           if constexpr (REG) {
             if (labs[k] != rcur) rflush(labs[k]);
-            racc0 += (double)ctr.pi[k] * (double)o[0][k];
-            racc1 += (double)ctr.pi[k] * (double)o[1][k];
+            racc[0] += (double)ctr.pi[k] * (double)o[0][k];
+            racc[1] += (double)ctr.pi[k] * (double)o[1][k];
           }
         }
       }
@@ -353,18 +386,23 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
   if (p < nplanes) { plane(x0 + p, sc, P0, P1, P2); next_stage(); ++p; }
   if (p < nplanes) { plane(x0 + p, sc, P1, P2, P0); next_stage(); ++p; }
 
+  constexpr int RNC = MAX_REGIONS * RNV;   // regional columns
   if constexpr (REG) {
-    // block partial of every (region, component) column: warp w adds the slots of columns 2w, 2w+1 in a fixed order
+    // block partial of every (region, component) column: warp sums, then thread q adds the warps of column q in order
     rflush(255);
-    __syncthreads();
     const int warp = threadIdx.x >> 5;
-    for (int q = warp; q < 2 * MAX_REGIONS; q += K::NTHREADS / 32) {
-      double v = 0.0;
-      for (int t = lane; t < K::NTHREADS; t += 32) v += rslot[q * K::NTHREADS + t];
-      v = warp_sum(v);
-      if (lane == 0) a.rpartials[(size_t)blockIdx.x * 2 * MAX_REGIONS + q] = v;
+#pragma unroll
+    for (int q = 0; q < RNC; ++q) {
+      const double v = warp_sum(rall[q]);
+      if (lane == 0) rred[warp * RNC + q] = v;
     }
-    __threadfence();
+    __syncthreads();
+    if (threadIdx.x < RNC) {
+      double v = 0.0;
+      for (int w = 0; w < K::NTHREADS / 32; ++w) v += rred[w * RNC + threadIdx.x];
+      a.rpartials[(size_t)blockIdx.x * RNC + threadIdx.x] = v;
+      __threadfence();
+    }
   }
   if constexpr (EQ) {
     block_max_finalize(acc[0], red, a.partials, a.ctl, gridDim.x, blockIdx.x);
@@ -374,19 +412,27 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
                                                                                       a.vacf_stride, a.zscale, gridDim.x, blockIdx.x);
   if constexpr (REG) {
     if (!last) return;
-    // the last CTA adds the block partials: thread t takes column t % 16 over the blocks t/16, t/16 + P, ...
+    // the last CTA adds the block partials: thread t takes column t % RNC over the blocks t / RNC, t / RNC + P, ...
     __threadfence();
-    constexpr int NC = 2 * MAX_REGIONS, P = K::NTHREADS / NC;
-    const int col = threadIdx.x % NC, part = threadIdx.x / NC;
+    constexpr int P = K::NTHREADS / RNC;
+    const int col = threadIdx.x % RNC, part = threadIdx.x / RNC;
     double v = 0.0;
-    for (unsigned int b = part; b < gridDim.x; b += P) v += __ldcg(&a.rpartials[(size_t)b * NC + col]);
+    if (part < P)
+      for (unsigned int b = part; b < gridDim.x; b += P) v += __ldcg(&a.rpartials[(size_t)b * RNC + col]);
     __syncthreads();
-    rslot[part * NC + col] = v;
+    if (part < P) rred[part * RNC + col] = v;
     __syncthreads();
-    if (threadIdx.x < NC && (threadIdx.x >> 1) < a.n_regions) {
+    if (threadIdx.x < RNC && threadIdx.x / RNV < a.n_regions) {
       double t = 0.0;
-      for (int q = 0; q < P; ++q) t += rslot[q * NC + threadIdx.x];
-      reinterpret_cast<double*>(a.fidr + (threadIdx.x >> 1) * a.fidr_stride + a.region_sample)[threadIdx.x & 1] = t;
+      for (int q = 0; q < P; ++q) t += rred[q * RNC + threadIdx.x];
+      const int r = threadIdx.x / RNV, c = threadIdx.x % RNV;
+      if (NH == 2) {
+        reinterpret_cast<double*>(a.fidr + r * a.fidr_stride + a.region_sample)[c] = t;
+      } else {
+        // Z^r_d[index] = (a alpha / 6) sum_{i in r} q^d_i (m_{i,+d} - m_{i,-d}) / w_r   (region_moment_kernel, Q27)
+        const double w = a.wr[r];
+        a.vacfr[((long long)r * 3 + c) * a.vacfr_stride + a.region_sample] = (w > 0.0) ? a.zscale * t / w : 0.0;
+      }
     }
   }
 }
