@@ -892,3 +892,38 @@ def test_slab_equilibration_loop_matches_oracle(lpc, oracle_mod, bc, n_slabs):
     it_g, d_g = ss.equilibrate(thr, 500)
     assert it_g == it_o and abs(d_g - deltas[-1]) <= 1e-10 * rho0.max()
     assert np.max(np.abs(ss.gather_field(lpc.LPC_FIELD_RHO) - rho_o)) <= 1e-10 * rho0.max()
+
+
+@pytest.mark.parametrize("seed", [7, 11])
+def test_random_shapes_and_features_tma_against_direct(lpc, seed):
+    """Seeded random lattices (1..120 x 1..70 x 1..300 and tiny ones), boundary conditions, precision, channels, link
+    weights and region labels: the TMA march and the per-pair kernel must agree bit for bit on every field and to
+    rounding on every series (the sums are taken in a different order)."""
+    rng = np.random.default_rng(seed)
+    for case in range(60):
+        shape = tuple(int(rng.integers(1, hi)) for hi in ((120, 70, 300) if case % 2 else (12, 12, 20)))
+        bc = tuple(int(v) for v in rng.integers(0, 2, size=3))
+        prec, nm, nd = int(rng.integers(0, 2)), int(rng.choice([0, 3])), int(rng.integers(0, 2))
+        use_link, nreg, n = bool(rng.integers(0, 2)), int(rng.choice([0, 3])), int(rng.integers(1, 12))
+        lat = lpc_inputs.random_small(shape, bc=bc, p_block=0.25 if np.prod(shape) > 8 else 0.0, alpha=0.9, seed=1000 + case, n_moments=nm)
+        link = lpc_inputs.random_links(shape, seed=case, lo=0.0) if use_link else None
+        region = rng.integers(0, 4, size=shape).astype(np.uint8)
+        out = []
+        for kernel in (1, 2):
+            g = lpc.Lattice.from_inputs(lat, precision=prec, n_moments=nm, n_density=nd, max_steps=n + 1, n_regions=nreg, link=link)
+            g.set_kernel(kernel)
+            if nreg:
+                g.set_regions(region)
+            g.step(n)
+            fields = [g.field(lpc.LPC_FIELD_G)] + ([g.field(lpc.LPC_FIELD_PX + d) for d in range(3)] if nm else [])
+            fields += [g.field(lpc.LPC_FIELD_RHO)] if nd else []
+            series = [g.fid()] + ([g.moments()[0]] if nm else [])
+            series += [np.array([g.fid_region(r) for r in range(nreg)])] if nreg else []
+            series += [np.array([g.moments_region(r)[0] for r in range(nreg)])] if nreg and nm else []
+            out.append((fields, series))
+            g.close()
+        what = f"case {case}: {shape} bc={bc} prec={prec} nm={nm} nd={nd} link={use_link} nreg={nreg} n={n}"
+        assert all(np.array_equal(a, b) for a, b in zip(out[0][0], out[1][0])), what
+        tol = 2e-5 if prec else 1e-12
+        for a, b in zip(out[0][1], out[1][1]):
+            assert np.all(np.abs(a - b) <= tol * max(np.abs(a).max(), 1e-300)), what
