@@ -199,11 +199,11 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
     rcur = next;
   };
 
-  // one x-plane as a thread holds it: the group's values of every channel and of pi, kappa, and mlo = the link
+  // one x-plane as a thread holds it: the group's values of every channel and of pi, and mlo = the link
   // weight towards the plane below (LK: the plane's own +x link weight, i.e. the -x weight of the plane above)
   struct Plane {
     T f[C][VW];
-    T pi[VW], kap[VW], mlo[VW];
+    T pi[VW], mlo[VW];
   };
   Plane P0, P1, P2;
   int sj = 0;
@@ -215,8 +215,6 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
 #pragma unroll
     for (int c = 0; c < C; ++c) ldv<T, VW>(sf + c * TYH * TZW + ec, n.f[c]);
     ldv<T, VW>(sp + (LK ? ek : ec), n.pi);
-#pragma unroll
-    for (int k = 0; k < VW; ++k) n.kap[k] = kappa_of(n.pi[k], a.a6);
     if constexpr (LK) {
       ldv<T, VW>(reinterpret_cast<const T*>(smem + sj * K::STAGE_BYTES + K::MX_OFF) + ek, n.mlo);
     } else if (below) {
@@ -289,7 +287,7 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
 #pragma unroll
     for (int k = 0; k < VW; ++k) {
       u[k].pc = ctr.pi[k];
-      u[k].kap = ctr.kap[k];
+      u[k].kap = kappa_of(ctr.pi[k], a.a6);   // once per site and plane, when the plane is the centre one
       u[k].sum_weights();
     }
 
