@@ -61,8 +61,9 @@ def parse():
                    help="run the workload as ONE lattice cut into x-slabs, S per rank (SURVEY 8(e)): a plane exchange after every step, "
                         "strong scaling over --gpus; 0 (default) = independent replicas")
     p.add_argument("--slab-direct", action="store_true",
-                   help="with --slabs: let the sweeps store their outermost planes into the ghost planes of neighbour slabs of the "
-                        "same process (lpc_set_halo_peers) instead of copying them afterwards")
+                   help="with --slabs: let the sweeps store their outermost planes into the neighbours' ghost planes themselves "
+                        "(lpc_set_halo_peers; other ranks' workspaces are mapped through CUDA IPC) instead of copying / sending them "
+                        "after the sweep")
     p.add_argument("--no-cpu-baseline", action="store_true")
     p.add_argument("--no-e2e", action="store_true")
     p.add_argument("--ref-sample-size", type=int, default=int(os.environ.get("LPC_REF_SAMPLE_L", "256")),
@@ -359,7 +360,7 @@ def run_slabs(args, lat, lpc, world, rank, local, dev):
     ss = slab.SlabSet(lat.shape, bc=lat.bc, slabs_per_rank=args.slabs, lattice_factory=factory, precision=args.precision,
                       n_moments=args.moments, dt=lat.dt, a=lat.a, alpha=lat.alpha, max_steps=K + W + 8)
     ss.set_site_params(lat.dF, lat.blocked, lat.omega)
-    n_direct = ss.enable_direct_stores() if args.slab_direct else 0
+    n_direct = ss.enable_direct_stores(remote=world > 1) if args.slab_direct else 0
     ss.step(W)
 
     def barrier():

@@ -87,22 +87,69 @@ class SlabSet:
             self.lat[s] = lattice_factory((hi - lo,) + self.global_shape[1:], bc=(LPC_BC_HALO, self.bc[1], self.bc[2]), **cfg)
         self.steps = 0
         self.direct = set()   # (src slab, src side) whose plane the step kernel stores into the neighbour itself
+        self.remote_direct = False
+        self._peer_storages = []   # mappings of other ranks' workspaces (kept alive while the peers are set)
 
-    def enable_direct_stores(self):
-        """Let the step kernel write a slab's outermost planes straight into the ghost planes of neighbours that live
-        in this process (same device: plain device addresses; several devices of one process: peer access must be
-        enabled) -- the transfer rides on the sweep's own stores and `exchange` has nothing left to do for those
-        faces.  Faces towards other ranks keep the send / recv.  Call after set_site_params."""
+    def enable_direct_stores(self, remote=False):
+        """Let the step kernel write a slab's outermost planes straight into the neighbours' ghost planes -- the
+        transfer rides on the sweep's own stores and `exchange` has nothing left to do for those faces.  Neighbours in
+        this process: plain device addresses.  remote=True: neighbours on other ranks of the SAME NODE as well -- every
+        rank exports its workspace allocation as a CUDA IPC handle (torch's shared-storage handle), the ranks swap
+        handles and ghost-plane offsets once (all_gather_object) and map each other's workspaces; after every step a
+        fence (`_step_fence`) makes sure all ranks' sweeps have finished before any rank starts the next one.  Faces
+        that are not direct keep the copy / send-recv.  Call after set_site_params.  Returns the direct faces here."""
         self.direct = set()
+        self._peer_storages = []
+        remote = bool(remote) and self.dist is not None and self.world > 1
+        table = {}
+        if remote:
+            import torch
+
+            mine = {}
+            for s in self.owned:
+                ws = self.lat[s].workspace
+                base = ws.data_ptr()
+                mine[s] = (ws.untyped_storage()._share_cuda_(),
+                           [tuple(a - base for a in self.lat[s].ghost_plane_addresses(side)[:2]) for side in (0, 1)],
+                           self.lat[s].ghost_plane_addresses(0)[2])
+            gathered = [None] * self.world
+            self.dist.all_gather_object(gathered, mine, group=self.group)
+            for part in gathered:
+                table.update(part)
         for s in self.owned:
             peers = [None, None]
             for side in (0, 1):
                 t = neighbour(self.n_slabs, s, side, self.periodic)
-                if t is not None and self.owner(t) == self.rank and hasattr(self.lat[t], "ghost_plane_addresses"):
-                    peers[side] = self.lat[t].ghost_plane_addresses(1 - side)
+                if t is None:
+                    continue
+                if self.owner(t) == self.rank:
+                    if hasattr(self.lat[t], "ghost_plane_addresses"):
+                        peers[side] = self.lat[t].ghost_plane_addresses(1 - side)
+                        self.direct.add((s, side))
+                elif remote:
+                    import torch
+
+                    handle, offsets, stride = table[t]
+                    st = torch.UntypedStorage._new_shared_cuda(*handle)   # maps the other rank's workspace here
+                    self._peer_storages.append(st)
+                    off0, off1 = offsets[1 - side]
+                    peers[side] = (st.data_ptr() + off0, st.data_ptr() + off1, stride)
                     self.direct.add((s, side))
             self.lat[s].set_halo_peers(lo=peers[0], hi=peers[1])
+        self.remote_direct = remote
         return len(self.direct)
+
+    def _step_fence(self):
+        """All ranks' sweeps of this step have finished (their direct stores have landed) before anyone goes on."""
+        import torch
+
+        if self.dist.get_backend(self.group) == "nccl":
+            # a one-element all-reduce on the compute stream orders the ranks' streams without stopping the host
+            t = torch.zeros(1, device="cuda")
+            self.dist.all_reduce(t, group=self.group)
+        else:
+            torch.cuda.synchronize()
+            self.dist.barrier(group=self.group)
 
     def owner(self, s: int) -> int:
         return s // self.spr
@@ -133,7 +180,7 @@ class SlabSet:
         plane.  Same process: one device copy per plane.  Other rank: one send / recv per channel plane, all of one
         exchange batched into a single group; both ends enumerate `messages()` in the same order, which is what
         matches the two planes a pair of ranks swaps in each direction on a periodic ring of two."""
-        ops, keep = [], []
+        ops, keep, landed = [], [], []
         for src, sside, dst, dside in messages(self.n_slabs, self.periodic):
             so, do = self.owner(src), self.owner(dst)
             if so != self.rank and do != self.rank:
@@ -143,18 +190,26 @@ class SlabSet:
             if so == self.rank and do == self.rank:
                 self.lat[dst].halo_planes(which, dside, RECV).copy_(self.lat[src].halo_planes(which, sside, SEND))
                 continue
+            # gloo cannot send device tensors: stage them through the host (tests; NCCL sends the planes in place)
+            via_host = self.dist.get_backend(self.group) != "nccl"
             if so == self.rank:
                 planes = self.lat[src].halo_planes(which, sside, SEND)
+                wire = planes.cpu() if via_host and planes.is_cuda else planes
                 for c in range(planes.shape[0]):
-                    ops.append(self.dist.P2POp(self.dist.isend, planes[c], self._global_rank(do), group=self.group))
+                    ops.append(self.dist.P2POp(self.dist.isend, wire[c], self._global_rank(do), group=self.group))
             else:
                 planes = self.lat[dst].halo_planes(which, dside, RECV)
+                wire = planes.cpu() if via_host and planes.is_cuda else planes
                 for c in range(planes.shape[0]):
-                    ops.append(self.dist.P2POp(self.dist.irecv, planes[c], self._global_rank(so), group=self.group))
-            keep.append(planes)
+                    ops.append(self.dist.P2POp(self.dist.irecv, wire[c], self._global_rank(so), group=self.group))
+                if wire is not planes:
+                    landed.append((planes, wire))
+            keep.append(wire)
         if ops:
             for req in self.dist.batch_isend_irecv(ops):
                 req.wait()
+        for planes, wire in landed:
+            planes.copy_(wire)
 
     def _global_rank(self, r):
         return r if self.group is None else self.dist.get_global_rank(self.group, r)
@@ -184,6 +239,8 @@ class SlabSet:
             for s in self.owned:
                 self.lat[s].step(1)
             self.exchange(HALO_STATE, after_step=True)
+            if self.remote_direct:
+                self._step_fence()
             self.steps += 1
 
     def _allreduce_max(self, v: float) -> float:
