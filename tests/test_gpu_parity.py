@@ -952,3 +952,51 @@ def test_random_lattices_against_oracle(lpc, oracle_mod):
         _check(lpc, lat, gpu, orc, n, tol_site=tol_site, tol_sum=tol_sum,
                what=f"case {case}: {shape} bc={bc} prec={prec} nm={nm} kernel={kernel} link={use_link} n={n}")
         gpu.close()
+
+
+@pytest.mark.parametrize("precision,nm,nd,nreg,use_link,bc", [(0, 3, 1, 3, True, (0, 0, 0)), (1, 3, 1, 3, True, (1, 0, 1)), (0, 0, 0, 0, False, (0, 1, 0)),
+                                                              (1, 0, 0, 2, False, (0, 0, 0)), (0, 3, 0, 0, False, (2, 0, 0))])
+def test_nothing_is_written_outside_the_workspace(lpc, precision, nm, nd, nreg, use_link, bc):
+    """Guard bytes before and after the workspace stay untouched through the precompute, every step kernel, the
+    equilibration sweeps, the regional passes and the read-outs (a bounds check of our own: the sanitizer is not
+    available on the GPU pool)."""
+    import torch
+
+    shape = (21, 19, 133)   # ragged against every tile shape
+    lat = lpc_inputs.random_small(shape, bc=tuple(b if b != 2 else 1 for b in bc), p_block=0.25, alpha=0.9, seed=95, n_moments=nm)
+    cfg = lpc.make_config(*shape, bc=bc, precision=precision, n_moments=nm, n_density=nd, dt=lat.dt, a=lat.a, alpha=lat.alpha,
+                          max_steps=40, stream=torch.cuda.current_stream().cuda_stream, n_regions=nreg,
+                          link_mobility=1 if use_link and bc[0] != 2 else 0)
+    nbytes = lpc.lpc_workspace_bytes(cfg)
+    guard = 1 << 20
+    buf = torch.full((nbytes + 2 * guard,), 0xAB, dtype=torch.uint8, device="cuda:0")
+    assert buf.data_ptr() % 256 == 0
+    handle = lpc.lpc_create_lattice(cfg, buf.data_ptr() + guard, nbytes)
+    try:
+        rng = np.random.default_rng(1)
+        for kernel in (1, 2, 3):
+            lpc.lpc_set_kernel(handle, kernel)
+            lpc.lpc_set_site_params(handle, lat.dF, lat.blocked, lat.omega)
+            if use_link and bc[0] != 2:
+                lpc.lpc_set_link_mobility(handle, lpc_inputs.random_links(shape, seed=9))
+            if bc[0] == 2:
+                lpc.lpc_slab_finish(handle)
+            if nreg:
+                lpc.lpc_set_regions(handle, rng.integers(0, 4, size=shape).astype(np.uint8))
+            if bc[0] == 2:
+                for _ in range(7):
+                    lpc.lpc_step_n(handle, 1)
+            else:
+                lpc.lpc_step_n(handle, 7)
+                lpc.lpc_step_n(handle, 1)
+            if nd and bc[0] != 2:
+                lpc.lpc_equilibrate(handle, 0.0, 5, 2)
+            lpc.lpc_read_fid(handle)
+            if nm:
+                lpc.lpc_moments(handle)
+            if nreg:
+                lpc.lpc_read_fid_region(handle, 0)
+        torch.cuda.synchronize()
+        assert bool((buf[:guard] == 0xAB).all()) and bool((buf[guard + nbytes:] == 0xAB).all())
+    finally:
+        lpc.lpc_destroy(handle)
