@@ -41,7 +41,9 @@
  * stationarity of Eq. 2, relaxation per connected cluster, free-diffusion
  * closed form (Eq. 7), uniform-shift single line, trajectory-enumeration brute
  * force of Eq. 8/11 and of <dx_1 dx_n> on 4^3 and smaller, Lorentz-gas first
- * lag, bounded-system sum rule, axis-permutation and translation symmetry.
+ * lag, bounded-system sum rule, axis-permutation and translation symmetry;
+ * lpco_set_g and the sum_i |g_i| tolerance-scale series against the dense
+ * (Phi W)^n on <= 4^3 (P18, P19).
  * Parity unpinned: the paper's application numbers (Table 1, peak ppm), whose
  * inputs are not available.
  */

@@ -2,8 +2,11 @@
 
 Only tests/, ``__graft_entry__.smoke()`` and bench.py's cpu_baseline /
 ``--impl reference`` legs may import this.  It does not import, and is not
-imported by, ``paper_2603_22553_b200``.  All arithmetic lives in the C file;
-this module only marshals numpy arrays.
+imported by, ``paper_2603_22553_b200``.  The propagation itself (O1-O10) lives in
+the C file and this module marshals numpy arrays for it; three read-outs that
+are plain sums over the oracle's own fields are written out here in numpy:
+``step_with_regions`` (Eq. 12 per region, pin P15), ``step_with_regional_moments``
+(Eq. 4 per region, pin P16) and ``spectrum`` (Eq. 9, pin P14).
 """
 from __future__ import annotations
 

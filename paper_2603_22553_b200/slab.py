@@ -86,8 +86,10 @@ class SlabSet:
             lo, hi = self.ranges[s]
             self.lat[s] = lattice_factory((hi - lo,) + self.global_shape[1:], bc=(LPC_BC_HALO, self.bc[1], self.bc[2]), **cfg)
         self.steps = 0
-        self.direct = set()   # (src slab, src side) whose plane the step kernel stores into the neighbour itself
+        self.direct = set()   # (src slab, src side) of OWNED slabs whose plane the step kernel stores into the neighbour itself
+        self.direct_all = set()   # the same over the slabs of all ranks: what both ends of a message skip after a step
         self.remote_direct = False
+        self.stats = {"copies": 0, "sends": 0, "recvs": 0}   # plane transfers `exchange` has issued so far
         self._peer_storages = []   # mappings of other ranks' workspaces (kept alive while the peers are set)
 
     def enable_direct_stores(self, remote=False):
@@ -137,6 +139,13 @@ class SlabSet:
                     self.direct.add((s, side))
             self.lat[s].set_halo_peers(lo=peers[0], hi=peers[1])
         self.remote_direct = remote
+        # the receiving end of a direct face must skip its receive as well: every rank learns all ranks' direct faces
+        self.direct_all = set(self.direct)
+        if self.dist is not None and self.world > 1:
+            gathered = [None] * self.world
+            self.dist.all_gather_object(gathered, sorted(self.direct), group=self.group)
+            for part in gathered:
+                self.direct_all.update(tuple(f) for f in part)
         return len(self.direct)
 
     def _step_fence(self):
@@ -185,10 +194,11 @@ class SlabSet:
             so, do = self.owner(src), self.owner(dst)
             if so != self.rank and do != self.rank:
                 continue
-            if after_step and (src, sside) in self.direct:
-                continue   # the sweep stored this plane into the neighbour's ghost plane already
+            if after_step and (src, sside) in self.direct_all:
+                continue   # the sweep stored this plane into the neighbour's ghost plane already (both ends skip it)
             if so == self.rank and do == self.rank:
                 self.lat[dst].halo_planes(which, dside, RECV).copy_(self.lat[src].halo_planes(which, sside, SEND))
+                self.stats["copies"] += 1
                 continue
             # gloo cannot send device tensors: stage them through the host (tests; NCCL sends the planes in place)
             via_host = self.dist.get_backend(self.group) != "nccl"
@@ -197,11 +207,13 @@ class SlabSet:
                 wire = planes.cpu() if via_host and planes.is_cuda else planes
                 for c in range(planes.shape[0]):
                     ops.append(self.dist.P2POp(self.dist.isend, wire[c], self._global_rank(do), group=self.group))
+                self.stats["sends"] += 1
             else:
                 planes = self.lat[dst].halo_planes(which, dside, RECV)
                 wire = planes.cpu() if via_host and planes.is_cuda else planes
                 for c in range(planes.shape[0]):
                     ops.append(self.dist.P2POp(self.dist.irecv, wire[c], self._global_rank(so), group=self.group))
+                self.stats["recvs"] += 1
                 if wire is not planes:
                     landed.append((planes, wire))
             keep.append(wire)

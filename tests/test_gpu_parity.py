@@ -584,35 +584,90 @@ def test_fp32_mode(lpc, oracle_mod, kernel):
 
 
 # ---------------------------------------------------------------------------------------------
-# BASELINE configs[1..3] at test sizes (and full length with LPC_FULL=1)
+# BASELINE configs[1..3]: the stated lattices in the default run (config 1 for 2000 steps, config 2 at 256^3 with the
+# moment fields for 200, config 3 at 2048 x 256 x 256 for 20), their full lengths (20000 / 20000 / 10000 steps) with
+# LPC_FULL=1 (profiles/r2_full_parity.md), and small copies of configs 2 and 3 that run longer per site
 # ---------------------------------------------------------------------------------------------
+def _report(name, res):
+    """One line per full-size case, also appended to gpurun_out/parity_full.log when that directory exists."""
+    line = f"PARITY {name}: " + ", ".join(f"{k}={v:.2e}" for k, v in res.items())
+    print(line)
+    out = os.path.join(ROOT, "gpurun_out")
+    if os.path.isdir(out):
+        with open(os.path.join(out, "parity_full.log"), "a") as f:
+            f.write(line + "\n")
+
+
 def test_config1_particle(lpc, oracle_mod):
-    n = 20000 if FULL else 300
+    n = 20000 if FULL else 2000
     lat = lpc_inputs.particle(n_steps=n)
+    assert lat.shape == (128, 128, 128)
     gpu, orc = _pair(lpc, oracle_mod, lat, n, 0)
     gpu.step(n)
     orc.step(n)
-    print(_check(lpc, lat, gpu, orc, n, what="config1"))
+    _report(f"config1 128^3 {n} steps", _check(lpc, lat, gpu, orc, n, what="config1"))
 
 
 def test_config2_monolith_scaled(lpc, oracle_mod):
-    L, n = (256, 200) if FULL else (96, 200)
+    L, n = 96, 200
     lat = lpc_inputs.monolith(L=L, n_steps=n)
     gpu, orc = _pair(lpc, oracle_mod, lat, n, 0)
     gpu.step(n)
     orc.step(n)
-    print(_check(lpc, lat, gpu, orc, n, what="config2"))
+    print(_check(lpc, lat, gpu, orc, n, what="config2 scaled"))
+
+
+def test_config2_monolith_full_size(lpc, oracle_mod):
+    n = 20000 if FULL else 200
+    lat = lpc_inputs.monolith(n_steps=n)
+    assert lat.shape == (256, 256, 256) and lat.n_moments == 3
+    gpu, orc = _pair(lpc, oracle_mod, lat, n, 0)
+    gpu.step(n)
+    orc.step(n)
+    _report(f"config2 256^3 + 3 moment fields {n} steps", _check(lpc, lat, gpu, orc, n, what="config2"))
 
 
 def test_config3_supercap_scaled(lpc, oracle_mod):
-    shape, n = ((2048, 256, 256), 20) if FULL else ((256, 32, 64), 200)
+    shape, n = (256, 32, 64), 200
     lat = lpc_inputs.supercap(*shape, n_steps=n)
     gpu, orc = _pair(lpc, oracle_mod, lat, n, 0)
     gpu.step(n)
     orc.step(n)
-    print(_check(lpc, lat, gpu, orc, n, what="config3"))
+    print(_check(lpc, lat, gpu, orc, n, what="config3 scaled"))
     # reflective x: nothing leaks through the walls -- total magnetisation magnitude is bounded by 1
     assert np.abs(gpu.fid()).max() <= 1 + 1e-12
+
+
+def test_config3_supercap_full_size(lpc, oracle_mod):
+    import torch
+
+    n = 10000 if FULL else 20
+    lat = lpc_inputs.supercap(n_steps=n)
+    assert lat.shape == (2048, 256, 256) and lat.bc == (1, 0, 0)
+    gpu, orc = _pair(lpc, oracle_mod, lat, n, 0)
+    gpu.step(n)
+    orc.step(n)
+    _report(f"config3 2048x256x256 {n} steps", _check(lpc, lat, gpu, orc, n, what="config3"))
+    assert np.abs(gpu.fid()).max() <= 1 + 1e-12
+    del gpu, orc
+    torch.cuda.empty_cache()
+
+
+# ---------------------------------------------------------------------------------------------
+# BASELINE configs[4]: every sweep size, both precisions, 50 steps against the oracle (SURVEY 8(d) "Parity runs"), in the
+# launch configuration bench.py times (kernel AUTO).  64^3 .. 256^3 element by element; 512^3 on sampled sites below.
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision", [0, 1])
+@pytest.mark.parametrize("L,nm", [(64, 0), (128, 0), (128, 3), (256, 0)])
+def test_sweep_sizes_50_steps(lpc, oracle_mod, L, nm, precision):
+    n = 50
+    lat = lpc_inputs.sweep(L, n_moments=nm, n_steps=n)
+    gpu, orc = _pair(lpc, oracle_mod, lat, n, 0, precision=precision)
+    gpu.step(n)
+    orc.step(n)
+    tol_site, tol_sum = (1e-5, 1e-5) if precision else (1e-10, 1e-9)
+    _report(f"sweep {L}^3 m{nm} {'fp32' if precision else 'fp64'} {n} steps",
+            _check(lpc, lat, gpu, orc, n, tol_site=tol_site, tol_sum=tol_sum, what=f"sweep {L} p{precision}"))
 
 
 # ---------------------------------------------------------------------------------------------
@@ -641,8 +696,20 @@ def test_bench_size_properties(lpc):
     torch.cuda.empty_cache()
 
 
-def test_bench_workload_sampled_sites_against_oracle(lpc, oracle_mod):
-    """The bench workload itself (512^3 sweep lattice, launch configuration of bench.py), sampled outputs.
+_SWEEP512 = {}
+
+
+def _sweep512():
+    """The bench lattice, generated once per test session (the 512^3 pore field takes a while)."""
+    if "lat" not in _SWEEP512:
+        _SWEEP512["lat"] = lpc_inputs.sweep(512)
+    return _SWEEP512["lat"]
+
+
+@pytest.mark.parametrize("precision", [0, 1])
+def test_bench_workload_sampled_sites_against_oracle(lpc, oracle_mod, precision):
+    """The bench workload itself (512^3 sweep lattice, launch configuration of bench.py, fp64 and fp32), sampled outputs
+    after 50 steps.
 
     g_i(n) depends only on the sites within n hops of i (Eq. 13, is a nearest-neighbour
     recurrence) and on dF one site further (Eq. 1).  The oracle therefore reproduces g_i(n) exactly on a
@@ -651,20 +718,24 @@ def test_bench_workload_sampled_sites_against_oracle(lpc, oracle_mod):
     """
     import torch
 
-    L, n = 512, 6
-    lat = lpc_inputs.sweep(L)
-    gpu = lpc.Lattice.from_inputs(lat, max_steps=n)
+    L, n = 512, 50
+    tol = 1e-5 if precision else 1e-10
+    lat = _sweep512()
+    gpu = lpc.Lattice.from_inputs(lat, precision=precision, max_steps=n)
     gpu.step(n)
     g_gpu = gpu.field(lpc.LPC_FIELD_G)
+    G_gpu = gpu.fid()
     del gpu
     torch.cuda.empty_cache()
+    # the reduction agrees with an independent fp64 sum of the field read back
+    assert abs(g_gpu.sum() - G_gpu[-1]) < (1e-6 if precision else 1e-12)
     opn = lat.blocked == 0
     z_full = np.exp(-lat.dF[opn]).sum()
     r = n + 2
     rng = np.random.default_rng(77)
-    sites = [(0, 0, 0), (L - 1, L - 1, L - 1), (0, 255, L - 1), (L - 1, 0, 256), (63, 64, 65), (7, 8, 63), (300, 7, 64)]
-    sites += [tuple(int(v) for v in rng.integers(0, L, 3)) for _ in range(9)]
-    checked = 0
+    sites = [(0, 0, 0), (L - 1, L - 1, L - 1), (0, 255, L - 1), (L - 1, 0, 256), (63, 64, 65), (7, 8, 63), (300, 7, 64), (31, 15, 127), (32, 16, 128)]
+    sites += [tuple(int(v) for v in rng.integers(0, L, 3)) for _ in range(7)]
+    worst = 0.0
     for c in sites:
         # nearest open site along z so that the sample carries a value
         while lat.blocked[c]:
@@ -678,10 +749,57 @@ def test_bench_workload_sampled_sites_against_oracle(lpc, oracle_mod):
         want = orc.g()[r, r, r] * (z_box / z_full)
         pi_c = np.exp(-lat.dF[c]) / z_full
         err = abs(g_gpu[c] - want) / pi_c
-        assert err <= 1e-10, f"site {c}: scaled error {err:.3e}"
+        assert err <= tol, f"site {c}: scaled error {err:.3e}"
         assert abs(want) > 0
-        checked += 1
-    assert checked == len(sites)
+        worst = max(worst, err)
+    _report(f"sweep 512^3 {'fp32' if precision else 'fp64'} {n} steps, {len(sites)} sampled sites", {"err_g": worst})
+
+
+# ---------------------------------------------------------------------------------------------
+# the features next to the step (regional FID inside the sweep, equilibration sweep, x-slabs) on a lattice of several
+# waves of CTAs (192 x 256 x 512: 1536 tiles-by-chunks on 296 resident CTAs), against the oracle
+# ---------------------------------------------------------------------------------------------
+def test_features_at_several_waves_against_oracle(lpc, oracle_mod):
+    from paper_2603_22553_b200 import slab
+
+    n, nreg = 12, 3
+    shape = (192, 256, 512)
+    lat = lpc_inputs.supercap(*shape, n_steps=n)          # reflective x, electrodes | bulk | electrodes
+    x = np.arange(lat.nx)[:, None, None] * np.ones(lat.shape, dtype=np.int64)
+    region = np.where(x < lat.nx * 3 // 8, 0, np.where(x < lat.nx * 5 // 8, 1, 2)).astype(np.uint8)
+    orc = oracle_mod.Oracle.from_lattice(lat, n_moments=0, max_steps=n)
+    Gr_o = orc.step_with_regions(region, nreg, n)
+    G_o, sabs = orc.fid(with_scale=True)
+    g_o, pi = orc.g(), orc.pi()
+    opn = lat.blocked == 0
+    for precision, tol_sum, tol_site in ((0, 1e-9, 1e-10), (1, 1e-5, 1e-5)):
+        gpu = lpc.Lattice.from_inputs(lat, precision=precision, max_steps=n, n_regions=nreg)
+        gpu.set_regions(region)
+        assert gpu.bytes_per_site_step == (4 if precision else 8) * 7 + 1      # the labels ride on the sweep
+        gpu.step(n)
+        for r in range(nreg):
+            assert np.max(np.abs(gpu.fid_region(r) - Gr_o[r]) / sabs) <= tol_sum, f"region {r} p{precision}"
+        assert np.max(np.abs(gpu.fid() - G_o) / sabs) <= tol_sum
+        assert np.max(np.abs(gpu.field(lpc.LPC_FIELD_G) - g_o)[opn] / pi[opn]) <= tol_site
+        gpu.close()
+    # the same lattice as three x-slabs (plane exchange after every step), sums of the slabs' series
+    ss = slab.SlabSet(lat.shape, bc=lat.bc, slabs_per_rank=3, dt=lat.dt, a=lat.a, alpha=lat.alpha, max_steps=n)
+    ss.set_site_params(lat.dF, lat.blocked, lat.omega)
+    ss.step(n)
+    assert np.max(np.abs(ss.fid() - G_o) / sabs) <= 1e-9
+    assert np.max(np.abs(ss.gather_field(lpc.LPC_FIELD_G, dtype=np.complex128) - g_o)[opn] / pi[opn]) <= 1e-10
+    del ss
+    # five sweeps of the equilibration loop from a random density, delta of every sweep
+    rng = np.random.default_rng(6)
+    rho0 = rng.random(lat.shape) * opn
+    rho0 /= rho0.sum()
+    rho_o, it_o, deltas = orc.equilibrate(rho0, 0.0, 5)
+    eq = lpc.Lattice.from_inputs(lat, n_density=1, max_steps=2)
+    eq.set_state(lpc.LPC_FIELD_RHO, rho0)
+    for k in range(5):
+        it, d = eq.equilibrate(0.0, 1, 1)
+        assert it == 1 and abs(d - deltas[k]) <= 1e-10 * rho0.max(), k
+    assert np.max(np.abs(eq.field(lpc.LPC_FIELD_RHO) - rho_o)) <= 1e-10 * rho0.max()
 
 
 # ---------------------------------------------------------------------------------------------
@@ -752,11 +870,15 @@ def test_slabs_match_unsplit_lattice_and_oracle(lpc, oracle_mod, bc, n_slabs, ke
     if direct:
         # the sweeps store their outermost planes into the neighbours' ghost planes themselves: nothing is copied
         assert ss.enable_direct_stores() == len(slab.messages(n_slabs, lat.bc[0] == 0))
-        ss.exchange = lambda which, after_step=False, _ex=ss.exchange: _ex(which, after_step) if not after_step else None
     orc = oracle_mod.Oracle.from_lattice(lat, n_moments=3, max_steps=n)
     orc.set_g(g0)
     assert abs(ss.fid()[0] - orc.fid()[0]) <= tol_sum * np.abs(g0).sum()
+    before = dict(ss.stats)
     ss.step(n)
+    if direct:
+        assert ss.stats == before      # the unpatched driver found nothing left to copy after any step
+    else:
+        assert ss.stats["copies"] - before["copies"] == n * len(slab.messages(n_slabs, lat.bc[0] == 0))
     orc.step(n)
     pi = orc.pi()
     opn = lat.blocked == 0

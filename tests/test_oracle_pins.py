@@ -562,9 +562,10 @@ def test_p7_trajectory_enumeration(oracle_mod, shape, bc, n, alpha):
     assert np.allclose(D, D_def, rtol=1e-10, atol=1e-10 * abs(D_def).max())
 
 
-def test_p7_dense_matrix_power_4cubed(oracle_mod):
-    """4^3: G[n] = 1^T (Phi W)^n pi with W built entry by entry from the move table."""
-    lat = lpc_inputs.config0(L=4, n_steps=50)
+def _dense_step_matrices(lat):
+    """The one-step matrices on a tiny lattice, entry by entry from the move table: W[j, i] = P(i -> j) (Eq. 1 with the
+    rest term) and Phi = diag(exp(i omega_i dt)) (Eq. 13 prefactor, :144).  Blocked sites have no moves:
+    their rows and columns are zero."""
     moves = _moves(lat)
     N = lat.n_sites
     flat = lambda idx: (idx[0] * lat.ny + idx[1]) * lat.nz + idx[2]
@@ -573,6 +574,13 @@ def test_p7_dense_matrix_power_4cubed(oracle_mod):
         for tgt, p, _ in lst:
             W[flat(tgt), flat(src)] += p
     Phi = np.diag(np.exp(1j * lat.omega.reshape(-1) * lat.dt))
+    return W, Phi
+
+
+def test_p7_dense_matrix_power_4cubed(oracle_mod):
+    """4^3: G[n] = 1^T (Phi W)^n pi with W built entry by entry from the move table."""
+    lat = lpc_inputs.config0(L=4, n_steps=50)
+    W, Phi = _dense_step_matrices(lat)
     v = _boltzmann(lat).reshape(-1).astype(complex)
     o = _mk(oracle_mod, lat)
     o.step(50)
@@ -581,6 +589,63 @@ def test_p7_dense_matrix_power_4cubed(oracle_mod):
         assert abs(G[n] - v.sum()) < 1e-13
         v = Phi @ (W @ v)
     assert np.max(np.abs(o.g().reshape(-1) - np.linalg.matrix_power(Phi @ W, 50) @ _boltzmann(lat).reshape(-1))) < 1e-15
+
+
+@pytest.mark.parametrize("shape,bc", [((4, 4, 4), (0, 0, 0)), ((3, 2, 4), (1, 0, 1))])
+def test_p18_set_g_against_dense_power(oracle_mod, shape, bc):
+    """lpco_set_g (an arbitrary initial magnetisation): Eq. 13 is linear, so from any complex g(0) the
+    state is (Phi W)^n g(0) and G[n] = 1^T (Phi W)^n g(0) (Eq. 12, :137).  g(0) has unrelated real and imaginary parts
+    (a re/im swap fails), non-zero values on blocked sites (they must be dropped: carbon holds no fluid, :47-55) and the
+    series must restart (G[0] = sum of g(0) over open sites, steps = 0) although steps were taken before."""
+    n = 12
+    lat = lpc_inputs.random_small(shape, bc=bc, p_block=0.25, alpha=0.8, seed=13, n_steps=n)
+    lat.dt = 2.0e-5
+    assert lat.blocked.any()
+    W, Phi = _dense_step_matrices(lat)
+    rng = np.random.default_rng(4)
+    g0 = rng.standard_normal(shape) * np.array(3.0) + 1j * (0.25 + rng.random(shape))   # |re| and im of different size and sign pattern
+    o = _mk(oracle_mod, lat, max_steps=n)
+    o.step(5)                                   # a series that set_g has to discard
+    o.set_g(g0)
+    assert o.steps == 0
+    opn = (lat.blocked == 0).reshape(-1)
+    v = np.where(opn, g0.reshape(-1), 0.0)
+    assert np.array_equal(o.g().reshape(-1), v)          # blocked sites zeroed, open ones taken as they are
+    G, sabs = o.fid(with_scale=True)
+    assert G.shape == (1,) and abs(G[0] - v.sum()) < 1e-14 * np.abs(v).sum()
+    assert abs(sabs[0] - np.abs(v).sum()) < 1e-14 * np.abs(v).sum()
+    o.step(n)
+    G, sabs = o.fid(with_scale=True)
+    scale = np.abs(v).sum()
+    for k in range(n + 1):
+        assert abs(G[k] - v.sum()) < 1e-14 * scale, k
+        assert abs(sabs[k] - np.abs(v).sum()) < 1e-14 * scale, k
+        if k == n:
+            assert np.max(np.abs(o.g().reshape(-1) - v)) < 1e-14 * np.abs(g0).max()
+            assert np.all(o.g().reshape(-1)[~opn] == 0)
+        v = Phi @ (W @ v)
+
+
+def test_p19_tolerance_scale_series_against_dense_power(oracle_mod):
+    """The sum_i |g_i(n)| series of the oracle is the denominator of every FID tolerance (SURVEY
+    Q12): it must be exactly sum_i |((Phi W)^n pi)_i|, not an upper bound of it.  Dense power on 4^3 with the chemical
+    shifts of configs[0] stretched so that the sites dephase and the series falls well below 1 (an oracle that returned
+    |G|, sum |Re g| + |Im g|, or the constant 1 fails)."""
+    lat = lpc_inputs.config0(L=4, n_steps=60)
+    lat.dt = 2.0e-5
+    W, Phi = _dense_step_matrices(lat)
+    v = _boltzmann(lat).reshape(-1).astype(complex)
+    o = _mk(oracle_mod, lat)
+    o.step(60)
+    G, sabs = o.fid(with_scale=True)
+    for n in range(61):
+        assert abs(sabs[n] - np.abs(v).sum()) < 1e-14, n
+        if n < 60:
+            v = Phi @ (W @ v)
+    # the case separates the candidates: each plausible wrong series is far outside the 1e-14 the right one meets
+    assert sabs[60] < 0.98
+    assert abs(G[60]) < 0.95 * sabs[60]
+    assert np.abs(v.real).sum() + np.abs(v.imag).sum() > 1.05 * sabs[60]
 
 
 # --------------------------------------------------------------------------
