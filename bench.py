@@ -64,6 +64,12 @@ def parse():
                    help="with --slabs: let the sweeps store their outermost planes into the neighbours' ghost planes themselves "
                         "(lpc_set_halo_peers; other ranks' workspaces are mapped through CUDA IPC) instead of copying / sending them "
                         "after the sweep")
+    p.add_argument("--sustained-s", type=float, default=2.0,
+                   help="after the K timed steps, time a further block of about this many seconds (at least 200 steps) with its own "
+                        "clock record: the rate under the board's power cap (0 = skip)")
+    p.add_argument("--time-block", type=int, default=0, choices=[0, 1, 2],
+                   help="LPC_OPT_TIME_BLOCK: 0 auto (two time steps per sweep where the lattice allows it), 1 one step per sweep, 2 two")
+    p.add_argument("--print-csrc-hash", action="store_true", help="print the hash profiles/traffic.csv is stamped with and exit")
     p.add_argument("--no-cpu-baseline", action="store_true")
     p.add_argument("--no-e2e", action="store_true")
     p.add_argument("--ref-sample-size", type=int, default=int(os.environ.get("LPC_REF_SAMPLE_L", "256")),
@@ -107,15 +113,67 @@ def make_workload(args):
     return lpc_inputs.supercap(n_moments=args.moments)
 
 
+def csrc_hash():
+    """Hash of the CUDA sources the library is built from.  profiles/traffic.csv carries the hash of the sources its ncu
+    captures were taken with; a row with another hash is stale and `roofline.traffic` is reported as null."""
+    import hashlib
+
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_2603_22553_b200", "csrc")
+    for name in sorted(os.listdir(csrc)):
+        if name.endswith((".cu", ".cuh")):
+            h.update(name.encode())
+            h.update(open(os.path.join(csrc, name), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def committed_traffic(key):
+    """dram read + write bytes per launch (and launches per step) of the step kernel from the committed `ncu --set full`
+    capture: profiles/traffic.csv rows are key,dram_bytes_per_step,csrc_hash,source.  None when missing or stale."""
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(tpath):
+        return None
+    want = csrc_hash()
+    for row in open(tpath):
+        cols = row.strip().split(",")
+        if len(cols) >= 3 and cols[0] == key and cols[2] == want:
+            return float(cols[1])
+    return None
+
+
 # --------------------------------------------------------------------------------------------
 # CPU oracle timing (cpu_baseline leg and --impl reference)
 # --------------------------------------------------------------------------------------------
-def oracle_sample(moments, steps=None, warmup=1, budget_s=12.0, L=256):
-    """Time the oracle on a bounded sample of the workload: an L^3 lattice with the same statistics."""
+def _omp_set_threads(n):
+    """Thread count of the OpenMP runtime the oracle library uses (the oracle itself is not touched)."""
+    import ctypes
+
+    try:
+        ctypes.CDLL("libgomp.so.1").omp_set_num_threads(int(n))
+        return True
+    except OSError:
+        return False
+
+
+def oracle_sample(moments, steps=None, warmup=1, budget_s=12.0, L=256, lat=None, threads=None):
+    """Time the oracle on a bounded sample of the workload: an L^3 lattice with the same statistics (or `lat` itself)."""
     orc_mod = load_oracle()
-    lat = lpc_inputs.sweep(L, n_moments=moments)
+    if lat is None:
+        lat = lpc_inputs.sweep(L, n_moments=moments)
+    cores_all = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    if threads is not None and not _omp_set_threads(threads):
+        return None, 0, 0.0
+    try:
+        return _oracle_sample(orc_mod, lat, moments, steps, warmup, budget_s, threads if threads is not None else cores_all)
+    finally:
+        if threads is not None:
+            _omp_set_threads(cores_all)
+
+
+def _oracle_sample(orc_mod, lat, moments, steps, warmup, budget_s, cores):
+    L = lat.nx
     cap = 100000
-    o = orc_mod.Oracle.from_lattice(lat, max_steps=cap)
+    o = orc_mod.Oracle.from_lattice(lat, n_moments=moments, max_steps=cap)
     o.step(warmup)
     if steps is None:
         t0 = time.perf_counter()
@@ -125,12 +183,25 @@ def oracle_sample(moments, steps=None, warmup=1, budget_s=12.0, L=256):
     t0 = time.perf_counter()
     o.step(steps)
     dt = time.perf_counter() - t0
-    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    o.close()
     return {
         "value": lat.n_sites * steps / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
-        "sample": f"{L}^3 sub-lattice with the workload's statistics, {steps} steps after {warmup} warm-up "
-                  f"(oracle/lpc_oracle.c, gcc -O2 -fopenmp, {dt:.1f} s)",
+        "sample": f"{lat.nx}x{lat.ny}x{lat.nz} lattice with the workload's statistics, {steps} steps after {warmup} warm-up "
+                  f"(oracle/lpc_oracle.c, gcc -O2 -fopenmp, {cores} thread(s), {dt:.1f} s)",
     }, steps, dt
+
+
+def cpu_baseline_record(args, lat):
+    """the oracle as it stands on the box's host cores -- OpenMP on all cores on the workload's own
+    lattice (>= 3 steps at 512^3), plus the 256^3 sample with all cores and single-threaded.  About 20-30 s in all."""
+    full, _, _ = oracle_sample(args.moments, steps=3, warmup=1, lat=lat)
+    rec = dict(full)
+    small, _, _ = oracle_sample(args.moments, budget_s=6.0, L=args.ref_sample_size)
+    rec["sample_256"] = {k: small[k] for k in ("value", "cores", "sample")}
+    single, _, _ = oracle_sample(args.moments, budget_s=5.0, L=min(args.ref_sample_size, 128), threads=1)
+    if single is not None:
+        rec["single_thread"] = {k: single[k] for k in ("value", "cores", "sample")}
+    return rec
 
 
 def run_reference(args):
@@ -216,10 +287,13 @@ def run_ours(args):
     host = [torch.from_numpy(a).pin_memory() for a in (lat.dF, lat.blocked, lat.omega)]
     h2d_job = sum(t.numel() * t.element_size() for t in host)
 
+    sus_cap = 20000 if args.sustained_s > 0 else 0
     sim = lpc.Lattice(lat.shape, bc=lat.bc, precision=args.precision, n_moments=args.moments, dt=lat.dt, a=lat.a,
-                      alpha=lat.alpha, max_steps=2 * K + W + 8, device=dev, link_mobility=1 if args.links else 0,
+                      alpha=lat.alpha, max_steps=2 * K + W + 8 + sus_cap, device=dev, link_mobility=1 if args.links else 0,
                       n_regions=args.regions)
     sim.set_kernel(args.kernel)
+    if args.time_block:
+        sim.set_option(lpc.LPC_OPT_TIME_BLOCK, args.time_block)
     link = None
     if args.links:
         # reduced mobility under confinement: every link that touches a porous (dF != 0) site
@@ -286,6 +360,30 @@ def run_ours(args):
     ms = ev0.elapsed_time(ev1)
     launches = sim.launch_count - l0
     value, ms_max = replicas.aggregate_glups(n_sites * K, ms, dev)
+
+    # ---- sustained block: the same loop for about args.sustained_s seconds, its own events and clock record.  The
+    # metric is "seconds per time step of propagation" over a long run: under the board's power cap the SM
+    # clock settles below the burst clock of a 20-step run.
+    sustained = None
+    if args.sustained_s > 0:
+        n_sus = int(max(200, min(sus_cap, args.sustained_s / max(ms / K * 1e-3, 1e-7))))
+        n_sus -= n_sus % 2
+        sampler2 = ClockSampler(local)
+        sampler2.start()
+        time.sleep(0.25)
+        es0, es1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        ts0 = time.perf_counter()
+        es0.record()
+        lpc.lpc_step_n(sim.handle, n_sus)
+        es1.record()
+        barrier()
+        ts1 = time.perf_counter()
+        clocks2 = sampler2.stop(ts0, ts1)
+        ms_sus = es0.elapsed_time(es1)
+        v_sus, ms_sus_max = replicas.aggregate_glups(n_sites * n_sus, ms_sus, dev)
+        sustained = {"steps": n_sus, "value": v_sus, "unit": UNIT, "ms_per_step": ms_sus_max / n_sus, "kernel_ms": ms_sus / n_sus,
+                     "clocks": clocks2}
     fid = sim.fid()
     assert np.isfinite(fid).all() and abs(fid[0] - 1.0) < (1e-4 if args.precision else 1e-12), "FID series is not sane"
 
@@ -301,20 +399,17 @@ def run_ours(args):
         # the step / time of the step.
         ms_kernel = ms / K                 # this rank's own time per step
         achieved = bps * n_sites / (ms_kernel * 1e-3) / 1e9
-        traffic = None
-        # dram read + write bytes per launch of the step kernel, from the committed `ncu --set full` capture
-        # (profiles/traffic.csv: key,dram_bytes_per_launch,source)
-        tpath = os.path.join(ROOT, "profiles", "traffic.csv")
-        if os.path.exists(tpath):
-            key = f"{L}^3/m{args.moments}/p{args.precision}" if args.workload == "sweep" else f"{args.workload}/m{args.moments}/p{args.precision}"
-            if args.links:
-                key += "/links"
-            if args.regions:
-                key += "/regions"
-            for row in open(tpath):
-                cols = row.strip().split(",")
-                if cols and cols[0] == key:
-                    traffic = float(cols[1])
+        # dram read + write bytes per LAUNCH of the dominant kernel from the committed `ncu --set full` capture of this very
+        # source tree (profiles/traffic.csv is stamped with csrc_hash(); a stale row reads as null)
+        key = f"{L}^3/m{args.moments}/p{args.precision}" if args.workload == "sweep" else f"{args.workload}/m{args.moments}/p{args.precision}"
+        if args.links:
+            key += "/links"
+        if args.regions:
+            key += "/regions"
+        if args.time_block == 1:
+            key += "/tb1"
+        traffic = committed_traffic(key)
+        steps_per_launch = K / max(launches, 1)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -329,13 +424,22 @@ def run_ours(args):
             "clocks": clocks,
             "e2e": e2e,
             "gpu_launches": int(launches),
+            # achieved = algorithmic bytes of the ONE-STEP-PER-SWEEP layout (56 B per site update in fp64) x site
+            # updates per launch / launch duration.  With two time steps per sweep a launch updates every site twice, so
+            # this EFFECTIVE rate can exceed the HBM peak; `dram` is what actually crossed HBM (ncu traffic / launch time).
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": traffic, "peak_source": peak_src, "bytes_per_site_step": bps,
-                         "kernel_ms": ms_kernel, "launches_per_step": launches / K,
+                         "kernel_ms": ms_kernel * steps_per_launch, "launches_per_step": launches / K,
+                         "time_steps_per_launch": steps_per_launch,
+                         "dram_gbs": (traffic / (ms_kernel * steps_per_launch * 1e-3) / 1e9) if traffic else None,
                          "frac_of_8TBs_spec": achieved / 8000.0},
         }
+        if sustained is not None:
+            a_sus = bps * n_sites / (sustained["kernel_ms"] * 1e-3) / 1e9
+            sustained["roofline"] = {"achieved": a_sus, "frac": a_sus / peak, "frac_of_8TBs_spec": a_sus / 8000.0}
+            line["sustained"] = sustained
         if world == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"] = oracle_sample(args.moments, L=args.ref_sample_size)[0]
+            line["cpu_baseline"] = cpu_baseline_record(args, lat) if args.workload == "sweep" else oracle_sample(args.moments, L=args.ref_sample_size)[0]
         print(json.dumps(line))
     if world > 1:
         dist.barrier()
@@ -417,6 +521,9 @@ def run_slabs(args, lat, lpc, world, rank, local, dev):
 
 def main():
     args = parse()
+    if args.print_csrc_hash:
+        print(csrc_hash())
+        return
     if args.impl == "reference":
         run_reference(args)
     else:

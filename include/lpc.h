@@ -66,6 +66,13 @@ extern "C" {
 #define LPC_KERNEL_PERSIST 3 /* all n steps of lpc_step_n in one cooperative launch, grid barrier
                                 between steps; for lattices that stay in L2 (launch-bound otherwise) */
 
+/* lpc_set_option keys */
+#define LPC_OPT_TIME_BLOCK 1     /* 0 auto (default), 1 one time step per sweep, 2 two time steps per sweep        */
+#define LPC_OPT_X_CHUNK 2        /* planes per x chunk of the one-step TMA sweeps; 0 = the library's choice         */
+#define LPC_OPT_X_CHUNK2 3       /* planes per x chunk of the two-step sweep; 0 = the library's choice              */
+#define LPC_OPT_PERSIST_MAX_MB 4 /* AUTO takes the persistent kernel up to this many MiB per step; 0 = 48           */
+#define LPC_OPT_REGION_FUSION 5  /* 0 regional sums inside the sweep when possible (default), 1 separate pass       */
+
 typedef struct lpc_lattice lpc_lattice; /* opaque, host struct owned by the library */
 
 typedef struct lpc_config {
@@ -128,7 +135,13 @@ int lpc_set_site_params(lpc_lattice* lat, const double* dF_kT, const uint8_t* bl
 int lpc_set_link_mobility(lpc_lattice* lat, const double* alpha_link);
 
 /* Advance n time steps (north star (b), (c); Eq. 13 + Eq. 12, Eq. 4): per step one fused sweep
- * that propagates, phase-rotates, reduces G[n] and (if enabled) Z_d[n+1], P^d, rho.
+ * that propagates, phase-rotates, reduces G[n] and (if enabled) Z_d[n+1], P^d, rho.  Eq. 13 is a
+ * Jacobi update (its right-hand side is at n-1), so a lattice that carries the
+ * magnetisation alone (n_moments = n_density = 0, no link factors, no region labels, not a slab,
+ * periodic axes of length >= 4) takes TWO steps per sweep while at least two are left
+ * ("temporal blocking": state and parameters cross HBM once per two steps; G[n] is still recorded
+ * for every step and the state after the call is bit for bit that of the one-step sweeps);
+ * LPC_OPT_TIME_BLOCK = 1 switches that off.
  * Asynchronous on the stream.  Errors: LPC_ESTATE (no site parameters yet), LPC_EINVAL (n < 0 or
  * steps_done + n > max_steps), LPC_ECUDA.                                                      */
 int lpc_step_n(lpc_lattice* lat, int64_t n);
@@ -263,6 +276,11 @@ int lpc_slab_finish(lpc_lattice* lat);
 /* Choose the step kernel (LPC_KERNEL_*).  AUTO picks PERSIST when one step's state and parameters
  * stay in L2 (<= 48 MB) and no region labels are set, else TMA.  Errors: LPC_EINVAL.             */
 int lpc_set_kernel(lpc_lattice* lat, int32_t which);
+
+/* Tuning and test switches (LPC_OPT_*): how the library schedules the sweeps, never what they
+ * compute.  Takes effect from the next lpc_step_n.  Errors: LPC_EINVAL (unknown key, value out
+ * of range, or LPC_OPT_TIME_BLOCK = 2 on a lattice that cannot run the two-step sweep).          */
+int lpc_set_option(lpc_lattice* lat, int32_t key, int64_t value);
 
 /* Steps taken since the last lpc_set_site_params / lpc_set_state(G).                           */
 int64_t lpc_steps_done(const lpc_lattice* lat);

@@ -24,11 +24,12 @@ LPC_BC_HALO = 2
 LPC_HALO_PARAMS, LPC_HALO_STATE, LPC_HALO_STATE0, LPC_HALO_STATE1 = 0, 1, 2, 3
 LPC_HALO_SEND, LPC_HALO_RECV = 0, 1
 LPC_KERNEL_AUTO, LPC_KERNEL_DIRECT, LPC_KERNEL_TMA, LPC_KERNEL_PERSIST = range(4)
+LPC_OPT_TIME_BLOCK, LPC_OPT_X_CHUNK, LPC_OPT_X_CHUNK2, LPC_OPT_PERSIST_MAX_MB, LPC_OPT_REGION_FUSION = 1, 2, 3, 4, 5
 
 EXPORTS = (
     "lpc_workspace_bytes", "lpc_create_lattice", "lpc_set_site_params", "lpc_set_link_mobility", "lpc_step_n", "lpc_read_fid",
     "lpc_moments", "lpc_read_field", "lpc_set_state", "lpc_equilibrate", "lpc_seed_from_density", "lpc_set_regions", "lpc_read_fid_region", "lpc_moments_region", "lpc_spectrum", "lpc_set_kernel",
-    "lpc_steps_done", "lpc_partition_sum", "lpc_set_partition_sum", "lpc_halo_view", "lpc_set_halo_peers", "lpc_slab_finish",
+    "lpc_set_option", "lpc_steps_done", "lpc_partition_sum", "lpc_set_partition_sum", "lpc_halo_view", "lpc_set_halo_peers", "lpc_slab_finish",
     "lpc_launch_count", "lpc_bytes_per_site_step", "lpc_destroy", "lpc_last_error",
 )
 
@@ -78,6 +79,7 @@ def _load():
     lib.lpc_read_field.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
     lib.lpc_set_state.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
     lib.lpc_set_kernel.argtypes = [C.c_void_p, C.c_int32]
+    lib.lpc_set_option.argtypes = [C.c_void_p, C.c_int32, C.c_int64]
     lib.lpc_equilibrate.argtypes = [C.c_void_p, C.c_double, C.c_int64, C.c_int64, C.POINTER(C.c_int64), C.POINTER(C.c_double)]
     lib.lpc_seed_from_density.argtypes = [C.c_void_p]
     lib.lpc_set_regions.argtypes = [C.c_void_p, C.c_void_p]
@@ -275,6 +277,10 @@ def lpc_set_kernel(handle, which):
     _check(_lib.lpc_set_kernel(handle, int(which)))
 
 
+def lpc_set_option(handle, key, value):
+    _check(_lib.lpc_set_option(handle, int(key), int(value)))
+
+
 def lpc_steps_done(handle) -> int:
     return int(_lib.lpc_steps_done(handle))
 
@@ -421,6 +427,9 @@ class Lattice:
 
     def set_kernel(self, which):
         lpc_set_kernel(self.handle, which)
+
+    def set_option(self, key, value):
+        lpc_set_option(self.handle, key, value)
 
     @property
     def steps_done(self):

@@ -18,6 +18,7 @@
 #include "lpc_internal.cuh"
 #include "lpc_precompute.cuh"
 #include "lpc_step.cuh"
+#include "lpc_step2.cuh"
 #include "lpc_equil.cuh"
 #include "lpc_regions.cuh"
 
@@ -79,6 +80,14 @@ struct lpc_lattice {
   long long steps;
   long long launches;
   int kernel;  // LPC_KERNEL_*
+  int device;  // CUDA device ordinal of the workspace
+  // two-step sweep (lpc_step2.cuh)
+  bool step2_ok;      // the lattice can run it (geometry, channels, boundary conditions)
+  int time_block;     // LPC_OPT_TIME_BLOCK: 0 auto, 1 one step per sweep, 2 two steps per sweep whenever possible
+  int xc2, chunks_x2; // its x chunks
+  bool ghosts_full;   // the whole ghost shell of the current state is valid (the one-step sweeps keep the face layer only)
+  CUtensorMap tm2_f[2], tm2_pi, tm2_cs;
+  int opt_xc, opt_persist_mb, opt_region_fusion;   // lpc_set_option overrides (0 = default)
   // TMA geometry
   int ty, tz, nstage, xc, tiles_z, tiles_y, chunks_x;
   bool tma_ok;
@@ -113,8 +122,9 @@ Layout make_layout(const lpc_config* c) {
   const int sT = c->precision ? 4 : 8;
   L.nx = c->nx; L.ny = c->ny; L.nz = c->nz;
   L.padz = 128 / sT;  // 128 bytes of ghost columns on each side keep every row 128-byte aligned
-  L.nxp = c->nx + 2;
-  L.nyp = c->ny + 2;
+  L.gh = GH;
+  L.nxp = c->nx + 2 * GH;
+  L.nyp = c->ny + 2 * GH;
   L.nzp = (c->nz + L.padz - 1) / L.padz * L.padz + 2 * L.padz;
   L.sy = L.nzp;
   L.sx = (long long)L.nyp * L.nzp;
@@ -127,7 +137,7 @@ Layout make_layout(const lpc_config* c) {
 // and slightly worse at 256^3, so there is one tile shape.)
 constexpr int SM_COUNT = 148;
 
-void tma_geometry(int C, bool f32, int nx, int ny, int nz, int* ty, int* tz, int* nstage, int* xc, int* tiles_z, int* tiles_y, int* chunks_x) {
+void tma_geometry(int C, bool f32, int nx, int ny, int nz, int xc_override, int* ty, int* tz, int* nstage, int* xc, int* tiles_z, int* tiles_y, int* chunks_x) {
   *ty = f32 ? 16 : 8; *tz = 64;   // fp32: a thread owns a z-quad (lpc_step_vec.cuh), 256 threads cover 16 rows
   *nstage = 4;   // 3 when the density rides along (3 channels); informational, the kernels fix it
   *tiles_z = (nz + *tz - 1) / *tz;
@@ -158,10 +168,17 @@ void tma_geometry(int C, bool f32, int nx, int ny, int nz, int* ty, int* tz, int
     }
     chunks = best;
   }
-  if (const char* e = getenv("LPC_XC")) {
-    const int v = atoi(e);
-    if (v > 0) chunks = (nx + v - 1) / v;
-  }
+  if (xc_override > 0) chunks = (nx + xc_override - 1) / xc_override;   // LPC_OPT_X_CHUNK
+  *xc = (int)((nx + chunks - 1) / chunks);
+  *chunks_x = (nx + *xc - 1) / *xc;
+}
+
+// x chunks of the two-step sweep: one CTA per SM; a chunk costs its planes + 4 halo planes of loads and 3 iterations of
+// pipeline fill, so chunks are long (64 planes) unless the lattice has too few tiles to give every SM a CTA
+void step2_geometry(int nx, long long tiles, int xc_override, int* xc, int* chunks_x) {
+  long long chunks = std::max(1, (nx + 32) / 64);
+  if (tiles * chunks < SM_COUNT) chunks = std::min<long long>(std::max(1, nx / 8), (SM_COUNT + tiles - 1) / tiles);
+  if (xc_override > 0) chunks = (nx + xc_override - 1) / xc_override;
   *xc = (int)((nx + chunks - 1) / chunks);
   *chunks_x = (nx + *xc - 1) / *xc;
 }
@@ -171,8 +188,8 @@ Offsets make_offsets(const lpc_config* c, const Layout& L) {
   const size_t sT = c->precision ? 4 : 8;
   const int C = 2 + c->n_density + c->n_moments;
   int ty, tz, ns, xc, tzs, tys, cxs;
-  tma_geometry(C, c->precision == 1, c->nx, c->ny, c->nz, &ty, &tz, &ns, &xc, &tzs, &tys, &cxs);
-  // the LPC_XC override may only shrink chunks at run time; size for the worst case (one plane per chunk)
+  tma_geometry(C, c->precision == 1, c->nx, c->ny, c->nz, 0, &ty, &tz, &ns, &xc, &tzs, &tys, &cxs);
+  // LPC_OPT_X_CHUNK may shrink the chunks at run time; size for the worst case (one plane per chunk)
   const size_t tma_blocks = (size_t)tzs * tys * (size_t)c->nx;
   o.partial_slots = std::max<size_t>(std::max<size_t>(DIRECT_MAX_BLOCKS, AUX_BLOCKS), std::min<size_t>(tma_blocks, 1u << 20));
   const long long N = (long long)c->nx * c->ny * c->nz;
@@ -249,13 +266,25 @@ int aux_grid(long long n) { return (int)std::max<long long>(1, std::min<long lon
 
 // the regional FID can ride on the TMA magnetisation sweep when there is no density channel next to it
 bool regions_fusable(const lpc_lattice* h) {
-  return h->have_regions && h->nrho == 0 && h->tma_ok && h->kernel != LPC_KERNEL_DIRECT && !getenv("LPC_NO_REGION_FUSION");
+  return h->have_regions && h->nrho == 0 && h->tma_ok && h->kernel != LPC_KERNEL_DIRECT && !h->opt_region_fusion;
 }
 
 // what launch_step_t will decide for the next step: regional sums inside the TMA sweeps (not with direct halo stores)
 bool will_fuse_regions(const lpc_lattice* h) {
   const bool peers = h->peer[0][h->cur ^ 1] || h->peer[1][h->cur ^ 1];
   return regions_fusable(h) && !peers;
+}
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device setting: remember per kernel AND device that it is made
+// (several lattices on several GPUs may live in one process)
+constexpr int MAX_DEVICES = 64;
+template <typename Kern>
+int ensure_dyn_smem(Kern kern, int bytes, int device, bool (&done)[MAX_DEVICES]) {
+  if (device < 0 || device >= MAX_DEVICES || !done[device]) {
+    CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    if (device >= 0 && device < MAX_DEVICES) done[device] = true;
+  }
+  return LPC_OK;
 }
 
 // ---- launch of one sweep ---------------------------------------------------------------------
@@ -279,6 +308,7 @@ int launch_step_t(lpc_lattice* h) {
   a.xc = h->xc; a.tiles_z = h->tiles_z; a.tiles_y = h->tiles_y; a.chunks_x = h->chunks_x;
 
   const bool use_tma = h->tma_ok && h->kernel != LPC_KERNEL_DIRECT;
+  h->ghosts_full = false;   // a one-step sweep renews the face layer of the ghosts only
   // slab mode with direct halo stores: the sweep writes into the buffer the neighbours write in this step (all slabs
   // step together, so that is their buffer cur ^ 1 as well)
   for (int s = 0; s < 2; ++s) {
@@ -304,11 +334,8 @@ int launch_step_t(lpc_lattice* h) {
     const unsigned grid = (unsigned)(h->tiles_z * h->tiles_y * h->chunks_x);
     auto launch = [&](auto kern, auto cfg, const CUtensorMap& tm, const StepArgs<T>& args) -> int {
       using K = decltype(cfg);
-      static bool attr_set = false;
-      if (!attr_set) {
-        CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, K::SMEM_BYTES));
-        attr_set = true;
-      }
+      static bool attr_done[MAX_DEVICES] = {};
+      if (int rc = ensure_dyn_smem(kern, K::SMEM_BYTES, h->device, attr_done)) return rc;
       kern<<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(tm, h->tm_pi, h->tm_cs, args);
       CUDA_TRY(cudaGetLastError());
       h->launches++;
@@ -322,11 +349,8 @@ int launch_step_t(lpc_lattice* h) {
     // stage less where the link boxes would not leave room for two CTAs per SM.
     auto launch_links = [&](auto kern, auto cfg, const CUtensorMap& tm, const StepArgs<T>& args) -> int {
       using K = decltype(cfg);
-      static bool attr_set = false;
-      if (!attr_set) {
-        CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, K::SMEM_BYTES));
-        attr_set = true;
-      }
+      static bool attr_done[MAX_DEVICES] = {};
+      if (int rc = ensure_dyn_smem(kern, K::SMEM_BYTES, h->device, attr_done)) return rc;
       kern<<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(tm, h->tm_cs, h->tm_l, args);
       CUDA_TRY(cudaGetLastError());
       h->launches++;
@@ -406,9 +430,14 @@ int launch_persist_t(lpc_lattice* h, int64_t n) {
   a.vacfr = nullptr; a.wr = nullptr; a.vacfr_stride = 0;
   a.c0 = 0; a.xc = 0; a.tiles_z = a.tiles_y = a.chunks_x = 0;
   auto kern = step_persist_kernel<T, NRHO, NMOM>;
-  static int per_sm = 0;
-  if (!per_sm) CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 256, 0));
+  static int per_sm_dev[MAX_DEVICES] = {};
+  int per_sm = (h->device >= 0 && h->device < MAX_DEVICES) ? per_sm_dev[h->device] : 0;
+  if (!per_sm) {
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 256, 0));
+    if (h->device >= 0 && h->device < MAX_DEVICES) per_sm_dev[h->device] = per_sm;
+  }
   if (per_sm < 1) return fail(LPC_ECUDA, "the persistent kernel does not fit on an SM");
+  h->ghosts_full = false;
   const long long npairs = (long long)((h->L.nz + 1) / 2) * h->L.ny * h->L.nx;
   const int grid = (int)std::max<long long>(1, std::min<long long>({(npairs + 255) / 256, (long long)per_sm * SM_COUNT, (long long)PERSIST_MAX_BLOCKS}));
   unsigned long long* bar = reinterpret_cast<unsigned long long*>(&wsp<Ctl>(h, h->off.ctl)->scratch[6]);
@@ -441,8 +470,7 @@ int launch_persist(lpc_lattice* h, int64_t n) {
 
 // AUTO takes the persistent kernel when one step's state and parameters stay in L2
 bool persist_by_default(const lpc_lattice* h) {
-  long long limit = 48ll << 20;
-  if (const char* e = getenv("LPC_PERSIST_MAX_MB")) limit = (long long)atoll(e) << 20;
+  const long long limit = (long long)(h->opt_persist_mb > 0 ? h->opt_persist_mb : 48) << 20;   // LPC_OPT_PERSIST_MAX_MB
   return (long long)h->N * h->sT * (2 * h->C + 3) <= limit;
 }
 
@@ -508,16 +536,66 @@ int region_moment(lpc_lattice* h) {
 // x ghost planes: 1 wrap (periodic), 0 zero (wall), 2 leave to the caller (slab)
 int xghost_mode(const lpc_lattice* h) { return h->halo ? 2 : (h->cfg.bc[0] == 0 ? 1 : 0); }
 
+// cells of the ghost shell of one channel (fill_ghosts_kernel)
+long long ghost_cells(const Layout& L) {
+  const long long wy = L.ny + 2 * L.gh, wz = L.nz + 2 * GHZ;
+  return 2ll * L.gh * wy * wz + (long long)L.nx * 2 * L.gh * wz + (long long)L.nx * L.ny * 2 * GHZ;
+}
+
 template <typename T>
 int fill_state_ghosts(lpc_lattice* h) {
   const Layout& L = h->L;
-  const long long cells = 2ll * ((long long)L.nx * L.ny + (long long)L.nx * L.nz + (long long)L.ny * L.nz) * h->C;
+  const long long cells = ghost_cells(L) * h->C;
   fill_ghosts_kernel<T><<<aux_grid(cells), 256, 0, h->stream>>>(wsp<T>(h, h->cur ? h->off.f1 : h->off.f0), h->C, L, xghost_mode(h),
                                                                  h->cfg.bc[1] == 0, h->cfg.bc[2] == 0);
   CUDA_TRY(cudaGetLastError());
   h->launches++;
+  h->ghosts_full = true;
   return LPC_OK;
 }
+
+// ---- two time steps in one sweep (lpc_step2.cuh) ----------------------------------------------
+// may the next steps of this lattice run two at a time?
+bool step2_usable(const lpc_lattice* h) {
+  if (!h->step2_ok || h->time_block == 1 || h->have_links || h->have_regions) return false;
+  if (h->kernel == LPC_KERNEL_DIRECT || h->kernel == LPC_KERNEL_PERSIST) return false;
+  return true;
+}
+
+template <typename T>
+int launch_step2_t(lpc_lattice* h) {
+  constexpr int VW = 16 / (int)sizeof(T);
+  using K = Step2Cfg<T, VW>;
+  if (!h->ghosts_full) {   // the sweep reads two ghost layers, edges included
+    int rc = fill_state_ghosts<T>(h);
+    if (rc) return rc;
+  }
+  StepArgs<T> a;
+  memset(&a, 0, sizeof(a));
+  a.L = h->L;
+  a.fin = wsp<T>(h, h->cur ? h->off.f1 : h->off.f0);
+  a.fout = wsp<T>(h, h->cur ? h->off.f0 : h->off.f1);
+  a.pi = wsp<T>(h, h->off.pi);
+  a.cs = wsp<T>(h, h->off.cs);
+  a.a6 = (T)(h->cfg.alpha / 6.0);
+  a.partials = wsp<double>(h, h->off.partials);
+  a.ctl = wsp<Ctl>(h, h->off.ctl);
+  a.fid = wsp<double2>(h, h->off.fid);
+  a.vacf = wsp<double>(h, h->off.vacf);
+  a.vacf_stride = h->cfg.max_steps + 2;
+  for (int d = 0; d < 3; ++d) a.per[d] = h->cfg.bc[d] == 0;
+  a.xc = h->xc2; a.tiles_z = h->tiles_z; a.tiles_y = h->tiles_y; a.chunks_x = h->chunks_x2;
+  static bool attr_done[MAX_DEVICES] = {};
+  if (int rc = ensure_dyn_smem(step2_kernel<T, VW>, K::SMEM_BYTES, h->device, attr_done)) return rc;
+  const unsigned grid = (unsigned)(h->tiles_z * h->tiles_y * h->chunks_x2);
+  step2_kernel<T, VW><<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(h->tm2_f[h->cur], h->tm2_pi, h->tm2_cs, a);
+  CUDA_TRY(cudaGetLastError());
+  h->launches++;
+  h->cur ^= 1;
+  return LPC_OK;   // the sweep stores every ghost image itself: the shell stays valid
+}
+
+int launch_step2(lpc_lattice* h) { return h->cfg.precision ? launch_step2_t<float>(h) : launch_step2_t<double>(h); }
 
 template <typename T>
 int set_g_from(lpc_lattice* h, const void* g) {
@@ -622,11 +700,15 @@ int set_site_params_t(lpc_lattice* h, const double* dF, const uint8_t* blocked, 
     return fail(LPC_EINVAL, "the equilibrium density underflows on %llu open sites: the spread of dF is too wide for %s", hc.bad,
                 h->cfg.precision ? "fp32" : "fp64");
   {
-    const long long cells = 2ll * ((long long)L.nx * L.ny + (long long)L.nx * L.nz + (long long)L.ny * L.nz);
+    // ghosts of pi (wrapped value, or 0 beyond a wall) and of cos, sin (the two-step sweep rotates ghost sites too)
+    const long long cells = ghost_cells(L);
     fill_ghosts_kernel<T><<<aux_grid(cells), 256, 0, h->stream>>>(wsp<T>(h, h->off.pi), 1, L, xghost_mode(h), h->cfg.bc[1] == 0,
                                                                    h->cfg.bc[2] == 0);
     CUDA_TRY(cudaGetLastError());
-    h->launches++;
+    fill_ghosts_kernel<T><<<aux_grid(2 * cells), 256, 0, h->stream>>>(wsp<T>(h, h->off.cs), 2, L, xghost_mode(h), h->cfg.bc[1] == 0,
+                                                                       h->cfg.bc[2] == 0);
+    CUDA_TRY(cudaGetLastError());
+    h->launches += 2;
   }
   // the scratch aliased the back buffer: clear it again so that its ghosts and carbon sites are 0
   CUDA_TRY(cudaMemsetAsync(h->ws + h->off.f1, 0, (size_t)h->C * L.np * h->sT, h->stream));
@@ -669,7 +751,7 @@ int set_link_mobility_t(lpc_lattice* h, const double* alpha_link) {
       });
       if (rc) return rc;
     }
-    const long long cells = 2ll * ((long long)L.nx * L.ny + (long long)L.nx * L.nz + (long long)L.ny * L.nz) * 3;
+    const long long cells = ghost_cells(L) * 3;
     fill_ghosts_kernel<T><<<aux_grid(cells), 256, 0, h->stream>>>(m, 3, L, h->cfg.bc[0] == 0, h->cfg.bc[1] == 0, h->cfg.bc[2] == 0);
     CUDA_TRY(cudaGetLastError());
     h->launches++;
@@ -788,13 +870,11 @@ int equilibrate_t(lpc_lattice* h, double threshold, int64_t max_iters, int64_t c
   using KP = TmaCfg<T, 0, 1, 0, TY, 64, 4, 0, VW>;
   using KL = TmaCfg<T, 0, 1, 0, TY, 64, 4, 1, VW>;
   if (use_tma) {
-    static bool attr_set = false;
-    if (!attr_set) {
-      CUDA_TRY(cudaFuncSetAttribute(step_tma_kernel<T, 0, 1, 0, TY, 64, 4, VW>, cudaFuncAttributeMaxDynamicSharedMemorySize, KP::SMEM_BYTES));
-      CUDA_TRY(cudaFuncSetAttribute(step_tma_links_kernel<T, 0, 1, 0, TY, 64, 4, VW>, cudaFuncAttributeMaxDynamicSharedMemorySize, KL::SMEM_BYTES));
-      attr_set = true;
-    }
+    static bool attr_done[MAX_DEVICES] = {}, attr_done_l[MAX_DEVICES] = {};
+    if (int rc = ensure_dyn_smem(step_tma_kernel<T, 0, 1, 0, TY, 64, 4, VW>, KP::SMEM_BYTES, h->device, attr_done)) return rc;
+    if (int rc = ensure_dyn_smem(step_tma_links_kernel<T, 0, 1, 0, TY, 64, 4, VW>, KL::SMEM_BYTES, h->device, attr_done_l)) return rc;
   }
+  h->ghosts_full = false;
   const unsigned tgrid = (unsigned)(h->tiles_z * h->tiles_y * h->chunks_x);
   int64_t done = 0;
   double delta = 0.0;
@@ -913,13 +993,19 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
   h->steps = 0;
   h->launches = 0;
   h->kernel = LPC_KERNEL_AUTO;
-  if (const char* e = getenv("LPC_KERNEL")) {
-    if (!strcmp(e, "direct")) h->kernel = LPC_KERNEL_DIRECT;
-    if (!strcmp(e, "tma")) h->kernel = LPC_KERNEL_TMA;
-    if (!strcmp(e, "persist")) h->kernel = LPC_KERNEL_PERSIST;
-  }
-  tma_geometry(h->C, cfg->precision == 1, cfg->nx, cfg->ny, cfg->nz, &h->ty, &h->tz, &h->nstage, &h->xc, &h->tiles_z, &h->tiles_y, &h->chunks_x);
+  h->device = dev;
+  h->time_block = 0;
+  h->ghosts_full = false;
+  h->opt_xc = h->opt_persist_mb = h->opt_region_fusion = 0;
+  tma_geometry(h->C, cfg->precision == 1, cfg->nx, cfg->ny, cfg->nz, 0, &h->ty, &h->tz, &h->nstage, &h->xc, &h->tiles_z, &h->tiles_y, &h->chunks_x);
   h->tma_ok = (size_t)h->tiles_z * h->tiles_y * h->chunks_x <= h->off.partial_slots;
+  // two steps per sweep: the magnetisation channels alone, no slab, and every periodic axis long enough for two ghost layers
+  step2_geometry(cfg->nx, h->tiles_z * h->tiles_y, 0, &h->xc2, &h->chunks_x2);
+  h->step2_ok = h->tma_ok && h->nrho == 0 && h->nmom == 0 && !h->halo;
+  for (int d = 0; d < 3; ++d) {
+    const int n = d == 0 ? cfg->nx : d == 1 ? cfg->ny : cfg->nz;
+    if (cfg->bc[d] == 0 && n < 4) h->step2_ok = false;
+  }
   if (h->tma_ok) {
     const Layout& L = h->L;
     const bool f32 = cfg->precision == 1;
@@ -939,6 +1025,16 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
     if (!rc && h->nrho == 1) rc = encode_map(&h->tm_r[1], f32, h->ws + h->off.f1, 4, d4, br);
     if (!rc) rc = encode_map(&h->tm_pi, f32, h->ws + h->off.pi, 3, d4, b4);
     if (!rc) rc = encode_map(&h->tm_cs, f32, h->ws + h->off.cs, 4, dk, bk);
+    if (!rc && h->step2_ok) {
+      // the two-step sweep: h and pi with two halo rows / one 16-byte halo group, cos and sin with one halo row
+      const cuuint32_t zw = (cuuint32_t)(h->tz + 2 * (16 / h->sT));
+      const cuuint32_t b2f[4] = {zw, (cuuint32_t)(h->ty + 4), 1, 2};
+      const cuuint32_t b2k[4] = {zw, (cuuint32_t)(h->ty + 2), 1, 2};
+      rc = encode_map(&h->tm2_f[0], f32, h->ws + h->off.f0, 4, d4, b2f);
+      if (!rc) rc = encode_map(&h->tm2_f[1], f32, h->ws + h->off.f1, 4, d4, b2f);
+      if (!rc) rc = encode_map(&h->tm2_pi, f32, h->ws + h->off.pi, 3, d4, b2f);
+      if (!rc) rc = encode_map(&h->tm2_cs, f32, h->ws + h->off.cs, 4, dk, b2k);
+    }
     if (!rc && cfg->link_mobility) {
       // pi centres and m_x: the tile itself; m_y: one more row below; m_z: 16 bytes of columns below
       const size_t chan = (size_t)L.np * h->sT;
@@ -1009,8 +1105,8 @@ int lpc_halo_view(lpc_lattice* h, int32_t set, int32_t side, int32_t role, void*
     return fail(LPC_EINVAL, "bad selector (set %d, side %d, role %d)", set, side, role);
   if (!plane || !plane_bytes || !stride_bytes || !n_channels) return fail(LPC_EINVAL, "output pointers must not be NULL");
   const Layout& L = h->L;
-  // padded x index: ghost 0, owned 1 .. nx, ghost nx + 1
-  const long long xp = side == 0 ? (role == LPC_HALO_SEND ? 1 : 0) : (role == LPC_HALO_SEND ? L.nx : L.nx + 1);
+  // padded x index: ghost planes 0 .. gh-1, owned gh .. gh+nx-1, ghost planes gh+nx ..; the exchange moves the innermost ghost plane
+  const long long xp = side == 0 ? (role == LPC_HALO_SEND ? L.gh : L.gh - 1) : (role == LPC_HALO_SEND ? L.gh + L.nx - 1 : L.gh + L.nx);
   const size_t base = set == LPC_HALO_PARAMS ? h->off.pi
                     : set == LPC_HALO_STATE0 ? h->off.f0
                     : set == LPC_HALO_STATE1 ? h->off.f1
@@ -1062,6 +1158,15 @@ int lpc_step_n(lpc_lattice* h, int64_t n) {
   const bool persist = !h->have_regions && n >= 2 &&
                        (h->kernel == LPC_KERNEL_PERSIST || (h->kernel == LPC_KERNEL_AUTO && persist_by_default(h)));
   if (persist) return h->cfg.precision ? launch_persist<float>(h, n) : launch_persist<double>(h, n);
+  // two steps per sweep while at least two are left (lpc_step2.cuh); an odd last step takes the one-step sweep
+  if (step2_usable(h)) {
+    while (n >= 2) {
+      int rc = launch_step2(h);
+      if (rc) return rc;
+      h->steps += 2;
+      n -= 2;
+    }
+  }
   for (int64_t k = 0; k < n; ++k) {
     if (h->region_moments && !will_fuse_regions(h)) {   // else the moment sweep books the regional VACF itself
       int rc = region_moment<false>(h);
@@ -1239,6 +1344,38 @@ int lpc_set_kernel(lpc_lattice* h, int32_t which) {
   if (which == LPC_KERNEL_TMA && !h->tma_ok) return fail(LPC_EINVAL, "the TMA kernel is not available for this lattice");
   h->kernel = which;
   return LPC_OK;
+}
+
+int lpc_set_option(lpc_lattice* h, int32_t key, int64_t value) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (value < 0) return fail(LPC_EINVAL, "option values are >= 0");
+  switch (key) {
+    case LPC_OPT_TIME_BLOCK:
+      if (value > 2) return fail(LPC_EINVAL, "LPC_OPT_TIME_BLOCK takes 0 (auto), 1 (one step per sweep) or 2 (two steps per sweep)");
+      if (value == 2 && !h->step2_ok) return fail(LPC_EINVAL, "this lattice cannot run the two-step sweep (channels, slab mode or a periodic axis shorter than 4)");
+      h->time_block = (int)value;
+      return LPC_OK;
+    case LPC_OPT_X_CHUNK: {
+      if (value > h->cfg.nx) value = h->cfg.nx;
+      h->opt_xc = (int)value;
+      tma_geometry(h->C, h->cfg.precision == 1, h->cfg.nx, h->cfg.ny, h->cfg.nz, h->opt_xc, &h->ty, &h->tz, &h->nstage, &h->xc, &h->tiles_z, &h->tiles_y, &h->chunks_x);
+      return LPC_OK;
+    }
+    case LPC_OPT_X_CHUNK2:
+      if (value > h->cfg.nx) value = h->cfg.nx;
+      step2_geometry(h->cfg.nx, (long long)h->tiles_z * h->tiles_y, (int)value, &h->xc2, &h->chunks_x2);
+      return LPC_OK;
+    case LPC_OPT_PERSIST_MAX_MB:
+      if (value > (1 << 20)) return fail(LPC_EINVAL, "LPC_OPT_PERSIST_MAX_MB is in MiB");
+      h->opt_persist_mb = (int)value;
+      return LPC_OK;
+    case LPC_OPT_REGION_FUSION:
+      if (value > 1) return fail(LPC_EINVAL, "LPC_OPT_REGION_FUSION takes 0 (inside the sweep when possible) or 1 (separate pass)");
+      h->opt_region_fusion = (int)value;
+      return LPC_OK;
+    default:
+      return fail(LPC_EINVAL, "unknown option %d", key);
+  }
 }
 
 int64_t lpc_steps_done(const lpc_lattice* h) { return h ? h->steps : 0; }

@@ -86,30 +86,48 @@ __global__ void site_params_kernel(const double* __restrict__ e, const double* _
   if (bad) atomicAdd(&ctl->bad, bad);
 }
 
-// Ghost layers of nch channel planes: periodic axis (1) -> wrapped interior value, reflective (0) -> 0;
-// perx = 2 (slab mode): the x ghost planes belong to the caller and are left alone.
+// Ghost layers of nch channel planes, all of them: L.gh planes / rows in x and y, GHZ columns in z, edges and corners
+// included.  A ghost cell takes the interior value it wraps to when every axis on which it lies outside is periodic (1),
+// and 0 as soon as one of them is reflective (0): nothing crosses a wall.  perx = 2 (slab mode): cells outside in x
+// belong to the caller and are left alone.  The shell is enumerated as x slabs (all of y, z), then y slabs (interior x,
+// all of z), then z columns (interior x and y).
 template <typename T>
 __global__ void fill_ghosts_kernel(T* __restrict__ f, int nch, Layout L, int perx, int pery, int perz) {
-  const long long fz = (long long)L.nx * L.ny, fy = (long long)L.nx * L.nz, fx = (long long)L.ny * L.nz;
-  const long long per_ch = 2 * (fz + fy + fx);
+  const int gh = L.gh;
+  const long long wy = L.ny + 2 * gh, wz = L.nz + 2 * GHZ;
+  const long long ca = 2ll * gh * wy * wz, cb = (long long)L.nx * 2 * gh * wz, cc = (long long)L.nx * L.ny * 2 * GHZ;
+  const long long per_ch = ca + cb + cc;
   for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < per_ch * nch; t += (long long)gridDim.x * blockDim.x) {
     const int c = (int)(t / per_ch);
     long long r = t % per_ch;
-    const int side = (int)(r & 1);
-    r >>= 1;
-    T* g = f + (long long)c * L.np;
-    if (r < fz) {
-      const int x = (int)(r / L.ny), y = (int)(r % L.ny);
-      g[L.idx(x, y, side ? L.nz : -1)] = perz ? g[L.idx(x, y, side ? 0 : L.nz - 1)] : (T)0;
-    } else if (r < fz + fy) {
-      r -= fz;
-      const int x = (int)(r / L.nz), z = (int)(r % L.nz);
-      g[L.idx(x, side ? L.ny : -1, z)] = pery ? g[L.idx(x, side ? 0 : L.ny - 1, z)] : (T)0;
+    int x, y, z;
+    if (r < ca) {
+      z = (int)(r % wz) - GHZ; r /= wz;
+      y = (int)(r % wy) - gh; r /= wy;
+      x = (int)r; x = x < gh ? x - gh : L.nx + (x - gh);
+    } else if (r < ca + cb) {
+      r -= ca;
+      z = (int)(r % wz) - GHZ; r /= wz;
+      y = (int)(r % (2 * gh)); r /= 2 * gh;
+      y = y < gh ? y - gh : L.ny + (y - gh);
+      x = (int)r;
     } else {
-      r -= fz + fy;
-      const int y = (int)(r / L.nz), z = (int)(r % L.nz);
-      if (perx != 2) g[L.idx(side ? L.nx : -1, y, z)] = perx ? g[L.idx(side ? 0 : L.nx - 1, y, z)] : (T)0;
+      r -= ca + cb;
+      z = (int)(r % (2 * GHZ)); r /= 2 * GHZ;
+      z = z < GHZ ? z - GHZ : L.nz + (z - GHZ);
+      y = (int)(r % L.ny);
+      x = (int)(r / L.ny);
     }
+    const bool ox = x < 0 || x >= L.nx, oy = y < 0 || y >= L.ny, oz = z < 0 || z >= L.nz;
+    if (ox && perx == 2) continue;
+    const bool wall = (ox && !perx) || (oy && !pery) || (oz && !perz);
+    T* g = f + (long long)c * L.np;
+    T v = (T)0;
+    if (!wall) {
+      const int sx = ((x % L.nx) + L.nx) % L.nx, sy = ((y % L.ny) + L.ny) % L.ny, sz = ((z % L.nz) + L.nz) % L.nz;
+      v = g[L.idx(sx, sy, sz)];
+    }
+    g[L.idx(x, y, z)] = v;
   }
 }
 

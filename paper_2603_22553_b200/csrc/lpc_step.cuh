@@ -100,8 +100,7 @@ __device__ __forceinline__ void direct_sweep(const StepArgs<T>& a, const T* __re
                              ld_state<T, COHERENT>(f + j - 1), ld_state<T, COHERENT>(f + j + 1));
       }
       const T hr = out[s][0], hi = out[s][1];
-      out[s][0] = u.cs * hr - u.sn * hi;
-      out[s][1] = u.cs * hi + u.sn * hr;
+      phase_rotate(u.cs, u.sn, hr, hi, out[s][0], out[s][1]);
       acc[0] += (double)u.pc * (double)out[s][0];
       acc[1] += (double)u.pc * (double)out[s][1];
     }

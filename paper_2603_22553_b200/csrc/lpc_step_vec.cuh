@@ -132,16 +132,18 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
     unsigned char* st = smem + s * K::STAGE_BYTES;
     const bool need_kcs = (NH == 2) && (jl >= 1 && jl <= nplanes);
     mbar_expect_tx(&full[s], K::TX_BYTES + (need_kcs ? K::KCS_RAW : 0));
-    tma_load_4d(st, &tm_f, &full[s], L.padz + z0 - HZ, y0, x0 + jl, a.c0);
+    // padded coordinates: plane x0 - 1 + jl, rows from y0 - 1 (boxes with halo) or y0 (boxes without)
+    const int px = x0 + jl + L.gh - 1, py = y0 + L.gh - 1;
+    tma_load_4d(st, &tm_f, &full[s], L.padz + z0 - HZ, py, px, a.c0);
     if constexpr (LK) {
-      tma_load_3d(st + K::F_BYTES, &lm.pic, &full[s], L.padz + z0, y0 + 1, x0 + jl);
-      tma_load_3d(st + K::MX_OFF, &lm.mx, &full[s], L.padz + z0, y0 + 1, x0 + jl);
-      tma_load_3d(st + K::MY_OFF, &lm.my, &full[s], L.padz + z0, y0, x0 + jl);
-      tma_load_3d(st + K::MZ_OFF, &lm.mz, &full[s], L.padz + z0 - HZ, y0 + 1, x0 + jl);
+      tma_load_3d(st + K::F_BYTES, &lm.pic, &full[s], L.padz + z0, py + 1, px);
+      tma_load_3d(st + K::MX_OFF, &lm.mx, &full[s], L.padz + z0, py + 1, px);
+      tma_load_3d(st + K::MY_OFF, &lm.my, &full[s], L.padz + z0, py, px);
+      tma_load_3d(st + K::MZ_OFF, &lm.mz, &full[s], L.padz + z0 - HZ, py + 1, px);
     } else {
-      tma_load_3d(st + K::F_BYTES, &tm_pi, &full[s], L.padz + z0 - HZ, y0, x0 + jl);
+      tma_load_3d(st + K::F_BYTES, &tm_pi, &full[s], L.padz + z0 - HZ, py, px);
     }
-    if (need_kcs) tma_load_4d(st + K::F_BYTES + K::PI_BYTES, &tm_cs, &full[s], L.padz + z0, y0 + 1, x0 + jl, 0);
+    if (need_kcs) tma_load_4d(st + K::F_BYTES + K::PI_BYTES, &tm_cs, &full[s], L.padz + z0, py + 1, px, 0);
     ++jl;
   };
   if (threadIdx.x == 0) {
@@ -336,8 +338,7 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
 #pragma unroll
       for (int k = 0; k < VW; ++k) {
         const T hr = o[0][k], hi = o[1][k];
-        o[0][k] = csv[k] * hr - snv[k] * hi;
-        o[1][k] = csv[k] * hi + snv[k] * hr;
+        phase_rotate(csv[k], snv[k], hr, hi, o[0][k], o[1][k]);
         if (k < nvalid) {
           acc[0] += (double)ctr.pi[k] * (double)o[0][k];
           acc[1] += (double)ctr.pi[k] * (double)o[1][k];
@@ -357,7 +358,7 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
           store_face_vec<T, VW>(a.fout + (long long)c * L.np, i, L.nx, L.ny, L.nz, L.sy, L.sx, permask, x, y, z, packv<T, VW>(o[c]), nvalid);
           if constexpr (PEER)   // the neighbours' ghost planes: same offset inside the padded plane
             store_peer_vec<T, VW>(a.peer[0] ? a.peer[0] + c * a.peer_stride[0] : nullptr, a.peer[1] ? a.peer[1] + c * a.peer_stride[1] : nullptr,
-                                  i - (long long)(x + 1) * L.sx, L.nx, x, packv<T, VW>(o[c]), nvalid);
+                                  i - (long long)(x + L.gh) * L.sx, L.nx, x, packv<T, VW>(o[c]), nvalid);
         }
       } else {
 #pragma unroll

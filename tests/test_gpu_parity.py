@@ -187,6 +187,83 @@ def test_kernels_agree_bitwise_on_state_and_are_deterministic(lpc):
 
 
 # ---------------------------------------------------------------------------------------------
+# the two-step sweep (temporal blocking, lpc_step2.cuh): same per-site arithmetic as the one-step sweeps, so the state
+# agrees bit for bit; G[n] of every step is still recorded; against the oracle like everything else
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision", [0, 1])
+@pytest.mark.parametrize("shape,bc,alpha", [
+    ((70, 19, 133), (1, 0, 0), 0.8),    # ragged in y and z, 3 z-tiles, 3 y-tiles, reflective x
+    ((33, 40, 64), (0, 1, 1), 1.0),     # exact z tile, reflective y and z, periodic x with an odd length
+    ((9, 8, 200), (0, 0, 0), 0.5),      # short x, 4 z-tiles, periodic everywhere
+    ((20, 13, 37), (0, 0, 0), 0.9),     # odd ny and nz: the last group of a row is ragged
+    ((4, 4, 4), (0, 0, 0), 1.0),        # every site lies within two of every periodic face
+    ((6, 5, 7), (0, 0, 1), 0.7),
+    ((130, 12, 70), (0, 0, 0), 1.0),    # several x chunks
+])
+def test_two_step_sweep_matches_one_step_sweep_and_oracle(lpc, oracle_mod, shape, bc, alpha, precision):
+    lat = lpc_inputs.random_small(shape, bc=bc, p_block=0.3, alpha=alpha, seed=61, n_moments=0)
+    lat.dt = 2.0e-5
+    n = 41                               # odd: twenty two-step sweeps and one one-step sweep
+    rng = np.random.default_rng(12)
+    g0 = (rng.standard_normal(shape) + 1j * rng.standard_normal(shape)) * (lat.blocked == 0)
+    two, orc = _pair(lpc, oracle_mod, lat, n, 2, precision=precision, g0=g0)
+    two.set_option(lpc.LPC_OPT_TIME_BLOCK, 2)
+    one = lpc.Lattice.from_inputs(lat, precision=precision, max_steps=n, g0=g0)
+    one.set_kernel(2)
+    one.set_option(lpc.LPC_OPT_TIME_BLOCK, 1)
+    l2, l1 = two.launch_count, one.launch_count
+    for k in (6, 1, 3, 20, 11):          # even and odd calls in turn: the sweeps alternate, the ghost shell is refilled when needed
+        two.step(k)
+        one.step(k)
+    assert one.launch_count - l1 == n
+    assert two.launch_count - l2 < n     # two steps per launch wherever a call had two left
+    assert two.steps_done == one.steps_done == n
+    assert np.array_equal(two.field(lpc.LPC_FIELD_G), one.field(lpc.LPC_FIELD_G))
+    scale = np.abs(g0).sum()
+    assert np.max(np.abs(two.fid() - one.fid())) <= (1e-6 if precision else 1e-14) * scale
+    orc.step(n)
+    G_o, sabs = orc.fid(with_scale=True)
+    tol_site, tol_sum = (1e-5, 1e-5) if precision else (1e-10, 1e-9)
+    assert np.max(np.abs(two.fid() - G_o) / sabs) <= tol_sum
+    pi, opn = orc.pi(), lat.blocked == 0
+    hmax = np.max(np.abs(g0)[opn] / pi[opn])
+    assert np.max(np.abs(two.field(lpc.LPC_FIELD_G) - orc.g())[opn] / pi[opn]) <= tol_site * hmax
+    # x chunks of other lengths give the same state bits (the chunk seams carry no arithmetic)
+    for xc in (5, 16):
+        alt = lpc.Lattice.from_inputs(lat, precision=precision, max_steps=n, g0=g0)
+        alt.set_option(lpc.LPC_OPT_X_CHUNK2, xc)
+        alt.step(n - 1)
+        alt.step(1)
+        assert np.array_equal(alt.field(lpc.LPC_FIELD_G), one.field(lpc.LPC_FIELD_G)), xc
+
+
+def test_two_step_sweep_default_and_eligibility(lpc, oracle_mod):
+    lat = lpc_inputs.random_small((24, 16, 70), bc=(0, 0, 0), p_block=0.2, seed=62, n_moments=0)
+    n = 10
+    # AUTO takes two steps per sweep on a lattice that carries the magnetisation alone
+    gpu, orc = _pair(lpc, oracle_mod, lat, n, 2)
+    l0 = gpu.launch_count
+    gpu.step(n)
+    assert gpu.launch_count - l0 == n // 2
+    orc.step(n)
+    _check(lpc, lat, gpu, orc, n, what="two-step default")
+    # the series is bitwise reproducible
+    again = lpc.Lattice.from_inputs(lat, max_steps=n)
+    again.set_kernel(2)
+    again.step(n)
+    assert np.array_equal(again.fid(), gpu.fid())
+    # lattices that cannot: moment fields, a density channel, a periodic axis shorter than four
+    for kw, shape in ((dict(n_moments=3), lat.shape), (dict(n_density=1), lat.shape), (dict(), (24, 3, 70))):
+        m = lpc.Lattice(shape, max_steps=4, **kw)
+        with pytest.raises(lpc.LpcError) as e:
+            m.set_option(lpc.LPC_OPT_TIME_BLOCK, 2)
+        assert e.value.code == lpc.LPC_EINVAL
+    with pytest.raises(lpc.LpcError) as e:
+        gpu.set_option(99, 1)
+    assert e.value.code == lpc.LPC_EINVAL
+
+
+# ---------------------------------------------------------------------------------------------
 # states set from outside, device-resident inputs
 # ---------------------------------------------------------------------------------------------
 def test_arbitrary_initial_magnetisation_and_relaxation(lpc, oracle_mod):
@@ -931,7 +1008,7 @@ def test_slab_mode_errors(lpc):
     assert e.value.code == lpc.LPC_ESTATE
     # the plane views address the workspace: shape [channels, (ny+2) * padded nz]
     v = plain.halo_planes(lpc.LPC_HALO_STATE, 0, lpc.LPC_HALO_SEND)
-    assert v.shape[0] == 2 + lat.n_moments and v.shape[1] % 12 == 0 and float(v[0].max()) == 1.0
+    assert v.shape[0] == 2 + lat.n_moments and v.shape[1] % 14 == 0 and float(v[0].max()) == 1.0   # ny + 4 padded rows
 
 
 def test_regional_fid_fused_sweep_matches_separate_pass(lpc, oracle_mod):
@@ -949,19 +1026,16 @@ def test_regional_fid_fused_sweep_matches_separate_pass(lpc, oracle_mod):
     for precision, tol in ((0, 1e-9), (1, 1e-5)):
         out = {}
         for fused in (True, False):
+            gpu = lpc.Lattice.from_inputs(lat, precision=precision, max_steps=n, n_regions=nreg)
+            gpu.set_kernel(2)
             if not fused:
-                os.environ["LPC_NO_REGION_FUSION"] = "1"
-            try:
-                gpu = lpc.Lattice.from_inputs(lat, precision=precision, max_steps=n, n_regions=nreg)
-                gpu.set_kernel(2)
-                gpu.set_regions(region)
-                assert gpu.bytes_per_site_step == (4 if precision else 8) * 7 + (1 if fused else (4 if precision else 8) * 3 + 1)
-                l0 = gpu.launch_count
-                gpu.step(n)
-                assert gpu.launch_count - l0 == (n if fused else 2 * n)
-                out[fused] = np.array([gpu.fid_region(r) for r in range(nreg)])
-            finally:
-                os.environ.pop("LPC_NO_REGION_FUSION", None)
+                gpu.set_option(lpc.LPC_OPT_REGION_FUSION, 1)      # the separate reduction pass after every sweep
+            gpu.set_regions(region)
+            assert gpu.bytes_per_site_step == (4 if precision else 8) * 7 + (1 if fused else (4 if precision else 8) * 3 + 1)
+            l0 = gpu.launch_count
+            gpu.step(n)
+            assert gpu.launch_count - l0 == (n if fused else 2 * n)
+            out[fused] = np.array([gpu.fid_region(r) for r in range(nreg)])
         assert np.max(np.abs(out[True] - Gr_o) / sabs) <= tol
         assert np.max(np.abs(out[True] - out[False]) / sabs) <= (1e-5 if precision else 1e-13)
     # with stored link weights the fused sweep is the links kernel

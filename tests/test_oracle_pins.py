@@ -795,3 +795,17 @@ def test_result_does_not_depend_on_thread_count():
         env = dict(os.environ, OMP_NUM_THREADS=nt)
         outs.append(subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, check=True).stdout)
     assert outs[0] == outs[1] == outs[2] and len(outs[0]) > 100
+
+
+def test_oracle_is_clean_under_asan_and_ubsan(tmp_path):
+    """the oracle built with -fsanitize=address,undefined (no OpenMP, so that every access is the
+    calling thread's) and driven through all its entry points by tests/c_client/oracle_sanitize.c."""
+    exe = str(tmp_path / "oracle_sanitize")
+    subprocess.check_call(["gcc", "-std=gnu11", "-O1", "-g", "-fno-omit-frame-pointer", "-ffp-contract=off", "-fsanitize=address,undefined",
+                           "-fno-sanitize-recover=all", "-Wall", "-Wextra", "-Wno-unknown-pragmas",
+                           os.path.join(ROOT, "oracle", "lpc_oracle.c"), os.path.join(ROOT, "tests", "c_client", "oracle_sanitize.c"),
+                           "-o", exe, "-lm"])
+    out = subprocess.run([exe], capture_output=True, text=True, timeout=300,
+                         env=dict(os.environ, ASAN_OPTIONS="detect_leaks=1:abort_on_error=0", UBSAN_OPTIONS="print_stacktrace=1"))
+    assert out.returncode == 0, out.stdout + out.stderr
+    assert out.stdout.strip() == "CLEAN" and "runtime error" not in out.stderr and "AddressSanitizer" not in out.stderr
