@@ -47,7 +47,8 @@ size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 constexpr int DIRECT_MAX_BLOCKS = 148 * 8;
 constexpr int AUX_BLOCKS = 148 * 8;
-constexpr long long STAGE_SITES = 4ll << 20;  // sites per host<->device staging chunk
+constexpr long long STAGE_SITES = 4ll << 20;  // sites in the host<->device staging region (two halves)
+inline long long stage_chunk_sites(long long N) { return std::max<long long>(1, std::min<long long>(N, STAGE_SITES / 2)); }
 constexpr long long SPEC_BATCH = 4096;        // frequencies per spectrum launch
 
 struct Offsets {
@@ -209,7 +210,7 @@ Offsets make_offsets(const lpc_config* c, const Layout& L) {
   o.wr = p; p += align_up(c->n_regions ? MAX_REGIONS * sizeof(double) : 0);
   o.rpartials = p; p += align_up(c->n_regions ? std::max<size_t>((size_t)AUX_BLOCKS * 4, o.partial_slots * 2) * MAX_REGIONS * sizeof(double) : 0);
   o.spec = p; p += align_up((size_t)SPEC_BATCH * sizeof(double2));
-  o.staging = p; p += align_up((size_t)std::min<long long>(N, STAGE_SITES) * 16);
+  o.staging = p; p += align_up(2 * (size_t)stage_chunk_sites(N) * 16);   // two halves of stage_chunk_sites(N) sites x 16 B
   o.total = p;
   return o;
 }
@@ -486,16 +487,20 @@ int launch_step(lpc_lattice* h) {
 template <typename F>
 int for_chunks_in(lpc_lattice* h, const void* src, size_t bytes_per_site, F body) {
   if (is_device_ptr(src)) return body(src, 0ll, h->N);
-  const long long chunk = std::min<long long>(h->N, STAGE_SITES);
+  // Two halves of the staging region in turn, no host synchronisation: the copies and the kernels that consume them are
+  // ordered by the stream, the host runs ahead and keeps the copy queue full (from pinned memory the upload then runs at
+  // the PCIe rate; the kernels are about 1% of it, so a second stream would buy nothing measurable)
+  const long long chunk = stage_chunk_sites(h->N);
+  const size_t half_bytes = (size_t)chunk * 16;
   unsigned char* stg = h->ws + h->off.staging;
+  int half = 0;
   for (long long i0 = 0; i0 < h->N; i0 += chunk) {
     const long long n = std::min(chunk, h->N - i0);
-    CUDA_TRY(cudaMemcpyAsync(stg, static_cast<const unsigned char*>(src) + (size_t)i0 * bytes_per_site, (size_t)n * bytes_per_site,
-                             cudaMemcpyHostToDevice, h->stream));
-    int rc = body(stg, i0, n);
+    CUDA_TRY(cudaMemcpyAsync(stg + (size_t)half * half_bytes, static_cast<const unsigned char*>(src) + (size_t)i0 * bytes_per_site,
+                             (size_t)n * bytes_per_site, cudaMemcpyHostToDevice, h->stream));
+    int rc = body(stg + (size_t)half * half_bytes, i0, n);
     if (rc) return rc;
-    // the staging buffer is reused by the next chunk
-    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    half ^= 1;
   }
   return LPC_OK;
 }
@@ -625,17 +630,20 @@ int boltzmann_pass(lpc_lattice* h, const double* dF, const uint8_t* blocked, Ctl
     CUDA_TRY(cudaGetLastError());
     h->launches++;
   } else {
-    const long long chunk = std::min<long long>(h->N, STAGE_SITES);
-    unsigned char* stg = h->ws + h->off.staging;
+    // as for_chunks_in: two halves of the staging region, ordered by the stream alone
+    const long long chunk = stage_chunk_sites(h->N);
+    const size_t half_bytes = (size_t)chunk * 16;
+    int half = 0;
     for (long long i0 = 0; i0 < h->N; i0 += chunk) {
       const long long n = std::min(chunk, h->N - i0);
+      unsigned char* stg = h->ws + h->off.staging + (size_t)half * half_bytes;
       CUDA_TRY(cudaMemcpyAsync(stg, dF + i0, (size_t)n * 8, cudaMemcpyDefault, h->stream));
       CUDA_TRY(cudaMemcpyAsync(stg + (size_t)chunk * 8, blocked + i0, (size_t)n, cudaMemcpyDefault, h->stream));
       boltzmann_factor_kernel<<<aux_grid(n), 256, 0, h->stream>>>(reinterpret_cast<const double*>(stg), stg + (size_t)chunk * 8, i0, n, e,
                                                                    ctl);
       CUDA_TRY(cudaGetLastError());
       h->launches++;
-      CUDA_TRY(cudaStreamSynchronize(h->stream));
+      half ^= 1;
     }
   }
   sum_kernel<<<aux_grid(h->N), 256, 0, h->stream>>>(e, h->N, wsp<double>(h, h->off.partials), ctl);
@@ -793,15 +801,16 @@ int read_field_t(lpc_lattice* h, int which, void* out) {
     CUDA_TRY(cudaGetLastError());
     h->launches++;
   } else {
-    const long long chunk = std::min<long long>(h->N, STAGE_SITES);
-    double* stg = wsp<double>(h, h->off.staging);
+    const long long chunk = stage_chunk_sites(h->N);
+    int half = 0;
     for (long long i0 = 0; i0 < h->N; i0 += chunk) {
       const long long n = std::min(chunk, h->N - i0);
+      double* stg = wsp<double>(h, h->off.staging) + (size_t)half * chunk * 2;
       gather_field_kernel<T><<<aux_grid(n), 256, 0, h->stream>>>(mode, i0, n, L, pi, ch, stg);
       CUDA_TRY(cudaGetLastError());
       h->launches++;
       CUDA_TRY(cudaMemcpyAsync(static_cast<unsigned char*>(out) + (size_t)i0 * bps, stg, (size_t)n * bps, cudaMemcpyDeviceToHost, h->stream));
-      CUDA_TRY(cudaStreamSynchronize(h->stream));
+      half ^= 1;
     }
   }
   CUDA_TRY(cudaStreamSynchronize(h->stream));

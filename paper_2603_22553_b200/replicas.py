@@ -1,10 +1,9 @@
-"""Multi-GPU plumbing of the benchmark: independent replicas, one lattice per rank.
+"""Timing plumbing of the multi-GPU benchmark: rank environment, MAX over ranks of the device time, whole-job GLUPS.
 
-The LPC3D step is benchmarked at N > 1 as N independent lattices (DESIGN.md "Multi-GPU":
-"replicas only"): there is no data-path collective.  The only communication is the
-aggregation of the timing -- barrier, MAX over ranks of the device time -- which is what this
-module holds.  It works on any ``torch.distributed`` backend (nccl on the GPU box, gloo in the
-CPU tests) and holds none of the method's arithmetic.
+The lattice itself is split over the ranks as x-slabs by ``slab.py`` (``bench.py --gpus N``);
+``bench.py --replicas`` instead runs N independent lattices, one per rank, with no data-path communication.  Either way
+the only thing this module does is aggregate the timing -- barrier, MAX over ranks of the device time.  It works on any
+``torch.distributed`` backend (nccl on the GPU box, gloo in the CPU tests) and holds none of the method's arithmetic.
 """
 from __future__ import annotations
 
