@@ -10,9 +10,12 @@ BASELINE.json configs[4] (monolith statistics, fp64, NMR kernel alone).  One ste
 moves 7.5 GB of state and parameters, far more than the 126 MB L2, so no L2 flush is
 needed between steps.
 
-N > 1 (torchrun): the path is benchmarked as independent replicas, one lattice per
-GPU, no data-path collective; value = all ranks' site updates
-divided by the slowest rank's time.
+N > 1 (torchrun): ONE lattice split into x-slabs over the ranks: weak
+scaling on N stacked copies of the 512^3 lattice (a (512 N) x 512 x 512 lattice; the 512^3 lattice is periodic, so
+the stack is continuous across the seams), each rank generating its own planes only, one boundary-plane exchange
+per step (NCCL send/recv, or the sweeps' own stores into the neighbours' ghost planes with --slab-direct) and no
+per-step collective; value = all sites x steps / the slowest rank's device time.  --replicas runs N independent
+lattices instead (no data-path communication).
 
 --impl reference times the CPU oracle (oracle/) as it stands on the host cores.
 """
@@ -58,8 +61,12 @@ def parse():
     p.add_argument("--regions", type=int, default=0, metavar="R",
                    help="label R (1..8) equal x-ranges as regions and record the region-resolved FID G_r[n] as well")
     p.add_argument("--slabs", type=int, default=0, metavar="S",
-                   help="run the workload as ONE lattice cut into x-slabs, S per rank (SURVEY 8(e)): a plane exchange after every step, "
-                        "strong scaling over --gpus; 0 (default) = independent replicas")
+                   help="run ONE lattice cut into x-slabs, S per rank (SURVEY 8(e)): a plane exchange after every step.  Default: 0 on "
+                        "one GPU (the unsplit lattice), 1 with --gpus N > 1")
+    p.add_argument("--replicas", action="store_true", help="with --gpus N > 1: N independent lattices instead of one split lattice")
+    p.add_argument("--strong", action="store_true",
+                   help="with slabs: split the workload's own lattice over the ranks (strong scaling) instead of stacking one copy "
+                        "per rank along x (weak scaling, the default)")
     p.add_argument("--slab-direct", action="store_true",
                    help="with --slabs: let the sweeps store their outermost planes into the neighbours' ghost planes themselves "
                         "(lpc_set_halo_peers; other ranks' workspaces are mapped through CUDA IPC) instead of copying / sending them "
@@ -280,6 +287,8 @@ def run_ours(args):
 
     L, K, W = args.size, args.steps, args.warmup
     lat = make_workload(args)
+    if world > 1 and not args.replicas and not args.slabs:
+        args.slabs = 1            # the default multi-GPU run: one lattice, one x-slab per rank
     if args.slabs:
         return run_slabs(args, lat, lpc, world, rank, local, dev)
     n_sites = lat.n_sites
@@ -461,9 +470,15 @@ def run_slabs(args, lat, lpc, world, rank, local, dev):
         m.set_kernel(args.kernel)
         return m
 
-    ss = slab.SlabSet(lat.shape, bc=lat.bc, slabs_per_rank=args.slabs, lattice_factory=factory, precision=args.precision,
+    # weak scaling (default): the global lattice is `world` copies of the workload's lattice stacked along x, and every rank
+    # hands in its own copy only (local=True); that needs a lattice that continues into itself (periodic x).  Strong scaling
+    # (--strong, or a lattice with walls in x): the workload's own lattice is cut over the ranks.
+    weak = (not args.strong) and lat.bc[0] == 0
+    gshape = (lat.nx * world, lat.ny, lat.nz) if weak else lat.shape
+    ss = slab.SlabSet(gshape, bc=lat.bc, slabs_per_rank=args.slabs, lattice_factory=factory, precision=args.precision,
                       n_moments=args.moments, dt=lat.dt, a=lat.a, alpha=lat.alpha, max_steps=K + W + 8)
-    ss.set_site_params(lat.dF, lat.blocked, lat.omega)
+    ss.set_site_params(lat.dF, lat.blocked, lat.omega, local=weak)
+    n_global = gshape[0] * gshape[1] * gshape[2]
     n_direct = ss.enable_direct_stores(remote=world > 1) if args.slab_direct else 0
     ss.step(W)
 
@@ -493,6 +508,7 @@ def run_slabs(args, lat, lpc, world, rank, local, dev):
     launches = sum(m.launch_count for m in ss.lat.values()) - l0
     fid = ss.fid()
     assert np.isfinite(fid).all() and abs(fid[0] - 1.0) < (1e-4 if args.precision else 1e-12), "FID series is not sane"
+    backend = dist.get_backend() if world > 1 else "none"
     if rank == 0:
         peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
         peak = float(json.load(open(peaks_path))["hbm_gbs"]) if os.path.exists(peaks_path) else FALLBACK_HBM_GBS
@@ -500,15 +516,19 @@ def run_slabs(args, lat, lpc, world, rank, local, dev):
         bps = m0.bytes_per_site_step
         own = sum(hi - lo for s, (lo, hi) in ss.ranges.items() if s in ss.lat) * lat.ny * lat.nz
         achieved = bps * own / (ms / K * 1e-3) / 1e9      # this rank's sites over this rank's time
-        plane_bytes = (lat.ny + 2) * m0.halo_planes(lpc.LPC_HALO_STATE, 0, lpc.LPC_HALO_SEND).shape[1] // (lat.ny + 2) * (4 if args.precision else 8)
+        plane_bytes = m0.halo_planes(lpc.LPC_HALO_STATE, 0, lpc.LPC_HALO_SEND).shape[1] * (4 if args.precision else 8)
+        n_faces = len(slab.messages(ss.n_slabs, ss.periodic))
         print(json.dumps({
-            "metric": METRIC, "value": lat.n_sites * K / (ms_max * 1e-3) / 1e9, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "metric": METRIC, "value": n_global * K / (ms_max * 1e-3) / 1e9, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak" if weak else "strong", "vs_baseline": None,
             "dtype": "f32" if args.precision else "f64", "data": "synthetic",
-            "config": {"workload": workload_name(args.size, args.moments, args.precision, args.workload), "lattice": list(lat.shape),
-                       "sites": lat.n_sites, "parallelism": f"x-slabs: {ss.n_slabs} slabs over {world} rank(s), one plane exchange per step "
-                                                           f"({2 + args.moments} channel planes of {plane_bytes} B per face); "
-                                                           f"{n_direct} faces stored by the sweeps themselves, the rest copied / sent",
+            "config": {"workload": workload_name(args.size, args.moments, args.precision, args.workload)
+                                   + (f", {world} copies stacked along x" if weak and world > 1 else ""),
+                       "lattice": list(gshape), "sites": n_global,
+                       "parallelism": f"x-slabs: {ss.n_slabs} slabs over {world} rank(s) (backend {backend}), one plane exchange per step "
+                                      f"({2 + args.moments} channel planes of {plane_bytes} B per face, {n_faces} faces); "
+                                      f"{n_direct} of this rank's faces stored by the sweeps themselves, the rest copied / sent; no per-step collective",
+                       "exchange_bytes_per_step": n_faces * (2 + args.moments) * plane_bytes,
                        "l2": "per-rank working set >> 126 MB L2" if bps * own > 4 * 126e6 else "per-rank working set is L2-sized"},
             "clocks": clocks, "e2e": None, "gpu_launches": int(launches),
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,

@@ -269,6 +269,22 @@ int lpc_halo_view(lpc_lattice* lat, int32_t set, int32_t side, int32_t role, voi
 int lpc_set_halo_peers(lpc_lattice* lat, void* lo0, void* lo1, size_t lo_channel_stride_bytes, void* hi0, void* hi1,
                        size_t hi_channel_stride_bytes);
 
+/* Slab mode between PROCESSES of one node (one process per GPU): export the device allocation that holds this lattice's
+ * workspace as a CUDA IPC handle, so that a neighbour rank can map it and hand the ghost-plane addresses inside it to
+ * lpc_set_halo_peers.  handle_out: host, LPC_IPC_HANDLE_BYTES bytes (a cudaIpcMemHandle_t; send it to the other rank as
+ * plain bytes).  offset_out: host, byte offset of the workspace inside the exported allocation (an allocator may have
+ * carved the workspace out of a larger block; the handle always names the whole block).
+ * Errors: LPC_EINVAL, LPC_ECUDA (e.g. the allocation does not come from cudaMalloc).                               */
+#define LPC_IPC_HANDLE_BYTES 64
+int lpc_ipc_export(lpc_lattice* lat, void* handle_out, size_t* offset_out);
+
+/* Map an allocation another process exported with lpc_ipc_export into this process (cudaIpcOpenMemHandle, peer access
+ * enabled when it lives on another GPU).  handle: host, LPC_IPC_HANDLE_BYTES bytes.  base_out: host, receives the device
+ * address of the allocation's first byte in THIS process; the neighbour's workspace starts at base + its offset.
+ * lpc_ipc_close unmaps it (after the lattices that store into it are done).  Errors: LPC_EINVAL, LPC_ECUDA.          */
+int lpc_ipc_open(const void* handle, void** base_out);
+int lpc_ipc_close(void* base);
+
 /* Slab mode: build the initial state once the pi ghost planes are in place (see the order above).  Resets the
  * step counter and the series.  Synchronises.  Errors: LPC_ESTATE (not a slab, or no site parameters).         */
 int lpc_slab_finish(lpc_lattice* lat);

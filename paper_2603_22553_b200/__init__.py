@@ -29,7 +29,7 @@ LPC_OPT_TIME_BLOCK, LPC_OPT_X_CHUNK, LPC_OPT_X_CHUNK2, LPC_OPT_PERSIST_MAX_MB, L
 EXPORTS = (
     "lpc_workspace_bytes", "lpc_create_lattice", "lpc_set_site_params", "lpc_set_link_mobility", "lpc_step_n", "lpc_read_fid",
     "lpc_moments", "lpc_read_field", "lpc_set_state", "lpc_equilibrate", "lpc_seed_from_density", "lpc_set_regions", "lpc_read_fid_region", "lpc_moments_region", "lpc_spectrum", "lpc_set_kernel",
-    "lpc_set_option", "lpc_steps_done", "lpc_partition_sum", "lpc_set_partition_sum", "lpc_halo_view", "lpc_set_halo_peers", "lpc_slab_finish",
+    "lpc_set_option", "lpc_ipc_export", "lpc_ipc_open", "lpc_ipc_close", "lpc_steps_done", "lpc_partition_sum", "lpc_set_partition_sum", "lpc_halo_view", "lpc_set_halo_peers", "lpc_slab_finish",
     "lpc_launch_count", "lpc_bytes_per_site_step", "lpc_destroy", "lpc_last_error",
 )
 
@@ -72,6 +72,9 @@ def _load():
     lib.lpc_halo_view.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_void_p), C.POINTER(C.c_size_t),
                                   C.POINTER(C.c_size_t), C.POINTER(C.c_int32)]
     lib.lpc_slab_finish.argtypes = [C.c_void_p]
+    lib.lpc_ipc_export.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_size_t)]
+    lib.lpc_ipc_open.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
+    lib.lpc_ipc_close.argtypes = [C.c_void_p]
     lib.lpc_set_halo_peers.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p, C.c_size_t]
     lib.lpc_step_n.argtypes = [C.c_void_p, C.c_int64]
     lib.lpc_read_fid.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_void_p]
@@ -193,6 +196,26 @@ def lpc_set_halo_peers(handle, lo=None, hi=None):
     hi = hi or (None, None, 0)
     _check(_lib.lpc_set_halo_peers(handle, C.c_void_p(lo[0]), C.c_void_p(lo[1]), C.c_size_t(lo[2]), C.c_void_p(hi[0]), C.c_void_p(hi[1]),
                                    C.c_size_t(hi[2])))
+
+
+def lpc_ipc_export(handle):
+    """(64-byte CUDA IPC handle of the allocation the workspace lies in, byte offset of the workspace inside it)."""
+    buf = C.create_string_buffer(64)
+    off = C.c_size_t()
+    _check(_lib.lpc_ipc_export(handle, buf, C.byref(off)))
+    return bytes(buf.raw), int(off.value)
+
+
+def lpc_ipc_open(handle_bytes) -> int:
+    """Map an exported allocation into this process; returns its base device address here."""
+    buf = C.create_string_buffer(bytes(handle_bytes), 64)
+    base = C.c_void_p()
+    _check(_lib.lpc_ipc_open(buf, C.byref(base)))
+    return int(base.value)
+
+
+def lpc_ipc_close(base):
+    _check(_lib.lpc_ipc_close(C.c_void_p(int(base))))
 
 
 def lpc_slab_finish(handle):
@@ -374,6 +397,18 @@ class Lattice:
         p0, _, st, _ = lpc_halo_view(self.handle, LPC_HALO_STATE0, side, LPC_HALO_RECV)
         p1, _, _, _ = lpc_halo_view(self.handle, LPC_HALO_STATE1, side, LPC_HALO_RECV)
         return p0, p1, st
+
+    def ipc_export(self):
+        """What another process needs to store into this lattice's ghost planes: the IPC handle of the workspace's
+        allocation, the workspace's offset in it, and per side the ghost-plane offsets (buffer 0, buffer 1) inside the
+        workspace plus the channel stride."""
+        handle, off = lpc_ipc_export(self.handle)
+        base = self.workspace.data_ptr()
+        ghosts = []
+        for side in (0, 1):
+            p0, p1, st = self.ghost_plane_addresses(side)
+            ghosts.append((p0 - base, p1 - base, st))
+        return handle, off, ghosts
 
     def set_halo_peers(self, lo=None, hi=None):
         lpc_set_halo_peers(self.handle, lo, hi)

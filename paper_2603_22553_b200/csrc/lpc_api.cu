@@ -1139,6 +1139,47 @@ int lpc_set_halo_peers(lpc_lattice* h, void* lo0, void* lo1, size_t lo_stride, v
   return LPC_OK;
 }
 
+int lpc_ipc_export(lpc_lattice* h, void* handle_out, size_t* offset_out) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (!handle_out || !offset_out) return fail(LPC_EINVAL, "output pointers must not be NULL");
+  static_assert(sizeof(cudaIpcMemHandle_t) == LPC_IPC_HANDLE_BYTES, "LPC_IPC_HANDLE_BYTES is the size of a cudaIpcMemHandle_t");
+  // the handle names the whole allocation the workspace lies in: find its base
+  typedef CUresult (*RangeFn)(CUdeviceptr*, size_t*, CUdeviceptr);
+  static RangeFn range_fn = nullptr;
+  if (!range_fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    CUDA_TRY(cudaGetDriverEntryPoint("cuMemGetAddressRange", &p, cudaEnableDefault, &q));
+    if (q != cudaDriverEntryPointSuccess || !p) return fail(LPC_ECUDA, "cuMemGetAddressRange not available in this driver");
+    range_fn = reinterpret_cast<RangeFn>(p);
+  }
+  CUdeviceptr base = 0;
+  size_t size = 0;
+  const CUresult r = range_fn(&base, &size, reinterpret_cast<CUdeviceptr>(h->ws));
+  if (r != CUDA_SUCCESS) return fail(LPC_ECUDA, "cuMemGetAddressRange failed with CUresult %d", (int)r);
+  cudaIpcMemHandle_t hd;
+  CUDA_TRY(cudaIpcGetMemHandle(&hd, reinterpret_cast<void*>(base)));
+  memcpy(handle_out, &hd, sizeof(hd));
+  *offset_out = (size_t)(reinterpret_cast<CUdeviceptr>(h->ws) - base);
+  return LPC_OK;
+}
+
+int lpc_ipc_open(const void* handle, void** base_out) {
+  if (!handle || !base_out) return fail(LPC_EINVAL, "handle and base_out must not be NULL");
+  cudaIpcMemHandle_t hd;
+  memcpy(&hd, handle, sizeof(hd));
+  void* p = nullptr;
+  CUDA_TRY(cudaIpcOpenMemHandle(&p, hd, cudaIpcMemLazyEnablePeerAccess));
+  *base_out = p;
+  return LPC_OK;
+}
+
+int lpc_ipc_close(void* base) {
+  if (!base) return fail(LPC_EINVAL, "base is NULL");
+  CUDA_TRY(cudaIpcCloseMemHandle(base));
+  return LPC_OK;
+}
+
 int lpc_slab_finish(lpc_lattice* h) {
   if (!h) return fail(LPC_EINVAL, "lattice is NULL");
   if (!h->halo) return fail(LPC_ESTATE, "the lattice was not created with bc[0] = LPC_BC_HALO");

@@ -90,30 +90,24 @@ class SlabSet:
         self.direct_all = set()   # the same over the slabs of all ranks: what both ends of a message skip after a step
         self.remote_direct = False
         self.stats = {"copies": 0, "sends": 0, "recvs": 0}   # plane transfers `exchange` has issued so far
-        self._peer_storages = []   # mappings of other ranks' workspaces (kept alive while the peers are set)
+        self._peer_maps = {}       # IPC handle -> base address here of another rank's workspace allocation
 
     def enable_direct_stores(self, remote=False):
         """Let the step kernel write a slab's outermost planes straight into the neighbours' ghost planes -- the
         transfer rides on the sweep's own stores and `exchange` has nothing left to do for those faces.  Neighbours in
         this process: plain device addresses.  remote=True: neighbours on other ranks of the SAME NODE as well -- every
-        rank exports its workspace allocation as a CUDA IPC handle (torch's shared-storage handle), the ranks swap
-        handles and ghost-plane offsets once (all_gather_object) and map each other's workspaces; after every step a
+        rank exports its workspace allocation as a CUDA IPC handle (lpc_ipc_export), the ranks swap handles and
+        ghost-plane offsets once (all_gather_object) and map each other's workspaces (lpc_ipc_open); after every step a
         fence (`_step_fence`) makes sure all ranks' sweeps have finished before any rank starts the next one.  Faces
         that are not direct keep the copy / send-recv.  Call after set_site_params.  Returns the direct faces here."""
         self.direct = set()
-        self._peer_storages = []
+        self._close_peers()
         remote = bool(remote) and self.dist is not None and self.world > 1
         table = {}
         if remote:
-            import torch
-
-            mine = {}
-            for s in self.owned:
-                ws = self.lat[s].workspace
-                base = ws.data_ptr()
-                mine[s] = (ws.untyped_storage()._share_cuda_(),
-                           [tuple(a - base for a in self.lat[s].ghost_plane_addresses(side)[:2]) for side in (0, 1)],
-                           self.lat[s].ghost_plane_addresses(0)[2])
+            # every rank publishes, per owned slab, the CUDA IPC handle of its workspace allocation and where the ghost
+            # planes lie in it (lpc_ipc_export behind the C ABI); a rank maps each remote allocation once (lpc_ipc_open)
+            mine = {s: self.lat[s].ipc_export() for s in self.owned}
             gathered = [None] * self.world
             self.dist.all_gather_object(gathered, mine, group=self.group)
             for part in gathered:
@@ -129,13 +123,12 @@ class SlabSet:
                         peers[side] = self.lat[t].ghost_plane_addresses(1 - side)
                         self.direct.add((s, side))
                 elif remote:
-                    import torch
-
-                    handle, offsets, stride = table[t]
-                    st = torch.UntypedStorage._new_shared_cuda(*handle)   # maps the other rank's workspace here
-                    self._peer_storages.append(st)
-                    off0, off1 = offsets[1 - side]
-                    peers[side] = (st.data_ptr() + off0, st.data_ptr() + off1, stride)
+                    handle, ws_off, ghosts = table[t]
+                    if handle not in self._peer_maps:
+                        self._peer_maps[handle] = self._ipc_open(handle)      # maps the other rank's allocation here
+                    base = self._peer_maps[handle] + ws_off
+                    off0, off1, stride = ghosts[1 - side]
+                    peers[side] = (base + off0, base + off1, stride)
                     self.direct.add((s, side))
             self.lat[s].set_halo_peers(lo=peers[0], hi=peers[1])
         self.remote_direct = remote
@@ -147,6 +140,19 @@ class SlabSet:
             for part in gathered:
                 self.direct_all.update(tuple(f) for f in part)
         return len(self.direct)
+
+    def _ipc_open(self, handle):
+        from . import lpc_ipc_open
+
+        return lpc_ipc_open(handle)
+
+    def _close_peers(self):
+        if self._peer_maps:
+            from . import lpc_ipc_close
+
+            for base in self._peer_maps.values():
+                lpc_ipc_close(base)
+        self._peer_maps = {}
 
     def _step_fence(self):
         """All ranks' sweeps of this step have finished (their direct stores have landed) before anyone goes on."""
@@ -163,10 +169,22 @@ class SlabSet:
     def owner(self, s: int) -> int:
         return s // self.spr
 
-    def local_part(self, arr, s):
-        """The planes of slab s of an array over the whole lattice (leading axes before x are kept)."""
+    def rank_range(self):
+        """Planes [lo, hi) of the whole lattice that this rank's slabs cover (they are contiguous)."""
+        return self.ranges[self.owned[0]][0], self.ranges[self.owned[-1]][1]
+
+    def local_part(self, arr, s, local=False):
+        """The planes of slab s of an array over the whole lattice -- or, with local=True, of an array that holds this
+        rank's planes only (`rank_range`); leading axes before x are kept."""
         lo, hi = self.ranges[s]
         a = np.asarray(arr)
+        if local:
+            r0, r1 = self.rank_range()
+            if a.shape[-3] != r1 - r0:
+                raise ValueError(f"a local array must hold this rank's {r1 - r0} planes, got {a.shape[-3]}")
+            lo, hi = lo - r0, hi - r0
+        elif a.shape[-3] != self.global_shape[0]:
+            raise ValueError(f"a global array must hold all {self.global_shape[0]} planes, got {a.shape[-3]}")
         lead = a.ndim - 3
         return np.ascontiguousarray(a[(slice(None),) * lead + (slice(lo, hi),)])
 
@@ -227,9 +245,12 @@ class SlabSet:
         return r if self.group is None else self.dist.get_global_rank(self.group, r)
 
     # ---- the call sequence of include/lpc.h "Slabs" ---------------------------------------------
-    def set_site_params(self, dF, blocked, omega, g0=None):
-        """dF, blocked, omega (and g0) are arrays over the WHOLE lattice (host); every rank cuts out its planes."""
-        parts = {s: (self.local_part(dF, s), self.local_part(blocked, s).astype(np.uint8), self.local_part(omega, s)) for s in self.owned}
+    def set_site_params(self, dF, blocked, omega, g0=None, local=False):
+        """dF, blocked, omega (and g0): host arrays over the WHOLE lattice, of which every rank cuts out its planes, or
+        (local=True) over this rank's own planes only (`rank_range`) -- nothing of the other ranks' input is needed here:
+        Eq. 2's normalisation travels as one scalar, the neighbours' pi as one plane."""
+        parts = {s: (self.local_part(dF, s, local), self.local_part(blocked, s, local).astype(np.uint8), self.local_part(omega, s, local))
+                 for s in self.owned}
         z_local = np.array([sum(self.lat[s].partition_sum(parts[s][0], parts[s][1]) for s in self.owned)], dtype=np.float64)
         Z = float(self._allreduce(z_local)[0])
         for s in self.owned:
@@ -240,7 +261,7 @@ class SlabSet:
             self.lat[s].slab_finish()
         if g0 is not None:
             for s in self.owned:
-                self.lat[s].set_state(0, self.local_part(g0, s))
+                self.lat[s].set_state(0, self.local_part(g0, s, local))
         self.exchange(HALO_STATE)
         self.steps = 0
         return Z

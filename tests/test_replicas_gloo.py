@@ -1,5 +1,6 @@
-"""The N > 1 path of the benchmark is "replicas only": the one thing that
-crosses ranks is the timing aggregation.  Covered here with world_size 2 on the gloo backend."""
+"""Timing aggregation of the multi-GPU benchmark (barrier, MAX over ranks of the device time, summed work) and the
+rank-0-only reference arm, with world_size 2 on the gloo backend.  The data path of the N > 1 run -- one lattice split into
+x-slabs -- is covered by tests/test_slab_gloo.py."""
 import json
 import os
 import subprocess

@@ -117,6 +117,23 @@ def _run(shape, bc, spr, n):
     return ss
 
 
+def _run_local(shape, bc, spr, n):
+    """Every rank hands in its own planes only (local=True), as bench.py does for the weak-scaling run."""
+    dF, blocked, g0 = _inputs(shape)
+    g0 = g0 * (blocked == 0)
+    ss = slab.SlabSet(shape, bc=bc, slabs_per_rank=spr, lattice_factory=FakeLattice, max_steps=n)
+    lo, hi = ss.rank_range()
+    Z = ss.set_site_params(dF[lo:hi], blocked[lo:hi], np.zeros(shape)[lo:hi], g0[lo:hi].astype(np.complex128), local=True)
+    ss.step(n)
+    f_ref, G_ref = _reference(dF, blocked, g0, bc[0] == 0, n)
+    assert abs(Z - np.exp(-dF)[blocked == 0].sum()) < 1e-9        # Eq. 2 normalises over the whole lattice
+    assert np.max(np.abs(ss.fid().real - G_ref)) < 1e-13
+    assert np.max(np.abs(ss.gather_field(0) - f_ref)) < 1e-12
+    with pytest.raises(ValueError):
+        ss.set_site_params(dF, blocked, np.zeros(shape), local=True) if ss.world > 1 else ss.local_part(dF[:-1], ss.owned[0])
+    return ss
+
+
 def _worker(rank, world, port, q):
     import torch.distributed as dist
 
@@ -126,6 +143,7 @@ def _worker(rank, world, port, q):
             for spr in (1, 2):
                 ss = _run((11, 3, 4), bc, spr, 9)
                 assert ss.world == 2 and ss.n_slabs == 2 * spr and ss.owned == list(range(rank * spr, (rank + 1) * spr))
+                _run_local((11, 3, 4), bc, spr, 9)
         q.put((rank, "ok"))
     except Exception as exc:  # report instead of hanging the other rank
         q.put((rank, repr(exc)))
@@ -151,6 +169,7 @@ def test_two_ranks_exchange_planes_and_add_series():
 @pytest.mark.parametrize("spr", [1, 2, 5])
 def test_single_process_slabs(bc, spr):
     _run((11, 3, 4), bc, spr, 9)
+    _run_local((11, 3, 4), bc, spr, 9)
 
 
 def test_ranges_neighbours_and_message_order():
