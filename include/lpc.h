@@ -56,8 +56,11 @@ extern "C" {
 #define LPC_HALO_STATE 1  /* the current state: 2 + n_density + n_moments channel planes      */
 #define LPC_HALO_STATE0 2 /* the same planes of state buffer 0 / 1 explicitly (the two buffers  */
 #define LPC_HALO_STATE1 3 /* alternate from step to step; for lpc_set_halo_peers)               */
-#define LPC_HALO_SEND 0   /* the outermost owned plane on that side                           */
-#define LPC_HALO_RECV 1   /* the ghost plane beyond it                                        */
+#define LPC_HALO_STATE2 4  /* the current state, TWO planes per face (for slabs that take two steps per sweep)  */
+#define LPC_HALO_PARAMS2 5 /* pi, two planes per face                                                            */
+#define LPC_HALO_PHASE2 6  /* cos and sin of omega dt (2 channels), two planes per face                          */
+#define LPC_HALO_SEND 0   /* the outermost owned plane(s) on that side                        */
+#define LPC_HALO_RECV 1   /* the ghost plane(s) beyond                                        */
 
 /* lpc_set_kernel selectors */
 #define LPC_KERNEL_AUTO 0
@@ -234,9 +237,15 @@ int lpc_spectrum(lpc_lattice* lat, int32_t region, int64_t count, double f0_hz, 
  * G[n], Z_d[m] of a slab are the sums over its own sites: the caller adds the ranks' series (one reduction
  * when the series is read, none per step); D follows from the summed Z_d as in lpc_moments.  The equilibration
  * loop runs the same way: lpc_equilibrate(lat, threshold, 1, 1, ...) is one sweep, the caller exchanges
- * LPC_HALO_STATE and takes the largest delta of all slabs.  Not available in slab mode: lpc_step_n with n > 1,
- * lpc_equilibrate with max_iters > 1 (LPC_ESTATE), the persistent kernel (never chosen), link factors
- * (LPC_EINVAL at creation).                                                                                  */
+ * LPC_HALO_STATE and takes the largest delta of all slabs.
+ * Two steps per sweep on slabs: when lpc_time_block_steps(lat) == 2 (magnetisation alone, at least two planes), the
+ * caller may exchange TWO planes per face -- LPC_HALO_PARAMS2 and LPC_HALO_PHASE2 once before lpc_slab_finish,
+ * LPC_HALO_STATE2 instead of LPC_HALO_STATE every time -- and then call lpc_step_n(lat, 2): one sweep, one exchange of
+ * the same bytes per step.  The two planes of a face are one contiguous run.  A caller that exchanges one plane keeps
+ * to lpc_step_n(lat, 1).
+ * Not available in slab mode: lpc_step_n with n > 2 (or n = 2 without the two-plane exchange), lpc_equilibrate with
+ * max_iters > 1 (LPC_ESTATE), the persistent kernel (never chosen), link factors (LPC_EINVAL at creation), direct halo
+ * stores together with two steps per sweep.                                                                    */
 
 /* Z_local = sum of exp(-dF_i) over the open sites of this lattice (Eq. 2).  dF_kT, blocked: host
  * or device, as lpc_set_site_params.  out: host.  Synchronises.  Errors: LPC_EINVAL, LPC_ECUDA.              */
@@ -297,6 +306,9 @@ int lpc_set_kernel(lpc_lattice* lat, int32_t which);
  * compute.  Takes effect from the next lpc_step_n.  Errors: LPC_EINVAL (unknown key, value out
  * of range, or LPC_OPT_TIME_BLOCK = 2 on a lattice that cannot run the two-step sweep).          */
 int lpc_set_option(lpc_lattice* lat, int32_t key, int64_t value);
+
+/* 2 if the next lpc_step_n(lat, n >= 2) takes two time steps per sweep (see lpc_step_n), else 1.  */
+int32_t lpc_time_block_steps(const lpc_lattice* lat);
 
 /* Steps taken since the last lpc_set_site_params / lpc_set_state(G).                           */
 int64_t lpc_steps_done(const lpc_lattice* lat);

@@ -22,6 +22,7 @@ LPC_OK, LPC_EINVAL, LPC_ESTATE, LPC_ENOMEM, LPC_ECUDA = 0, -1, -2, -3, -4
 LPC_FIELD_G, LPC_FIELD_PI, LPC_FIELD_PX, LPC_FIELD_PY, LPC_FIELD_PZ, LPC_FIELD_RHO = range(6)
 LPC_BC_HALO = 2
 LPC_HALO_PARAMS, LPC_HALO_STATE, LPC_HALO_STATE0, LPC_HALO_STATE1 = 0, 1, 2, 3
+LPC_HALO_STATE2, LPC_HALO_PARAMS2, LPC_HALO_PHASE2 = 4, 5, 6
 LPC_HALO_SEND, LPC_HALO_RECV = 0, 1
 LPC_KERNEL_AUTO, LPC_KERNEL_DIRECT, LPC_KERNEL_TMA, LPC_KERNEL_PERSIST = range(4)
 LPC_OPT_TIME_BLOCK, LPC_OPT_X_CHUNK, LPC_OPT_X_CHUNK2, LPC_OPT_PERSIST_MAX_MB, LPC_OPT_REGION_FUSION = 1, 2, 3, 4, 5
@@ -29,7 +30,7 @@ LPC_OPT_TIME_BLOCK, LPC_OPT_X_CHUNK, LPC_OPT_X_CHUNK2, LPC_OPT_PERSIST_MAX_MB, L
 EXPORTS = (
     "lpc_workspace_bytes", "lpc_create_lattice", "lpc_set_site_params", "lpc_set_link_mobility", "lpc_step_n", "lpc_read_fid",
     "lpc_moments", "lpc_read_field", "lpc_set_state", "lpc_equilibrate", "lpc_seed_from_density", "lpc_set_regions", "lpc_read_fid_region", "lpc_moments_region", "lpc_spectrum", "lpc_set_kernel",
-    "lpc_set_option", "lpc_ipc_export", "lpc_ipc_open", "lpc_ipc_close", "lpc_steps_done", "lpc_partition_sum", "lpc_set_partition_sum", "lpc_halo_view", "lpc_set_halo_peers", "lpc_slab_finish",
+    "lpc_set_option", "lpc_time_block_steps", "lpc_ipc_export", "lpc_ipc_open", "lpc_ipc_close", "lpc_steps_done", "lpc_partition_sum", "lpc_set_partition_sum", "lpc_halo_view", "lpc_set_halo_peers", "lpc_slab_finish",
     "lpc_launch_count", "lpc_bytes_per_site_step", "lpc_destroy", "lpc_last_error",
 )
 
@@ -89,6 +90,8 @@ def _load():
     lib.lpc_read_fid_region.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_int64, C.c_void_p]
     lib.lpc_moments_region.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_void_p, C.c_void_p]
     lib.lpc_spectrum.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_double, C.c_double, C.c_int64, C.c_double, C.c_void_p]
+    lib.lpc_time_block_steps.argtypes = [C.c_void_p]
+    lib.lpc_time_block_steps.restype = C.c_int32
     lib.lpc_steps_done.argtypes = [C.c_void_p]
     lib.lpc_steps_done.restype = C.c_int64
     lib.lpc_launch_count.argtypes = [C.c_void_p]
@@ -304,6 +307,10 @@ def lpc_set_option(handle, key, value):
     _check(_lib.lpc_set_option(handle, int(key), int(value)))
 
 
+def lpc_time_block_steps(handle) -> int:
+    return int(_lib.lpc_time_block_steps(handle))
+
+
 def lpc_steps_done(handle) -> int:
     return int(_lib.lpc_steps_done(handle))
 
@@ -465,6 +472,10 @@ class Lattice:
 
     def set_option(self, key, value):
         lpc_set_option(self.handle, key, value)
+
+    @property
+    def time_block_steps(self):
+        return lpc_time_block_steps(self.handle)
 
     @property
     def steps_done(self):

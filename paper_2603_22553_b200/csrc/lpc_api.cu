@@ -563,6 +563,7 @@ int fill_state_ghosts(lpc_lattice* h) {
 // may the next steps of this lattice run two at a time?
 bool step2_usable(const lpc_lattice* h) {
   if (!h->step2_ok || h->time_block == 1 || h->have_links || h->have_regions) return false;
+  if (h->peer[0][0] || h->peer[1][0]) return false;   // direct halo stores belong to the one-step sweep
   if (h->kernel == LPC_KERNEL_DIRECT || h->kernel == LPC_KERNEL_PERSIST) return false;
   return true;
 }
@@ -1010,7 +1011,7 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
   h->tma_ok = (size_t)h->tiles_z * h->tiles_y * h->chunks_x <= h->off.partial_slots;
   // two steps per sweep: the magnetisation channels alone, no slab, and every periodic axis long enough for two ghost layers
   step2_geometry(cfg->nx, h->tiles_z * h->tiles_y, 0, &h->xc2, &h->chunks_x2);
-  h->step2_ok = h->tma_ok && h->nrho == 0 && h->nmom == 0 && !h->halo;
+  h->step2_ok = h->tma_ok && h->nrho == 0 && h->nmom == 0 && !(h->halo && cfg->nx < 2);
   for (int d = 0; d < 3; ++d) {
     const int n = d == 0 ? cfg->nx : d == 1 ? cfg->ny : cfg->nz;
     if (cfg->bc[d] == 0 && n < 4) h->step2_ok = false;
@@ -1110,10 +1111,21 @@ int lpc_halo_view(lpc_lattice* h, int32_t set, int32_t side, int32_t role, void*
                   int32_t* n_channels) {
   if (!h) return fail(LPC_EINVAL, "lattice is NULL");
   if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
-  if ((set != LPC_HALO_PARAMS && set != LPC_HALO_STATE && set != LPC_HALO_STATE0 && set != LPC_HALO_STATE1) || (side != 0 && side != 1) || (role != LPC_HALO_SEND && role != LPC_HALO_RECV))
+  if (set < LPC_HALO_PARAMS || set > LPC_HALO_PHASE2 || (side != 0 && side != 1) || (role != LPC_HALO_SEND && role != LPC_HALO_RECV))
     return fail(LPC_EINVAL, "bad selector (set %d, side %d, role %d)", set, side, role);
   if (!plane || !plane_bytes || !stride_bytes || !n_channels) return fail(LPC_EINVAL, "output pointers must not be NULL");
   const Layout& L = h->L;
+  if (set >= LPC_HALO_STATE2) {
+    // two planes per face, one contiguous run: owned planes gh, gh+1 / gh+nx-2, gh+nx-1; ghost planes 0, 1 / gh+nx, gh+nx+1
+    if (L.nx < 2) return fail(LPC_ESTATE, "a two-plane halo needs at least two owned planes");
+    const long long xp2 = side == 0 ? (role == LPC_HALO_SEND ? L.gh : L.gh - 2) : (role == LPC_HALO_SEND ? L.gh + L.nx - 2 : L.gh + L.nx);
+    const size_t base2 = set == LPC_HALO_PARAMS2 ? h->off.pi : set == LPC_HALO_PHASE2 ? h->off.cs : (h->cur ? h->off.f1 : h->off.f0);
+    *plane = h->ws + base2 + (size_t)xp2 * L.sx * h->sT;
+    *plane_bytes = 2 * (size_t)L.sx * h->sT;
+    *stride_bytes = (size_t)L.np * h->sT;
+    *n_channels = set == LPC_HALO_PARAMS2 ? 1 : set == LPC_HALO_PHASE2 ? 2 : h->C;
+    return LPC_OK;
+  }
   // padded x index: ghost planes 0 .. gh-1, owned gh .. gh+nx-1, ghost planes gh+nx ..; the exchange moves the innermost ghost plane
   const long long xp = side == 0 ? (role == LPC_HALO_SEND ? L.gh : L.gh - 1) : (role == LPC_HALO_SEND ? L.gh + L.nx - 1 : L.gh + L.nx);
   const size_t base = set == LPC_HALO_PARAMS ? h->off.pi
@@ -1204,7 +1216,8 @@ int lpc_step_n(lpc_lattice* h, int64_t n) {
   if (n < 0) return fail(LPC_EINVAL, "n must be >= 0");
   if (h->steps + n > h->cfg.max_steps) return fail(LPC_EINVAL, "steps_done + n = %lld exceeds max_steps = %lld", (long long)(h->steps + n), (long long)h->cfg.max_steps);
   if (h->halo && !h->halo_ready) return fail(LPC_ESTATE, "slab mode: lpc_slab_finish has not been called");
-  if (h->halo && n > 1) return fail(LPC_ESTATE, "slab mode: the x ghost planes must be exchanged after every step (n <= 1)");
+  if (h->halo && n > 1 && !(n == 2 && step2_usable(h)))
+    return fail(LPC_ESTATE, "slab mode: the x ghost planes must be exchanged after every sweep (n <= 1, or n = 2 on a lattice with lpc_time_block_steps = 2 and two-plane exchanges)");
   const bool persist = !h->have_regions && n >= 2 &&
                        (h->kernel == LPC_KERNEL_PERSIST || (h->kernel == LPC_KERNEL_AUTO && persist_by_default(h)));
   if (persist) return h->cfg.precision ? launch_persist<float>(h, n) : launch_persist<double>(h, n);
@@ -1229,6 +1242,12 @@ int lpc_step_n(lpc_lattice* h, int64_t n) {
       rc = region_reduce(h, h->steps);
       if (rc) return rc;
     }
+  }
+  // a slab that may take two steps per sweep hands whole planes to its neighbours, y and z ghosts included: after a
+  // one-step sweep bring the full shell of the owned planes up to date before the caller's exchange
+  if (h->halo && n > 0 && step2_usable(h) && !h->ghosts_full) {
+    int rc = h->cfg.precision ? fill_state_ghosts<float>(h) : fill_state_ghosts<double>(h);
+    if (rc) return rc;
   }
   return LPC_OK;
 }
@@ -1428,6 +1447,7 @@ int lpc_set_option(lpc_lattice* h, int32_t key, int64_t value) {
   }
 }
 
+int32_t lpc_time_block_steps(const lpc_lattice* h) { return (h && step2_usable(h)) ? 2 : 1; }
 int64_t lpc_steps_done(const lpc_lattice* h) { return h ? h->steps : 0; }
 int64_t lpc_launch_count(const lpc_lattice* h) { return h ? h->launches : 0; }
 

@@ -17,6 +17,7 @@ import numpy as np
 
 LPC_BC_HALO = 2
 HALO_PARAMS, HALO_STATE = 0, 1
+HALO_STATE2, HALO_PARAMS2, HALO_PHASE2 = 4, 5, 6   # two planes per face: slabs that take two time steps per sweep
 SEND, RECV = 0, 1
 
 
@@ -86,6 +87,10 @@ class SlabSet:
             lo, hi = self.ranges[s]
             self.lat[s] = lattice_factory((hi - lo,) + self.global_shape[1:], bc=(LPC_BC_HALO, self.bc[1], self.bc[2]), **cfg)
         self.steps = 0
+        # two time steps per sweep (include/lpc.h "Slabs"): every slab of every rank must be able to, because all slabs
+        # exchange two planes per face then
+        can = all(getattr(m, "time_block_steps", 1) == 2 for m in self.lat.values())
+        self.two_step = bool(self._allreduce_min(1.0 if can else 0.0) > 0.5)
         self.direct = set()   # (src slab, src side) of OWNED slabs whose plane the step kernel stores into the neighbour itself
         self.direct_all = set()   # the same over the slabs of all ranks: what both ends of a message skip after a step
         self.remote_direct = False
@@ -102,6 +107,7 @@ class SlabSet:
         that are not direct keep the copy / send-recv.  Call after set_site_params.  Returns the direct faces here."""
         self.direct = set()
         self._close_peers()
+        self.two_step = False   # the direct stores ride on the one-step sweep
         remote = bool(remote) and self.dist is not None and self.world > 1
         table = {}
         if remote:
@@ -256,25 +262,40 @@ class SlabSet:
         for s in self.owned:
             self.lat[s].set_partition_sum(Z)
             self.lat[s].set_site_params(*parts[s])
-        self.exchange(HALO_PARAMS)
+        if self.two_step:
+            self.exchange(HALO_PARAMS2)
+            self.exchange(HALO_PHASE2)     # the two-step sweep rotates the ring of neighbour sites as well
+        else:
+            self.exchange(HALO_PARAMS)
         for s in self.owned:
             self.lat[s].slab_finish()
         if g0 is not None:
             for s in self.owned:
                 self.lat[s].set_state(0, self.local_part(g0, s, local))
-        self.exchange(HALO_STATE)
+        self.exchange(self.state_set)
         self.steps = 0
         return Z
 
+    @property
+    def state_set(self):
+        """Which planes of the state an exchange moves: two per face for slabs that take two steps per sweep."""
+        return HALO_STATE2 if self.two_step else HALO_STATE
+
     def step(self, n=1):
-        """n time steps: per step one sweep per slab, then the plane exchange."""
-        for _ in range(int(n)):
+        """n time steps: per sweep (one step, or two on slabs that can) one launch per slab, then the plane exchange."""
+        n = int(n)
+        while n > 0:
+            k = 2 if (self.two_step and n >= 2) else 1
             for s in self.owned:
-                self.lat[s].step(1)
-            self.exchange(HALO_STATE, after_step=True)
+                self.lat[s].step(k)
+            self.exchange(self.state_set, after_step=True)
             if self.remote_direct:
                 self._step_fence()
-            self.steps += 1
+            self.steps += k
+            n -= k
+
+    def _allreduce_min(self, v: float) -> float:
+        return -self._allreduce_max(-v)
 
     def _allreduce_max(self, v: float) -> float:
         if self.dist is None or self.world == 1:
@@ -291,7 +312,7 @@ class SlabSet:
         """arr over the WHOLE lattice (e.g. an initial density for the equilibration loop)."""
         for s in self.owned:
             self.lat[s].set_state(which, self.local_part(arr, s))
-        self.exchange(HALO_STATE)
+        self.exchange(self.state_set)
 
     def equilibrate(self, threshold, max_iters):
         """The equilibration loop over all slabs: one sweep per slab, the plane exchange, and the
@@ -302,7 +323,7 @@ class SlabSet:
             for s in self.owned:
                 _, d = self.lat[s].equilibrate(0.0, 1, 1)
                 delta = max(delta, d)
-            self.exchange(HALO_STATE)
+            self.exchange(self.state_set)
             delta = self._allreduce_max(delta)
             done += 1
             if delta < threshold:

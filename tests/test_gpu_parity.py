@@ -263,6 +263,44 @@ def test_two_step_sweep_default_and_eligibility(lpc, oracle_mod):
     assert e.value.code == lpc.LPC_EINVAL
 
 
+@pytest.mark.parametrize("bc,n_slabs,precision", [((0, 0, 0), 2, 0), ((1, 0, 0), 3, 0), ((0, 1, 0), 1, 0), ((0, 0, 1), 4, 1)])
+def test_two_step_sweep_on_slabs(lpc, oracle_mod, bc, n_slabs, precision):
+    """Slabs that carry the magnetisation alone take two steps per sweep and exchange two planes per face (include/lpc.h
+    "Slabs"): against the oracle and, bit for bit, against the unsplit lattice."""
+    from paper_2603_22553_b200 import slab
+
+    n = 31
+    lat = lpc_inputs.random_small((46, 18, 70), bc=bc, p_block=0.25, alpha=0.9, seed=83, n_steps=n, n_moments=0)
+    rng = np.random.default_rng(5)
+    g0 = (rng.random(lat.shape) + 1j * rng.random(lat.shape)) * (lat.blocked == 0)
+    ss = slab.SlabSet(lat.shape, bc=lat.bc, slabs_per_rank=n_slabs, precision=precision, dt=lat.dt, a=lat.a, alpha=lat.alpha, max_steps=n)
+    assert ss.two_step
+    ss.set_site_params(lat.dF, lat.blocked, lat.omega, g0)
+    l0 = sum(m.launch_count for m in ss.lat.values())
+    ss.step(n)                  # fifteen two-step sweeps and one one-step sweep per slab (plus one ghost refill)
+    assert sum(m.launch_count for m in ss.lat.values()) - l0 <= n_slabs * (n // 2 + 3)
+    orc = oracle_mod.Oracle.from_lattice(lat, n_moments=0, max_steps=n)
+    orc.set_g(g0)
+    orc.step(n)
+    G_o, sabs = orc.fid(with_scale=True)
+    tol_site, tol_sum = (1e-5, 1e-5) if precision else (1e-10, 1e-9)
+    assert np.max(np.abs(ss.fid() - G_o) / sabs) <= tol_sum
+    pi, opn = orc.pi(), lat.blocked == 0
+    hmax = np.max(np.abs(g0)[opn] / pi[opn])
+    g = ss.gather_field(lpc.LPC_FIELD_G, dtype=np.complex128)
+    assert np.max(np.abs(g - orc.g())[opn] / pi[opn]) <= tol_site * hmax
+    # more steps after an odd count: the one-step sweep left the shells to be refilled before the next exchange
+    ss2 = slab.SlabSet(lat.shape, bc=lat.bc, slabs_per_rank=n_slabs, precision=precision, dt=lat.dt, a=lat.a, alpha=lat.alpha, max_steps=n)
+    ss2.set_site_params(lat.dF, lat.blocked, lat.omega, g0)
+    for k in (3, 1, 8, 19):
+        ss2.step(k)
+    assert np.array_equal(ss2.gather_field(lpc.LPC_FIELD_G, dtype=np.complex128), g)
+    if precision == 0:
+        whole = lpc.Lattice.from_inputs(lat, max_steps=n, g0=g0)
+        whole.step(n)
+        assert np.max(np.abs(g - whole.field(lpc.LPC_FIELD_G))[opn] / pi[opn]) <= 1e-12 * hmax
+
+
 # ---------------------------------------------------------------------------------------------
 # states set from outside, device-resident inputs
 # ---------------------------------------------------------------------------------------------
