@@ -87,7 +87,7 @@ struct lpc_lattice {
   int time_block;     // LPC_OPT_TIME_BLOCK: 0 auto, 1 one step per sweep, 2 two steps per sweep whenever possible
   int xc2, chunks_x2; // its x chunks
   bool ghosts_full;   // the whole ghost shell of the current state is valid (the one-step sweeps keep the face layer only)
-  CUtensorMap tm2_f[2], tm2_pi, tm2_cs;
+  CUtensorMap tm2_f[2], tm2_m[2], tm2_pi, tm2_cs;   // tm2_m: the three moment channels
   int opt_xc, opt_persist_mb, opt_region_fusion;   // lpc_set_option overrides (0 = default)
   // TMA geometry
   int ty, tz, nstage, xc, tiles_z, tiles_y, chunks_x;
@@ -571,7 +571,7 @@ bool step2_usable(const lpc_lattice* h) {
 template <typename T>
 int launch_step2_t(lpc_lattice* h) {
   constexpr int VW = 16 / (int)sizeof(T);
-  using K = Step2Cfg<T, VW>;
+  using K = Step2Cfg<T, VW, 2>;
   if (!h->ghosts_full) {   // the sweep reads two ghost layers, edges included
     int rc = fill_state_ghosts<T>(h);
     if (rc) return rc;
@@ -591,14 +591,28 @@ int launch_step2_t(lpc_lattice* h) {
   a.vacf_stride = h->cfg.max_steps + 2;
   for (int d = 0; d < 3; ++d) a.per[d] = h->cfg.bc[d] == 0;
   a.xc = h->xc2; a.tiles_z = h->tiles_z; a.tiles_y = h->tiles_y; a.chunks_x = h->chunks_x2;
-  static bool attr_done[MAX_DEVICES] = {};
-  if (int rc = ensure_dyn_smem(step2_kernel<T, VW>, K::SMEM_BYTES, h->device, attr_done)) return rc;
+  a.zscale = h->cfg.a * h->cfg.alpha / 6.0;
   const unsigned grid = (unsigned)(h->tiles_z * h->tiles_y * h->chunks_x2);
-  step2_kernel<T, VW><<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(h->tm2_f[h->cur], h->tm2_pi, h->tm2_cs, a);
+  if (h->nmom == 3) {
+    // the three moment channels first (Z_d of both steps; they read the step counter the magnetisation sweep advances)
+    using KM = Step2Cfg<T, VW, 3>;
+    StepArgs<T> am = a;
+    am.c0 = 2;
+    am.fout = a.fout + 2 * h->L.np;
+    static bool attr_done_m[MAX_DEVICES] = {};
+    if (int rc = ensure_dyn_smem(step2_kernel<T, VW, 3>, KM::SMEM_BYTES, h->device, attr_done_m)) return rc;
+    step2_kernel<T, VW, 3><<<grid, KM::NTHREADS, KM::SMEM_BYTES, h->stream>>>(h->tm2_m[h->cur], h->tm2_pi, h->tm2_cs, am);
+    CUDA_TRY(cudaGetLastError());
+    h->launches++;
+  }
+  a.c0 = 0;
+  static bool attr_done[MAX_DEVICES] = {};
+  if (int rc = ensure_dyn_smem(step2_kernel<T, VW, 2>, K::SMEM_BYTES, h->device, attr_done)) return rc;
+  step2_kernel<T, VW, 2><<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(h->tm2_f[h->cur], h->tm2_pi, h->tm2_cs, a);
   CUDA_TRY(cudaGetLastError());
   h->launches++;
   h->cur ^= 1;
-  return LPC_OK;   // the sweep stores every ghost image itself: the shell stays valid
+  return LPC_OK;   // the sweeps store every ghost image themselves: the shell stays valid
 }
 
 int launch_step2(lpc_lattice* h) { return h->cfg.precision ? launch_step2_t<float>(h) : launch_step2_t<double>(h); }
@@ -1011,7 +1025,7 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
   h->tma_ok = (size_t)h->tiles_z * h->tiles_y * h->chunks_x <= h->off.partial_slots;
   // two steps per sweep: the magnetisation channels alone, no slab, and every periodic axis long enough for two ghost layers
   step2_geometry(cfg->nx, h->tiles_z * h->tiles_y, 0, &h->xc2, &h->chunks_x2);
-  h->step2_ok = h->tma_ok && h->nrho == 0 && h->nmom == 0 && !(h->halo && cfg->nx < 2);
+  h->step2_ok = h->tma_ok && h->nrho == 0 && !(h->halo && cfg->nx < 2);
   for (int d = 0; d < 3; ++d) {
     const int n = d == 0 ? cfg->nx : d == 1 ? cfg->ny : cfg->nz;
     if (cfg->bc[d] == 0 && n < 4) h->step2_ok = false;
@@ -1042,6 +1056,9 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
       const cuuint32_t b2k[4] = {zw, (cuuint32_t)(h->ty + 2), 1, 2};
       rc = encode_map(&h->tm2_f[0], f32, h->ws + h->off.f0, 4, d4, b2f);
       if (!rc) rc = encode_map(&h->tm2_f[1], f32, h->ws + h->off.f1, 4, d4, b2f);
+      const cuuint32_t b2m[4] = {zw, (cuuint32_t)(h->ty + 4), 1, 3};
+      if (!rc && h->nmom == 3) rc = encode_map(&h->tm2_m[0], f32, h->ws + h->off.f0, 4, d4, b2m);
+      if (!rc && h->nmom == 3) rc = encode_map(&h->tm2_m[1], f32, h->ws + h->off.f1, 4, d4, b2m);
       if (!rc) rc = encode_map(&h->tm2_pi, f32, h->ws + h->off.pi, 3, d4, b2f);
       if (!rc) rc = encode_map(&h->tm2_cs, f32, h->ws + h->off.cs, 4, dk, b2k);
     }

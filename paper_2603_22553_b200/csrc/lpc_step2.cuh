@@ -1,6 +1,6 @@
 // lpc_step2.cuh -- TWO time steps per sweep (temporal blocking of Eq. 13; north star (b) "optional temporal
-// blocking of several steps per pass").  The magnetisation kernel alone (h_re, h_im; no density, moment or
-// link channels, no region labels, no slabs).
+// blocking of several steps per pass").  The magnetisation channels (h_re, h_im) or the three moment
+// channels of the VACF; no density or link channels, no region labels, no direct halo stores.
 //
 // Eq. 13 is a Jacobi update: g(n+1) depends on g(n) at the site and its six neighbours only.  Two steps therefore depend
 // on the sites within two hops, and a CTA that stages a (TY+4) x (TZ+2 VW) window of the y-z plane can advance its
@@ -32,8 +32,12 @@
 
 namespace lpc {
 
-template <typename T, int VW, int TZ_ = 64>
+// NC = 2: the magnetisation (h_re, h_im; phase rotation; G of both steps).  NC = 3: the three moment fields q^d of the
+// VACF (Eq. 4; no phase, no cos / sin traffic; Z_d of both steps) -- they propagate independently of the
+// magnetisation, so a lattice with moment fields runs one two-step sweep of each kind per two steps.
+template <typename T, int VW, int NC = 2, int TZ_ = 64>
 struct Step2Cfg {
+  static constexpr bool MAG = (NC == 2);
   static constexpr int TZ = TZ_;
   static constexpr int TY = 4 * VW;                 // 8 rows of z-pairs in fp64, 16 rows of z-quads in fp32: 256 own groups
   static constexpr int GZ = TZ / VW;                // own groups per row
@@ -45,25 +49,26 @@ struct Step2Cfg {
   static constexpr int N2 = TY * GZ;                // thread slots of the second step (256)
   static constexpr int NTHREADS = (N1 + 31) / 32 * 32;
   static constexpr int NSTAGE = 6;                  // a plane is in use for four iterations; two more are in flight
-  static constexpr int F_BYTES = 2 * R0 * TZW * (int)sizeof(T);
+  static constexpr int F_BYTES = NC * R0 * TZW * (int)sizeof(T);
   static constexpr int PI_BYTES = R0 * TZW * (int)sizeof(T);
-  static constexpr int CS_BYTES = 2 * R1 * TZW * (int)sizeof(T);
+  static constexpr int CS_BYTES = MAG ? 2 * R1 * TZW * (int)sizeof(T) : 0;
   static constexpr int STAGE_BYTES = F_BYTES + PI_BYTES + CS_BYTES;
-  static constexpr int RING_PLANE = 2 * R1 * TZW * (int)sizeof(T);
+  static constexpr int RING_PLANE = NC * R1 * TZW * (int)sizeof(T);
   static constexpr int RING_OFF = NSTAGE * STAGE_BYTES;
   static constexpr int BAR_OFF = RING_OFF + 3 * RING_PLANE;
   static constexpr int RED_OFF = BAR_OFF + NSTAGE * 8;
-  static constexpr int NRED = 4;
+  static constexpr int NRED = 2 * (MAG ? 2 : 3);    // G_re, G_im (or Z_x, Z_y, Z_z) of the first and of the second step
   static constexpr int SMEM_BYTES = RED_OFF + ((NTHREADS / 32) * NRED + 2) * 8 + 128;   // +128: manual alignment slack
-  static_assert(F_BYTES % 128 == 0 && PI_BYTES % 128 == 0 && CS_BYTES % 128 == 0 && RING_PLANE % 128 == 0, "TMA boxes land 128-byte aligned");
+  static_assert(F_BYTES % 128 == 0 && PI_BYTES % 128 == 0 && CS_BYTES % 128 == 0, "TMA boxes land 128-byte aligned");
+  static_assert(RING_PLANE % 16 == 0 && RING_OFF % 128 == 0, "16-byte vector accesses to the ring");
   static_assert(SMEM_BYTES <= 227 * 1024, "one CTA per SM");
 };
 
 // A group of a periodic face region and all its ghost images: every combination of the shifts that map the site into the
 // ghost shell (two layers in x, y and z; edges and corners included).  Rare, out of line.
 template <typename T, int VW>
-__device__ __noinline__ void store_images(T* __restrict__ base, long long sx, long long sy, int gh, int nzp_pad, int nyp, int nx, int ny, int nz, int permask,
-                                          int x, int y, int z, typename VecN<T, VW>::type v, int nvalid) {
+__device__ __noinline__ void store_images(T* __restrict__ base, long long sx, long long sy, int gh, int padz, int nx, int ny, int nz, int permask, int x,
+                                          int y, int z, typename VecN<T, VW>::type v, int nvalid) {
   T o[VW];
   o[0] = v.x; o[1] = v.y;
   if constexpr (VW == 4) { o[2] = v.z; o[3] = v.w; }
@@ -77,10 +82,7 @@ __device__ __noinline__ void store_images(T* __restrict__ base, long long sx, lo
     if (y < GH) dy[ndy++] = ny;
     if (y >= ny - GH) dy[ndy++] = -ny;
   }
-  (void)nyp;
-#pragma unroll
-  for (int k = 0; k < VW; ++k) {
-    if (k >= nvalid) break;
+  for (int k = 0; k < VW && k < nvalid; ++k) {
     const int zk = z + k;
     int dz[3], ndz = 1;
     dz[0] = 0;
@@ -91,17 +93,19 @@ __device__ __noinline__ void store_images(T* __restrict__ base, long long sx, lo
     for (int a = 0; a < ndx; ++a)
       for (int b = 0; b < ndy; ++b)
         for (int c = 0; c < ndz; ++c)
-          base[(long long)(x + dx[a] + gh) * sx + (long long)(y + dy[b] + gh) * sy + (zk + dz[c] + nzp_pad)] = o[k];
+          base[(long long)(x + dx[a] + gh) * sx + (long long)(y + dy[b] + gh) * sy + (zk + dz[c] + padz)] = o[k];
   }
 }
 
-template <typename T, int VW>
-__global__ void __launch_bounds__(Step2Cfg<T, VW>::NTHREADS, 1)
+template <typename T, int VW, int NC>
+__global__ void __launch_bounds__(Step2Cfg<T, VW, NC>::NTHREADS, 1)
     step2_kernel(const __grid_constant__ CUtensorMap tm_f, const __grid_constant__ CUtensorMap tm_pi, const __grid_constant__ CUtensorMap tm_cs,
                  StepArgs<T> a) {
-  using K = Step2Cfg<T, VW>;
+  using K = Step2Cfg<T, VW, NC>;
   using V = typename VecN<T, VW>::type;
   constexpr int TZW = K::TZW, R0 = K::R0, R1 = K::R1, NS = K::NSTAGE;
+  constexpr bool MAG = K::MAG;
+  constexpr int HR = K::NRED / 2;   // reductions per step
   extern __shared__ __align__(128) unsigned char smem_raw[];
   unsigned char* smem = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
   uint64_t* full = reinterpret_cast<uint64_t*>(smem + K::BAR_OFF);
@@ -128,14 +132,14 @@ __global__ void __launch_bounds__(Step2Cfg<T, VW>::NTHREADS, 1)
     unsigned char* st = smem + s * K::STAGE_BYTES;
     mbar_expect_tx(&full[s], K::STAGE_BYTES);
     const int pz = L.padz + z0 - VW, py = y0 + L.gh - 2, px = x0 + j + L.gh - 2;
-    tma_load_4d(st, &tm_f, &full[s], pz, py, px, 0);
+    tma_load_4d(st, &tm_f, &full[s], pz, py, px, a.c0);
     tma_load_3d(st + K::F_BYTES, &tm_pi, &full[s], pz, py, px);
-    tma_load_4d(st + K::F_BYTES + K::PI_BYTES, &tm_cs, &full[s], pz, py + 1, px, 0);
+    if constexpr (MAG) tma_load_4d(st + K::F_BYTES + K::PI_BYTES, &tm_cs, &full[s], pz, py + 1, px, 0);
   };
   if (tid == 0) {
     tma_prefetch_desc(&tm_f);
     tma_prefetch_desc(&tm_pi);
-    tma_prefetch_desc(&tm_cs);
+    if constexpr (MAG) tma_prefetch_desc(&tm_cs);
     for (int j = 0; j < 4 && j < nin; ++j) issue(j);
   }
 
@@ -164,7 +168,7 @@ __global__ void __launch_bounds__(Step2Cfg<T, VW>::NTHREADS, 1)
 
   // one x-plane as a thread holds it: the group's h and pi, and mlo = the link weight towards the plane below
   struct Plane {
-    T f[2][VW];
+    T f[NC][VW];
     T pi[VW], mlo[VW];
   };
   auto stage_of = [&](int j) -> const unsigned char* { return smem + (j % NS) * K::STAGE_BYTES; };
@@ -172,13 +176,16 @@ __global__ void __launch_bounds__(Step2Cfg<T, VW>::NTHREADS, 1)
 
   // the update of one group whose plane is the centre one: sf = h_re of the centre plane at the group (h_im is fch elements
   // further), sp = pi, sc = cos (sin is kch further); in-plane neighbours at +-TZW (y) and -1 / +VW (z)
-  auto update = [&](const Plane& prv, const Plane& ctr, const Plane& nxt, const T* sf, int fch, const T* sp, const T* sc, int kch, T (&o)[2][VW]) {
+  auto update = [&](const Plane& prv, const Plane& ctr, const Plane& nxt, const T* sf, int fch, const T* sp, const T* sc, int kch, T (&o)[NC][VW],
+                    double* zacc, int nvz) {
     T pym[VW], pyp[VW], csv[VW], snv[VW];
     ldv<T, VW>(sp - TZW, pym);
     ldv<T, VW>(sp + TZW, pyp);
     const T pzm = sp[-1], pzp = sp[VW];
-    ldv<T, VW>(sc, csv);
-    ldv<T, VW>(sc + kch, snv);
+    if constexpr (MAG) {
+      ldv<T, VW>(sc, csv);
+      ldv<T, VW>(sc + kch, snv);
+    }
     SiteUpdate<T, 0, 0> u[VW];
 #pragma unroll
     for (int k = 0; k < VW; ++k) {
@@ -196,21 +203,36 @@ __global__ void __launch_bounds__(Step2Cfg<T, VW>::NTHREADS, 1)
       u[k].sum_weights();
     }
 #pragma unroll
-    for (int c = 0; c < 2; ++c) {
+    for (int c = 0; c < NC; ++c) {
       const T* fcn = sf + c * fch;
       T fym[VW], fyp[VW];
       ldv<T, VW>(fcn - TZW, fym);
       ldv<T, VW>(fcn + TZW, fyp);
       const T fzm = fcn[-1], fzp = fcn[VW];
+      if constexpr (!MAG) {
+        // Z_d of this step (Eq. 4): sum over the tile's own sites of q^d_i (m_{i,+d} - m_{i,-d}), from the values BEFORE the update
+        if (zacc) {
+          double t = 0.0;
+#pragma unroll
+          for (int k = 0; k < VW; ++k) {
+            const T dm = (c == 0) ? (u[k].mxp - u[k].mxm) : (c == 1) ? (u[k].myp - u[k].mym) : (u[k].mzp - u[k].mzm);
+            const double qd = (double)ctr.f[c][k] * (double)dm;
+            if (k < nvz) t += qd;
+          }
+          zacc[c] += t;
+        }
+      }
 #pragma unroll
       for (int k = 0; k < VW; ++k)
         o[c][k] = u[k].gather(ctr.f[c][k], prv.f[c][k], nxt.f[c][k], fym[k], fyp[k], k == 0 ? fzm : ctr.f[c][k ? k - 1 : 0],
                               k == VW - 1 ? fzp : ctr.f[c][k == VW - 1 ? k : k + 1]);
     }
+    if constexpr (MAG) {
 #pragma unroll
-    for (int k = 0; k < VW; ++k) {
-      const T hr = o[0][k], hi = o[1][k];
-      phase_rotate(csv[k], snv[k], hr, hi, o[0][k], o[1][k]);
+      for (int k = 0; k < VW; ++k) {
+        const T hr = o[0][k], hi = o[1][k];
+        phase_rotate(csv[k], snv[k], hr, hi, o[0][k], o[1][k]);
+      }
     }
   };
 
@@ -218,8 +240,8 @@ __global__ void __launch_bounds__(Step2Cfg<T, VW>::NTHREADS, 1)
   auto take1 = [&](Plane& n, int j, const Plane* below) {
     const T* sf = reinterpret_cast<const T*>(stage_of(j));
     const T* sp = reinterpret_cast<const T*>(stage_of(j) + K::F_BYTES);
-    ldv<T, VW>(sf + e1, n.f[0]);
-    ldv<T, VW>(sf + R0 * TZW + e1, n.f[1]);
+#pragma unroll
+    for (int c = 0; c < NC; ++c) ldv<T, VW>(sf + c * R0 * TZW + e1, n.f[c]);
     ldv<T, VW>(sp + e1, n.pi);
     if (below) {
 #pragma unroll
@@ -230,8 +252,8 @@ __global__ void __launch_bounds__(Step2Cfg<T, VW>::NTHREADS, 1)
   auto take2 = [&](Plane& n, int j, const Plane& below) {
     const T* rf = reinterpret_cast<const T*>(smem + K::RING_OFF + (j % 3) * K::RING_PLANE);
     const T* sp = reinterpret_cast<const T*>(stage_of(j) + K::F_BYTES);
-    ldv<T, VW>(rf + k2, n.f[0]);
-    ldv<T, VW>(rf + R1 * TZW + k2, n.f[1]);
+#pragma unroll
+    for (int c = 0; c < NC; ++c) ldv<T, VW>(rf + c * R1 * TZW + k2, n.f[c]);
     ldv<T, VW>(sp + e2, n.pi);
 #pragma unroll
     for (int k = 0; k < VW; ++k) n.mlo[k] = tmin(n.pi[k], below.pi[k]);
@@ -249,12 +271,13 @@ __global__ void __launch_bounds__(Step2Cfg<T, VW>::NTHREADS, 1)
       const T* sf = reinterpret_cast<const T*>(st) + e1;
       const T* sp = reinterpret_cast<const T*>(st + K::F_BYTES) + e1;
       const T* sc = reinterpret_cast<const T*>(st + K::F_BYTES + K::PI_BYTES) + k1;
-      T o[2][VW];
-      update(Aprv, Actr, Anxt, sf, R0 * TZW, sp, sc, R1 * TZW, o);
+      T o[NC][VW];
+      const bool own_plane = j >= 2 && j <= nplanes + 1;   // a plane of this CTA's own chunk: its own sites count towards the sums
+      update(Aprv, Actr, Anxt, sf, R0 * TZW, sp, sc, R1 * TZW, o, (!MAG && own_plane) ? acc : nullptr, nv1);
       T* rf = reinterpret_cast<T*>(smem + K::RING_OFF + (j % 3) * K::RING_PLANE);
-      *reinterpret_cast<V*>(rf + k1) = packv<T, VW>(o[0]);
-      *reinterpret_cast<V*>(rf + R1 * TZW + k1) = packv<T, VW>(o[1]);
-      if (j >= 2 && j <= nplanes + 1) {   // a plane of this CTA's own chunk: its own sites count towards G[n+1]
+#pragma unroll
+      for (int c = 0; c < NC; ++c) *reinterpret_cast<V*>(rf + c * R1 * TZW + k1) = packv<T, VW>(o[c]);
+      if (MAG && own_plane) {   // G[n+1]
 #pragma unroll
         for (int k = 0; k < VW; ++k)
           if (k < nv1) {
@@ -271,22 +294,24 @@ __global__ void __launch_bounds__(Step2Cfg<T, VW>::NTHREADS, 1)
         const T* rf = reinterpret_cast<const T*>(smem + K::RING_OFF + (j % 3) * K::RING_PLANE) + k2;
         const T* sp = reinterpret_cast<const T*>(st + K::F_BYTES) + e2;
         const T* sc = reinterpret_cast<const T*>(st + K::F_BYTES + K::PI_BYTES) + k2;
-        T o[2][VW];
-        update(Bprv, Bctr, Bnxt, rf, R1 * TZW, sp, sc, R1 * TZW, o);
+        T o[NC][VW];
+        update(Bprv, Bctr, Bnxt, rf, R1 * TZW, sp, sc, R1 * TZW, o, MAG ? nullptr : acc + HR, nv2);
+        if constexpr (MAG) {   // G[n+2]
 #pragma unroll
-        for (int k = 0; k < VW; ++k)
-          if (k < nv2) {
-            acc[2] += (double)Bctr.pi[k] * (double)o[0][k];
-            acc[3] += (double)Bctr.pi[k] * (double)o[1][k];
-          }
+          for (int k = 0; k < VW; ++k)
+            if (k < nv2) {
+              acc[2] += (double)Bctr.pi[k] * (double)o[0][k];
+              acc[3] += (double)Bctr.pi[k] * (double)o[1][k];
+            }
+        }
         if (nv2 > 0) {
           if (edge_yz || (a.per[0] && (x < GH || x >= L.nx - GH))) {
 #pragma unroll
-            for (int c = 0; c < 2; ++c)
-              store_images<T, VW>(a.fout + (long long)c * L.np, L.sx, L.sy, L.gh, L.padz, L.nyp, L.nx, L.ny, L.nz, permask, x, y2, z2, packv<T, VW>(o[c]), nv2);
+            for (int c = 0; c < NC; ++c)
+              store_images<T, VW>(a.fout + (long long)c * L.np, L.sx, L.sy, L.gh, L.padz, L.nx, L.ny, L.nz, permask, x, y2, z2, packv<T, VW>(o[c]), nv2);
           } else {
 #pragma unroll
-            for (int c = 0; c < 2; ++c) store_vec<T, VW>(outp + (long long)c * L.np, packv<T, VW>(o[c]), nv2);
+            for (int c = 0; c < NC; ++c) store_vec<T, VW>(outp + (long long)c * L.np, packv<T, VW>(o[c]), nv2);
           }
         }
         outp += L.sx;
@@ -318,7 +343,8 @@ __global__ void __launch_bounds__(Step2Cfg<T, VW>::NTHREADS, 1)
   if (t < niter) { iteration(t, A0, A1, A2, B1, B2, B0); ++t; }
   if (t < niter) { iteration(t, A1, A2, A0, B2, B0, B1); ++t; }
 
-  block_reduce_finalize<K::NRED, FIN_STEP2, 0>(acc, red, a.partials, a.ctl, a.fid, a.vacf, a.vacf_stride, a.zscale, gridDim.x, blockIdx.x);
+  block_reduce_finalize<K::NRED, MAG ? FIN_STEP2 : FIN_MOM2, MAG ? 0 : 3>(acc, red, a.partials, a.ctl, a.fid, a.vacf, a.vacf_stride, a.zscale, gridDim.x,
+                                                                          blockIdx.x);
 }
 
 }  // namespace lpc

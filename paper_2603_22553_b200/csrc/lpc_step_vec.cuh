@@ -105,7 +105,13 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
   const Layout& L = a.L;
   const int bz = blockIdx.x % a.tiles_z;
   const int by = (blockIdx.x / a.tiles_z) % a.tiles_y;
-  const int bx = blockIdx.x / (a.tiles_z * a.tiles_y);
+  int bx = blockIdx.x / (a.tiles_z * a.tiles_y);
+  if constexpr (PEER) {
+    // direct halo stores: the two x chunks at the ends of the slab go first (block order is launch order), so that their
+    // planes are on their way to the neighbours' ghost planes while the interior chunks are still being swept
+    const int last = a.chunks_x - 1;
+    bx = (bx == 0) ? 0 : (bx == 1) ? last : bx - 1;
+  }
   const int z0 = bz * TZ, y0 = by * TY, x0 = bx * a.xc;
   const int nplanes = min(a.xc, L.nx - x0);
   const int nloads = nplanes + 2;

@@ -237,6 +237,37 @@ def test_two_step_sweep_matches_one_step_sweep_and_oracle(lpc, oracle_mod, shape
         assert np.array_equal(alt.field(lpc.LPC_FIELD_G), one.field(lpc.LPC_FIELD_G)), xc
 
 
+@pytest.mark.parametrize("precision", [0, 1])
+@pytest.mark.parametrize("shape,bc,alpha", [((70, 19, 133), (1, 0, 0), 0.8), ((33, 40, 64), (0, 1, 1), 1.0), ((20, 13, 37), (0, 0, 0), 0.9),
+                                            ((6, 5, 7), (0, 0, 1), 0.7)])
+def test_two_step_sweep_with_moment_fields(lpc, oracle_mod, shape, bc, alpha, precision):
+    """The moment fields take two steps per sweep as well (a sweep of their own before the magnetisation's): Z_d[m] of every
+    step, P^d bit for bit as from the one-step sweeps, everything against the oracle."""
+    lat = lpc_inputs.random_small(shape, bc=bc, p_block=0.3, alpha=alpha, seed=63, n_moments=3)
+    lat.dt = 2.0e-5
+    n = 31
+    two, orc = _pair(lpc, oracle_mod, lat, n, 2, precision=precision)
+    two.set_option(lpc.LPC_OPT_TIME_BLOCK, 2)
+    one = lpc.Lattice.from_inputs(lat, precision=precision, max_steps=n)
+    one.set_kernel(2)
+    one.set_option(lpc.LPC_OPT_TIME_BLOCK, 1)
+    l2 = two.launch_count
+    for k in (4, 1, 7, 19):
+        two.step(k)
+        one.step(k)
+    assert two.launch_count - l2 < 2 * n
+    for w in (lpc.LPC_FIELD_G, lpc.LPC_FIELD_PX, lpc.LPC_FIELD_PY, lpc.LPC_FIELD_PZ):
+        assert np.array_equal(two.field(w), one.field(w)), w
+    Z2, D2 = two.moments()
+    Z1, D1 = one.moments()
+    z1 = np.abs(Z1[:, :1]).max()
+    assert np.max(np.abs(Z2 - Z1)) <= (1e-6 if precision else 1e-14) * z1
+    assert np.max(np.abs(two.fid() - one.fid())) <= (1e-6 if precision else 1e-14)
+    orc.step(n)
+    tol_site, tol_sum = (1e-5, 1e-5) if precision else (1e-10, 1e-9)
+    _check(lpc, lat, two, orc, n, tol_site=tol_site, tol_sum=tol_sum, what=f"two-step moments {shape} p{precision}")
+
+
 def test_two_step_sweep_default_and_eligibility(lpc, oracle_mod):
     lat = lpc_inputs.random_small((24, 16, 70), bc=(0, 0, 0), p_block=0.2, seed=62, n_moments=0)
     n = 10
@@ -252,8 +283,8 @@ def test_two_step_sweep_default_and_eligibility(lpc, oracle_mod):
     again.set_kernel(2)
     again.step(n)
     assert np.array_equal(again.fid(), gpu.fid())
-    # lattices that cannot: moment fields, a density channel, a periodic axis shorter than four
-    for kw, shape in ((dict(n_moments=3), lat.shape), (dict(n_density=1), lat.shape), (dict(), (24, 3, 70))):
+    # lattices that cannot: a density channel, a periodic axis shorter than four
+    for kw, shape in ((dict(n_density=1), lat.shape), (dict(n_moments=3, n_density=1), lat.shape), (dict(), (24, 3, 70))):
         m = lpc.Lattice(shape, max_steps=4, **kw)
         with pytest.raises(lpc.LpcError) as e:
             m.set_option(lpc.LPC_OPT_TIME_BLOCK, 2)
