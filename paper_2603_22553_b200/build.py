@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblpc.so")
 SOURCES = [os.path.join(CSRC, "lpc_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("lpc_internal.cuh", "lpc_step.cuh", "lpc_step_vec.cuh", "lpc_precompute.cuh", "lpc_equil.cuh", "lpc_regions.cuh")] + [
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("lpc_internal.cuh", "lpc_step.cuh", "lpc_step_vec.cuh", "lpc_step2.cuh", "lpc_precompute.cuh", "lpc_equil.cuh", "lpc_regions.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "lpc.h")]
 
 NVCC_FLAGS = [

@@ -1235,7 +1235,8 @@ int lpc_step_n(lpc_lattice* h, int64_t n) {
   if (h->halo && !h->halo_ready) return fail(LPC_ESTATE, "slab mode: lpc_slab_finish has not been called");
   if (h->halo && n > 1 && !(n == 2 && step2_usable(h)))
     return fail(LPC_ESTATE, "slab mode: the x ghost planes must be exchanged after every sweep (n <= 1, or n = 2 on a lattice with lpc_time_block_steps = 2 and two-plane exchanges)");
-  const bool persist = !h->have_regions && n >= 2 &&
+  // (never on a slab: the persistent kernel would take both steps of a two-step call without the ghost planes of the second)
+  const bool persist = !h->have_regions && !h->halo && n >= 2 &&
                        (h->kernel == LPC_KERNEL_PERSIST || (h->kernel == LPC_KERNEL_AUTO && persist_by_default(h)));
   if (persist) return h->cfg.precision ? launch_persist<float>(h, n) : launch_persist<double>(h, n);
   // two steps per sweep while at least two are left (lpc_step2.cuh); an odd last step takes the one-step sweep
