@@ -86,6 +86,7 @@ struct lpc_lattice {
   bool step2_ok;      // the lattice can run it (geometry, channels, boundary conditions)
   int time_block;     // LPC_OPT_TIME_BLOCK: 0 auto, 1 one step per sweep, 2 two steps per sweep whenever possible
   int xc2, chunks_x2; // its x chunks
+  int ty2, tz2, tiles_z2, tiles_y2;   // its tiles: 8 rows of 32 16-byte groups (lpc_step2.cuh)
   bool ghosts_full;   // the whole ghost shell of the current state is valid (the one-step sweeps keep the face layer only)
   CUtensorMap tm2_f[2], tm2_m[2], tm2_pi, tm2_cs;   // tm2_m: the three moment channels
   int opt_xc, opt_persist_mb, opt_region_fusion;   // lpc_set_option overrides (0 = default)
@@ -590,9 +591,9 @@ int launch_step2_t(lpc_lattice* h) {
   a.vacf = wsp<double>(h, h->off.vacf);
   a.vacf_stride = h->cfg.max_steps + 2;
   for (int d = 0; d < 3; ++d) a.per[d] = h->cfg.bc[d] == 0;
-  a.xc = h->xc2; a.tiles_z = h->tiles_z; a.tiles_y = h->tiles_y; a.chunks_x = h->chunks_x2;
+  a.xc = h->xc2; a.tiles_z = h->tiles_z2; a.tiles_y = h->tiles_y2; a.chunks_x = h->chunks_x2;
   a.zscale = h->cfg.a * h->cfg.alpha / 6.0;
-  const unsigned grid = (unsigned)(h->tiles_z * h->tiles_y * h->chunks_x2);
+  const unsigned grid = (unsigned)(h->tiles_z2 * h->tiles_y2 * h->chunks_x2);
   if (h->nmom == 3) {
     // the three moment channels first (Z_d of both steps; they read the step counter the magnetisation sweep advances)
     using KM = Step2Cfg<T, VW, 3>;
@@ -1024,8 +1025,12 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
   tma_geometry(h->C, cfg->precision == 1, cfg->nx, cfg->ny, cfg->nz, 0, &h->ty, &h->tz, &h->nstage, &h->xc, &h->tiles_z, &h->tiles_y, &h->chunks_x);
   h->tma_ok = (size_t)h->tiles_z * h->tiles_y * h->chunks_x <= h->off.partial_slots;
   // two steps per sweep: the magnetisation channels alone, no slab, and every periodic axis long enough for two ghost layers
-  step2_geometry(cfg->nx, h->tiles_z * h->tiles_y, 0, &h->xc2, &h->chunks_x2);
-  h->step2_ok = h->tma_ok && h->nrho == 0 && !(h->halo && cfg->nx < 2);
+  h->ty2 = 8; h->tz2 = 32 * (16 / h->sT);
+  h->tiles_z2 = (cfg->nz + h->tz2 - 1) / h->tz2;
+  h->tiles_y2 = (cfg->ny + h->ty2 - 1) / h->ty2;
+  step2_geometry(cfg->nx, (long long)h->tiles_z2 * h->tiles_y2, 0, &h->xc2, &h->chunks_x2);
+  h->step2_ok = h->tma_ok && h->nrho == 0 && !(h->halo && cfg->nx < 2) &&
+                (size_t)h->tiles_z2 * h->tiles_y2 * h->chunks_x2 <= h->off.partial_slots;
   for (int d = 0; d < 3; ++d) {
     const int n = d == 0 ? cfg->nx : d == 1 ? cfg->ny : cfg->nz;
     if (cfg->bc[d] == 0 && n < 4) h->step2_ok = false;
@@ -1051,12 +1056,12 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
     if (!rc) rc = encode_map(&h->tm_cs, f32, h->ws + h->off.cs, 4, dk, bk);
     if (!rc && h->step2_ok) {
       // the two-step sweep: h and pi with two halo rows / one 16-byte halo group, cos and sin with one halo row
-      const cuuint32_t zw = (cuuint32_t)(h->tz + 2 * (16 / h->sT));
-      const cuuint32_t b2f[4] = {zw, (cuuint32_t)(h->ty + 4), 1, 2};
-      const cuuint32_t b2k[4] = {zw, (cuuint32_t)(h->ty + 2), 1, 2};
+      const cuuint32_t zw = (cuuint32_t)(h->tz2 + 2 * (16 / h->sT));
+      const cuuint32_t b2f[4] = {zw, (cuuint32_t)(h->ty2 + 4), 1, 2};
+      const cuuint32_t b2k[4] = {zw, (cuuint32_t)(h->ty2 + 2), 1, 2};
       rc = encode_map(&h->tm2_f[0], f32, h->ws + h->off.f0, 4, d4, b2f);
       if (!rc) rc = encode_map(&h->tm2_f[1], f32, h->ws + h->off.f1, 4, d4, b2f);
-      const cuuint32_t b2m[4] = {zw, (cuuint32_t)(h->ty + 4), 1, 3};
+      const cuuint32_t b2m[4] = {zw, (cuuint32_t)(h->ty2 + 4), 1, 3};
       if (!rc && h->nmom == 3) rc = encode_map(&h->tm2_m[0], f32, h->ws + h->off.f0, 4, d4, b2m);
       if (!rc && h->nmom == 3) rc = encode_map(&h->tm2_m[1], f32, h->ws + h->off.f1, 4, d4, b2m);
       if (!rc) rc = encode_map(&h->tm2_pi, f32, h->ws + h->off.pi, 3, d4, b2f);
@@ -1450,7 +1455,11 @@ int lpc_set_option(lpc_lattice* h, int32_t key, int64_t value) {
     }
     case LPC_OPT_X_CHUNK2:
       if (value > h->cfg.nx) value = h->cfg.nx;
-      step2_geometry(h->cfg.nx, (long long)h->tiles_z * h->tiles_y, (int)value, &h->xc2, &h->chunks_x2);
+      step2_geometry(h->cfg.nx, (long long)h->tiles_z2 * h->tiles_y2, (int)value, &h->xc2, &h->chunks_x2);
+      if ((size_t)h->tiles_z2 * h->tiles_y2 * h->chunks_x2 > h->off.partial_slots) {   // too many CTAs for the partial sums: back to the default
+        step2_geometry(h->cfg.nx, (long long)h->tiles_z2 * h->tiles_y2, 0, &h->xc2, &h->chunks_x2);
+        return fail(LPC_EINVAL, "LPC_OPT_X_CHUNK2 = %lld gives more CTAs than the workspace has partial-sum slots", (long long)value);
+      }
       return LPC_OK;
     case LPC_OPT_PERSIST_MAX_MB:
       if (value > (1 << 20)) return fail(LPC_EINVAL, "LPC_OPT_PERSIST_MAX_MB is in MiB");
