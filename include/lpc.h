@@ -70,11 +70,12 @@ extern "C" {
                                 between steps; for lattices that stay in L2 (launch-bound otherwise) */
 
 /* lpc_set_option keys */
-#define LPC_OPT_TIME_BLOCK 1     /* 0 auto (default), 1 one time step per sweep, 2 two time steps per sweep        */
+#define LPC_OPT_TIME_BLOCK 1     /* 0 auto (default; = 1 on B200), 1 one time step per sweep, 2 two per sweep      */
 #define LPC_OPT_X_CHUNK 2        /* planes per x chunk of the one-step TMA sweeps; 0 = the library's choice         */
 #define LPC_OPT_X_CHUNK2 3       /* planes per x chunk of the two-step sweep; 0 = the library's choice              */
 #define LPC_OPT_PERSIST_MAX_MB 4 /* AUTO takes the persistent kernel up to this many MiB per step; 0 = 48           */
 #define LPC_OPT_REGION_FUSION 5  /* 0 regional sums inside the sweep when possible (default), 1 separate pass       */
+#define LPC_OPT_FULL_PHASE 6     /* 0 sweeps read sin alone where every phase angle is small (default), 1 cos + sin  */
 
 typedef struct lpc_lattice lpc_lattice; /* opaque, host struct owned by the library */
 
@@ -141,10 +142,11 @@ int lpc_set_link_mobility(lpc_lattice* lat, const double* alpha_link);
  * that propagates, phase-rotates, reduces G[n] and (if enabled) Z_d[n+1], P^d, rho.  Eq. 13 is a
  * Jacobi update (its right-hand side is at n-1), so a lattice that carries the
  * magnetisation alone (n_moments = n_density = 0, no link factors, no region labels, not a slab,
- * periodic axes of length >= 4) takes TWO steps per sweep while at least two are left
+ * periodic axes of length >= 4) can take TWO steps per sweep while at least two are left
  * ("temporal blocking": state and parameters cross HBM once per two steps; G[n] is still recorded
- * for every step and the state after the call is bit for bit that of the one-step sweeps);
- * LPC_OPT_TIME_BLOCK = 1 switches that off.
+ * for every step and the state after the call is bit for bit that of the one-step sweeps).
+ * LPC_OPT_TIME_BLOCK = 2 asks for it; the default is one step per sweep, which measures faster on
+ * B200 (the two-step sweep is bound by its instruction count, not by HBM: DESIGN.md 6.1c).
  * Asynchronous on the stream.  Errors: LPC_ESTATE (no site parameters yet), LPC_EINVAL (n < 0 or
  * steps_done + n > max_steps), LPC_ECUDA.                                                      */
 int lpc_step_n(lpc_lattice* lat, int64_t n);

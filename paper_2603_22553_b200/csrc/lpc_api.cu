@@ -84,17 +84,19 @@ struct lpc_lattice {
   int device;  // CUDA device ordinal of the workspace
   // two-step sweep (lpc_step2.cuh)
   bool step2_ok;      // the lattice can run it (geometry, channels, boundary conditions)
-  int time_block;     // LPC_OPT_TIME_BLOCK: 0 auto, 1 one step per sweep, 2 two steps per sweep whenever possible
+  int time_block;     // LPC_OPT_TIME_BLOCK: 0 auto (= 1), 1 one step per sweep, 2 two steps per sweep whenever possible
   int xc2, chunks_x2; // its x chunks
   int ty2, tz2, tiles_z2, tiles_y2;   // its tiles: 8 rows of 32 16-byte groups (lpc_step2.cuh)
   bool ghosts_full;   // the whole ghost shell of the current state is valid (the one-step sweeps keep the face layer only)
-  CUtensorMap tm2_f[2], tm2_m[2], tm2_pi, tm2_cs;   // tm2_m: the three moment channels
+  CUtensorMap tm2_f[2], tm2_m[2], tm2_pi, tm2_cs, tm2_sn;   // tm2_m: the three moment channels; tm2_sn: the sine channel alone
+  bool phase_small;   // every open site has cos(omega dt) >= 1/2: sweeps may read sin alone (cos_from_sin)
+  int opt_full_phase; // LPC_OPT_FULL_PHASE: 1 = always read cos and sin
   int opt_xc, opt_persist_mb, opt_region_fusion;   // lpc_set_option overrides (0 = default)
   // TMA geometry
   int ty, tz, nstage, xc, tiles_z, tiles_y, chunks_x;
   bool tma_ok;
   TmaLinkMaps tm_l;  // pi centres and the three link-weight channels (link_mobility = 1)
-  CUtensorMap tm_f[2], tm_m[2], tm_r[2], tm_pi, tm_cs;  // tm_r: one channel per box (the density channel alone, equilibration)  // tm_f: magnetisation (+ density) channels, tm_m: the 3 moment channels
+  CUtensorMap tm_f[2], tm_m[2], tm_r[2], tm_pi, tm_cs, tm_sn;  // tm_r: one channel per box (the density channel alone, equilibration)  // tm_f: magnetisation (+ density) channels, tm_m: the 3 moment channels
 };
 
 namespace {
@@ -289,6 +291,9 @@ int ensure_dyn_smem(Kern kern, int bytes, int device, bool (&done)[MAX_DEVICES])
   return LPC_OK;
 }
 
+// may the sweeps read sin alone and rebuild cos from it?
+bool sin_only(const lpc_lattice* h) { return h->phase_small && !h->opt_full_phase; }
+
 // ---- launch of one sweep ---------------------------------------------------------------------
 template <typename T, int NRHO, int NMOM>
 int launch_step_t(lpc_lattice* h) {
@@ -343,6 +348,15 @@ int launch_step_t(lpc_lattice* h) {
       h->launches++;
       return LPC_OK;
     };
+    auto launch_sn = [&](auto kern, auto cfg, const CUtensorMap& tm, const StepArgs<T>& args) -> int {
+      using K = decltype(cfg);
+      static bool attr_done[MAX_DEVICES] = {};
+      if (int rc = ensure_dyn_smem(kern, K::SMEM_BYTES, h->device, attr_done)) return rc;
+      kern<<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(tm, h->tm_pi, h->tm_sn, args);
+      CUDA_TRY(cudaGetLastError());
+      h->launches++;
+      return LPC_OK;
+    };
     // With moment fields the step is two sweeps over the same pair of buffers: the three moment
     // channels first (Z_d[k+1], P^d <- W P^d; no phase, no cos/sin traffic), then the magnetisation
     // (and density) channels, which also advance the step counter.  One 5-channel sweep needs more
@@ -380,7 +394,10 @@ int launch_step_t(lpc_lattice* h) {
     a.c0 = 0;
     int rc;
     if constexpr (NRHO == 0) {
-      if (fuse_regions)
+      if (sin_only(h) && !fuse_regions && !h->have_links && !peers)
+        // every phase angle is small: stage sin alone and rebuild cos (8 bytes per site less in fp64)
+        rc = launch_sn(step_tma_kernel<T, 2, 0, 0, TY, 64, NS, VW, 4>, TmaCfg<T, 2, 0, 0, TY, 64, NS, 0, VW, 4>(), h->tm_f[h->cur], a);
+      else if (fuse_regions)
         rc = h->have_links ? launch_links(step_tma_links_kernel<T, 2, 0, 0, TY, 64, NSL, VW, 1>, TmaCfg<T, 2, 0, 0, TY, 64, NSL, 1, VW, 1>(), h->tm_f[h->cur], a)
                            : launch(step_tma_kernel<T, 2, 0, 0, TY, 64, NS, VW, 1>, TmaCfg<T, 2, 0, 0, TY, 64, NS, 0, VW, 1>(), h->tm_f[h->cur], a);
       else
@@ -563,7 +580,8 @@ int fill_state_ghosts(lpc_lattice* h) {
 // ---- two time steps in one sweep (lpc_step2.cuh) ----------------------------------------------
 // may the next steps of this lattice run two at a time?
 bool step2_usable(const lpc_lattice* h) {
-  if (!h->step2_ok || h->time_block == 1 || h->have_links || h->have_regions) return false;
+  // on request only (LPC_OPT_TIME_BLOCK = 2): on B200 the one-step sweep measures faster at every size tried
+  if (!h->step2_ok || h->time_block != 2 || h->have_links || h->have_regions) return false;
   if (h->peer[0][0] || h->peer[1][0]) return false;   // direct halo stores belong to the one-step sweep
   if (h->kernel == LPC_KERNEL_DIRECT || h->kernel == LPC_KERNEL_PERSIST) return false;
   return true;
@@ -572,7 +590,6 @@ bool step2_usable(const lpc_lattice* h) {
 template <typename T>
 int launch_step2_t(lpc_lattice* h) {
   constexpr int VW = 16 / (int)sizeof(T);
-  using K = Step2Cfg<T, VW, 2>;
   if (!h->ghosts_full) {   // the sweep reads two ghost layers, edges included
     int rc = fill_state_ghosts<T>(h);
     if (rc) return rc;
@@ -596,20 +613,28 @@ int launch_step2_t(lpc_lattice* h) {
   const unsigned grid = (unsigned)(h->tiles_z2 * h->tiles_y2 * h->chunks_x2);
   if (h->nmom == 3) {
     // the three moment channels first (Z_d of both steps; they read the step counter the magnetisation sweep advances)
-    using KM = Step2Cfg<T, VW, 3>;
+    using KM = Step2Cfg<T, VW, 3, false>;
     StepArgs<T> am = a;
     am.c0 = 2;
     am.fout = a.fout + 2 * h->L.np;
     static bool attr_done_m[MAX_DEVICES] = {};
-    if (int rc = ensure_dyn_smem(step2_kernel<T, VW, 3>, KM::SMEM_BYTES, h->device, attr_done_m)) return rc;
-    step2_kernel<T, VW, 3><<<grid, KM::NTHREADS, KM::SMEM_BYTES, h->stream>>>(h->tm2_m[h->cur], h->tm2_pi, h->tm2_cs, am);
+    if (int rc = ensure_dyn_smem(step2_kernel<T, VW, 3, false>, KM::SMEM_BYTES, h->device, attr_done_m)) return rc;
+    step2_kernel<T, VW, 3, false><<<grid, KM::NTHREADS, KM::SMEM_BYTES, h->stream>>>(h->tm2_m[h->cur], h->tm2_pi, h->tm2_cs, am);
     CUDA_TRY(cudaGetLastError());
     h->launches++;
   }
   a.c0 = 0;
-  static bool attr_done[MAX_DEVICES] = {};
-  if (int rc = ensure_dyn_smem(step2_kernel<T, VW, 2>, K::SMEM_BYTES, h->device, attr_done)) return rc;
-  step2_kernel<T, VW, 2><<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(h->tm2_f[h->cur], h->tm2_pi, h->tm2_cs, a);
+  if (sin_only(h)) {
+    using K = Step2Cfg<T, VW, 2, true>;
+    static bool attr_done[MAX_DEVICES] = {};
+    if (int rc = ensure_dyn_smem(step2_kernel<T, VW, 2, true>, K::SMEM_BYTES, h->device, attr_done)) return rc;
+    step2_kernel<T, VW, 2, true><<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(h->tm2_f[h->cur], h->tm2_pi, h->tm2_sn, a);
+  } else {
+    using K = Step2Cfg<T, VW, 2, false>;
+    static bool attr_done[MAX_DEVICES] = {};
+    if (int rc = ensure_dyn_smem(step2_kernel<T, VW, 2, false>, K::SMEM_BYTES, h->device, attr_done)) return rc;
+    step2_kernel<T, VW, 2, false><<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(h->tm2_f[h->cur], h->tm2_pi, h->tm2_cs, a);
+  }
   CUDA_TRY(cudaGetLastError());
   h->launches++;
   h->cur ^= 1;
@@ -723,6 +748,7 @@ int set_site_params_t(lpc_lattice* h, const double* dF, const uint8_t* blocked, 
   if (hc.bad != 0)
     return fail(LPC_EINVAL, "the equilibrium density underflows on %llu open sites: the spread of dF is too wide for %s", hc.bad,
                 h->cfg.precision ? "fp32" : "fp64");
+  h->phase_small = (hc.wide_phase == 0);
   {
     // ghosts of pi (wrapped value, or 0 beyond a wall) and of cos, sin (the two-step sweep rotates ghost sites too)
     const long long cells = ghost_cells(L);
@@ -1021,7 +1047,8 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
   h->device = dev;
   h->time_block = 0;
   h->ghosts_full = false;
-  h->opt_xc = h->opt_persist_mb = h->opt_region_fusion = 0;
+  h->opt_xc = h->opt_persist_mb = h->opt_region_fusion = h->opt_full_phase = 0;
+  h->phase_small = false;
   tma_geometry(h->C, cfg->precision == 1, cfg->nx, cfg->ny, cfg->nz, 0, &h->ty, &h->tz, &h->nstage, &h->xc, &h->tiles_z, &h->tiles_y, &h->chunks_x);
   h->tma_ok = (size_t)h->tiles_z * h->tiles_y * h->chunks_x <= h->off.partial_slots;
   // two steps per sweep: the magnetisation channels alone, no slab, and every periodic axis long enough for two ghost layers
@@ -1054,6 +1081,8 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
     if (!rc && h->nrho == 1) rc = encode_map(&h->tm_r[1], f32, h->ws + h->off.f1, 4, d4, br);
     if (!rc) rc = encode_map(&h->tm_pi, f32, h->ws + h->off.pi, 3, d4, b4);
     if (!rc) rc = encode_map(&h->tm_cs, f32, h->ws + h->off.cs, 4, dk, bk);
+    const cuuint32_t bs[4] = {bk[0], bk[1], 1, 1};   // the sine channel alone
+    if (!rc) rc = encode_map(&h->tm_sn, f32, h->ws + h->off.cs, 4, dk, bs);
     if (!rc && h->step2_ok) {
       // the two-step sweep: h and pi with two halo rows / one 16-byte halo group, cos and sin with one halo row
       const cuuint32_t zw = (cuuint32_t)(h->tz2 + 2 * (16 / h->sT));
@@ -1066,6 +1095,8 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
       if (!rc && h->nmom == 3) rc = encode_map(&h->tm2_m[1], f32, h->ws + h->off.f1, 4, d4, b2m);
       if (!rc) rc = encode_map(&h->tm2_pi, f32, h->ws + h->off.pi, 3, d4, b2f);
       if (!rc) rc = encode_map(&h->tm2_cs, f32, h->ws + h->off.cs, 4, dk, b2k);
+      const cuuint32_t b2s[4] = {zw, (cuuint32_t)(h->ty2 + 2), 1, 1};
+      if (!rc) rc = encode_map(&h->tm2_sn, f32, h->ws + h->off.cs, 4, dk, b2s);
     }
     if (!rc && cfg->link_mobility) {
       // pi centres and m_x: the tile itself; m_y: one more row below; m_z: 16 bytes of columns below
@@ -1465,6 +1496,10 @@ int lpc_set_option(lpc_lattice* h, int32_t key, int64_t value) {
       if (value > (1 << 20)) return fail(LPC_EINVAL, "LPC_OPT_PERSIST_MAX_MB is in MiB");
       h->opt_persist_mb = (int)value;
       return LPC_OK;
+    case LPC_OPT_FULL_PHASE:
+      if (value > 1) return fail(LPC_EINVAL, "LPC_OPT_FULL_PHASE takes 0 (sin alone where every phase angle is small) or 1 (always cos and sin)");
+      h->opt_full_phase = (int)value;
+      return LPC_OK;
     case LPC_OPT_REGION_FUSION:
       if (value > 1) return fail(LPC_EINVAL, "LPC_OPT_REGION_FUSION takes 0 (inside the sweep when possible) or 1 (separate pass)");
       h->opt_region_fusion = (int)value;
@@ -1485,7 +1520,11 @@ double lpc_bytes_per_site_step(const lpc_lattice* h) {
   // with per-link mobility factors the sweep also reads three stored link weights per site
   // region labels: one byte per site inside the sweep, or one more pass over h (2 channels), pi and the label
   const double regions = !h->have_regions ? 0.0 : regions_fusable(h) ? 1.0 : 3.0 * h->sT + 1.0;
-  return (double)h->sT * (2.0 * h->C + 3.0 + (h->have_links ? 3.0 : 0.0)) + regions;
+  // lattices whose phase angles are all small: the plain magnetisation sweeps read sin alone
+  const bool sn = sin_only(h) && h->tma_ok && h->kernel != LPC_KERNEL_DIRECT && h->kernel != LPC_KERNEL_PERSIST &&
+                  !(h->kernel == LPC_KERNEL_AUTO && persist_by_default(h)) && h->nrho == 0 && !h->have_links &&
+                  !(h->have_regions && regions_fusable(h)) && !(h->peer[0][0] || h->peer[1][0]);
+  return (double)h->sT * (2.0 * h->C + (sn ? 2.0 : 3.0) + (h->have_links ? 3.0 : 0.0)) + regions;
 }
 
 void lpc_destroy(lpc_lattice* h) { delete h; }

@@ -71,19 +71,26 @@ __global__ void site_params_kernel(const double* __restrict__ e, const double* _
                                    Layout L, double dt, Ctl* ctl, T* __restrict__ pi, T* __restrict__ cs) {
   const double Z = ctl->zsum;
   unsigned long long bad = 0;
+  bool wide = false;
   for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (long long)gridDim.x * blockDim.x) {
     const long long i = i0 + k;
     const long long j = dense_to_padded(L, i);
     const double p = e[i] / Z;
     double c = 1.0, s = 0.0;
     if (p > 0.0) sincos(omega[k] * dt, &s, &c);
+    // small phase angles (every BASELINE config: |omega dt| <= 0.13): the stored cosine is the one a sweep rebuilds from
+    // the stored sine (cos_from_sin), so sweeps that read sin alone agree bit for bit with those that read both
+    T sT = (T)s, cT = (T)c;
+    if (c >= COMPACT_PHASE_MIN_COS) cT = cos_from_sin(sT);
+    else wide = true;
     // kappa_of() needs pi to be a normal number of T on every open site
     if (e[i] > 0.0 && !((T)p >= (sizeof(T) == 8 ? (T)2.2250738585072014e-308 : (T)1.17549435e-38f))) bad++;
     pi[j] = (T)p;
-    cs[j] = (T)c;
-    cs[L.np + j] = (T)s;
+    cs[j] = cT;
+    cs[L.np + j] = sT;
   }
   if (bad) atomicAdd(&ctl->bad, bad);
+  if (wide) ctl->wide_phase = 1u;
 }
 
 // Ghost layers of nch channel planes, all of them: L.gh planes / rows in x and y, GHZ columns in z, edges and corners

@@ -220,6 +220,7 @@ struct TmaLinkMaps {
 // VW: sites per thread along z (one 16-byte vector: 2 in fp64, 4 in the fp32 march of lpc_step_vec.cuh).
 // FEAT bit 0: the region-resolved FID (magnetisation sweep) or VACF (moment sweep) is accumulated in the same sweep;
 // bit 1: slab mode with direct halo stores (no shared memory of its own).
+// bit 2: the sweep stages sin alone and rebuilds cos (cos_from_sin): 8 bytes per site less (fp64).
 template <typename T, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int LK = 0, int VW = 2, int FEAT = 0>
 struct TmaCfg {
   static constexpr int C = NH + NRHO + NMOM;
@@ -239,7 +240,7 @@ struct TmaCfg {
   static constexpr int MX_BYTES = (MX_RAW + 127) / 128 * 128;
   static constexpr int MY_BYTES = (MY_RAW + 127) / 128 * 128;
   static constexpr int MZ_BYTES = (MZ_RAW + 127) / 128 * 128;
-  static constexpr int KCS_RAW = NH * TY * TZ * (int)sizeof(T);  // cos, sin (no halo); none without the magnetisation
+  static constexpr int KCS_RAW = ((FEAT & 4) ? 1 : NH) * TY * TZ * (int)sizeof(T);  // cos, sin (no halo), or sin alone (FEAT bit 2); none without the magnetisation
   static constexpr int F_BYTES = (F_RAW + 127) / 128 * 128;
   static constexpr int PI_BYTES = (PI_RAW + 127) / 128 * 128;
   static constexpr int KCS_BYTES = (KCS_RAW + 127) / 128 * 128;

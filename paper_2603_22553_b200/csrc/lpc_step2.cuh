@@ -43,7 +43,8 @@ namespace lpc {
 // NC = 2: the magnetisation (h_re, h_im; phase rotation; G of both steps).  NC = 3: the three moment fields q^d of the
 // VACF (Eq. 4; no phase, no cos / sin traffic; Z_d of both steps) -- they propagate independently of the
 // magnetisation, so a lattice with moment fields runs one two-step sweep of each kind per two steps.
-template <typename T, int VW, int NC = 2, int TY_ = 8>
+// CPH: the phase factors are staged as sin alone and cos is rebuilt (cos_from_sin; lattices whose phase angles are all small).
+template <typename T, int VW, int NC = 2, bool CPH = false, int TY_ = 8>
 struct Step2Cfg {
   static constexpr bool MAG = (NC == 2);
   static constexpr int GZ = 32;                     // own groups per row: one per lane of a row warp
@@ -56,26 +57,29 @@ struct Step2Cfg {
   static constexpr int NA = R1 + 1;                 // step-1 warps: one per row + the edge warp (groups 0 and G1-1 of every row)
   static constexpr int NB = TY;                     // step-2 warps: one per row
   static constexpr int NTHREADS = 32 * (NA + NB + 1);   // + the warp that issues the loads
-  static constexpr int NSTAGE = 4;                  // step 1 reads a plane in two iterations; two more are in flight
+  static constexpr int NSTAGE = CPH ? 5 : 4;        // step 1 reads a plane in two iterations; the others are in flight
   static constexpr int NRING = 4;                   // planes of the intermediate state: three in use by step 2, one being written
   static constexpr int ND = 4;                      // hand-over barriers per direction (iterations in flight)
   static constexpr int PF = 0;                      // > 0: every load also sends plane j + PF towards L2 (measured: no gain)
   static constexpr int F_BYTES = NC * R0 * TZW * (int)sizeof(T);
   static constexpr int PI_BYTES = R0 * TZW * (int)sizeof(T);
-  static constexpr int CS_BYTES = MAG ? 2 * R1 * TZW * (int)sizeof(T) : 0;
+  static constexpr int NPH = MAG ? (CPH ? 1 : 2) : 0;   // staged phase channels: cos and sin, or sin alone
+  static constexpr int CS_RAW = NPH * R1 * TZW * (int)sizeof(T);
+  static constexpr int CS_BYTES = (CS_RAW + 127) / 128 * 128;
   static constexpr int STAGE_BYTES = F_BYTES + PI_BYTES + CS_BYTES;
+  static constexpr int TX_BYTES = F_BYTES + PI_BYTES + CS_RAW;
   static constexpr int RCH = R1 * TZW;              // elements of one channel of a ring plane
   static constexpr int RING_PLANE = (NC + 1) * RCH * (int)sizeof(T);   // the intermediate state and pi (step 2 reads no stage)
   static constexpr int RING_OFF = NSTAGE * STAGE_BYTES;
   static constexpr int CSB_OFF = RING_OFF + NRING * RING_PLANE;        // step 2's own cos / sin: 16 bytes of each per thread
-  static constexpr int CSB_BYTES = MAG ? 2 * 2 * NB * 32 * 16 : 0;   // two slots: the plane in use and the next one
+  static constexpr int CSB_BYTES = 2 * NPH * NB * 32 * 16;   // two slots: the plane in use and the next one
   static constexpr int BAR_OFF = CSB_OFF + CSB_BYTES;
   static constexpr int RED_OFF = BAR_OFF + (NSTAGE + 2 * ND) * 8;
   static constexpr int NRED = 2 * (MAG ? 2 : 3);    // G_re, G_im (or Z_x, Z_y, Z_z) of the first and of the second step
   static constexpr int SMEM_BYTES = RED_OFF + ((NTHREADS / 32) * NRED + 2) * 8 + 128;   // +128: manual alignment slack
   static_assert(2 * R1 <= 32, "the edge warp holds two groups of every row");
   static_assert((NRING & (NRING - 1)) == 0 && (ND & (ND - 1)) == 0, "slots are picked with a mask");
-  static_assert(F_BYTES % 128 == 0 && PI_BYTES % 128 == 0 && CS_BYTES % 128 == 0, "TMA boxes land 128-byte aligned");
+  static_assert(F_BYTES % 128 == 0 && PI_BYTES % 128 == 0 && CS_BYTES % 128 == 0 && (!MAG ? !CPH : true), "TMA boxes land 128-byte aligned");
   static_assert(RING_PLANE % 16 == 0 && RING_OFF % 128 == 0 && CSB_OFF % 16 == 0, "16-byte vector accesses to the ring");
   static_assert(SMEM_BYTES <= 227 * 1024, "one CTA per SM");
 };
@@ -113,11 +117,11 @@ __device__ __noinline__ void store_images(T* __restrict__ base, long long sx, lo
   }
 }
 
-template <typename T, int VW, int NC>
-__global__ void __launch_bounds__(Step2Cfg<T, VW, NC>::NTHREADS, 1)
+template <typename T, int VW, int NC, bool CPH>
+__global__ void __launch_bounds__(Step2Cfg<T, VW, NC, CPH>::NTHREADS, 1)
     step2_kernel(const __grid_constant__ CUtensorMap tm_f, const __grid_constant__ CUtensorMap tm_pi, const __grid_constant__ CUtensorMap tm_cs,
                  StepArgs<T> a) {
-  using K = Step2Cfg<T, VW, NC>;
+  using K = Step2Cfg<T, VW, NC, CPH>;
   using V = typename VecN<T, VW>::type;
   constexpr int TZW = K::TZW, R0 = K::R0, R1 = K::R1, NS = K::NSTAGE, RCH = K::RCH;
   constexpr bool MAG = K::MAG;
@@ -226,15 +230,15 @@ __global__ void __launch_bounds__(Step2Cfg<T, VW, NC>::NTHREADS, 1)
       auto issue = [&](int j) {
         const int s = j % NS;
         unsigned char* st = smem + s * K::STAGE_BYTES;
-        mbar_expect_tx(&full[s], K::STAGE_BYTES);
+        mbar_expect_tx(&full[s], K::TX_BYTES);
         const int pz = L.padz + z0 - VW, py = y0 + L.gh - 2, px = x0 + j + L.gh - 2;
         tma_load_4d(st, &tm_f, &full[s], pz, py, px, a.c0);
         tma_load_3d(st + K::F_BYTES, &tm_pi, &full[s], pz, py, px);
-        if constexpr (MAG) tma_load_4d(st + K::F_BYTES + K::PI_BYTES, &tm_cs, &full[s], pz, py + 1, px, 0);
+        if constexpr (MAG) tma_load_4d(st + K::F_BYTES + K::PI_BYTES, &tm_cs, &full[s], pz, py + 1, px, CPH ? 1 : 0);
         if (K::PF > 0 && j + K::PF < nin) {
           tma_prefetch_4d(&tm_f, pz, py, px + K::PF, a.c0);
           tma_prefetch_3d(&tm_pi, pz, py, px + K::PF);
-          if constexpr (MAG) tma_prefetch_4d(&tm_cs, pz, py + 1, px + K::PF, 0);
+          if constexpr (MAG) tma_prefetch_4d(&tm_cs, pz, py + 1, px + K::PF, CPH ? 1 : 0);
         }
       };
       tma_prefetch_desc(&tm_f);
@@ -285,8 +289,14 @@ __global__ void __launch_bounds__(Step2Cfg<T, VW, NC>::NTHREADS, 1)
         const bool own_plane = t >= 1 && t <= nplanes;   // plane j = t + 1 of this CTA's own chunk: its own sites count towards the sums
         update(prv, ctr, nxt, sf, R0 * TZW, sp,
                [&](T (&csv)[VW], T (&snv)[VW]) {
-                 ldv<T, VW>(sk, csv);
-                 ldv<T, VW>(sk + R1 * TZW, snv);
+                 if constexpr (CPH) {
+                   ldv<T, VW>(sk, snv);
+#pragma unroll
+                   for (int k = 0; k < VW; ++k) csv[k] = cos_from_sin(snv[k]);
+                 } else {
+                   ldv<T, VW>(sk, csv);
+                   ldv<T, VW>(sk + R1 * TZW, snv);
+                 }
                },
                o, (!MAG && own_plane) ? acc : nullptr, nv1);
         // ring slot (t + 1) & 3 held plane t - 3, which step 2 read last in its iteration t - 2
@@ -342,7 +352,7 @@ __global__ void __launch_bounds__(Step2Cfg<T, VW, NC>::NTHREADS, 1)
     T* outp = a.fout + L.idx(x0, y2, z2);
     // cos and sin of the thread's own group come straight from global memory into a 16-byte slot of its own (cp.async),
     // one plane ahead: step 2 reads no stage, so the stages turn over at the pace of step 1 alone
-    constexpr int CSLOT = 2 * K::NB * 32 * VW;           // elements of one slot: cos of every thread, then sin
+    constexpr int CSLOT = K::NPH * K::NB * 32 * VW;      // elements of one slot: cos of every thread, then sin (CPH: sin alone)
     T* csb = reinterpret_cast<T*>(smem + K::CSB_OFF) + (r2 * 32 + lane) * VW;
     const T* csg = a.cs + L.idx(x0, y2, z2);
     // output plane j (absolute x0 - 2 + j) into slot j & 1; one group per call, so that wait<1> leaves only the latest in flight
@@ -350,8 +360,12 @@ __global__ void __launch_bounds__(Step2Cfg<T, VW, NC>::NTHREADS, 1)
       if constexpr (MAG) {
         if (nv2 > 0 && j <= nplanes + 1) {
           T* dst = csb + (j & 1) * CSLOT;
-          cp_async16(dst, csg);
-          cp_async16(dst + K::NB * 32 * VW, csg + L.np);
+          if constexpr (CPH) {
+            cp_async16(dst, csg + L.np);
+          } else {
+            cp_async16(dst, csg);
+            cp_async16(dst + K::NB * 32 * VW, csg + L.np);
+          }
           csg += L.sx;
         }
         cp_async_commit();
@@ -379,8 +393,14 @@ __global__ void __launch_bounds__(Step2Cfg<T, VW, NC>::NTHREADS, 1)
         update(prv, ctr, nxt, rf, RCH, rf + NC * RCH,
                [&](T (&csv)[VW], T (&snv)[VW]) {
                  cp_async_wait<1>();
-                 ldv<T, VW>(csb + (j & 1) * CSLOT, csv);
-                 ldv<T, VW>(csb + (j & 1) * CSLOT + K::NB * 32 * VW, snv);
+                 if constexpr (CPH) {
+                   ldv<T, VW>(csb + (j & 1) * CSLOT, snv);
+#pragma unroll
+                   for (int k = 0; k < VW; ++k) csv[k] = cos_from_sin(snv[k]);
+                 } else {
+                   ldv<T, VW>(csb + (j & 1) * CSLOT, csv);
+                   ldv<T, VW>(csb + (j & 1) * CSLOT + K::NB * 32 * VW, snv);
+                 }
                },
                o, MAG ? nullptr : acc + HR, nv2);
         if constexpr (MAG) {   // G[n+2]

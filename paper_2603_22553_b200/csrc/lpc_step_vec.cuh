@@ -79,12 +79,15 @@ __device__ __noinline__ void store_face_vec(T* __restrict__ base, long long i, i
   }
 }
 
-// FEAT bit 0 (REG): region-resolved FID inside the sweep; bit 1 (PEER): slab mode with direct halo stores.
+// FEAT bit 0 (REG): region-resolved FID inside the sweep; bit 1 (PEER): slab mode with direct halo stores; bit 2 (CPH): tm_cs
+// stages the sine alone (one channel) and the cosine is rebuilt from it (lattices whose phase angles are all small).
 template <typename T, int VW, int NH, int NRHO, int NMOM, int TY, int TZ, int NSTAGE, int LK, int FEAT, typename LM>
 __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUtensorMap& tm_pi, const CUtensorMap& tm_cs, const LM& lm,
                                                 const StepArgs<T>& a) {
   constexpr int REG = FEAT & 1;
   constexpr bool PEER = (FEAT & 2) != 0;
+  constexpr bool CPH = (FEAT & 4) != 0;
+  static_assert(!CPH || NH == 2, "only a sweep that rotates reads the phase factors");
   using K = TmaCfg<T, NH, NRHO, NMOM, TY, TZ, NSTAGE, LK, VW, FEAT>;
   // REG on the magnetisation sweep: G_r (2 values per site); on the moment sweep: the regional VACF (3 values per site)
   static_assert(!REG || NH == 2 || NMOM == 3, "regional sums ride on the magnetisation or on the moment sweep");
@@ -149,7 +152,7 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
     } else {
       tma_load_3d(st + K::F_BYTES, &tm_pi, &full[s], L.padz + z0 - HZ, py, px);
     }
-    if (need_kcs) tma_load_4d(st + K::F_BYTES + K::PI_BYTES, &tm_cs, &full[s], L.padz + z0, py + 1, px, 0);
+    if (need_kcs) tma_load_4d(st + K::F_BYTES + K::PI_BYTES, &tm_cs, &full[s], L.padz + z0, py + 1, px, CPH ? 1 : 0);
     ++jl;
   };
   if (threadIdx.x == 0) {
@@ -257,8 +260,12 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
     const T* sk = reinterpret_cast<const T*>(smem + sc * K::STAGE_BYTES + K::F_BYTES + K::PI_BYTES);
     T csv[VW], snv[VW];
     if (NH == 2) {
-      ldv<T, VW>(sk + ek, csv);
-      ldv<T, VW>(sk + TY * TZ + ek, snv);
+      if constexpr (CPH) {
+        ldv<T, VW>(sk + ek, snv);
+      } else {
+        ldv<T, VW>(sk + ek, csv);
+        ldv<T, VW>(sk + TY * TZ + ek, snv);
+      }
     }
     SiteUpdate<T, NRHO, NMOM> u[VW];
     if constexpr (LK) {
@@ -344,6 +351,7 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
 #pragma unroll
       for (int k = 0; k < VW; ++k) {
         const T hr = o[0][k], hi = o[1][k];
+        if constexpr (CPH) csv[k] = cos_from_sin(snv[k]);
         phase_rotate(csv[k], snv[k], hr, hi, o[0][k], o[1][k]);
         if (k < nvalid) {
           acc[0] += (double)ctr.pi[k] * (double)o[0][k];

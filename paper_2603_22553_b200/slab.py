@@ -57,7 +57,7 @@ class SlabSet:
     torch.distributed is initialised, else a single process).
     """
 
-    def __init__(self, global_shape, bc=(0, 0, 0), slabs_per_rank=1, lattice_factory=None, group=None, **cfg):
+    def __init__(self, global_shape, bc=(0, 0, 0), slabs_per_rank=1, lattice_factory=None, group=None, time_block=0, **cfg):
         self.dist = None
         self.rank, self.world = 0, 1
         try:
@@ -87,8 +87,15 @@ class SlabSet:
             lo, hi = self.ranges[s]
             self.lat[s] = lattice_factory((hi - lo,) + self.global_shape[1:], bc=(LPC_BC_HALO, self.bc[1], self.bc[2]), **cfg)
         self.steps = 0
-        # two time steps per sweep (include/lpc.h "Slabs"): every slab of every rank must be able to, because all slabs
-        # exchange two planes per face then
+        # two time steps per sweep (include/lpc.h "Slabs"; on request, time_block=2 -> LPC_OPT_TIME_BLOCK): every slab of
+        # every rank must be able to, because all slabs exchange two planes per face then
+        if time_block:
+            for m in self.lat.values():
+                if hasattr(m, "set_option"):
+                    try:
+                        m.set_option(1, int(time_block))   # LPC_OPT_TIME_BLOCK
+                    except Exception:
+                        pass                               # a slab that cannot: `can` below turns out False
         can = all(getattr(m, "time_block_steps", 1) == 2 for m in self.lat.values())
         self.two_step = bool(self._allreduce_min(1.0 if can else 0.0) > 0.5)
         self.direct = set()   # (src slab, src side) of OWNED slabs whose plane the step kernel stores into the neighbour itself

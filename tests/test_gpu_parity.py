@@ -271,8 +271,11 @@ def test_two_step_sweep_with_moment_fields(lpc, oracle_mod, shape, bc, alpha, pr
 def test_two_step_sweep_default_and_eligibility(lpc, oracle_mod):
     lat = lpc_inputs.random_small((24, 16, 70), bc=(0, 0, 0), p_block=0.2, seed=62, n_moments=0)
     n = 10
-    # AUTO takes two steps per sweep on a lattice that carries the magnetisation alone
+    # the default is one step per sweep; on request a lattice that carries the magnetisation alone takes two
     gpu, orc = _pair(lpc, oracle_mod, lat, n, 2)
+    assert gpu.time_block_steps == 1
+    gpu.set_option(lpc.LPC_OPT_TIME_BLOCK, 2)
+    assert gpu.time_block_steps == 2
     l0 = gpu.launch_count
     gpu.step(n)
     assert gpu.launch_count - l0 == n // 2
@@ -281,6 +284,7 @@ def test_two_step_sweep_default_and_eligibility(lpc, oracle_mod):
     # the series is bitwise reproducible
     again = lpc.Lattice.from_inputs(lat, max_steps=n)
     again.set_kernel(2)
+    again.set_option(lpc.LPC_OPT_TIME_BLOCK, 2)
     again.step(n)
     assert np.array_equal(again.fid(), gpu.fid())
     # lattices that cannot: a density channel, a periodic axis shorter than four
@@ -304,7 +308,7 @@ def test_two_step_sweep_on_slabs(lpc, oracle_mod, bc, n_slabs, precision):
     lat = lpc_inputs.random_small((46, 18, 70), bc=bc, p_block=0.25, alpha=0.9, seed=83, n_steps=n, n_moments=0)
     rng = np.random.default_rng(5)
     g0 = (rng.random(lat.shape) + 1j * rng.random(lat.shape)) * (lat.blocked == 0)
-    ss = slab.SlabSet(lat.shape, bc=lat.bc, slabs_per_rank=n_slabs, precision=precision, dt=lat.dt, a=lat.a, alpha=lat.alpha, max_steps=n)
+    ss = slab.SlabSet(lat.shape, bc=lat.bc, slabs_per_rank=n_slabs, precision=precision, dt=lat.dt, a=lat.a, alpha=lat.alpha, max_steps=n, time_block=2)
     assert ss.two_step
     ss.set_site_params(lat.dF, lat.blocked, lat.omega, g0)
     l0 = sum(m.launch_count for m in ss.lat.values())
@@ -321,7 +325,7 @@ def test_two_step_sweep_on_slabs(lpc, oracle_mod, bc, n_slabs, precision):
     g = ss.gather_field(lpc.LPC_FIELD_G, dtype=np.complex128)
     assert np.max(np.abs(g - orc.g())[opn] / pi[opn]) <= tol_site * hmax
     # more steps after an odd count: the one-step sweep left the shells to be refilled before the next exchange
-    ss2 = slab.SlabSet(lat.shape, bc=lat.bc, slabs_per_rank=n_slabs, precision=precision, dt=lat.dt, a=lat.a, alpha=lat.alpha, max_steps=n)
+    ss2 = slab.SlabSet(lat.shape, bc=lat.bc, slabs_per_rank=n_slabs, precision=precision, dt=lat.dt, a=lat.a, alpha=lat.alpha, max_steps=n, time_block=2)
     ss2.set_site_params(lat.dF, lat.blocked, lat.omega, g0)
     for k in (3, 1, 8, 19):
         ss2.step(k)
@@ -330,6 +334,46 @@ def test_two_step_sweep_on_slabs(lpc, oracle_mod, bc, n_slabs, precision):
         whole = lpc.Lattice.from_inputs(lat, max_steps=n, g0=g0)
         whole.step(n)
         assert np.max(np.abs(g - whole.field(lpc.LPC_FIELD_G))[opn] / pi[opn]) <= 1e-12 * hmax
+
+
+@pytest.mark.parametrize("precision", [0, 1])
+def test_sweeps_that_read_sin_alone(lpc, oracle_mod, precision):
+    """Lattices whose phase angles are all small (cos(omega dt) >= 1/2) store cos as sqrt(1 - sin^2) and the plain
+    magnetisation sweeps read sin alone (48 instead of 56 bytes per site update in fp64): same state bit for
+    bit as the sweeps that read both, parity with the oracle (which takes cos and sin from libm); a lattice with one wide
+    angle reads cos and sin everywhere."""
+    n = 60
+    sT = 4 if precision else 8
+    tol_site, tol_sum = (1e-5, 1e-5) if precision else (1e-10, 1e-9)
+    lat = lpc_inputs.random_small((40, 19, 150), bc=(0, 1, 0), p_block=0.25, alpha=0.9, seed=71, n_steps=n, n_moments=0)
+    lat.dt = 4.0e-5                                           # |omega dt| up to 1.0: cos >= 0.54
+    assert np.cos(lat.omega * lat.dt).min() >= 0.5
+    out = {}
+    for full in (0, 1):
+        for tb in (1, 2):
+            gpu, orc = _pair(lpc, oracle_mod, lat, n, 2, precision=precision)
+            gpu.set_option(lpc.LPC_OPT_FULL_PHASE, full)
+            gpu.set_option(lpc.LPC_OPT_TIME_BLOCK, tb)
+            assert gpu.bytes_per_site_step == sT * (7 if full else 6)
+            gpu.step(n)
+            orc.step(n)
+            _check(lpc, lat, gpu, orc, n, tol_site=tol_site, tol_sum=tol_sum, what=f"sin alone full={full} tb={tb} p{precision}")
+            out[full, tb] = (gpu.field(lpc.LPC_FIELD_G), gpu.fid())
+    for tb in (1, 2):
+        assert np.array_equal(out[0, tb][0], out[1, tb][0])
+    assert np.array_equal(out[0, 1][1], out[1, 1][1])
+    # one site beyond the limit: the whole lattice reads cos and sin, whatever the option says
+    wide = lpc_inputs.random_small((40, 19, 150), bc=(0, 1, 0), p_block=0.25, alpha=0.9, seed=71, n_steps=n, n_moments=0)
+    wide.dt = 4.0e-5
+    i = tuple(np.argwhere(wide.blocked == 0)[5])
+    wide.omega[i] = 2.0 / wide.dt                             # cos = -0.42
+    for tb in (1, 2):
+        gpu, orc = _pair(lpc, oracle_mod, wide, n, 2, precision=precision)
+        gpu.set_option(lpc.LPC_OPT_TIME_BLOCK, tb)
+        assert gpu.bytes_per_site_step == sT * 7
+        gpu.step(n)
+        orc.step(n)
+        _check(lpc, wide, gpu, orc, n, tol_site=tol_site, tol_sum=tol_sum, what=f"wide angle tb={tb} p{precision}")
 
 
 # ---------------------------------------------------------------------------------------------
@@ -1100,7 +1144,8 @@ def test_regional_fid_fused_sweep_matches_separate_pass(lpc, oracle_mod):
             if not fused:
                 gpu.set_option(lpc.LPC_OPT_REGION_FUSION, 1)      # the separate reduction pass after every sweep
             gpu.set_regions(region)
-            assert gpu.bytes_per_site_step == (4 if precision else 8) * 7 + (1 if fused else (4 if precision else 8) * 3 + 1)
+            # (the sweep next to a separate pass reads sin alone: this lattice's phase angles are all small)
+            assert gpu.bytes_per_site_step == (4 if precision else 8) * (7 if fused else 6) + (1 if fused else (4 if precision else 8) * 3 + 1)
             l0 = gpu.launch_count
             gpu.step(n)
             assert gpu.launch_count - l0 == (n if fused else 2 * n)
