@@ -76,6 +76,7 @@ def parse():
                         "clock record: the rate under the board's power cap (0 = skip)")
     p.add_argument("--time-block", type=int, default=0, choices=[0, 1, 2],
                    help="LPC_OPT_TIME_BLOCK: 0 auto (two time steps per sweep where the lattice allows it), 1 one step per sweep, 2 two")
+    p.add_argument("--x-chunk", type=int, default=0, help="LPC_OPT_X_CHUNK: planes per x chunk of the one-step sweeps (0: the library's choice)")
     p.add_argument("--full-phase", action="store_true",
                    help="LPC_OPT_FULL_PHASE = 1: the sweeps read cos and sin even where every phase angle is small (default: sin alone)")
     p.add_argument("--print-csrc-hash", action="store_true", help="print the hash profiles/traffic.csv is stamped with and exit")
@@ -307,6 +308,8 @@ def run_ours(args):
         sim.set_option(lpc.LPC_OPT_TIME_BLOCK, args.time_block)
     if args.full_phase:
         sim.set_option(lpc.LPC_OPT_FULL_PHASE, 1)
+    if args.x_chunk:
+        sim.set_option(lpc.LPC_OPT_X_CHUNK, args.x_chunk)
     link = None
     if args.links:
         # reduced mobility under confinement: every link that touches a porous (dF != 0) site

@@ -102,6 +102,7 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
   unsigned char* smem = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
   uint64_t* full = reinterpret_cast<uint64_t*>(smem + K::BAR_OFF);
   uint64_t* empty = full + NSTAGE;
+  const uint32_t full_a = smem_u32(full), empty_a = full_a + NSTAGE * 8;   // the consumers' barrier addresses, converted once
   double* red = reinterpret_cast<double*>(smem + K::RED_OFF);
   double* rred = reinterpret_cast<double*>(smem + K::RSLOT_OFF);   // REG: warp partials of the regional columns
 
@@ -178,6 +179,10 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
   const bool edge_yz = (a.per[1] && (y == 0 || y == L.ny - 1)) || (a.per[2] && (z == 0 || z + VW >= L.nz));
   const int permask = (a.per[0] ? 1 : 0) | (a.per[1] ? 2 : 0) | (a.per[2] ? 4 : 0);
   const bool xface = a.per[0] || PEER;   // the outermost x planes have copies to write
+  // planes of this chunk whose groups have copies to write (-1: none), and whether the thread's group takes the plain
+  // 16-byte store on all other planes
+  const int xlo = (xface && x0 == 0) ? 0 : -1, xhi = (xface && x0 + nplanes == L.nx) ? L.nx - 1 : -1;
+  const bool plain = (nvalid == VW) && !edge_yz;
   T* outp = a.fout + L.idx(x0, y, z);
   // REG: the running sum of the region the thread is in; it moves to the thread's slot when the label changes
   const uint8_t* labp = REG ? a.label + ((long long)x0 * L.ny + y) * L.nz + z : nullptr;
@@ -220,7 +225,7 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
   int sj = 0;
   uint32_t phj = 0;
   auto take = [&](Plane& n, const Plane* below) {
-    mbar_wait(&full[sj], phj);
+    mbar_wait_a(full_a + sj * 8, phj);
     const T* sf = reinterpret_cast<const T*>(smem + sj * K::STAGE_BYTES);
     const T* sp = reinterpret_cast<const T*>(smem + sj * K::STAGE_BYTES + K::F_BYTES);
 #pragma unroll
@@ -340,7 +345,7 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
     }
     // every shared-memory read of stage sc is done: hand it back to the producer
     __syncwarp();
-    if (lane == 0) mbar_arrive(&empty[sc]);
+    if (lane == 0) mbar_arrive_a(empty_a + sc * 8);
 
     if constexpr (EQ) {
 #pragma unroll
@@ -353,7 +358,12 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
         const T hr = o[0][k], hi = o[1][k];
         if constexpr (CPH) csv[k] = cos_from_sin(snv[k]);
         phase_rotate(csv[k], snv[k], hr, hi, o[0][k], o[1][k]);
-        if (k < nvalid) {
+        if constexpr (!REG) {
+          // sites beyond the lattice (ragged tiles) count with weight 0; a full group takes the product as it is
+          const double w = (nvalid == VW || k < nvalid) ? (double)ctr.pi[k] : 0.0;
+          acc[0] = fma(w, (double)o[0][k], acc[0]);
+          acc[1] = fma(w, (double)o[1][k], acc[1]);
+        } else if (k < nvalid) {
           acc[0] += (double)ctr.pi[k] * (double)o[0][k];
           acc[1] += (double)ctr.pi[k] * (double)o[1][k];
           if constexpr (REG) {
@@ -364,8 +374,11 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
         }
       }
     }
-    if (nvalid > 0) {
-      if (edge_yz || (xface && (x == 0 || x == L.nx - 1))) {
+    if (plain && x != xlo && x != xhi) {
+#pragma unroll
+      for (int c = 0; c < C; ++c) *reinterpret_cast<V*>(outp + (long long)c * L.np) = packv<T, VW>(o[c]);
+    } else if (nvalid > 0) {
+      if (edge_yz || x == xlo || x == xhi) {
         const long long i = L.idx(x, y, z);
 #pragma unroll
         for (int c = 0; c < C; ++c) {
@@ -384,7 +397,7 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
 
   take(P0, nullptr);
   __syncwarp();
-  if (lane == 0) mbar_arrive(&empty[0]);   // the plane below the chunk is only needed for its centres
+  if (lane == 0) mbar_arrive_a(empty_a);   // the plane below the chunk is only needed for its centres
   take(P1, &P0);
 
   // the march, unrolled by three so that the planes keep their registers while their roles rotate
