@@ -75,8 +75,9 @@ def parse():
                    help="after the K timed steps, time a further block of about this many seconds (at least 200 steps) with its own "
                         "clock record: the rate under the board's power cap (0 = skip)")
     p.add_argument("--time-block", type=int, default=0, choices=[0, 1, 2],
-                   help="LPC_OPT_TIME_BLOCK: 0 auto (two time steps per sweep where the lattice allows it), 1 one step per sweep, 2 two")
+                   help="LPC_OPT_TIME_BLOCK: 0 auto (one step per sweep: measured faster on B200), 1 one step per sweep, 2 two steps per sweep where the lattice allows it")
     p.add_argument("--x-chunk", type=int, default=0, help="LPC_OPT_X_CHUNK: planes per x chunk of the one-step sweeps (0: the library's choice)")
+    p.add_argument("--serial-launch", action="store_true", help="LPC_OPT_SERIAL_LAUNCH = 1: plain launches (no programmatic dependent launch)")
     p.add_argument("--full-phase", action="store_true",
                    help="LPC_OPT_FULL_PHASE = 1: the sweeps read cos and sin even where every phase angle is small (default: sin alone)")
     p.add_argument("--print-csrc-hash", action="store_true", help="print the hash profiles/traffic.csv is stamped with and exit")
@@ -260,7 +261,7 @@ class ClockSampler:
         time.sleep(0.15)
         self.proc.terminate()
         rows = [r for t, r in self.rows if t0 <= t <= t1] or [r for _, r in self.rows]
-        sm, mx, reasons = [], None, set()
+        sm, mx, reasons, power = [], None, set(), []
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for r in rows:
             try:
@@ -268,10 +269,15 @@ class ClockSampler:
                 mx = float(r[1])
             except Exception:
                 continue
+            try:
+                power.append(float(r[2]))
+            except Exception:
+                pass
             for name, v in zip(names, r[3:7]):
                 if v.lower().startswith("active"):
                     reasons.add(name)
-        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm)}
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm),
+                "power_w": statistics.median(power) if power else None}
 
 
 # --------------------------------------------------------------------------------------------
@@ -310,6 +316,8 @@ def run_ours(args):
         sim.set_option(lpc.LPC_OPT_FULL_PHASE, 1)
     if args.x_chunk:
         sim.set_option(lpc.LPC_OPT_X_CHUNK, args.x_chunk)
+    if args.serial_launch:
+        sim.set_option(lpc.LPC_OPT_SERIAL_LAUNCH, 1)
     link = None
     if args.links:
         # reduced mobility under confinement: every link that touches a porous (dF != 0) site
@@ -422,8 +430,10 @@ def run_ours(args):
             key += "/links"
         if args.regions:
             key += "/regions"
-        if args.time_block == 1:
-            key += "/tb1"
+        if args.time_block == 2:
+            key += "/tb2"
+        if args.full_phase:
+            key += "/fullphase"
         traffic = committed_traffic(key)
         steps_per_launch = K / max(launches, 1)
         line = {

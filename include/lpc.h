@@ -76,6 +76,7 @@ extern "C" {
 #define LPC_OPT_PERSIST_MAX_MB 4 /* AUTO takes the persistent kernel up to this many MiB per step; 0 = 48           */
 #define LPC_OPT_REGION_FUSION 5  /* 0 regional sums inside the sweep when possible (default), 1 separate pass       */
 #define LPC_OPT_FULL_PHASE 6     /* 0 sweeps read sin alone where every phase angle is small (default), 1 cos + sin  */
+#define LPC_OPT_SERIAL_LAUNCH 7  /* 0 a sweep may start behind the tail of the one before it (default), 1 plain launches */
 
 typedef struct lpc_lattice lpc_lattice; /* opaque, host struct owned by the library */
 
@@ -318,7 +319,10 @@ int64_t lpc_steps_done(const lpc_lattice* lat);
 /* Kernel launches this lattice has enqueued so far (all kernels, for accounting).              */
 int64_t lpc_launch_count(const lpc_lattice* lat);
 
-/* Algorithmic HBM bytes one step moves per lattice site with this configuration.   */
+/* Algorithmic HBM bytes one step moves per lattice site with this configuration and kernel
+ * choice: state channels in and out, pi, cos and sin -- sin alone where the sweep
+ * rebuilds cos --, pi a second time where the moment fields have a sweep of their own, stored link
+ * weights and region labels if set.  Halo re-reads of the tiles are not in it.                  */
 double lpc_bytes_per_site_step(const lpc_lattice* lat);
 
 /* Free the host handle (the workspace stays with the caller).  NULL is allowed.                */

@@ -25,7 +25,7 @@ LPC_HALO_PARAMS, LPC_HALO_STATE, LPC_HALO_STATE0, LPC_HALO_STATE1 = 0, 1, 2, 3
 LPC_HALO_STATE2, LPC_HALO_PARAMS2, LPC_HALO_PHASE2 = 4, 5, 6
 LPC_HALO_SEND, LPC_HALO_RECV = 0, 1
 LPC_KERNEL_AUTO, LPC_KERNEL_DIRECT, LPC_KERNEL_TMA, LPC_KERNEL_PERSIST = range(4)
-LPC_OPT_TIME_BLOCK, LPC_OPT_X_CHUNK, LPC_OPT_X_CHUNK2, LPC_OPT_PERSIST_MAX_MB, LPC_OPT_REGION_FUSION, LPC_OPT_FULL_PHASE = 1, 2, 3, 4, 5, 6
+LPC_OPT_TIME_BLOCK, LPC_OPT_X_CHUNK, LPC_OPT_X_CHUNK2, LPC_OPT_PERSIST_MAX_MB, LPC_OPT_REGION_FUSION, LPC_OPT_FULL_PHASE, LPC_OPT_SERIAL_LAUNCH = 1, 2, 3, 4, 5, 6, 7
 
 EXPORTS = (
     "lpc_workspace_bytes", "lpc_create_lattice", "lpc_set_site_params", "lpc_set_link_mobility", "lpc_step_n", "lpc_read_fid",

@@ -91,6 +91,7 @@ struct lpc_lattice {
   CUtensorMap tm2_f[2], tm2_m[2], tm2_pi, tm2_cs, tm2_sn;   // tm2_m: the three moment channels; tm2_sn: the sine channel alone
   bool phase_small;   // every open site has cos(omega dt) >= 1/2: sweeps may read sin alone (cos_from_sin)
   int opt_full_phase; // LPC_OPT_FULL_PHASE: 1 = always read cos and sin
+  int opt_serial_launch;   // LPC_OPT_SERIAL_LAUNCH: 1 = no programmatic dependent launch
   int opt_xc, opt_persist_mb, opt_region_fusion;   // lpc_set_option overrides (0 = default)
   // TMA geometry
   int ty, tz, nstage, xc, tiles_z, tiles_y, chunks_x;
@@ -294,6 +295,23 @@ int ensure_dyn_smem(Kern kern, int bytes, int device, bool (&done)[MAX_DEVICES])
 // may the sweeps read sin alone and rebuild cos from it?
 bool sin_only(const lpc_lattice* h) { return h->phase_small && !h->opt_full_phase; }
 
+// A sweep launch that may overlap the tail of the launch before it in the stream (programmatic dependent launch: the
+// kernels call griddepcontrol.launch_dependents / .wait); LPC_OPT_SERIAL_LAUNCH = 1 launches them the plain way.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_sweep(const lpc_lattice* h, void (*kern)(KArgs...), unsigned grid, unsigned threads, size_t smem, Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(threads);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = h->stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = h->opt_serial_launch ? 0 : 1;
+  return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 // ---- launch of one sweep ---------------------------------------------------------------------
 template <typename T, int NRHO, int NMOM>
 int launch_step_t(lpc_lattice* h) {
@@ -343,8 +361,7 @@ int launch_step_t(lpc_lattice* h) {
       using K = decltype(cfg);
       static bool attr_done[MAX_DEVICES] = {};
       if (int rc = ensure_dyn_smem(kern, K::SMEM_BYTES, h->device, attr_done)) return rc;
-      kern<<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(tm, h->tm_pi, h->tm_cs, args);
-      CUDA_TRY(cudaGetLastError());
+      CUDA_TRY(launch_sweep(h, kern, grid, K::NTHREADS, K::SMEM_BYTES, tm, h->tm_pi, h->tm_cs, args));
       h->launches++;
       return LPC_OK;
     };
@@ -352,8 +369,7 @@ int launch_step_t(lpc_lattice* h) {
       using K = decltype(cfg);
       static bool attr_done[MAX_DEVICES] = {};
       if (int rc = ensure_dyn_smem(kern, K::SMEM_BYTES, h->device, attr_done)) return rc;
-      kern<<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(tm, h->tm_pi, h->tm_sn, args);
-      CUDA_TRY(cudaGetLastError());
+      CUDA_TRY(launch_sweep(h, kern, grid, K::NTHREADS, K::SMEM_BYTES, tm, h->tm_pi, h->tm_sn, args));
       h->launches++;
       return LPC_OK;
     };
@@ -367,8 +383,7 @@ int launch_step_t(lpc_lattice* h) {
       using K = decltype(cfg);
       static bool attr_done[MAX_DEVICES] = {};
       if (int rc = ensure_dyn_smem(kern, K::SMEM_BYTES, h->device, attr_done)) return rc;
-      kern<<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(tm, h->tm_cs, h->tm_l, args);
-      CUDA_TRY(cudaGetLastError());
+      CUDA_TRY(launch_sweep(h, kern, grid, K::NTHREADS, K::SMEM_BYTES, tm, h->tm_cs, h->tm_l, args));
       h->launches++;
       return LPC_OK;
     };
@@ -619,8 +634,7 @@ int launch_step2_t(lpc_lattice* h) {
     am.fout = a.fout + 2 * h->L.np;
     static bool attr_done_m[MAX_DEVICES] = {};
     if (int rc = ensure_dyn_smem(step2_kernel<T, VW, 3, false>, KM::SMEM_BYTES, h->device, attr_done_m)) return rc;
-    step2_kernel<T, VW, 3, false><<<grid, KM::NTHREADS, KM::SMEM_BYTES, h->stream>>>(h->tm2_m[h->cur], h->tm2_pi, h->tm2_cs, am);
-    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(launch_sweep(h, step2_kernel<T, VW, 3, false>, grid, KM::NTHREADS, KM::SMEM_BYTES, h->tm2_m[h->cur], h->tm2_pi, h->tm2_cs, am));
     h->launches++;
   }
   a.c0 = 0;
@@ -628,12 +642,12 @@ int launch_step2_t(lpc_lattice* h) {
     using K = Step2Cfg<T, VW, 2, true>;
     static bool attr_done[MAX_DEVICES] = {};
     if (int rc = ensure_dyn_smem(step2_kernel<T, VW, 2, true>, K::SMEM_BYTES, h->device, attr_done)) return rc;
-    step2_kernel<T, VW, 2, true><<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(h->tm2_f[h->cur], h->tm2_pi, h->tm2_sn, a);
+    CUDA_TRY(launch_sweep(h, step2_kernel<T, VW, 2, true>, grid, K::NTHREADS, K::SMEM_BYTES, h->tm2_f[h->cur], h->tm2_pi, h->tm2_sn, a));
   } else {
     using K = Step2Cfg<T, VW, 2, false>;
     static bool attr_done[MAX_DEVICES] = {};
     if (int rc = ensure_dyn_smem(step2_kernel<T, VW, 2, false>, K::SMEM_BYTES, h->device, attr_done)) return rc;
-    step2_kernel<T, VW, 2, false><<<grid, K::NTHREADS, K::SMEM_BYTES, h->stream>>>(h->tm2_f[h->cur], h->tm2_pi, h->tm2_cs, a);
+    CUDA_TRY(launch_sweep(h, step2_kernel<T, VW, 2, false>, grid, K::NTHREADS, K::SMEM_BYTES, h->tm2_f[h->cur], h->tm2_pi, h->tm2_cs, a));
   }
   CUDA_TRY(cudaGetLastError());
   h->launches++;
@@ -1047,7 +1061,7 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
   h->device = dev;
   h->time_block = 0;
   h->ghosts_full = false;
-  h->opt_xc = h->opt_persist_mb = h->opt_region_fusion = h->opt_full_phase = 0;
+  h->opt_xc = h->opt_persist_mb = h->opt_region_fusion = h->opt_full_phase = h->opt_serial_launch = 0;
   h->phase_small = false;
   tma_geometry(h->C, cfg->precision == 1, cfg->nx, cfg->ny, cfg->nz, 0, &h->ty, &h->tz, &h->nstage, &h->xc, &h->tiles_z, &h->tiles_y, &h->chunks_x);
   h->tma_ok = (size_t)h->tiles_z * h->tiles_y * h->chunks_x <= h->off.partial_slots;
@@ -1500,6 +1514,10 @@ int lpc_set_option(lpc_lattice* h, int32_t key, int64_t value) {
       if (value > 1) return fail(LPC_EINVAL, "LPC_OPT_FULL_PHASE takes 0 (sin alone where every phase angle is small) or 1 (always cos and sin)");
       h->opt_full_phase = (int)value;
       return LPC_OK;
+    case LPC_OPT_SERIAL_LAUNCH:
+      if (value > 1) return fail(LPC_EINVAL, "LPC_OPT_SERIAL_LAUNCH takes 0 (a sweep may start behind the one before it) or 1 (plain launches)");
+      h->opt_serial_launch = (int)value;
+      return LPC_OK;
     case LPC_OPT_REGION_FUSION:
       if (value > 1) return fail(LPC_EINVAL, "LPC_OPT_REGION_FUSION takes 0 (inside the sweep when possible) or 1 (separate pass)");
       h->opt_region_fusion = (int)value;
@@ -1524,7 +1542,10 @@ double lpc_bytes_per_site_step(const lpc_lattice* h) {
   const bool sn = sin_only(h) && h->tma_ok && h->kernel != LPC_KERNEL_DIRECT && h->kernel != LPC_KERNEL_PERSIST &&
                   !(h->kernel == LPC_KERNEL_AUTO && persist_by_default(h)) && h->nrho == 0 && !h->have_links &&
                   !(h->have_regions && regions_fusable(h)) && !(h->peer[0][0] || h->peer[1][0]);
-  return (double)h->sT * (2.0 * h->C + (sn ? 2.0 : 3.0) + (h->have_links ? 3.0 : 0.0)) + regions;
+  // moment fields on the TMA path: the step is two sweeps (moment channels, then magnetisation) and each stages pi
+  const bool tma = h->tma_ok && h->kernel != LPC_KERNEL_DIRECT && h->kernel != LPC_KERNEL_PERSIST && !(h->kernel == LPC_KERNEL_AUTO && persist_by_default(h));
+  const double pi_again = (h->nmom == 3 && tma) ? 1.0 : 0.0;
+  return (double)h->sT * (2.0 * h->C + (sn ? 2.0 : 3.0) + pi_again + (h->have_links ? 3.0 : 0.0)) + regions;
 }
 
 void lpc_destroy(lpc_lattice* h) { delete h; }

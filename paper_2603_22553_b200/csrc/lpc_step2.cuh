@@ -151,6 +151,8 @@ __global__ void __launch_bounds__(Step2Cfg<T, VW, NC, CPH>::NTHREADS, 1)
     mbar_fence_init();
   }
   __syncthreads();
+  pdl_launch_dependents();   // as in the one-step sweep (lpc_step_vec.cuh)
+  pdl_wait();
 
   double acc[K::NRED];
 #pragma unroll

@@ -103,6 +103,7 @@ class SlabSet:
         self.remote_direct = False
         self.stats = {"copies": 0, "sends": 0, "recvs": 0}   # plane transfers `exchange` has issued so far
         self._peer_maps = {}       # IPC handle -> base address here of another rank's workspace allocation
+        self._fence = None         # the one-element tensor of the per-step fence
 
     def enable_direct_stores(self, remote=False):
         """Let the step kernel write a slab's outermost planes straight into the neighbours' ghost planes -- the
@@ -117,6 +118,16 @@ class SlabSet:
         self.two_step = False   # the direct stores ride on the one-step sweep
         remote = bool(remote) and self.dist is not None and self.world > 1
         table = {}
+        if remote:
+            # CUDA IPC handles open on the same node only, and the fence and the plane copies are ordered by torch's current
+            # stream: every rank must sit on one host and every slab must run on that stream, else the faces between ranks
+            # keep their send / recv
+            import socket
+
+            ok = all(self._on_current_stream(m) for m in self.lat.values())
+            names = [None] * self.world
+            self.dist.all_gather_object(names, (socket.gethostname(), ok), group=self.group)
+            remote = len({n for n, _ in names}) == 1 and all(o for _, o in names)
         if remote:
             # every rank publishes, per owned slab, the CUDA IPC handle of its workspace allocation and where the ghost
             # planes lie in it (lpc_ipc_export behind the C ABI); a rank maps each remote allocation once (lpc_ipc_open)
@@ -154,6 +165,16 @@ class SlabSet:
                 self.direct_all.update(tuple(f) for f in part)
         return len(self.direct)
 
+    @staticmethod
+    def _on_current_stream(m):
+        """True if the slab's sweeps are ordered with torch's current stream (what the copies and the fence use)."""
+        st = getattr(m, "stream", None)
+        if st is None or not hasattr(st, "cuda_stream"):
+            return True
+        import torch
+
+        return st.cuda_stream == torch.cuda.current_stream(getattr(m, "device", None)).cuda_stream
+
     def _ipc_open(self, handle):
         from . import lpc_ipc_open
 
@@ -173,8 +194,10 @@ class SlabSet:
 
         if self.dist.get_backend(self.group) == "nccl":
             # a one-element all-reduce on the compute stream orders the ranks' streams without stopping the host
-            t = torch.zeros(1, device="cuda")
-            self.dist.all_reduce(t, group=self.group)
+            # (the slabs run on torch's current stream: checked when the direct stores were enabled)
+            if self._fence is None:
+                self._fence = torch.zeros(1, device="cuda")
+            self.dist.all_reduce(self._fence, group=self.group)
         else:
             torch.cuda.synchronize()
             self.dist.barrier(group=self.group)
