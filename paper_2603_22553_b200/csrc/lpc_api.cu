@@ -409,9 +409,13 @@ int launch_step_t(lpc_lattice* h) {
     a.c0 = 0;
     int rc;
     if constexpr (NRHO == 0) {
-      if (sin_only(h) && !fuse_regions && !h->have_links && !peers)
+      if (sin_only(h) && !fuse_regions && !h->have_links && peers)
+        rc = launch_sn(step_tma_kernel<T, 2, 0, 0, TY, 64, NS, VW, 6>, TmaCfg<T, 2, 0, 0, TY, 64, NS, 0, VW, 6>(), h->tm_f[h->cur], a);
+      else if (sin_only(h) && !fuse_regions && !h->have_links && !peers)
         // every phase angle is small: stage sin alone and rebuild cos (8 bytes per site less in fp64)
         rc = launch_sn(step_tma_kernel<T, 2, 0, 0, TY, 64, NS, VW, 4>, TmaCfg<T, 2, 0, 0, TY, 64, NS, 0, VW, 4>(), h->tm_f[h->cur], a);
+      else if (fuse_regions && sin_only(h) && !h->have_links)
+        rc = launch_sn(step_tma_kernel<T, 2, 0, 0, TY, 64, NS, VW, 5>, TmaCfg<T, 2, 0, 0, TY, 64, NS, 0, VW, 5>(), h->tm_f[h->cur], a);
       else if (fuse_regions)
         rc = h->have_links ? launch_links(step_tma_links_kernel<T, 2, 0, 0, TY, 64, NSL, VW, 1>, TmaCfg<T, 2, 0, 0, TY, 64, NSL, 1, VW, 1>(), h->tm_f[h->cur], a)
                            : launch(step_tma_kernel<T, 2, 0, 0, TY, 64, NS, VW, 1>, TmaCfg<T, 2, 0, 0, TY, 64, NS, 0, VW, 1>(), h->tm_f[h->cur], a);
@@ -949,9 +953,9 @@ int equilibrate_t(lpc_lattice* h, double threshold, int64_t max_iters, int64_t c
       if (use_tma) {
         sa.fout = ch[src ^ 1];
         if (h->have_links)
-          step_tma_links_kernel<T, 0, 1, 0, TY, 64, 4, VW><<<tgrid, KL::NTHREADS, KL::SMEM_BYTES, h->stream>>>(h->tm_r[src], h->tm_cs, h->tm_l, sa);
+          CUDA_TRY(launch_sweep(h, step_tma_links_kernel<T, 0, 1, 0, TY, 64, 4, VW>, tgrid, KL::NTHREADS, KL::SMEM_BYTES, h->tm_r[src], h->tm_cs, h->tm_l, sa));
         else
-          step_tma_kernel<T, 0, 1, 0, TY, 64, 4, VW><<<tgrid, KP::NTHREADS, KP::SMEM_BYTES, h->stream>>>(h->tm_r[src], h->tm_pi, h->tm_cs, sa);
+          CUDA_TRY(launch_sweep(h, step_tma_kernel<T, 0, 1, 0, TY, 64, 4, VW>, tgrid, KP::NTHREADS, KP::SMEM_BYTES, h->tm_r[src], h->tm_pi, h->tm_cs, sa));
       } else {
         a.rin = ch[src];
         a.rout = ch[src ^ 1];
@@ -1540,10 +1544,10 @@ double lpc_bytes_per_site_step(const lpc_lattice* h) {
   const double regions = !h->have_regions ? 0.0 : regions_fusable(h) ? 1.0 : 3.0 * h->sT + 1.0;
   // lattices whose phase angles are all small: the plain magnetisation sweeps read sin alone
   const bool sn = sin_only(h) && h->tma_ok && h->kernel != LPC_KERNEL_DIRECT && h->kernel != LPC_KERNEL_PERSIST &&
-                  !(h->kernel == LPC_KERNEL_AUTO && persist_by_default(h)) && h->nrho == 0 && !h->have_links &&
-                  !(h->have_regions && regions_fusable(h)) && !(h->peer[0][0] || h->peer[1][0]);
+                  !(h->kernel == LPC_KERNEL_AUTO && persist_by_default(h) && !h->have_regions) && h->nrho == 0 && !h->have_links;
   // moment fields on the TMA path: the step is two sweeps (moment channels, then magnetisation) and each stages pi
-  const bool tma = h->tma_ok && h->kernel != LPC_KERNEL_DIRECT && h->kernel != LPC_KERNEL_PERSIST && !(h->kernel == LPC_KERNEL_AUTO && persist_by_default(h));
+  const bool tma = h->tma_ok && h->kernel != LPC_KERNEL_DIRECT && h->kernel != LPC_KERNEL_PERSIST &&
+                   !(h->kernel == LPC_KERNEL_AUTO && persist_by_default(h) && !h->have_regions);
   const double pi_again = (h->nmom == 3 && tma) ? 1.0 : 0.0;
   return (double)h->sT * (2.0 * h->C + (sn ? 2.0 : 3.0) + pi_again + (h->have_links ? 3.0 : 0.0)) + regions;
 }

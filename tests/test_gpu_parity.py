@@ -509,7 +509,7 @@ def test_regional_fid_and_spectrum_match_oracle(lpc, oracle_mod, kernel, precisi
     gpu.set_kernel(kernel)
     gpu.set_regions(region)
     # the TMA sweep reads the labels itself (+1 B); the direct kernel is followed by a pass over h, pi and the labels
-    assert gpu.bytes_per_site_step == (4 if precision else 8) * (7 if kernel == 2 else 10) + 1
+    assert gpu.bytes_per_site_step == (4 if precision else 8) * (6 if kernel == 2 else 10) + 1
     gpu.step(n)
     orc = oracle_mod.Oracle.from_lattice(lat, n_moments=0, max_steps=n)
     Gr_o = orc.step_with_regions(region, nreg, n)
@@ -967,7 +967,7 @@ def test_features_at_several_waves_against_oracle(lpc, oracle_mod):
     for precision, tol_sum, tol_site in ((0, 1e-9, 1e-10), (1, 1e-5, 1e-5)):
         gpu = lpc.Lattice.from_inputs(lat, precision=precision, max_steps=n, n_regions=nreg)
         gpu.set_regions(region)
-        assert gpu.bytes_per_site_step == (4 if precision else 8) * 7 + 1      # the labels ride on the sweep
+        assert gpu.bytes_per_site_step == (4 if precision else 8) * 6 + 1      # the labels ride on the sweep (which reads sin alone)
         gpu.step(n)
         for r in range(nreg):
             assert np.max(np.abs(gpu.fid_region(r) - Gr_o[r]) / sabs) <= tol_sum, f"region {r} p{precision}"
@@ -1147,7 +1147,7 @@ def test_regional_fid_fused_sweep_matches_separate_pass(lpc, oracle_mod):
                 gpu.set_option(lpc.LPC_OPT_REGION_FUSION, 1)      # the separate reduction pass after every sweep
             gpu.set_regions(region)
             # (the sweep next to a separate pass reads sin alone: this lattice's phase angles are all small)
-            assert gpu.bytes_per_site_step == (4 if precision else 8) * (7 if fused else 6) + (1 if fused else (4 if precision else 8) * 3 + 1)
+            assert gpu.bytes_per_site_step == (4 if precision else 8) * 6 + (1 if fused else (4 if precision else 8) * 3 + 1)
             l0 = gpu.launch_count
             gpu.step(n)
             assert gpu.launch_count - l0 == (n if fused else 2 * n)
