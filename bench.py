@@ -436,6 +436,11 @@ def run_ours(args):
             key += "/fullphase"
         traffic = committed_traffic(key)
         steps_per_launch = K / max(launches, 1)
+        # the same step with cos AND sin read (the round-1 layout, SURVEY 8(d)'s "stored phase" row: 56 B in fp64): the rate
+        # this run would need on those bytes, i.e. what the byte diet of DESIGN.md section 5 is worth
+        sim.set_option(lpc.LPC_OPT_FULL_PHASE, 1)
+        bps_cs = sim.bytes_per_site_step
+        sim.set_option(lpc.LPC_OPT_FULL_PHASE, 1 if args.full_phase else 0)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -450,15 +455,17 @@ def run_ours(args):
             "clocks": clocks,
             "e2e": e2e,
             "gpu_launches": int(launches),
-            # achieved = algorithmic bytes of the ONE-STEP-PER-SWEEP layout (56 B per site update in fp64) x site
-            # updates per launch / launch duration.  With two time steps per sweep a launch updates every site twice, so
-            # this EFFECTIVE rate can exceed the HBM peak; `dram` is what actually crossed HBM (ncu traffic / launch time).
+            # achieved = algorithmic bytes of the one-step-per-sweep layout (lpc_bytes_per_site_step: 48 B per site update in
+            # fp64 where the sweep reads sin alone) x site updates per launch / launch duration.  With two
+            # time steps per sweep a launch updates every site twice, so this EFFECTIVE rate can exceed the HBM peak; `dram_gbs`
+            # is what actually crossed HBM (ncu traffic / launch time).
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": traffic, "peak_source": peak_src, "bytes_per_site_step": bps,
                          "kernel_ms": ms_kernel * steps_per_launch, "launches_per_step": launches / K,
                          "time_steps_per_launch": steps_per_launch,
                          "dram_gbs": (traffic / (ms_kernel * steps_per_launch * 1e-3) / 1e9) if traffic else None,
-                         "frac_of_8TBs_spec": achieved / 8000.0},
+                         "frac_of_8TBs_spec": achieved / 8000.0,
+                         "bytes_per_site_step_cos_and_sin": bps_cs, "frac_on_cos_and_sin_bytes": achieved * bps_cs / bps / peak},
         }
         if sustained is not None:
             a_sus = bps * n_sites / (sustained["kernel_ms"] * 1e-3) / 1e9
