@@ -310,6 +310,12 @@ int lpc_set_kernel(lpc_lattice* lat, int32_t which);
  * of range, or LPC_OPT_TIME_BLOCK = 2 on a lattice that cannot run the two-step sweep).          */
 int lpc_set_option(lpc_lattice* lat, int32_t key, int64_t value);
 
+/* 1 if the plain magnetisation sweeps of this lattice read sin alone and rebuild cos (every open
+ * site has cos(omega dt) >= 1/2 and LPC_OPT_FULL_PHASE is 0), else 0.  Slabs that take two steps
+ * per sweep rotate their neighbours' boundary sites as well, so the slabs of one lattice must agree:
+ * a caller sets LPC_OPT_FULL_PHASE = 1 on all of them unless every slab answers 1.               */
+int32_t lpc_reads_sin_alone(const lpc_lattice* lat);
+
 /* 2 if the next lpc_step_n(lat, n >= 2) takes two time steps per sweep (see lpc_step_n), else 1.  */
 int32_t lpc_time_block_steps(const lpc_lattice* lat);
 

@@ -30,7 +30,7 @@ LPC_OPT_TIME_BLOCK, LPC_OPT_X_CHUNK, LPC_OPT_X_CHUNK2, LPC_OPT_PERSIST_MAX_MB, L
 EXPORTS = (
     "lpc_workspace_bytes", "lpc_create_lattice", "lpc_set_site_params", "lpc_set_link_mobility", "lpc_step_n", "lpc_read_fid",
     "lpc_moments", "lpc_read_field", "lpc_set_state", "lpc_equilibrate", "lpc_seed_from_density", "lpc_set_regions", "lpc_read_fid_region", "lpc_moments_region", "lpc_spectrum", "lpc_set_kernel",
-    "lpc_set_option", "lpc_time_block_steps", "lpc_ipc_export", "lpc_ipc_open", "lpc_ipc_close", "lpc_steps_done", "lpc_partition_sum", "lpc_set_partition_sum", "lpc_halo_view", "lpc_set_halo_peers", "lpc_slab_finish",
+    "lpc_set_option", "lpc_time_block_steps", "lpc_reads_sin_alone", "lpc_ipc_export", "lpc_ipc_open", "lpc_ipc_close", "lpc_steps_done", "lpc_partition_sum", "lpc_set_partition_sum", "lpc_halo_view", "lpc_set_halo_peers", "lpc_slab_finish",
     "lpc_launch_count", "lpc_bytes_per_site_step", "lpc_destroy", "lpc_last_error",
 )
 
@@ -92,6 +92,8 @@ def _load():
     lib.lpc_spectrum.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_double, C.c_double, C.c_int64, C.c_double, C.c_void_p]
     lib.lpc_time_block_steps.argtypes = [C.c_void_p]
     lib.lpc_time_block_steps.restype = C.c_int32
+    lib.lpc_reads_sin_alone.argtypes = [C.c_void_p]
+    lib.lpc_reads_sin_alone.restype = C.c_int32
     lib.lpc_steps_done.argtypes = [C.c_void_p]
     lib.lpc_steps_done.restype = C.c_int64
     lib.lpc_launch_count.argtypes = [C.c_void_p]
@@ -311,6 +313,10 @@ def lpc_time_block_steps(handle) -> int:
     return int(_lib.lpc_time_block_steps(handle))
 
 
+def lpc_reads_sin_alone(handle) -> int:
+    return int(_lib.lpc_reads_sin_alone(handle))
+
+
 def lpc_steps_done(handle) -> int:
     return int(_lib.lpc_steps_done(handle))
 
@@ -476,6 +482,10 @@ class Lattice:
     @property
     def time_block_steps(self):
         return lpc_time_block_steps(self.handle)
+
+    @property
+    def reads_sin_alone(self):
+        return bool(lpc_reads_sin_alone(self.handle))
 
     @property
     def steps_done(self):

@@ -141,9 +141,12 @@ Layout make_layout(const lpc_config* c) {
 // SM (a sweep carries at most 3 channels: the moment fields have a sweep of their own).  (16 x 64 tiles with one 16-warp CTA per SM measured the same at 512^3
 // and slightly worse at 256^3, so there is one tile shape.)
 constexpr int SM_COUNT = 148;
+#ifndef LPC_TY64
+#define LPC_TY64 8   // rows of an fp64 tile (-DLPC_TY64=16: one 16-warp CTA per SM, 512^3 fp64 118.0 / 104.8 GLUPS burst / sustained against 120.4 / 105.5)
+#endif
 
 void tma_geometry(int C, bool f32, int nx, int ny, int nz, int xc_override, int* ty, int* tz, int* nstage, int* xc, int* tiles_z, int* tiles_y, int* chunks_x) {
-  *ty = f32 ? 16 : 8; *tz = 64;   // fp32: a thread owns a z-quad (lpc_step_vec.cuh), 256 threads cover 16 rows
+  *ty = f32 ? 16 : LPC_TY64; *tz = 64;   // fp32: a thread owns a z-quad (lpc_step_vec.cuh), 256 threads cover 16 rows
   *nstage = 4;   // 3 when the density rides along (3 channels); informational, the kernels fix it
   *tiles_z = (nz + *tz - 1) / *tz;
   *tiles_y = (ny + *ty - 1) / *ty;
@@ -388,7 +391,7 @@ int launch_step_t(lpc_lattice* h) {
       return LPC_OK;
     };
     // fp64: a thread owns a z-pair on 8 x 64 tiles; fp32: a z-quad on 16 x 64 tiles (one 16-byte group either way)
-    constexpr int VW = 16 / (int)sizeof(T), TY = 4 * VW;
+    constexpr int VW = 16 / (int)sizeof(T), TY = sizeof(T) == 8 ? LPC_TY64 : 4 * VW;
     constexpr int NS = (NRHO == 0) ? 4 : 3;   // two CTAs per SM must fit in shared memory
     constexpr int NSL = (NRHO == 0) ? 3 : 2;  // with the link-weight boxes
     if constexpr (NMOM == 3) {
@@ -935,7 +938,7 @@ int equilibrate_t(lpc_lattice* h, double threshold, int64_t max_iters, int64_t c
   sa.label = nullptr; sa.rpartials = nullptr; sa.fidr = nullptr; sa.fidr_stride = 0; sa.region_sample = 0; sa.n_regions = 0;
   sa.vacfr = nullptr; sa.wr = nullptr; sa.vacfr_stride = 0;
   sa.c0 = 2; sa.xc = h->xc; sa.tiles_z = h->tiles_z; sa.tiles_y = h->tiles_y; sa.chunks_x = h->chunks_x;
-  constexpr int VW = 16 / (int)sizeof(T), TY = 4 * VW;
+  constexpr int VW = 16 / (int)sizeof(T), TY = sizeof(T) == 8 ? LPC_TY64 : 4 * VW;
   using KP = TmaCfg<T, 0, 1, 0, TY, 64, 4, 0, VW>;
   using KL = TmaCfg<T, 0, 1, 0, TY, 64, 4, 1, VW>;
   if (use_tma) {
@@ -1532,6 +1535,7 @@ int lpc_set_option(lpc_lattice* h, int32_t key, int64_t value) {
 }
 
 int32_t lpc_time_block_steps(const lpc_lattice* h) { return (h && step2_usable(h)) ? 2 : 1; }
+int32_t lpc_reads_sin_alone(const lpc_lattice* h) { return (h && h->have_params && sin_only(h)) ? 1 : 0; }
 int64_t lpc_steps_done(const lpc_lattice* h) { return h ? h->steps : 0; }
 int64_t lpc_launch_count(const lpc_lattice* h) { return h ? h->launches : 0; }
 

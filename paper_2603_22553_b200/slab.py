@@ -292,6 +292,14 @@ class SlabSet:
         for s in self.owned:
             self.lat[s].set_partition_sum(Z)
             self.lat[s].set_site_params(*parts[s])
+        # slabs that take two steps per sweep rotate their neighbours' boundary sites too: all slabs read the phase factors the
+        # same way (sin alone only if every slab of every rank may, include/lpc.h lpc_reads_sin_alone)
+        if self.two_step:
+            mine = all(getattr(self.lat[s], "reads_sin_alone", True) for s in self.owned)
+            if self._allreduce_min(1.0 if mine else 0.0) < 0.5:
+                for s in self.owned:
+                    if hasattr(self.lat[s], "set_option"):
+                        self.lat[s].set_option(6, 1)   # LPC_OPT_FULL_PHASE
         if self.two_step:
             self.exchange(HALO_PARAMS2)
             self.exchange(HALO_PHASE2)     # the two-step sweep rotates the ring of neighbour sites as well

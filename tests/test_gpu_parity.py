@@ -336,6 +336,34 @@ def test_two_step_sweep_on_slabs(lpc, oracle_mod, bc, n_slabs, precision):
         assert np.max(np.abs(g - whole.field(lpc.LPC_FIELD_G))[opn] / pi[opn]) <= 1e-12 * hmax
 
 
+def test_two_step_slabs_agree_on_the_phase_factors(lpc, oracle_mod):
+    """One wide phase angle on a boundary plane of one slab: the neighbour slab rotates that site in its first step too, so
+    every slab has to read cos and sin (lpc_reads_sin_alone); against the oracle and against the unsplit lattice."""
+    from paper_2603_22553_b200 import slab
+
+    n = 20
+    lat = lpc_inputs.random_small((40, 18, 70), bc=(0, 0, 0), p_block=0.2, alpha=0.9, seed=84, n_steps=n, n_moments=0)
+    lat.blocked[19, 5, 7] = 0
+    lat.omega[19, 5, 7] = 2.0 / lat.dt                        # cos = -0.42, on the last plane of slab 0 of 2
+    ss = slab.SlabSet(lat.shape, bc=lat.bc, slabs_per_rank=2, dt=lat.dt, a=lat.a, alpha=lat.alpha, max_steps=n, time_block=2)
+    assert ss.two_step
+    ss.set_site_params(lat.dF, lat.blocked, lat.omega)
+    assert not any(m.reads_sin_alone for m in ss.lat.values())
+    ss.step(n)
+    orc = oracle_mod.Oracle.from_lattice(lat, n_moments=0, max_steps=n)
+    orc.step(n)
+    G_o, sabs = orc.fid(with_scale=True)
+    assert np.max(np.abs(ss.fid() - G_o) / sabs) <= 1e-9
+    pi, opn = orc.pi(), lat.blocked == 0
+    g = ss.gather_field(lpc.LPC_FIELD_G, dtype=np.complex128)
+    assert np.max(np.abs(g - orc.g())[opn] / pi[opn]) <= 1e-10
+    whole = lpc.Lattice.from_inputs(lat, max_steps=n)
+    whole.set_kernel(2)
+    whole.step(n)
+    # (the slabs add their partition sums in another order than the unsplit lattice: pi may differ in the last bit)
+    assert np.max(np.abs(g - whole.field(lpc.LPC_FIELD_G))[opn] / pi[opn]) <= 1e-12
+
+
 @pytest.mark.parametrize("precision", [0, 1])
 def test_sweeps_that_read_sin_alone(lpc, oracle_mod, precision):
     """Lattices whose phase angles are all small (cos(omega dt) >= 1/2) store cos as sqrt(1 - sin^2) and the plain
