@@ -1295,7 +1295,7 @@ def test_random_lattices_against_oracle(lpc, oracle_mod):
 
 
 @pytest.mark.parametrize("precision,nm,nd,nreg,use_link,bc", [(0, 3, 1, 3, True, (0, 0, 0)), (1, 3, 1, 3, True, (1, 0, 1)), (0, 0, 0, 0, False, (0, 1, 0)),
-                                                              (1, 0, 0, 2, False, (0, 0, 0)), (0, 3, 0, 0, False, (2, 0, 0))])
+                                                              (1, 0, 0, 2, False, (0, 0, 0)), (0, 3, 0, 0, False, (2, 0, 0)), (1, 3, 0, 0, False, (0, 0, 0))])
 def test_nothing_is_written_outside_the_workspace(lpc, precision, nm, nd, nreg, use_link, bc):
     """Guard bytes before and after the workspace stay untouched through the precompute, every step kernel, the
     equilibration sweeps, the regional passes and the read-outs (a bounds check of our own: the sanitizer is not
@@ -1336,6 +1336,17 @@ def test_nothing_is_written_outside_the_workspace(lpc, precision, nm, nd, nreg, 
                 lpc.lpc_moments(handle)
             if nreg:
                 lpc.lpc_read_fid_region(handle, 0)
+        # the two-step sweep (own tiles, two ghost layers, ghost images of the face sites) where the lattice can run it, and the
+        # sweeps that read cos and sin
+        if nd == 0 and nreg == 0 and bc[0] != 2:
+            lpc.lpc_set_kernel(handle, 2)
+            lpc.lpc_set_site_params(handle, lat.dF, lat.blocked, lat.omega)
+            lpc.lpc_set_option(handle, lpc.LPC_OPT_TIME_BLOCK, 2)
+            assert lpc.lpc_time_block_steps(handle) == 2
+            lpc.lpc_step_n(handle, 6)
+            lpc.lpc_set_option(handle, lpc.LPC_OPT_FULL_PHASE, 1)
+            lpc.lpc_step_n(handle, 5)
+            lpc.lpc_read_fid(handle)
         torch.cuda.synchronize()
         assert bool((buf[:guard] == 0xAB).all()) and bool((buf[guard + nbytes:] == 0xAB).all())
     finally:
