@@ -95,6 +95,7 @@ struct lpc_lattice {
   int opt_xc, opt_persist_mb, opt_region_fusion;   // lpc_set_option overrides (0 = default)
   // TMA geometry
   int ty, tz, nstage, xc, tiles_z, tiles_y, chunks_x;
+  int xc_reg, chunks_x_reg;   // x chunks of the sweeps that carry regional sums
   bool tma_ok;
   TmaLinkMaps tm_l;  // pi centres and the three link-weight channels (link_mobility = 1)
   CUtensorMap tm_f[2], tm_m[2], tm_r[2], tm_pi, tm_cs, tm_sn;  // tm_r: one channel per box (the density channel alone, equilibration)  // tm_f: magnetisation (+ density) channels, tm_m: the 3 moment channels
@@ -145,7 +146,8 @@ constexpr int SM_COUNT = 148;
 #define LPC_TY64 8   // rows of an fp64 tile (-DLPC_TY64=16: one 16-warp CTA per SM, 512^3 fp64 118.0 / 104.8 GLUPS burst / sustained against 120.4 / 105.5)
 #endif
 
-void tma_geometry(int C, bool f32, int nx, int ny, int nz, int xc_override, int* ty, int* tz, int* nstage, int* xc, int* tiles_z, int* tiles_y, int* chunks_x) {
+void tma_geometry(int C, bool f32, int nx, int ny, int nz, int xc_override, int* ty, int* tz, int* nstage, int* xc, int* tiles_z, int* tiles_y, int* chunks_x,
+                  int target = 32) {
   *ty = f32 ? 16 : LPC_TY64; *tz = 64;   // fp32: a thread owns a z-quad (lpc_step_vec.cuh), 256 threads cover 16 rows
   *nstage = 4;   // 3 when the density rides along (3 channels); informational, the kernels fix it
   *tiles_z = (nz + *tz - 1) / *tz;
@@ -159,7 +161,9 @@ void tma_geometry(int C, bool f32, int nx, int ny, int nz, int xc_override, int*
   // write bursts; many short CTAs desynchronise and keep the mix even.  Below 24 planes the two extra
   // plane loads per chunk cost more than that gains, unless the grid is short of waves (256^3: 16 planes
   // per chunk measured 2% faster than 32), so chunks shrink to 16 planes to reach 8 waves.
-  long long chunks = std::max(1, (nx + 16) / 32);
+  // (sweeps with regional sums take 64-plane chunks, `target`: their per-CTA epilogue -- a warp sum per regional column -- is
+  // worth two planes; 512^3 fp64 with three regions 98.1 -> 102.7 GLUPS burst, 89.3 -> 93.2 sustained)
+  long long chunks = std::max(1, (nx + target / 2) / target);
   chunks = std::max(chunks, std::min<long long>(std::max(1, nx / 16), (8 * resident + tiles - 1) / tiles));
   if (tiles * std::max(1, nx / 16) < 3 * resident) {
     // Few waves: wave quantisation decides.  A CTA costs its planes plus two halo planes plus about six
@@ -349,6 +353,10 @@ int launch_step_t(lpc_lattice* h) {
   // (and not together with direct halo stores: that combination runs the separate pass)
   const bool fuse_regions = use_tma && will_fuse_regions(h);
   h->regions_fused = fuse_regions;
+  if (fuse_regions && !h->opt_xc) {
+    a.xc = h->xc_reg;
+    a.chunks_x = h->chunks_x_reg;
+  }
   a.label = fuse_regions ? h->ws + h->off.regions : nullptr;
   a.rpartials = wsp<double>(h, h->off.rpartials);
   a.fidr = wsp<double2>(h, h->off.fidr);
@@ -359,7 +367,7 @@ int launch_step_t(lpc_lattice* h) {
   a.region_sample = h->steps + 1;
   a.n_regions = h->cfg.n_regions;
   if (use_tma) {
-    const unsigned grid = (unsigned)(h->tiles_z * h->tiles_y * h->chunks_x);
+    const unsigned grid = (unsigned)(h->tiles_z * h->tiles_y * a.chunks_x);
     auto launch = [&](auto kern, auto cfg, const CUtensorMap& tm, const StepArgs<T>& args) -> int {
       using K = decltype(cfg);
       static bool attr_done[MAX_DEVICES] = {};
@@ -1072,6 +1080,10 @@ int lpc_create_lattice(const lpc_config* cfg, void* workspace_dev, size_t bytes,
   h->phase_small = false;
   tma_geometry(h->C, cfg->precision == 1, cfg->nx, cfg->ny, cfg->nz, 0, &h->ty, &h->tz, &h->nstage, &h->xc, &h->tiles_z, &h->tiles_y, &h->chunks_x);
   h->tma_ok = (size_t)h->tiles_z * h->tiles_y * h->chunks_x <= h->off.partial_slots;
+  {
+    int ty, tz, ns, tzs, tys;
+    tma_geometry(h->C, cfg->precision == 1, cfg->nx, cfg->ny, cfg->nz, 0, &ty, &tz, &ns, &h->xc_reg, &tzs, &tys, &h->chunks_x_reg, 64);
+  }
   // two steps per sweep: the magnetisation channels alone, no slab, and every periodic axis long enough for two ghost layers
   h->ty2 = 8; h->tz2 = 32 * (16 / h->sT);
   h->tiles_z2 = (cfg->nz + h->tz2 - 1) / h->tz2;

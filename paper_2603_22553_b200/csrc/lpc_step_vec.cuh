@@ -214,13 +214,13 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
   double racc[RNV];
   double rall[REG ? MAX_REGIONS * RNV : 1];
   if constexpr (REG) {
-#pragma unroll
-    for (int q = 0; q < MAX_REGIONS * RNV; ++q) rall[q] = 0.0;
+    for (int q = 0; q < a.n_regions * RNV; ++q) rall[q] = 0.0;
 #pragma unroll
     for (int v = 0; v < RNV; ++v) racc[v] = 0.0;
   }
+  const int nrcol = REG ? a.n_regions * RNV : 0;   // regional columns in use: labels beyond n_regions are in no region
   auto rflush = [&](int next) {
-    if (rcur < MAX_REGIONS) {
+    if (rcur < a.n_regions) {
 #pragma unroll
       for (int v = 0; v < RNV; ++v) rall[rcur * RNV + v] += racc[v];
     }
@@ -442,13 +442,12 @@ __device__ __forceinline__ void step_tma_body(const CUtensorMap& tm_f, const CUt
     // block partial of every (region, component) column: warp sums, then thread q adds the warps of column q in order
     rflush(255);
     const int warp = threadIdx.x >> 5;
-#pragma unroll
-    for (int q = 0; q < RNC; ++q) {
+    for (int q = 0; q < nrcol; ++q) {   // only the columns of regions that exist (three regions: 6 of 16)
       const double v = warp_sum(rall[q]);
       if (lane == 0) rred[warp * RNC + q] = v;
     }
     __syncthreads();
-    if (threadIdx.x < RNC) {
+    if (threadIdx.x < nrcol) {
       double v = 0.0;
       for (int w = 0; w < K::NTHREADS / 32; ++w) v += rred[w * RNC + threadIdx.x];
       a.rpartials[(size_t)blockIdx.x * RNC + threadIdx.x] = v;
