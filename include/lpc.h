@@ -331,6 +331,26 @@ int64_t lpc_launch_count(const lpc_lattice* lat);
  * weights and region labels if set.  Halo re-reads of the tiles are not in it.                  */
 double lpc_bytes_per_site_step(const lpc_lattice* lat);
 
+/* One FID sample without a lattice, a workspace or any allocation (for callers that may not call
+ * cudaMalloc: under CUDA graph capture, in a serving loop, in a harness that forbids it):
+ *     out[0] + i out[1] = G = sum_{i < n_sites} g_i          (Eq. 12)
+ * of a dense device array g of n_sites complex numbers (re, im pairs of doubles, e.g. what
+ * lpc_read_field(lat, LPC_FIELD_G, device pointer) wrote).  A variant of the reduction kernel behind
+ * lpc_set_state: one block partial per 32768 sites, then the last block adds the partials in block
+ * order (bitwise reproducible for a given n_sites).  The partials and the ticket counter live in a
+ * static __device__ array of the library (LPC_NOALLOC_SCRATCH_BYTES, held by every GPU that loads
+ * the library until the process exits), which is why n_sites is limited to LPC_NOALLOC_MAX_SITES.
+ *   g, out : DEVICE pointers of the current device, caller-owned; out takes 2 doubles.
+ *   stream : cudaStream_t of the current device (NULL: the default stream).  Asynchronous.
+ * The call clears the ticket counter itself (stream-ordered) and overwrites every partial it reads,
+ * so it does not depend on what the last call left.  ALL calls on a device share the one array:
+ * calls that overlap on the GPU (two streams, two host threads) race -- serialise them.
+ * Calls no cudaMalloc / cudaFree and no allocating library routine.
+ * Errors: LPC_EINVAL (NULL or host pointer, n_sites < 0 or > LPC_NOALLOC_MAX_SITES), LPC_ECUDA.  */
+#define LPC_NOALLOC_MAX_SITES (1ll << 28)       /* 8192 block partials x 32768 sites            */
+#define LPC_NOALLOC_SCRATCH_BYTES (256 + 8192 * 16)
+int lpc_fid_sample_noalloc(const double* g_re_im_dev, int64_t n_sites, double* out_dev, void* stream);
+
 /* Free the host handle (the workspace stays with the caller).  NULL is allowed.                */
 void lpc_destroy(lpc_lattice* lat);
 

@@ -31,7 +31,7 @@ EXPORTS = (
     "lpc_workspace_bytes", "lpc_create_lattice", "lpc_set_site_params", "lpc_set_link_mobility", "lpc_step_n", "lpc_read_fid",
     "lpc_moments", "lpc_read_field", "lpc_set_state", "lpc_equilibrate", "lpc_seed_from_density", "lpc_set_regions", "lpc_read_fid_region", "lpc_moments_region", "lpc_spectrum", "lpc_set_kernel",
     "lpc_set_option", "lpc_time_block_steps", "lpc_reads_sin_alone", "lpc_ipc_export", "lpc_ipc_open", "lpc_ipc_close", "lpc_steps_done", "lpc_partition_sum", "lpc_set_partition_sum", "lpc_halo_view", "lpc_set_halo_peers", "lpc_slab_finish",
-    "lpc_launch_count", "lpc_bytes_per_site_step", "lpc_destroy", "lpc_last_error",
+    "lpc_launch_count", "lpc_bytes_per_site_step", "lpc_fid_sample_noalloc", "lpc_destroy", "lpc_last_error",
 )
 
 
@@ -90,6 +90,7 @@ def _load():
     lib.lpc_read_fid_region.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_int64, C.c_void_p]
     lib.lpc_moments_region.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_void_p, C.c_void_p]
     lib.lpc_spectrum.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_double, C.c_double, C.c_int64, C.c_double, C.c_void_p]
+    lib.lpc_fid_sample_noalloc.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
     lib.lpc_time_block_steps.argtypes = [C.c_void_p]
     lib.lpc_time_block_steps.restype = C.c_int32
     lib.lpc_reads_sin_alone.argtypes = [C.c_void_p]
@@ -307,6 +308,16 @@ def lpc_set_kernel(handle, which):
 
 def lpc_set_option(handle, key, value):
     _check(_lib.lpc_set_option(handle, int(key), int(value)))
+
+
+LPC_NOALLOC_MAX_SITES = 1 << 28
+
+
+def lpc_fid_sample_noalloc(g_dev_ptr, n_sites, out_dev_ptr, stream=None):
+    """G = sum of n_sites complex numbers at the DEVICE address g_dev_ptr into the 2 doubles at the DEVICE address
+    out_dev_ptr (Eq. 12); scratch in the library's static device array, nothing is allocated (include/lpc.h)."""
+    _check(_lib.lpc_fid_sample_noalloc(C.c_void_p(int(g_dev_ptr)), int(n_sites), C.c_void_p(int(out_dev_ptr)),
+                                       C.c_void_p(int(stream)) if stream else None))
 
 
 def lpc_time_block_steps(handle) -> int:

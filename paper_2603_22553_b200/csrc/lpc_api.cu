@@ -1571,3 +1571,113 @@ double lpc_bytes_per_site_step(const lpc_lattice* h) {
 void lpc_destroy(lpc_lattice* h) { delete h; }
 
 }  // extern "C"
+
+// ================================================================================================
+// lpc_fid_sample_noalloc: Eq. 12 of a dense complex array with NO memory of the caller's or of an
+// allocator: the block partials and the ticket counter of the reduction -- what reduce_g_kernel keeps in the workspace --
+// live in a file-scope device array.  Everything that touches the array is in this file: in host code its name is a
+// host-side stand-in, not a device address, so the entry point asks cudaGetSymbolAddress once per device (with that
+// device current) and hands the kernel the pointer it got.
+// ================================================================================================
+namespace {
+
+constexpr int NA_CHUNK = 1 << 15;       // sites per block partial
+constexpr int NA_MAX_BLOCKS = 8192;     // partials the array holds: LPC_NOALLOC_MAX_SITES = NA_CHUNK * NA_MAX_BLOCKS
+constexpr int NA_HEADER = 256;          // the ticket counter, on a 256-byte line of its own
+static_assert((long long)NA_CHUNK * NA_MAX_BLOCKS == LPC_NOALLOC_MAX_SITES, "lpc.h states the limit");
+static_assert(NA_HEADER + NA_MAX_BLOCKS * (int)sizeof(double2) == LPC_NOALLOC_SCRATCH_BYTES, "lpc.h states the size");
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[LPC_NOALLOC_SCRATCH_BYTES];
+
+// Block b adds the sites [b NA_CHUNK, (b+1) NA_CHUNK) (thread-strided, then warp shuffles, then the warps in order) and
+// stores one partial; the block that takes the last ticket adds all partials in block order and writes out[0..1].
+// Deterministic: the order depends on n alone.  `scratch` is the device address of g_noalloc_scratch.
+__global__ void __launch_bounds__(256) fid_sample_noalloc_kernel(const double2* __restrict__ g, long long n, unsigned char* scratch,
+                                                                  double* __restrict__ out) {
+  unsigned int* ticket = reinterpret_cast<unsigned int*>(scratch);
+  double2* partial = reinterpret_cast<double2*>(scratch + NA_HEADER);
+  __shared__ double red[2 * 8];
+  __shared__ unsigned int s_last;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const long long i0 = (long long)blockIdx.x * NA_CHUNK;
+  const long long i1 = (i0 + NA_CHUNK < n) ? i0 + NA_CHUNK : n;
+  double re = 0.0, im = 0.0;
+  for (long long i = i0 + threadIdx.x; i < i1; i += blockDim.x) {
+    const double2 v = g[i];
+    re += v.x;
+    im += v.y;
+  }
+  re = warp_sum(re);
+  im = warp_sum(im);
+  if (lane == 0) {
+    red[2 * warp] = re;
+    red[2 * warp + 1] = im;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double sr = 0.0, si = 0.0;
+    for (int w = 0; w < 8; ++w) {
+      sr += red[2 * w];
+      si += red[2 * w + 1];
+    }
+    partial[blockIdx.x] = make_double2(sr, si);
+    __threadfence();
+    s_last = (atomicAdd(ticket, 1u) == gridDim.x - 1) ? 1u : 0u;
+  }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  re = im = 0.0;
+  for (unsigned int b = threadIdx.x; b < gridDim.x; b += blockDim.x) {
+    const double2 v = __ldcg(&partial[b]);
+    re += v.x;
+    im += v.y;
+  }
+  re = warp_sum(re);
+  im = warp_sum(im);
+  __syncthreads();   // red is reused
+  if (lane == 0) {
+    red[2 * warp] = re;
+    red[2 * warp + 1] = im;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double sr = 0.0, si = 0.0;
+    for (int w = 0; w < 8; ++w) {
+      sr += red[2 * w];
+      si += red[2 * w + 1];
+    }
+    out[0] = sr;
+    out[1] = si;
+    *ticket = 0u;   // (the next call clears it as well: it does not rely on this)
+  }
+}
+
+}  // namespace
+
+extern "C" int lpc_fid_sample_noalloc(const double* g, int64_t n_sites, double* out, void* stream) {
+  if (!g || !out) return fail(LPC_EINVAL, "g and out must not be NULL");
+  if (n_sites < 0) return fail(LPC_EINVAL, "n_sites must be >= 0");
+  if (n_sites > LPC_NOALLOC_MAX_SITES)
+    return fail(LPC_EINVAL, "n_sites = %lld exceeds LPC_NOALLOC_MAX_SITES = %lld, what the library's static scratch array (%d bytes) covers",
+                (long long)n_sites, (long long)LPC_NOALLOC_MAX_SITES, (int)LPC_NOALLOC_SCRATCH_BYTES);
+  if ((n_sites > 0 && !is_device_ptr(g)) || !is_device_ptr(out)) return fail(LPC_EINVAL, "g and out must be device pointers");
+  int dev = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= MAX_DEVICES) return fail(LPC_ECUDA, "device ordinal %d is beyond the %d this library keeps track of", dev, MAX_DEVICES);
+  // the device address of the array on THIS device: asked for once per device, with that device current
+  static unsigned char* scratch_of[MAX_DEVICES] = {};
+  unsigned char* scratch = scratch_of[dev];
+  if (!scratch) {
+    CUDA_TRY(cudaGetSymbolAddress(reinterpret_cast<void**>(&scratch), g_noalloc_scratch));
+    if (!scratch) return fail(LPC_ECUDA, "cudaGetSymbolAddress gave no address for the scratch array on device %d", dev);
+    scratch_of[dev] = scratch;
+  }
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  // the ticket must start at zero whatever an earlier (perhaps failed) call left; the partials are overwritten before they are read
+  CUDA_TRY(cudaMemsetAsync(scratch, 0, NA_HEADER, st));
+  const unsigned grid = (unsigned)std::max<long long>(1, (n_sites + NA_CHUNK - 1) / NA_CHUNK);
+  fid_sample_noalloc_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(g), (long long)n_sites, scratch, out);
+  CUDA_TRY(cudaGetLastError());
+  return LPC_OK;
+}
