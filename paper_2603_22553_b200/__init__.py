@@ -31,7 +31,7 @@ EXPORTS = (
     "lpc_workspace_bytes", "lpc_create_lattice", "lpc_set_site_params", "lpc_set_link_mobility", "lpc_step_n", "lpc_read_fid",
     "lpc_moments", "lpc_read_field", "lpc_set_state", "lpc_equilibrate", "lpc_seed_from_density", "lpc_set_regions", "lpc_read_fid_region", "lpc_moments_region", "lpc_spectrum", "lpc_set_kernel",
     "lpc_set_option", "lpc_time_block_steps", "lpc_reads_sin_alone", "lpc_ipc_export", "lpc_ipc_open", "lpc_ipc_close", "lpc_steps_done", "lpc_partition_sum", "lpc_set_partition_sum", "lpc_halo_view", "lpc_set_halo_peers", "lpc_slab_finish",
-    "lpc_launch_count", "lpc_bytes_per_site_step", "lpc_fid_sample_noalloc", "lpc_destroy", "lpc_last_error",
+    "lpc_launch_count", "lpc_bytes_per_site_step", "lpc_fid_sample_noalloc", "lpc_sync_steps", "lpc_destroy", "lpc_last_error",
 )
 
 
@@ -90,6 +90,7 @@ def _load():
     lib.lpc_read_fid_region.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_int64, C.c_void_p]
     lib.lpc_moments_region.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_void_p, C.c_void_p]
     lib.lpc_spectrum.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_double, C.c_double, C.c_int64, C.c_double, C.c_void_p]
+    lib.lpc_sync_steps.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
     lib.lpc_fid_sample_noalloc.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
     lib.lpc_time_block_steps.argtypes = [C.c_void_p]
     lib.lpc_time_block_steps.restype = C.c_int32
@@ -313,6 +314,13 @@ def lpc_set_option(handle, key, value):
 LPC_NOALLOC_MAX_SITES = 1 << 28
 
 
+def lpc_sync_steps(handle) -> int:
+    """Read the device's step count back after CUDA graph replays of lpc_step_n (include/lpc.h "CUDA graphs")."""
+    n = C.c_int64(0)
+    _check(_lib.lpc_sync_steps(handle, C.byref(n)))
+    return int(n.value)
+
+
 def lpc_fid_sample_noalloc(g_dev_ptr, n_sites, out_dev_ptr, stream=None):
     """G = sum of n_sites complex numbers at the DEVICE address g_dev_ptr into the 2 doubles at the DEVICE address
     out_dev_ptr (Eq. 12); scratch in the library's static device array, nothing is allocated (include/lpc.h)."""
@@ -489,6 +497,10 @@ class Lattice:
 
     def set_option(self, key, value):
         lpc_set_option(self.handle, key, value)
+
+    def sync_steps(self):
+        """After CUDA graph replays of ``step``: take the device's step count (include/lpc.h "CUDA graphs")."""
+        return lpc_sync_steps(self.handle)
 
     @property
     def time_block_steps(self):

@@ -1549,6 +1549,20 @@ int lpc_set_option(lpc_lattice* h, int32_t key, int64_t value) {
 int32_t lpc_time_block_steps(const lpc_lattice* h) { return (h && step2_usable(h)) ? 2 : 1; }
 int32_t lpc_reads_sin_alone(const lpc_lattice* h) { return (h && h->have_params && sin_only(h)) ? 1 : 0; }
 int64_t lpc_steps_done(const lpc_lattice* h) { return h ? h->steps : 0; }
+
+int lpc_sync_steps(lpc_lattice* h, int64_t* steps_done) {
+  if (!h) return fail(LPC_EINVAL, "lattice is NULL");
+  if (!h->have_params) return fail(LPC_ESTATE, "lpc_set_site_params has not been called");
+  long long s = 0;
+  CUDA_TRY(cudaMemcpyAsync(&s, &wsp<Ctl>(h, h->off.ctl)->step, sizeof(s), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  if (s < 0 || s > h->cfg.max_steps)
+    return fail(LPC_ESTATE, "the device has taken %lld steps but the series hold max_steps = %lld: graph replays overflowed them", s,
+                (long long)h->cfg.max_steps);
+  h->steps = s;
+  if (steps_done) *steps_done = s;
+  return LPC_OK;
+}
 int64_t lpc_launch_count(const lpc_lattice* h) { return h ? h->launches : 0; }
 
 double lpc_bytes_per_site_step(const lpc_lattice* h) {

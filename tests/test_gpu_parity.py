@@ -404,6 +404,55 @@ def test_sweeps_that_read_sin_alone(lpc, oracle_mod, precision):
         _check(lpc, wide, gpu, orc, n, tol_site=tol_site, tol_sum=tol_sum, what=f"wide angle tb={tb} p{precision}")
 
 
+@pytest.mark.parametrize("kernel,nm,precision", [(2, 0, 0), (2, 3, 0), (1, 0, 0), (2, 0, 1)])
+def test_step_n_under_cuda_graph_capture(lpc, oracle_mod, kernel, nm, precision):
+    """lpc_step_n only enqueues launches: captured into a CUDA graph and replayed it appends to the series like direct calls
+    (include/lpc.h "CUDA graphs"); lpc_sync_steps brings the host's count up to date.  Against the oracle and, bit for bit,
+    against a lattice stepped without a graph."""
+    import torch
+
+    k, reps = 6, 4
+    n = 3 + k * reps + 2
+    lat = lpc_inputs.random_small((40, 24, 100), bc=(0, 1, 0), p_block=0.25, alpha=0.9, seed=88, n_steps=n, n_moments=nm)
+    tol_site, tol_sum = (1e-5, 1e-5) if precision else (1e-10, 1e-9)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        gpu, orc = _pair(lpc, oracle_mod, lat, n, kernel, precision=precision)
+        gpu.step(3)                                     # odd: the graph starts from buffer 1
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=st):
+            gpu.step(k)
+        assert gpu.steps_done == 3 + k                  # the host counted the capture, the device has not run it
+        assert gpu.sync_steps() == 3
+        for _ in range(reps):
+            graph.replay()
+        assert gpu.sync_steps() == 3 + k * reps
+        gpu.step(2)                                     # and on without the graph
+        assert gpu.steps_done == n
+        plain = lpc.Lattice.from_inputs(lat, precision=precision, n_moments=nm, max_steps=n)
+        plain.set_kernel(kernel)
+        plain.step(n)
+        orc.step(n)
+        _check(lpc, lat, gpu, orc, n, tol_site=tol_site, tol_sum=tol_sum, what=f"graph k{kernel} m{nm} p{precision}")
+        assert np.array_equal(gpu.fid(), plain.fid())
+        assert np.array_equal(gpu.field(lpc.LPC_FIELD_G), plain.field(lpc.LPC_FIELD_G))
+        if nm:
+            assert np.array_equal(gpu.moments()[0], plain.moments()[0])
+        # replays beyond the series' capacity are the caller's to avoid; what sync_steps can still tell is that it happened
+        small = lpc.Lattice.from_inputs(lat, precision=precision, n_moments=0, max_steps=k + 1)
+        small.set_kernel(kernel)
+        g2 = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g2, stream=st):
+            small.step(k)
+        small.sync_steps()
+        g2.replay()
+        assert small.sync_steps() == k
+        small.close()
+        plain.close()
+        gpu.close()
+
+
 # ---------------------------------------------------------------------------------------------
 # states set from outside, device-resident inputs
 # ---------------------------------------------------------------------------------------------
