@@ -268,6 +268,32 @@ def test_two_step_sweep_with_moment_fields(lpc, oracle_mod, shape, bc, alpha, pr
     _check(lpc, lat, two, orc, n, tol_site=tol_site, tol_sum=tol_sum, what=f"two-step moments {shape} p{precision}")
 
 
+@pytest.mark.parametrize("precision", [0, 1])
+def test_two_step_sweep_on_several_waves_of_ctas(lpc, precision):
+    """The hand-over between the two groups of warps under load: a lattice of several waves of CTAs (one CTA per SM), 30 steps,
+    bit for bit the one-step sweeps and bitwise reproducible."""
+    n = 30
+    lat = lpc_inputs.sweep(128, n_steps=n)
+    shape = (130, 200, 384)                                   # 25 y-tiles x 6 (3 in fp32) z-tiles x 2 or 3 x chunks
+    rng = np.random.default_rng(2)
+    dF = -3.0 * rng.random(shape)
+    blocked = (rng.random(shape) < 0.2).astype(np.uint8)
+    omega = -12000.0 * rng.random(shape)
+    outs = []
+    for tb in (1, 2, 2):
+        gpu = lpc.Lattice(shape, bc=(0, 0, 0), precision=precision, dt=lat.dt, max_steps=n)
+        gpu.set_kernel(2)
+        gpu.set_option(lpc.LPC_OPT_TIME_BLOCK, tb)
+        gpu.set_site_params(dF, blocked, omega)
+        gpu.step(n)
+        outs.append((gpu.field(lpc.LPC_FIELD_G), gpu.fid()))
+        gpu.close()
+    assert np.array_equal(outs[0][0], outs[1][0])             # the state: same arithmetic per site
+    assert np.array_equal(outs[1][0], outs[2][0]) and np.array_equal(outs[1][1], outs[2][1])
+    scale = 1e-5 if precision else 1e-12                      # the series: another summation order
+    assert np.max(np.abs(outs[0][1] - outs[1][1])) <= scale
+
+
 def test_two_step_sweep_default_and_eligibility(lpc, oracle_mod):
     lat = lpc_inputs.random_small((24, 16, 70), bc=(0, 0, 0), p_block=0.2, seed=62, n_moments=0)
     n = 10
